@@ -1,0 +1,170 @@
+/* tcw.h -- C ABI of the B200-native tCW track-sum library (libtcw.so).
+ *
+ * The operation is the search statistic of arxiv 2507.07816 (Merou, Tenorio, Sintes):
+ * "templates ... describe the corresponding time-frequency evolution track of potential signals
+ *  in data ... The statistics are then summed across the data bins selected by the track"
+ * (section 2).  For a template (f0, tau, n, n-hat) and every SFT j with t_j >= T0
+ *
+ *     f_gw(t_j)  = f0 * ((t_j - T0)/tau + 1)^(1/(1-n))                  eq. (1)
+ *     f_hat(t_j) = f_gw(t_j) * (1 + v(t_j).n-hat / c)                   eq. (2)
+ *     k_j        = rint(f_hat(t_j) * T_sft) - k_min,  k_min = rint(f_min * T_sft)
+ *     stat       = sum over j with 0 <= k_j < n_bins of spectrogram[j][k_j]
+ *
+ * where spectrogram[j][k] is the normalised power rho_j[k] or the number count nu_j[k] of
+ * SFT j.  Every floating-point step of k_j is one IEEE-754 binary64 operation
+ * in the order ((f0*g)*D)*T_sft with g the correctly rounded power and D = 1 + beta,
+ * beta = ((vx*nx + vy*ny) + vz*nz)/c, c = 299792458 m/s (readings
+ * Q1-Q19).  rint is round-half-to-even.  Out-of-band bins are skipped.  The candidate
+ * reduction is the per-(sky, tau, n) maximum over f0 with the lowest f0 index attaining it
+ * (PAPER.md:79 compares the best template near a signal with a threshold).
+ *
+ * Template linear index = ((s*n_tau + a)*n_brk + b)*n_f0 + i   (f0 fastest, sky slowest);
+ * a "group" is the n_f0 templates sharing one (s, a, b); group index = (s*n_tau + a)*n_brk + b.
+ *
+ * All work runs in CUDA kernels for sm_100a on the device that is current at tcw_create.
+ * There is no CPU fallback: without a usable CUDA device tcw_create returns TCW_ECUDA.
+ *
+ * Error behaviour: every function returns an int code (below); nothing is thrown across the
+ * ABI; on error no output buffer is written.  tcw_last_error() gives a thread-local message.
+ * Argument validation happens before the first CUDA call, so TCW_EINVAL is returned for bad
+ * arguments even on a machine with no GPU.
+ */
+#ifndef TCW_H_
+#define TCW_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tcw_handle tcw_handle; /* opaque, owned by the library */
+
+enum {
+    TCW_OK = 0,
+    TCW_EINVAL = -1,       /* bad argument (NULL, size, ordering, range) */
+    TCW_ENOMEM = -2,       /* host or device allocation failed */
+    TCW_ECUDA = -3,        /* a CUDA runtime call failed (message in tcw_last_error) */
+    TCW_EUNSUPPORTED = -4  /* valid request the library cannot serve */
+};
+
+/* Spectrogram element formats (normalised power rho or number count nu). */
+enum {
+    TCW_F32_POWER = 0, /* float32 [n_sft][n_bins]                                            */
+    TCW_U8_COUNT = 1,  /* uint8   [n_sft][n_bins], value added as an integer (0/1 for nu)     */
+    TCW_BIT_COUNT = 2  /* uint32 words, bit k of row j = (word[k >> 5] >> (k & 31)) & 1       */
+};
+
+/* tcw_create -- bind a spectrogram and its per-SFT metadata to a handle.
+ *
+ *  out             receives the handle.
+ *  spectrogram     SFT-major rows, row j at byte offset j*row_pitch_bytes.  DEVICE pointer, or
+ *                  HOST pointer (pageable or pinned): the library copies it with
+ *                  cudaMemcpyDefault into its own 16-byte-aligned, zero-padded pitch, so the
+ *                  caller may free or overwrite it as soon as tcw_create returns.
+ *  format          one of TCW_F32_POWER / TCW_U8_COUNT / TCW_BIT_COUNT.
+ *  row_pitch_bytes >= the bytes of one row (4*n_bins, n_bins, 4*ceil(n_bins/32)).
+ *  n_sft, n_bins   > 0.  SFTs that are missing are simply absent from the list (reading Q16).
+ *  f_min, T_sft    band start (Hz) and SFT length (s); bin k is centred on (k_min + k)/T_sft.
+ *                  TCW_EINVAL if |f_min*T_sft - rint(f_min*T_sft)| > 1e-9.
+ *  timestamps      HOST, [n_sft], strictly increasing; timestamps[j] IS the time t_j at which
+ *                  eq. (1)-(2) are evaluated for SFT j (callers pass mid-SFT times, reading Q1).
+ *  velocities      HOST, [n_sft][3], detector velocity wrt the SSB in m/s, equatorial frame.
+ *  stream          cudaStream_t (NULL = default stream).  The stream is synchronised before
+ *                  tcw_create returns.
+ */
+int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes,
+               int n_sft, int n_bins, double f_min, double T_sft, const double *timestamps,
+               const double *velocities, void *stream);
+
+/* The cubic-lattice template bank: explicit axes, HOST pointers, copied during
+ * the call.  Spacing is the caller's business; only f0 must be ascending. */
+typedef struct {
+    double T0;          /* signal start time, same clock as timestamps; SFTs with t_j < T0 are skipped */
+    int n_f0;
+    const double *f0;   /* [n_f0] Hz, > 0, strictly ascending                     */
+    int n_tau;
+    const double *tau;  /* [n_tau] s, > 0                                          */
+    int n_brk;
+    const double *brk;  /* [n_brk] braking index n, > 1                            */
+    int n_sky;
+    const double *sky;  /* [n_sky][3] unit vectors n-hat towards the source, equatorial */
+} tcw_grid;
+
+/* Candidate record per group.  Power format: stat is float32.  Count formats: the same 8 bytes
+ * hold { int32 stat; int32 f0_index }. */
+typedef struct {
+    float stat;
+    int f0_index;
+} tcw_best_f32;
+typedef struct {
+    int stat;
+    int f0_index;
+} tcw_best_i32;
+
+/* tcw_search -- track sums for the whole grid, and the per-group best template.
+ *
+ *  out_stat  DEVICE, [n_sky][n_tau][n_brk][n_f0], float32 (power) or int32 (counts); may be NULL.
+ *  out_best  DEVICE, [n_sky*n_tau*n_brk] tcw_best_f32 / tcw_best_i32; may be NULL (not both).
+ *            Ties go to the lowest f0 index.  A template with no in-band SFT has stat 0 and
+ *            still takes part in the maximum.
+ *  stream    cudaStream_t.  The call enqueues its kernels and returns; outputs are valid once
+ *            the stream has been synchronised.  The grid arrays are copied before returning.
+ *            One search at a time per handle.
+ *
+ * Power sums are accumulated in float32 in a fixed order (run-to-run bit-identical); counts in
+ * int32, exact.  TCW_EINVAL for NULL / non-positive sizes, tau <= 0, n <= 1, f0 <= 0 or not
+ * ascending, | |n-hat| - 1 | > 1e-6, or f0_max*T_sft >= 2^31 - 2^20.
+ */
+int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_best, void *stream);
+
+/* tcw_search_host -- the same search with HOST output buffers (either may be NULL, not both):
+ * runs tcw_search into library scratch, copies the results to the host and synchronises the
+ * stream before returning. */
+int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host,
+                    void *stream);
+
+/* tcw_destroy -- free the handle and everything it owns.  NULL is a no-op returning TCW_OK. */
+int tcw_destroy(tcw_handle *h);
+
+/* tcw_last_error -- thread-local description of the last error on this thread; never NULL. */
+const char *tcw_last_error(void);
+
+/* ---- inspection entry points (used by the parity tests and by bench.py) ------------------- */
+
+/* tcw_track_indices -- the bin indices k_j themselves, for the listed templates.
+ *  sel      HOST, [n_sel] template linear indices.
+ *  out_k    DEVICE, int32 [n_sel][n_sft]; INT32_MIN where t_j < T0.  Computed by the same device
+ *           function the search kernels use.  Asynchronous like tcw_search. */
+int tcw_track_indices(tcw_handle *h, const tcw_grid *grid, long n_sel, const long *sel,
+                      int *out_k, void *stream);
+
+/* tcw_tables -- the two per-search tables of the last tcw_search / tcw_track_indices call:
+ *  out_g  HOST, float64 [n_tau][n_brk][n_sft], g = RN(((t_j - T0)/tau + 1)^(1/(1-n))), 0 where t_j < T0
+ *  out_d  HOST, float64 [n_sky][n_sft],        D = 1 + beta
+ * Either may be NULL.  Synchronises `stream`. */
+int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
+
+/* Options.  tcw_set_option returns TCW_EINVAL for an unknown key or value. */
+enum {
+    TCW_OPT_KERNEL = 0,     /* 0 auto (default), 1 force the global-memory gather kernel,
+                               2 force the TMA-staged kernel (TCW_EUNSUPPORTED at search if the
+                               f0 spacing makes the window exceed shared memory)              */
+    TCW_OPT_TIMING = 1,     /* 1: record CUDA events around each stage of tcw_search           */
+    TCW_OPT_F0_PER_LANE = 2 /* staged kernel: templates per lane, 4 or 8 (tile = 32x that); 0 auto */
+};
+int tcw_set_option(tcw_handle *h, int key, long value);
+
+/* tcw_get_timing -- device time of the stages of the last tcw_search, in milliseconds:
+ *  ms[0] Doppler + spin-down tables, ms[1] gather-accumulate kernel, ms[2] candidate reduction,
+ *  ms[3] whole call.  Needs TCW_OPT_TIMING = 1; synchronises the search's stream. */
+int tcw_get_timing(tcw_handle *h, float ms[4]);
+
+/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged),
+ * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
+ * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
+ * info[5] kernels launched by the call.  Synchronises the search's stream. */
+int tcw_get_info(tcw_handle *h, long info[6]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TCW_H_ */

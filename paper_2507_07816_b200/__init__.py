@@ -1,0 +1,290 @@
+"""paper_2507_07816_b200 -- thin Python binding of libtcw.so (include/tcw.h).
+
+Argument marshalling only: every step of the tCW track sum (eqs. (1)-(2),
+PAPER.md:57) runs in the CUDA kernels under csrc/.  PyTorch appears here for device memory and
+streams.  There is no CPU fallback: if the library cannot be loaded, or no CUDA device is
+usable, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+__all__ = [
+    "TcwError", "Handle", "Grid", "load_library", "library_path", "shard_groups",
+    "TCW_F32_POWER", "TCW_U8_COUNT", "TCW_BIT_COUNT", "FORMATS",
+]
+
+TCW_OK, TCW_EINVAL, TCW_ENOMEM, TCW_ECUDA, TCW_EUNSUPPORTED = 0, -1, -2, -3, -4
+TCW_F32_POWER, TCW_U8_COUNT, TCW_BIT_COUNT = 0, 1, 2
+TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE = 0, 1, 2
+FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
+
+EXPORTS = (
+    "tcw_create", "tcw_search", "tcw_search_host", "tcw_destroy", "tcw_last_error",
+    "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
+)
+
+
+class TcwError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"tcw error {code}: {message}")
+        self.code = code
+
+
+class _CGrid(ctypes.Structure):
+    _fields_ = [
+        ("T0", ctypes.c_double),
+        ("n_f0", ctypes.c_int), ("f0", ctypes.POINTER(ctypes.c_double)),
+        ("n_tau", ctypes.c_int), ("tau", ctypes.POINTER(ctypes.c_double)),
+        ("n_brk", ctypes.c_int), ("brk", ctypes.POINTER(ctypes.c_double)),
+        ("n_sky", ctypes.c_int), ("sky", ctypes.POINTER(ctypes.c_double)),
+    ]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library(rebuild: bool = False) -> ctypes.CDLL:
+    """dlopen libtcw.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None and not rebuild:
+        return _lib
+    path = _build.build(force=rebuild)
+    L = ctypes.CDLL(path)
+    vp, dp, ci, cl = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_long
+    L.tcw_create.restype = ci
+    L.tcw_create.argtypes = [ctypes.POINTER(vp), vp, ci, cl, ci, ci, ctypes.c_double, ctypes.c_double, dp, dp, vp]
+    L.tcw_search.restype = ci
+    L.tcw_search.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
+    L.tcw_search_host.restype = ci
+    L.tcw_search_host.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
+    L.tcw_destroy.restype = ci
+    L.tcw_destroy.argtypes = [vp]
+    L.tcw_last_error.restype = ctypes.c_char_p
+    L.tcw_last_error.argtypes = []
+    L.tcw_track_indices.restype = ci
+    L.tcw_track_indices.argtypes = [vp, ctypes.POINTER(_CGrid), cl, ctypes.POINTER(cl), vp, vp]
+    L.tcw_tables.restype = ci
+    L.tcw_tables.argtypes = [vp, dp, dp, vp]
+    L.tcw_set_option.restype = ci
+    L.tcw_set_option.argtypes = [vp, ci, cl]
+    L.tcw_get_timing.restype = ci
+    L.tcw_get_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.tcw_get_info.restype = ci
+    L.tcw_get_info.argtypes = [vp, ctypes.POINTER(cl)]
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != TCW_OK:
+        raise TcwError(rc, load_library().tcw_last_error().decode("utf-8", "replace"))
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _dp(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+@dataclass
+class Grid:
+    """The cubic-lattice template bank as explicit axes; mirrors tcw_grid."""
+    f0: np.ndarray
+    tau: np.ndarray
+    brk: np.ndarray
+    sky: np.ndarray            # [n_sky][3]
+    T0: float = 0.0
+
+    def __post_init__(self):
+        self.f0, self.tau, self.brk = _f64(self.f0), _f64(self.tau), _f64(self.brk)
+        self.sky = _f64(self.sky).reshape(-1, 3)
+
+    @classmethod
+    def of(cls, w) -> "Grid":
+        """From any object with attributes f0, tau, brk, sky, T0 (e.g. tcw_inputs.Workload)."""
+        return cls(w.f0, w.tau, w.brk, w.sky, float(w.T0))
+
+    @property
+    def n_groups(self) -> int:
+        return len(self.sky) * len(self.tau) * len(self.brk)
+
+    @property
+    def n_templates(self) -> int:
+        return self.n_groups * len(self.f0)
+
+    def _c(self) -> _CGrid:
+        return _CGrid(float(self.T0), len(self.f0), _dp(self.f0), len(self.tau), _dp(self.tau),
+                      len(self.brk), _dp(self.brk), len(self.sky), _dp(self.sky))
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Handle:
+    """tcw_create / tcw_search / tcw_destroy with the same argument meaning as include/tcw.h."""
+
+    def __init__(self, spectrogram, fmt, n_bins: int, f_min: float, T_sft: float, timestamps, velocities,
+                 stream=None):
+        """`spectrogram`: a CUDA torch tensor, or a host numpy array / CPU torch tensor, 2-D,
+        SFT-major, dtype float32 (fmt "f32"), uint8 ("u8") or int32/uint32 words ("bits")."""
+        import torch
+        L = load_library()
+        self._h = ctypes.c_void_p()
+        self.fmt = FORMATS[fmt] if isinstance(fmt, str) else int(fmt)
+        if isinstance(spectrogram, np.ndarray):
+            spec = np.ascontiguousarray(spectrogram)
+            ptr, pitch, n_sft = spec.ctypes.data, spec.strides[0], spec.shape[0]
+        else:
+            spec = spectrogram if spectrogram.stride(-1) == 1 else spectrogram.contiguous()
+            ptr, pitch, n_sft = spec.data_ptr(), spec.stride(0) * spec.element_size(), spec.shape[0]
+            if spec.is_cuda:
+                torch.cuda.set_device(spec.device)
+        ts, vel = _f64(timestamps), _f64(velocities)
+        if ts.shape != (n_sft,) or vel.shape != (n_sft, 3):
+            raise ValueError("timestamps must be [n_sft] and velocities [n_sft][3]")
+        self.n_sft, self.n_bins = int(n_sft), int(n_bins)
+        _check(L.tcw_create(ctypes.byref(self._h), ptr, self.fmt, pitch, self.n_sft, self.n_bins,
+                            float(f_min), float(T_sft), _dp(ts), _dp(vel), _stream_ptr(stream)))
+
+    @classmethod
+    def from_workload(cls, w, device="cuda", host: bool = False, stream=None) -> "Handle":
+        """Bind a tcw_inputs.Workload-like object.  host=False first moves the spectrogram to
+        `device` with torch; host=True hands the host array to tcw_create, which copies it."""
+        import torch
+        spec = w.spectrogram
+        if not host:
+            arr = np.ascontiguousarray(spec)
+            if arr.dtype == np.uint32:
+                arr = arr.view(np.int32)
+            spec = torch.from_numpy(arr).to(device)
+        return cls(spec, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, stream=stream)
+
+    # ------------------------------------------------------------------ the path
+    @property
+    def stat_dtype(self):
+        import torch
+        return torch.float32 if self.fmt == TCW_F32_POWER else torch.int32
+
+    def search(self, grid: Grid, out_stat=None, out_best=None, want_stat: bool = True, want_best: bool = True,
+               stream=None):
+        """tcw_search.  Returns (stat, best): stat a CUDA tensor [n_sky][n_tau][n_brk][n_f0]
+        (float32 or int32), best a CUDA int32 tensor [n_groups][2] whose column 0 holds the
+        statistic's bits (view as float32 for the power format) and column 1 the f0 index.
+        Asynchronous: synchronise the stream before reading."""
+        import torch
+        L = load_library()
+        dev = torch.device("cuda", torch.cuda.current_device())
+        if out_stat is None and want_stat:
+            out_stat = torch.empty((len(grid.sky), len(grid.tau), len(grid.brk), len(grid.f0)),
+                                   dtype=self.stat_dtype, device=dev)
+        if out_best is None and want_best:
+            out_best = torch.empty((grid.n_groups, 2), dtype=torch.int32, device=dev)
+        cg = grid._c()
+        _check(L.tcw_search(self._h, ctypes.byref(cg),
+                            out_stat.data_ptr() if out_stat is not None else None,
+                            out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
+        return out_stat, out_best
+
+    def search_host(self, grid: Grid, out_stat: np.ndarray | None = None, out_best: np.ndarray | None = None,
+                    want_stat: bool = True, stream=None):
+        """tcw_search_host: results land in host numpy arrays; synchronous."""
+        L = load_library()
+        if out_stat is None and want_stat:
+            out_stat = np.empty((len(grid.sky), len(grid.tau), len(grid.brk), len(grid.f0)),
+                                dtype=np.float32 if self.fmt == TCW_F32_POWER else np.int32)
+        if out_best is None:
+            out_best = np.empty((grid.n_groups, 2), dtype=np.int32)
+        cg = grid._c()
+        _check(L.tcw_search_host(self._h, ctypes.byref(cg),
+                                 out_stat.ctypes.data if out_stat is not None else None,
+                                 out_best.ctypes.data, _stream_ptr(stream)))
+        return out_stat, out_best
+
+    def best_fields(self, best):
+        """Split a best array ([n_groups][2] int32, torch or numpy) into (stat, f0_index)."""
+        if isinstance(best, np.ndarray):
+            stat = best[:, 0].copy().view(np.float32) if self.fmt == TCW_F32_POWER else best[:, 0].copy()
+            return stat, best[:, 1].copy()
+        b = best.cpu().numpy()
+        return self.best_fields(b)
+
+    # ------------------------------------------------------------------ inspection
+    def track_indices(self, grid: Grid, sel, stream=None):
+        """tcw_track_indices: int32 CUDA tensor [n_sel][n_sft] of bin indices k_j."""
+        import torch
+        L = load_library()
+        sel = np.ascontiguousarray(sel, dtype=np.int64)
+        out = torch.empty((len(sel), self.n_sft), dtype=torch.int32, device="cuda")
+        cg = grid._c()
+        _check(L.tcw_track_indices(self._h, ctypes.byref(cg), len(sel),
+                                   sel.ctypes.data_as(ctypes.POINTER(ctypes.c_long)), out.data_ptr(),
+                                   _stream_ptr(stream)))
+        return out
+
+    def tables(self, grid: Grid, stream=None):
+        """(g [n_tau][n_brk][n_sft], D [n_sky][n_sft]) of the last search, as host float64 arrays."""
+        L = load_library()
+        g = np.empty((len(grid.tau), len(grid.brk), self.n_sft), dtype=np.float64)
+        d = np.empty((len(grid.sky), self.n_sft), dtype=np.float64)
+        _check(L.tcw_tables(self._h, _dp(g), _dp(d), _stream_ptr(stream)))
+        return g, d
+
+    def set_option(self, key: int, value: int):
+        _check(load_library().tcw_set_option(self._h, int(key), int(value)))
+
+    def timing(self):
+        """Device milliseconds of the last search: (tables, sum kernel, best kernel, whole call)."""
+        ms = (ctypes.c_float * 4)()
+        _check(load_library().tcw_get_timing(self._h, ms))
+        return tuple(float(x) for x in ms)
+
+    def info(self) -> dict:
+        v = (ctypes.c_long * 6)()
+        _check(load_library().tcw_get_info(self._h, v))
+        return dict(kernel={1: "gather", 2: "staged"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
+                    smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load_library().tcw_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+
+def shard_groups(n_sky: int, rank: int, world_size: int) -> slice:
+    """Multi-GPU partition: whole sky points -- hence whole (sky, tau, n)
+    groups, so each per-group argmax stays on one rank -- split into contiguous, nearly equal
+    ranges.  No collective is needed on the data path; the spectrogram is replicated."""
+    if not (0 <= rank < world_size):
+        raise ValueError("rank out of range")
+    base, rem = divmod(n_sky, world_size)
+    lo = rank * base + min(rank, rem)
+    return slice(lo, lo + base + (1 if rank < rem else 0))

@@ -1,0 +1,583 @@
+// tcw_api.cu -- host runtime and C ABI of libtcw.so (declared in include/tcw.h).
+//
+// The host side validates arguments, owns the device copies (spectrogram re-laid to a 16-byte
+// aligned zero-padded pitch, timestamps, velocities), the grow-only scratch (tables, grid axes,
+// per-tile candidates) and the launch plan.  Every step of the path runs in the kernels of
+// tcw_tables.cuh and tcw_sum.cuh; there is no CPU fallback.
+#include "../../include/tcw.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tcw_sum.cuh"
+#include "tcw_tables.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(call)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(e_ == cudaErrorMemoryAllocation ? TCW_ENOMEM : TCW_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                               \
+    } while (0)
+
+constexpr double C_LIGHT = 299792458.0;
+constexpr size_t SMEM_MAX = 227 * 1024;
+
+template <typename T> struct DevBuf {
+    T *p = nullptr;
+    size_t cap = 0;  // elements
+    int reserve(size_t n)
+    {
+        if (n <= cap) return TCW_OK;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        CUDA_TRY(cudaMalloc((void **)&p, std::max<size_t>(n, 1) * sizeof(T)));
+        cap = n;
+        return TCW_OK;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+size_t row_bytes(int format, int n_bins)
+{
+    switch (format) {
+    case TCW_F32_POWER: return 4 * (size_t)n_bins;
+    case TCW_U8_COUNT: return (size_t)n_bins;
+    default: return 4 * (((size_t)n_bins + 31) / 32);
+    }
+}
+
+bool is_pow2(double x)
+{
+    int e;
+    return x > 0 && std::isfinite(x) && std::frexp(x, &e) == 0.5;
+}
+
+}  // namespace
+
+struct tcw_handle {
+    int device = 0;
+    int format = 0, n_sft = 0, n_bins = 0, k_min = 0;
+    long pitch = 0;
+    double f_min = 0, T = 0;
+    bool t_pow2 = false;
+    double vmax = 0;  // max |v_j|
+    std::vector<double> ts;
+    unsigned char *d_spec = nullptr;
+    double *d_ts = nullptr, *d_vel = nullptr;
+    // grow-only scratch
+    DevBuf<double> d_g, d_d, d_axes;
+    DevBuf<unsigned char> d_partial, d_stat, d_best;
+    DevBuf<long> d_sel;
+    int *d_status = nullptr;
+    double *h_stage = nullptr;  // pinned staging for the grid axes / selections
+    size_t h_stage_cap = 0;     // bytes
+    cudaEvent_t ev_stage = nullptr;
+    // options
+    int opt_kernel = 0, opt_timing = 0, opt_r = 0;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool timing_valid = false;
+    cudaStream_t last_stream = nullptr;
+    long info[6] = {0, 0, 0, 0, 0, 0};
+    // last tables
+    int tab_tau = 0, tab_brk = 0, tab_sky = 0;
+    // device axis pointers of the last prepared grid
+    const double *a_f0 = nullptr, *a_tau = nullptr, *a_brk = nullptr, *a_sky = nullptr;
+};
+
+namespace {
+
+int validate_grid(const tcw_handle *h, const tcw_grid *g)
+{
+    if (!g) return fail(TCW_EINVAL, "grid is NULL");
+    if (g->n_f0 <= 0 || g->n_tau <= 0 || g->n_brk <= 0 || g->n_sky <= 0)
+        return fail(TCW_EINVAL, "grid sizes must be positive");
+    if (!g->f0 || !g->tau || !g->brk || !g->sky) return fail(TCW_EINVAL, "grid axis pointer is NULL");
+    if (!std::isfinite(g->T0)) return fail(TCW_EINVAL, "T0 is not finite");
+    for (int i = 0; i < g->n_f0; ++i) {
+        if (!(g->f0[i] > 0) || !std::isfinite(g->f0[i])) return fail(TCW_EINVAL, "f0[%d] must be > 0", i);
+        if (i && !(g->f0[i] > g->f0[i - 1])) return fail(TCW_EINVAL, "f0 must be strictly ascending (at %d)", i);
+    }
+    if (g->f0[g->n_f0 - 1] * h->T >= 2147483648.0 - 1048576.0)
+        return fail(TCW_EINVAL, "f0_max*T_sft exceeds the 32-bit bin range");
+    for (int i = 0; i < g->n_tau; ++i)
+        if (!(g->tau[i] > 0) || !std::isfinite(g->tau[i])) return fail(TCW_EINVAL, "tau[%d] must be > 0", i);
+    for (int i = 0; i < g->n_brk; ++i)
+        if (!(g->brk[i] > 1) || !std::isfinite(g->brk[i])) return fail(TCW_EINVAL, "braking index brk[%d] must be > 1", i);
+    for (int i = 0; i < g->n_sky; ++i) {
+        const double *n = g->sky + 3 * (size_t)i;
+        double nrm = std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        if (!(std::fabs(nrm - 1.0) <= 1e-6)) return fail(TCW_EINVAL, "sky[%d] is not a unit vector", i);
+    }
+    long n_groups = (long)g->n_sky * g->n_tau * g->n_brk;
+    if (n_groups * (long)g->n_f0 / g->n_f0 != n_groups || n_groups > (1L << 40))
+        return fail(TCW_EINVAL, "grid too large");
+    return TCW_OK;
+}
+
+int ensure_stage(tcw_handle *h, size_t bytes)
+{
+    if (bytes <= h->h_stage_cap) return TCW_OK;
+    if (h->h_stage) cudaFreeHost(h->h_stage);
+    h->h_stage = nullptr;
+    h->h_stage_cap = 0;
+    CUDA_TRY(cudaMallocHost((void **)&h->h_stage, bytes));
+    h->h_stage_cap = bytes;
+    return TCW_OK;
+}
+
+// Copy the grid axes (and an optional selection list) to the device through pinned staging,
+// then build both tables on `st`.
+int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaStream_t st)
+{
+    CUDA_TRY(cudaSetDevice(h->device));
+    const size_t n_axes = (size_t)g->n_f0 + g->n_tau + g->n_brk + 3 * (size_t)g->n_sky;
+    const size_t stage_bytes = n_axes * sizeof(double) + (size_t)std::max<long>(n_sel, 0) * sizeof(long);
+    // the staging buffer may still feed the previous call's copy
+    CUDA_TRY(cudaEventSynchronize(h->ev_stage));
+    int rc;
+    if ((rc = ensure_stage(h, stage_bytes)) != TCW_OK) return rc;
+    if ((rc = h->d_axes.reserve(n_axes)) != TCW_OK) return rc;
+    if ((rc = h->d_g.reserve((size_t)g->n_tau * g->n_brk * h->n_sft)) != TCW_OK) return rc;
+    if ((rc = h->d_d.reserve((size_t)g->n_sky * h->n_sft)) != TCW_OK) return rc;
+    if (n_sel > 0 && (rc = h->d_sel.reserve((size_t)n_sel)) != TCW_OK) return rc;
+
+    double *w = h->h_stage;
+    std::memcpy(w, g->f0, sizeof(double) * g->n_f0);
+    std::memcpy(w + g->n_f0, g->tau, sizeof(double) * g->n_tau);
+    std::memcpy(w + g->n_f0 + g->n_tau, g->brk, sizeof(double) * g->n_brk);
+    std::memcpy(w + g->n_f0 + g->n_tau + g->n_brk, g->sky, sizeof(double) * 3 * (size_t)g->n_sky);
+    CUDA_TRY(cudaMemcpyAsync(h->d_axes.p, w, n_axes * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (n_sel > 0) {
+        std::memcpy(w + n_axes, sel, sizeof(long) * (size_t)n_sel);
+        CUDA_TRY(cudaMemcpyAsync(h->d_sel.p, w + n_axes, sizeof(long) * (size_t)n_sel, cudaMemcpyHostToDevice, st));
+    }
+    CUDA_TRY(cudaEventRecord(h->ev_stage, st));
+    h->a_f0 = h->d_axes.p;
+    h->a_tau = h->a_f0 + g->n_f0;
+    h->a_brk = h->a_tau + g->n_tau;
+    h->a_sky = h->a_brk + g->n_brk;
+
+    {
+        long total = (long)g->n_sky * h->n_sft;
+        tcw::doppler_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(h->d_vel, h->n_sft, h->a_sky,
+                                                                                 g->n_sky, h->d_d.p);
+        CUDA_TRY(cudaGetLastError());
+    }
+    {
+        long total = (long)g->n_tau * g->n_brk * h->n_sft;
+        tcw::spindown_table_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(
+            h->d_ts, h->n_sft, g->T0, h->a_tau, g->n_tau, h->a_brk, g->n_brk, h->d_g.p);
+        CUDA_TRY(cudaGetLastError());
+    }
+    h->tab_tau = g->n_tau;
+    h->tab_brk = g->n_brk;
+    h->tab_sky = g->n_sky;
+    h->last_stream = st;
+    return TCW_OK;
+}
+
+tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
+{
+    tcw::SumParams p;
+    std::memset(&p, 0, sizeof p);
+    p.spec = h->d_spec;
+    p.pitch = h->pitch;
+    p.n_sft = h->n_sft;
+    p.n_bins = h->n_bins;
+    p.k_min = h->k_min;
+    p.T = h->T;
+    p.gtab = h->d_g.p;
+    p.dtab = h->d_d.p;
+    p.f0 = h->a_f0;
+    p.n_f0 = g->n_f0;
+    p.n_ab = g->n_tau * g->n_brk;
+    p.j_begin = (int)(std::lower_bound(h->ts.begin(), h->ts.end(), g->T0) - h->ts.begin());
+    // |beta| <= |v| |n-hat| / c with | |n-hat| - 1 | <= 1e-6; a relative 1e-5 on beta is ample
+    const double dmax = 1.0 + (h->vmax / C_LIGHT) * (1.0 + 1e-5) + 1e-15;
+    p.dmaxT = dmax * h->T * (1.0 + 1e-12);
+    p.status = h->d_status;
+    return p;
+}
+
+// Upper bound of the number of bins a tile of `tile` consecutive f0 can select in one SFT:
+// k_last - k_first + 1 <= (f_last - f_first) * T * g * D + 2 with g <= 1, D*T <= dmaxT.
+long max_window_bins(const tcw_grid *g, int tile, double dmaxT)
+{
+    double df = 0;
+    for (int i0 = 0; i0 < g->n_f0; i0 += tile) {
+        int i1 = std::min(i0 + tile, g->n_f0) - 1;
+        df = std::max(df, g->f0[i1] - g->f0[i0]);
+    }
+    double w = std::floor(df * dmaxT) + 3.0;
+    return w > 1e9 ? (long)1e9 : (long)w;
+}
+
+int slab_pitch(int format, long w_bins)
+{
+    long b = format == TCW_F32_POWER ? 4 * w_bins + 32 : (format == TCW_U8_COUNT ? w_bins + 32 : (w_bins + 7) / 8 + 48);
+    b = (b + 15) & ~15L;
+    return b > (1L << 30) ? (1 << 30) : (int)b;
+}
+
+template <int FMT, int R, bool P2>
+int launch_staged_t(const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
+{
+    auto kern = tcw::sum_staged_kernel<FMT, R, P2>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)n_ctas, tcw::STAGED_THREADS, smem, st>>>(p);
+    CUDA_TRY(cudaGetLastError());
+    return TCW_OK;
+}
+
+template <int FMT, bool P2>
+int launch_staged_r(int r, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
+{
+    return r == 8 ? launch_staged_t<FMT, 8, P2>(p, n_ctas, smem, st) : launch_staged_t<FMT, 4, P2>(p, n_ctas, smem, st);
+}
+
+int launch_staged(int fmt, int r, bool p2, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
+{
+    switch (fmt) {
+    case TCW_F32_POWER:
+        return p2 ? launch_staged_r<tcw::FMT_F32, true>(r, p, n_ctas, smem, st)
+                  : launch_staged_r<tcw::FMT_F32, false>(r, p, n_ctas, smem, st);
+    case TCW_U8_COUNT:
+        return p2 ? launch_staged_r<tcw::FMT_U8, true>(r, p, n_ctas, smem, st)
+                  : launch_staged_r<tcw::FMT_U8, false>(r, p, n_ctas, smem, st);
+    default:
+        return p2 ? launch_staged_r<tcw::FMT_BITS, true>(r, p, n_ctas, smem, st)
+                  : launch_staged_r<tcw::FMT_BITS, false>(r, p, n_ctas, smem, st);
+    }
+}
+
+template <int FMT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
+{
+    if (p2) tcw::sum_gather_kernel<FMT, true><<<(unsigned)n_ctas, 128, 0, st>>>(p);
+    else tcw::sum_gather_kernel<FMT, false><<<(unsigned)n_ctas, 128, 0, st>>>(p);
+    CUDA_TRY(cudaGetLastError());
+    return TCW_OK;
+}
+
+int launch_gather(int fmt, bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
+{
+    switch (fmt) {
+    case TCW_F32_POWER: return launch_gather_t<tcw::FMT_F32>(p2, p, n_ctas, st);
+    case TCW_U8_COUNT: return launch_gather_t<tcw::FMT_U8>(p2, p, n_ctas, st);
+    default: return launch_gather_t<tcw::FMT_BITS>(p2, p, n_ctas, st);
+    }
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+extern "C" {
+
+const char *tcw_last_error(void) { return g_err; }
+
+int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes, int n_sft,
+               int n_bins, double f_min, double T_sft, const double *timestamps, const double *velocities,
+               void *stream)
+{
+    if (!out) return fail(TCW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!spectrogram || !timestamps || !velocities) return fail(TCW_EINVAL, "NULL input pointer");
+    if (format != TCW_F32_POWER && format != TCW_U8_COUNT && format != TCW_BIT_COUNT)
+        return fail(TCW_EINVAL, "unknown spectrogram format %d", format);
+    if (n_sft <= 0 || n_bins <= 0) return fail(TCW_EINVAL, "n_sft and n_bins must be positive");
+    if (row_pitch_bytes < (long)row_bytes(format, n_bins))
+        return fail(TCW_EINVAL, "row_pitch_bytes %ld is smaller than one row (%zu bytes)", row_pitch_bytes,
+                    row_bytes(format, n_bins));
+    if (!(T_sft > 0) || !std::isfinite(T_sft) || !(f_min >= 0) || !std::isfinite(f_min))
+        return fail(TCW_EINVAL, "f_min must be >= 0 and T_sft > 0");
+    const double km = std::rint(f_min * T_sft);
+    if (std::fabs(f_min * T_sft - km) > 1e-9) return fail(TCW_EINVAL, "f_min*T_sft must be an integer (bin-aligned band start)");
+    if (km + n_bins >= 2147483648.0 - 1048576.0) return fail(TCW_EINVAL, "band exceeds the 32-bit bin range");
+    double vmax = 0;
+    for (int j = 0; j < n_sft; ++j) {
+        if (!std::isfinite(timestamps[j])) return fail(TCW_EINVAL, "timestamps[%d] is not finite", j);
+        if (j && !(timestamps[j] > timestamps[j - 1]))
+            return fail(TCW_EINVAL, "timestamps must be strictly increasing (at %d)", j);
+        const double *v = velocities + 3 * (size_t)j;
+        double n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        if (!std::isfinite(n) || n >= 0.5 * C_LIGHT) return fail(TCW_EINVAL, "velocities[%d] is not a physical velocity", j);
+        vmax = std::max(vmax, n);
+    }
+
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    tcw_handle *h = new (std::nothrow) tcw_handle;
+    if (!h) return fail(TCW_ENOMEM, "out of host memory");
+    h->device = dev;
+    h->format = format;
+    h->n_sft = n_sft;
+    h->n_bins = n_bins;
+    h->f_min = f_min;
+    h->T = T_sft;
+    h->t_pow2 = is_pow2(T_sft);
+    h->k_min = (int)km;
+    h->vmax = vmax;
+    h->ts.assign(timestamps, timestamps + n_sft);
+    h->pitch = (long)((row_bytes(format, n_bins) + 15) & ~(size_t)15);
+    cudaStream_t st = (cudaStream_t)stream;
+
+#define CREATE_TRY(call)                                                                       \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            int rc_ = fail(e_ == cudaErrorMemoryAllocation ? TCW_ENOMEM : TCW_ECUDA, "%s: %s", #call, \
+                           cudaGetErrorString(e_));                                            \
+            tcw_destroy(h);                                                                    \
+            return rc_;                                                                        \
+        }                                                                                      \
+    } while (0)
+
+    CREATE_TRY(cudaMalloc((void **)&h->d_spec, (size_t)h->pitch * n_sft));
+    CREATE_TRY(cudaMalloc((void **)&h->d_ts, sizeof(double) * n_sft));
+    CREATE_TRY(cudaMalloc((void **)&h->d_vel, sizeof(double) * 3 * (size_t)n_sft));
+    CREATE_TRY(cudaMalloc((void **)&h->d_status, sizeof(int)));
+    CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
+    for (auto &e : h->ev) CREATE_TRY(cudaEventCreate(&e));
+    CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
+    if ((size_t)h->pitch != row_bytes(format, n_bins))
+        CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));
+    CREATE_TRY(cudaMemcpy2DAsync(h->d_spec, (size_t)h->pitch, spectrogram, (size_t)row_pitch_bytes,
+                                 row_bytes(format, n_bins), (size_t)n_sft, cudaMemcpyDefault, st));
+    CREATE_TRY(cudaMemcpyAsync(h->d_ts, timestamps, sizeof(double) * n_sft, cudaMemcpyHostToDevice, st));
+    CREATE_TRY(cudaMemcpyAsync(h->d_vel, velocities, sizeof(double) * 3 * (size_t)n_sft, cudaMemcpyHostToDevice, st));
+    CREATE_TRY(cudaEventRecord(h->ev_stage, st));
+    CREATE_TRY(cudaStreamSynchronize(st));
+#undef CREATE_TRY
+    *out = h;
+    return TCW_OK;
+}
+
+int tcw_destroy(tcw_handle *h)
+{
+    if (!h) return TCW_OK;
+    cudaSetDevice(h->device);
+    if (h->d_spec) cudaFree(h->d_spec);
+    if (h->d_ts) cudaFree(h->d_ts);
+    if (h->d_vel) cudaFree(h->d_vel);
+    if (h->d_status) cudaFree(h->d_status);
+    h->d_g.release();
+    h->d_d.release();
+    h->d_axes.release();
+    h->d_partial.release();
+    h->d_stat.release();
+    h->d_best.release();
+    h->d_sel.release();
+    if (h->h_stage) cudaFreeHost(h->h_stage);
+    if (h->ev_stage) cudaEventDestroy(h->ev_stage);
+    for (auto &e : h->ev)
+        if (e) cudaEventDestroy(e);
+    delete h;
+    return TCW_OK;
+}
+
+int tcw_set_option(tcw_handle *h, int key, long value)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    switch (key) {
+    case TCW_OPT_KERNEL:
+        if (value < 0 || value > 2) return fail(TCW_EINVAL, "TCW_OPT_KERNEL must be 0, 1 or 2");
+        h->opt_kernel = (int)value;
+        return TCW_OK;
+    case TCW_OPT_TIMING:
+        if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_TIMING must be 0 or 1");
+        h->opt_timing = (int)value;
+        return TCW_OK;
+    case TCW_OPT_F0_PER_LANE:
+        if (value != 0 && value != 4 && value != 8) return fail(TCW_EINVAL, "TCW_OPT_F0_PER_LANE must be 0, 4 or 8");
+        h->opt_r = (int)value;
+        return TCW_OK;
+    default: return fail(TCW_EINVAL, "unknown option %d", key);
+    }
+}
+
+int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_best, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    int rc = validate_grid(h, grid);
+    if (rc != TCW_OK) return rc;
+    if (!out_stat && !out_best) return fail(TCW_EINVAL, "out_stat and out_best are both NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
+
+    tcw::SumParams p = base_params(h, grid);
+    // ---- launch plan: staged kernel with the largest tile whose window fits shared memory
+    int kernel = 0, r = 0, stages = 0, pitch_s = 0;
+    size_t smem = 0;
+    if (h->opt_kernel != 1) {
+        const int cand[2] = {h->opt_r ? h->opt_r : 8, 4};
+        for (int c = 0; c < (h->opt_r ? 1 : 2) && !kernel; ++c) {
+            int ps = slab_pitch(h->format, max_window_bins(grid, 32 * cand[c], p.dmaxT));
+            size_t need_red = (size_t)tcw::NCW * 32 * cand[c] * 4;
+            for (int s = 4; s >= 2; --s) {
+                size_t b = tcw::staged_smem_bytes(s, ps);
+                if (b <= SMEM_MAX / 2 - 1024 || (s == 2 && b <= SMEM_MAX)) {
+                    if ((size_t)s * tcw::ROWS * ps < need_red) continue;
+                    kernel = 2; r = cand[c]; stages = s; pitch_s = ps; smem = b;
+                    break;
+                }
+            }
+        }
+        if (!kernel && h->opt_kernel == 2)
+            return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the staged kernel (window exceeds shared memory)");
+    }
+    if (!kernel) kernel = 1;
+    p.tile = kernel == 2 ? 32 * r : 128;
+    p.n_tiles = (grid->n_f0 + p.tile - 1) / p.tile;
+    p.stages = stages;
+    p.pitch_s = pitch_s;
+    const long n_ctas = n_groups * p.n_tiles;
+    if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "grid needs more than 2^31-1 CTAs; split the search");
+
+    CUDA_TRY(cudaSetDevice(h->device));
+    if ((rc = h->d_partial.reserve((size_t)n_ctas * 8)) != TCW_OK) return rc;
+    if (!out_best && (rc = h->d_best.reserve((size_t)n_groups * 8)) != TCW_OK) return rc;
+    p.partial = h->d_partial.p;
+    p.out_stat = out_stat;
+
+    const bool tm = h->opt_timing != 0;
+    h->timing_valid = false;
+    if (tm) CUDA_TRY(cudaEventRecord(h->ev[0], st));
+    if ((rc = prepare(h, grid, 0, nullptr, st)) != TCW_OK) return rc;
+    p.f0 = h->a_f0;
+    p.gtab = h->d_g.p;
+    p.dtab = h->d_d.p;
+    if (tm) CUDA_TRY(cudaEventRecord(h->ev[1], st));
+    if (kernel == 2) rc = launch_staged(h->format, r, h->t_pow2, p, n_ctas, smem, st);
+    else rc = launch_gather(h->format, h->t_pow2, p, n_ctas, st);
+    if (rc != TCW_OK) return rc;
+    if (tm) CUDA_TRY(cudaEventRecord(h->ev[2], st));
+    void *best_dst = out_best ? out_best : (void *)h->d_best.p;
+    if (h->format == TCW_F32_POWER)
+        tcw::best_kernel<float><<<(unsigned)((n_groups + 127) / 128), 128, 0, st>>>(
+            (const tcw::Best<float> *)h->d_partial.p, n_groups, p.n_tiles, (tcw::Best<float> *)best_dst);
+    else
+        tcw::best_kernel<int><<<(unsigned)((n_groups + 127) / 128), 128, 0, st>>>(
+            (const tcw::Best<int> *)h->d_partial.p, n_groups, p.n_tiles, (tcw::Best<int> *)best_dst);
+    CUDA_TRY(cudaGetLastError());
+    if (tm) {
+        CUDA_TRY(cudaEventRecord(h->ev[3], st));
+        h->timing_valid = true;
+    }
+    h->info[0] = kernel;
+    h->info[1] = p.tile;
+    h->info[2] = n_ctas;
+    h->info[3] = (long)smem;
+    h->info[5] = 4;  // doppler table, spin-down table, sum, best
+    return TCW_OK;
+}
+
+int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    int rc = validate_grid(h, grid);
+    if (rc != TCW_OK) return rc;
+    if (!out_stat_host && !out_best_host) return fail(TCW_EINVAL, "out_stat and out_best are both NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n_groups = (size_t)grid->n_sky * grid->n_tau * grid->n_brk;
+    const size_t n_templates = n_groups * grid->n_f0;
+    CUDA_TRY(cudaSetDevice(h->device));
+    if (out_stat_host && (rc = h->d_stat.reserve(n_templates * 4)) != TCW_OK) return rc;
+    if ((rc = h->d_best.reserve(n_groups * 8)) != TCW_OK) return rc;
+    rc = tcw_search(h, grid, out_stat_host ? (void *)h->d_stat.p : nullptr, h->d_best.p, stream);
+    if (rc != TCW_OK) return rc;
+    if (out_stat_host)
+        CUDA_TRY(cudaMemcpyAsync(out_stat_host, h->d_stat.p, n_templates * 4, cudaMemcpyDeviceToHost, st));
+    if (out_best_host)
+        CUDA_TRY(cudaMemcpyAsync(out_best_host, h->d_best.p, n_groups * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return TCW_OK;
+}
+
+int tcw_track_indices(tcw_handle *h, const tcw_grid *grid, long n_sel, const long *sel, int *out_k, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    int rc = validate_grid(h, grid);
+    if (rc != TCW_OK) return rc;
+    if (n_sel <= 0 || !sel || !out_k) return fail(TCW_EINVAL, "selection is empty or NULL");
+    const long n_templates = (long)grid->n_sky * grid->n_tau * grid->n_brk * grid->n_f0;
+    for (long q = 0; q < n_sel; ++q)
+        if (sel[q] < 0 || sel[q] >= n_templates) return fail(TCW_EINVAL, "sel[%ld] is not a template index", q);
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = prepare(h, grid, n_sel, sel, st)) != TCW_OK) return rc;
+    tcw::SumParams p = base_params(h, grid);
+    const long total = n_sel * h->n_sft;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (h->t_pow2) tcw::track_index_kernel<true><<<blocks, 256, 0, st>>>(p, h->d_sel.p, n_sel, p.n_ab, out_k);
+    else tcw::track_index_kernel<false><<<blocks, 256, 0, st>>>(p, h->d_sel.p, n_sel, p.n_ab, out_k);
+    CUDA_TRY(cudaGetLastError());
+    return TCW_OK;
+}
+
+int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    if (!h->tab_tau) return fail(TCW_EINVAL, "no search has been run on this handle");
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(cudaSetDevice(h->device));
+    if (out_g)
+        CUDA_TRY(cudaMemcpyAsync(out_g, h->d_g.p, sizeof(double) * (size_t)h->tab_tau * h->tab_brk * h->n_sft,
+                                 cudaMemcpyDeviceToHost, st));
+    if (out_d)
+        CUDA_TRY(cudaMemcpyAsync(out_d, h->d_d.p, sizeof(double) * (size_t)h->tab_sky * h->n_sft,
+                                 cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return TCW_OK;
+}
+
+int tcw_get_timing(tcw_handle *h, float ms[4])
+{
+    if (!h || !ms) return fail(TCW_EINVAL, "NULL argument");
+    if (!h->timing_valid) return fail(TCW_EINVAL, "no timed search: set TCW_OPT_TIMING = 1 before tcw_search");
+    CUDA_TRY(cudaEventSynchronize(h->ev[3]));
+    CUDA_TRY(cudaEventElapsedTime(&ms[0], h->ev[0], h->ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]));
+    CUDA_TRY(cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]));
+    CUDA_TRY(cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]));
+    return TCW_OK;
+}
+
+int tcw_get_info(tcw_handle *h, long info[6])
+{
+    if (!h || !info) return fail(TCW_EINVAL, "NULL argument");
+    if (!h->info[0]) return fail(TCW_EINVAL, "no search has been run on this handle");
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaStreamSynchronize(h->last_stream));
+    int status = 0;
+    CUDA_TRY(cudaMemcpy(&status, h->d_status, sizeof(int), cudaMemcpyDeviceToHost));
+    h->info[4] = status;
+    std::memcpy(info, h->info, sizeof h->info);
+    return TCW_OK;
+}
+
+}  // extern "C"

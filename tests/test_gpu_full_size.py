@@ -1,0 +1,123 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot evaluate 6.9e9 (cfg2) or 8.8e11 (cfg3) lookups in seconds, so the GPU runs
+the whole grid and the oracle recomputes seeded samples of whole (sky, tau, n) groups -- all f0
+of each, so the per-group best is checkable too -- plus properties that hold at any size.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import tcw_inputs
+
+from test_gpu_parity import TOL, assert_best_parity, assert_stat_parity, tcw  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def sampled_group_parity(tcw, w, groups, stat, bs, bi):
+    n_f0 = len(w.f0)
+    ref = oracle.evaluate(w, sel=oracle.group_templates(w, groups))
+    got = stat.reshape(-1, n_f0)[groups].reshape(-1)
+    assert_stat_parity(w, got, ref.stat)
+    assert_best_parity(w, n_f0, bs[groups], bi[groups], ref.stat)
+    return ref
+
+
+def test_cfg2_full_grid_sampled_groups(tcw):
+    """cfg2 exactly as bench.py runs it: 640 000 templates x 10 800 SFTs, float32 power."""
+    import torch
+    w = tcw_inputs.make_workload("cfg2")
+    with tcw.Handle.from_workload(w) as h:
+        grid = tcw.Grid.of(w)
+        stat, best = h.search(grid)
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == "staged" and info["status"] == 0
+        bs, bi = h.best_fields(best)
+        stat = stat.cpu().numpy()
+        # sampled bin indices, straight from the device function the kernel uses
+        rng = np.random.default_rng(22)
+        sel = rng.integers(0, w.n_templates, size=48)
+        k = h.track_indices(grid, sel)
+        torch.cuda.synchronize()
+    rk = oracle.evaluate(w, sel=sel, want_k=True)
+    clean = rk.n_ambig == 0
+    assert clean.sum() >= 40 and np.array_equal(k.cpu().numpy()[clean], rk.k[clean])
+    groups = np.array([0, 4, 37, 80, 121, 159])            # first, last, and a spread of (tau, n)
+    sampled_group_parity(tcw, w, groups, stat, bs, bi)
+    # properties at full size: per-group best equals the maximum of the group's own statistics
+    st = stat.reshape(-1, len(w.f0))
+    assert np.array_equal(bs, st.max(axis=1)) and np.array_equal(bi, st.argmax(axis=1))
+    assert np.all(st >= 0) and np.isfinite(st).all()
+    # the 20 injections raise the best statistic of the groups nearest to them: the global
+    # maximum must sit well above the noise-only expectation N + 5 sqrt(N)
+    assert bs.max() > 10800 * 0.3
+
+
+@pytest.mark.parametrize("fmt", ["u8", "bits"])
+def test_cfg3_sky_patch_subset_counts_bit_exact(tcw, fmt):
+    """cfg3 data (cfg2 thresholded at 1.6) with a 12-sky x 3-tau x 2-n slice of its grid, all
+    4000 f0: 72 groups on the GPU, 6 sampled by the oracle; u8 and bit-packed must agree exactly."""
+    import torch
+    w = tcw_inputs.make_workload("cfg3", fmt=fmt)
+    w = w.subgrid(tau=[0, 7, 15], brk=[0, 4], sky=np.arange(0, 256, 22))
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        assert h.info()["status"] == 0
+        bs, bi = h.best_fields(best)
+    stat = stat.cpu().numpy()
+    groups = np.array([0, 5, 17, 33, 50, w.n_groups - 1])
+    sampled_group_parity(tcw, w, groups, stat, bs, bi)
+    st = stat.reshape(-1, len(w.f0))
+    assert np.array_equal(bs, st.max(axis=1)) and np.array_equal(bi, st.argmax(axis=1))
+    test_cfg3_sky_patch_subset_counts_bit_exact.results = getattr(
+        test_cfg3_sky_patch_subset_counts_bit_exact, "results", {})
+    test_cfg3_sky_patch_subset_counts_bit_exact.results[fmt] = stat
+    res = test_cfg3_sky_patch_subset_counts_bit_exact.results
+    if len(res) == 2:
+        assert np.array_equal(res["u8"], res["bits"])
+
+
+def test_cfg4_like_gaps_wide_band(tcw):
+    """cfg4's structure at reduced size: 20 000 bins (500-3000 Hz), 30% of 4000 slots missing in
+    random gaps, 20 000 f0 (79 tiles with a ragged tail), half-integer braking indices."""
+    import torch
+    rng = np.random.default_rng(44)
+    n_slots, n_bins = 4000, 20000
+    present = np.ones(n_slots, dtype=bool)
+    while (~present).mean() < 0.30:
+        length = int(rng.uniform(60, 400))
+        start = int(rng.integers(0, n_slots - length))
+        present[start:start + length] = False
+    ts = (8.0 * np.arange(n_slots) + 4.0)[present]
+    rho = rng.standard_exponential((len(ts), n_bins), dtype=np.float32)
+    w = tcw_inputs.Workload("cfg4like", "f32", rho, len(ts), n_bins, 500.0, 8.0, ts,
+                            tcw_inputs.detector_velocity(ts), 0.0,
+                            500.0 + 0.125 * np.arange(20000), np.geomspace(3500.0, 35000.0, 4),
+                            np.array([3.0, 3.5, 6.5]), tcw_inputs.sky_vector(1.0, 0.3)[None])
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        assert h.info()["status"] == 0
+        bs, bi = h.best_fields(best)
+    sampled_group_parity(tcw, w, np.array([0, 5, 11]), stat.cpu().numpy(), bs, bi)
+
+
+def test_cfg5_all_sky_subset_bits(tcw):
+    """cfg5 data (non-stationary floor, bit-packed, band from 1000 Hz so k_min = 8000) with 40 of
+    its 4096 sky points: the full-sphere Doppler spread moves tracks by up to +-0.8 bin."""
+    import torch
+    w = tcw_inputs.make_workload("cfg5")
+    w = w.subgrid(sky=np.arange(0, 4096, 103))
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        assert h.info()["status"] == 0
+        bs, bi = h.best_fields(best)
+    groups = np.array([0, 100, 333, 500, w.n_groups - 1])
+    ref = sampled_group_parity(tcw, w, groups, stat.cpu().numpy(), bs, bi)
+    assert ref.stat.max() > 100
