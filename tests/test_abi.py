@@ -1,0 +1,138 @@
+"""CPU-side checks of the boundary: libtcw.so builds, loads without a GPU, exports every symbol
+include/tcw.h declares, and rejects bad arguments before touching CUDA.  No compute call is made."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2507_07816_b200 as tcw
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "tcw.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    return tcw.load_library()
+
+
+def declared_functions():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(tcw_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    names = declared_functions()
+    assert set(names) == set(tcw.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_header_constants_match_binding():
+    text = open(HEADER).read()
+    for name in ("TCW_OK", "TCW_EINVAL", "TCW_ENOMEM", "TCW_ECUDA", "TCW_EUNSUPPORTED",
+                 "TCW_F32_POWER", "TCW_U8_COUNT", "TCW_BIT_COUNT",
+                 "TCW_OPT_KERNEL", "TCW_OPT_TIMING", "TCW_OPT_F0_PER_LANE"):
+        m = re.search(rf"\b{name}\s*=\s*(-?\d+)", text)
+        assert m, name
+        assert int(m.group(1)) == getattr(tcw, name), name
+
+
+def test_library_is_sm100a_and_has_tma_bulk_copies():
+    """The .so carries sm_100a SASS and the staged kernel's TMA bulk copies (UBLKCP)."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump) and not shutil.which("cuobjdump"):
+        pytest.skip("cuobjdump not available")
+    elf = subprocess.run([cuobjdump, "-lelf", tcw.library_path()], capture_output=True, text=True).stdout
+    assert "sm_100a" in elf
+    sass = subprocess.run([cuobjdump, "-sass", "-fun", "_ZN3tcw17sum_staged_kernelILi0ELi8ELb1EEEvNS_9SumParamsE",
+                           tcw.library_path()], capture_output=True, text=True).stdout
+    assert "UBLKCP" in sass and "SYNCS" in sass
+    assert "DFMA" not in sass            # the index chain is never contracted
+    assert "DMUL" in sass and "DADD" in sass
+
+
+def _create_args(n_sft=4, n_bins=8):
+    spec = np.zeros((n_sft, n_bins), dtype=np.float32)
+    ts = 8.0 * np.arange(n_sft) + 4.0
+    vel = np.zeros((n_sft, 3))
+    return spec, ts, vel
+
+
+def _create(lib, spec, fmt, pitch, n_sft, n_bins, f_min, T, ts, vel):
+    h = ctypes.c_void_p()
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = lib.tcw_create(ctypes.byref(h), spec.ctypes.data if spec is not None else None, fmt, pitch, n_sft, n_bins,
+                        f_min, T, ts.ctypes.data_as(dp) if ts is not None else None,
+                        vel.ctypes.data_as(dp) if vel is not None else None, None)
+    return rc, h
+
+
+def test_create_rejects_bad_arguments_without_cuda(lib):
+    spec, ts, vel = _create_args()
+    bad = [
+        dict(spec=None),
+        dict(ts=None),
+        dict(vel=None),
+        dict(fmt=7),
+        dict(n_sft=0),
+        dict(n_bins=-1),
+        dict(pitch=16),                                   # smaller than a row of 8 floats
+        dict(T=0.0),
+        dict(f_min=500.03),                               # f_min*T_sft not an integer
+        dict(ts=np.array([4.0, 12.0, 12.0, 28.0])),       # not strictly increasing
+        dict(ts=np.array([4.0, np.nan, 20.0, 28.0])),
+        dict(vel=np.full((4, 3), 3e8)),                   # not a physical detector velocity
+    ]
+    for kw in bad:
+        a = dict(spec=spec, fmt=0, pitch=32, n_sft=4, n_bins=8, f_min=500.0, T=8.0, ts=ts, vel=vel)
+        a.update(kw)
+        rc, h = _create(lib, a["spec"], a["fmt"], a["pitch"], a["n_sft"], a["n_bins"], a["f_min"], a["T"],
+                        a["ts"], a["vel"])
+        assert rc == tcw.TCW_EINVAL, kw
+        assert not h.value
+        assert len(lib.tcw_last_error()) > 0
+    assert lib.tcw_create(None, None, 0, 0, 0, 0, 0.0, 0.0, None, None, None) == tcw.TCW_EINVAL
+
+
+def test_null_handle_calls(lib):
+    assert lib.tcw_destroy(None) == tcw.TCW_OK
+    assert lib.tcw_search(None, None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_search_host(None, None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_set_option(None, 0, 0) == tcw.TCW_EINVAL
+    assert lib.tcw_get_timing(None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_get_info(None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_tables(None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_track_indices(None, None, 0, None, None, None) == tcw.TCW_EINVAL
+    assert isinstance(lib.tcw_last_error(), bytes)
+
+
+def test_no_cuda_device_fails_loudly(lib):
+    """On a box without a GPU a valid tcw_create must fail with TCW_ECUDA, never fall back."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    spec, ts, vel = _create_args()
+    rc, h = _create(lib, spec, 0, 32, 4, 8, 500.0, 8.0, ts, vel)
+    assert rc == tcw.TCW_ECUDA and not h.value
+    with pytest.raises((tcw.TcwError, RuntimeError, AssertionError)):
+        tcw.Handle(spec, "f32", 8, 500.0, 8.0, ts, vel)
+
+
+def test_grid_marshalling_and_sharding():
+    g = tcw.Grid([500.0, 500.125], [3500.0], [3, 5, 7], [[1, 0, 0], [0, 1, 0]], T0=12.0)
+    c = g._c()
+    assert (c.n_f0, c.n_tau, c.n_brk, c.n_sky, c.T0) == (2, 1, 3, 2, 12.0)
+    assert c.brk[2] == 7.0 and c.sky[4] == 1.0
+    assert g.n_groups == 6 and g.n_templates == 12
+    for n_sky, world in [(256, 8), (7, 3), (2, 4), (4096, 5)]:
+        parts = [tcw.shard_groups(n_sky, r, world) for r in range(world)]
+        covered = np.concatenate([np.arange(n_sky)[p] for p in parts])
+        assert np.array_equal(covered, np.arange(n_sky))
+        sizes = [p.stop - p.start for p in parts]
+        assert max(sizes) - min(sizes) <= 1
