@@ -1,0 +1,381 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the tCW track-sum hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (Doppler table, spin-down table, gather-accumulate,
+candidate reduction: SURVEY.md section 8(a) rows a1-a6) over the whole template grid of the
+workload.  The default workload is cfg2 = BASELINE.json:configs[1] (one day of 8-s SFTs,
+500-1000 Hz, float32 normalised power, 4000 f0 x 32 tau x 5 n x 1 sky = 640 000 templates).
+
+Printed: ONE JSON line.  `value` = nominal template-SFT lookups/s (n_templates * n_sft per
+step, all ranks) with inputs resident in HBM; `e2e` = the same through tcw_create(HOST
+spectrogram) + tcw_search_host(HOST outputs) + tcw_destroy, copies inside the timed region;
+`roofline` = compulsory bytes B_comp of DESIGN.md section 6 over the gather-accumulate kernel's
+device time; `cpu_baseline` = oracle/ timed on this box's host cores on a bounded sample.
+
+N > 1 (torchrun): weak scaling.  Rank r searches the same grid at its own sky point, the
+spectrogram is replicated, and there is no data-path collective.
+
+`--impl reference` times the oracle (oracle/, the paper's definition on the host cores); for
+this paper there is no reference code to install.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "template-SFT lookups/s"
+UNIT = "lookups/s"
+C_LIGHT = 299792458.0
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the gather-accumulate kernel,
+# from the committed `ncu --set full` capture named beside each entry (None = not captured).
+NCU_TRAFFIC_BYTES = {
+    # "cfg2": (bytes, "profiles/r1_cfg2_sum_staged_full.md"),
+}
+
+
+# ----------------------------------------------------------------------------- helpers
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def compulsory_bytes(w, sky=None):
+    """B_comp of SURVEY.md section 8(d) / DESIGN.md section 6: for every (sky, tau, n) group and
+    SFT, the bins between the tracks of the group's first and last f0, clipped to the band, times
+    the bytes per bin; plus 4 B per template (out_stat) and 8 B per group (out_best).  This is a
+    byte model for the roofline, evaluated with numpy; it is not part of the search."""
+    sky = w.sky if sky is None else sky
+    bpb = {"f32": 4.0, "u8": 1.0, "bits": 0.125}[w.fmt]
+    k_min = int(round(w.f_min * w.T_sft))
+    t = w.timestamps
+    ok = t >= w.T0
+    total = 0.0
+    D = 1.0 + (w.velocities @ np.asarray(sky).T) / C_LIGHT           # [n_sft][n_sky]
+    for tau in w.tau:
+        base = np.where(ok, (t - w.T0) / tau + 1.0, 1.0)
+        for n in w.brk:
+            g = np.power(base, 1.0 / (1.0 - n))[:, None] * D * w.T_sft   # [n_sft][n_sky]
+            k_lo = np.rint(w.f0[0] * g) - k_min
+            k_hi = np.rint(w.f0[-1] * g) - k_min
+            lo = np.maximum(k_lo, 0)
+            hi = np.minimum(k_hi, w.n_bins - 1)
+            bins = np.where(ok[:, None], np.maximum(hi - lo + 1, 0), 0)
+            total += float(bins.sum()) * bpb
+    n_groups = len(sky) * len(w.tau) * len(w.brk)
+    return total + 4.0 * n_groups * len(w.f0) + 8.0 * n_groups
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(w, budget_s: float, max_groups: int | None = None):
+    """The oracle as it stands (oracle/tcw_oracle.c, OpenMP over templates) timed on ONE call over a
+    seeded random sample of whole (sky, tau, n) groups of `w`.  A first call on a few groups sizes
+    the sample so that the timed call takes about `budget_s` (never more than the whole grid)."""
+    import oracle
+    oracle.build()
+    rng = np.random.default_rng(7)
+    order = rng.permutation(w.n_groups)
+    n1 = min(4, w.n_groups)
+    t0 = time.perf_counter()
+    oracle.evaluate(w, sel=oracle.group_templates(w, order[:n1]))      # also loads the library
+    t1 = time.perf_counter() - t0
+    n = int(max(1, min(w.n_groups, budget_s / (t1 / n1))))
+    if max_groups is not None:
+        n = min(n, max_groups)
+    sel = oracle.group_templates(w, np.sort(order[:n]))
+    t0 = time.perf_counter()
+    oracle.evaluate(w, sel=sel)
+    t_used = time.perf_counter() - t0
+    lookups = n * len(w.f0) * w.n_sft
+    return dict(value=lookups / t_used, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"{n} of {w.n_groups} whole (sky,tau,n) groups of {w.name} in one call "
+                       f"({n * len(w.f0)} templates x {w.n_sft} SFTs = {lookups:.3e} nominal lookups) in {t_used:.1f} s",
+                seconds=t_used, templates=n * len(w.f0))
+
+
+def workload_config(w, extra=None):
+    cfg = {"workload": f"{w.name} (BASELINE.json:configs[{int(w.name[3:]) - 1}])", "format": w.fmt,
+           "n_sft": int(w.n_sft), "n_bins": int(w.n_bins), "n_f0": len(w.f0), "n_tau": len(w.tau),
+           "n_brk": len(w.brk), "n_sky": len(w.sky), "n_templates": int(w.n_templates),
+           "spectrogram_bytes": int(w.spectrogram.nbytes)}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import tcw_inputs
+    w = tcw_inputs.make_workload(args.config)
+    per_step = max(1.0, min(20.0, 60.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        time_oracle(w, per_step, max_groups=1)
+    tot_lookups, tot_s, cores, samples = 0.0, 0.0, 0, []
+    for _ in range(args.steps):
+        r = time_oracle(w, per_step)
+        tot_lookups += r["value"] * r["seconds"]
+        tot_s += r["seconds"]
+        cores = r["cores"]
+        samples.append(r["sample"])
+    value = tot_lookups / tot_s
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(w, {"note": "each step is a bounded sample of the workload on the host cores"}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": samples[-1]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2507_07816_b200 as tcw
+    import tcw_inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the tCW path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    tcw.load_library()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = tcw_inputs.make_workload(args.config, fmt=args.format)
+    if world > 1:
+        # weak scaling: the same (f0, tau, n) grid at this rank's own sky points, spectrogram replicated
+        n_sky = len(w.sky)
+        if n_sky == 1:
+            cap = tcw_inputs.fibonacci_cap(world, 1.0, 0.3, 10.0)
+            w = w.subgrid()
+            w.sky = np.ascontiguousarray(cap[rank:rank + 1])
+        # (multi-sky configs keep their own sky list on every rank: per-GPU work is fixed)
+    grid = tcw.Grid.of(w)
+    n_sft, n_templates, n_groups = w.n_sft, grid.n_templates, grid.n_groups
+    nominal = float(n_templates) * n_sft
+    stream = torch.cuda.current_stream()
+
+    h = tcw.Handle.from_workload(w, device=dev)
+    if args.kernel:
+        h.set_option(tcw.TCW_OPT_KERNEL, {"auto": 0, "gather": 1, "staged": 2}[args.kernel])
+    if args.f0_per_lane:
+        h.set_option(tcw.TCW_OPT_F0_PER_LANE, args.f0_per_lane)
+    out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
+    out_best = torch.empty((n_groups, 2), dtype=torch.int32, device=dev)
+
+    sampler = ClockSampler(local)
+    for _ in range(args.warmup):
+        h.search(grid, out_stat, out_best)
+    h.set_option(tcw.TCW_OPT_TIMING, 1)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    t_host0 = time.perf_counter()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        h.search(grid, out_stat, out_best)
+    ev1.record(stream)
+    barrier()
+    t_host = time.perf_counter() - t_host0
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = ev0.elapsed_time(ev1)
+    stage_ms, n_timed = h.timing()
+    h.set_option(tcw.TCW_OPT_TIMING, 0)
+    info = h.info()
+    if info["status"] != 0:
+        raise SystemExit(f"bench.py: device status word {info['status']} (window bound violated)")
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * nominal / (ms_step * 1e-3)
+
+    # in-band lookups: the same search over an all-ones uint8 spectrogram counts them exactly
+    ones = torch.ones((n_sft, w.n_bins), dtype=torch.uint8, device=dev)
+    with tcw.Handle(ones, "u8", w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities) as h1:
+        cnt, _ = h1.search(grid, want_best=False)
+        torch.cuda.synchronize()
+        inband = float(cnt.sum(dtype=torch.int64).item())
+    del ones, cnt
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    spec_np = np.ascontiguousarray(w.spectrogram)
+    if spec_np.dtype == np.uint32:
+        spec_np = spec_np.view(np.int32)
+    spec_pin = torch.from_numpy(spec_np).pin_memory()
+    stat_pin = torch.empty(out_stat.shape, dtype=h.stat_dtype).pin_memory()
+    best_pin = torch.empty((n_groups, 2), dtype=torch.int32).pin_memory()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+
+    def e2e_step():
+        with tcw.Handle(spec_pin, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities) as hh:
+            hh.search_host(grid, stat_pin.numpy(), best_pin.numpy())
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()                      # tcw_search_host synchronises the stream before returning
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = int(spec_np.nbytes + w.timestamps.nbytes + w.velocities.nbytes
+              + 8 * (len(w.f0) + len(w.tau) + len(w.brk) + 3 * len(w.sky)))
+    d2h = int(4 * n_templates + 8 * n_groups)
+    e2e_value = world * nominal * e2e_steps / e2e_s
+    h.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = load_peaks()
+    b_comp = compulsory_bytes(w)
+    sum_ms = stage_ms[1]
+    achieved = b_comp / (sum_ms * 1e-3) / 1e9
+    traffic = NCU_TRAFFIC_BYTES.get(args.config if args.format is None else f"{args.config}:{args.format}")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {"f32": "f64 index + f32 accumulate", "u8": "f64 index + i32 accumulate",
+                  "bits": "f64 index + i32 accumulate"}[w.fmt],
+        "data": "synthetic",
+        "config": workload_config(w, {
+            "parallelism": f"dp{world} (templates sharded by sky point, spectrogram replicated, no collective)",
+            "l2_policy": "inputs larger than L2 (no flush)" if w.spectrogram.nbytes > 126e6 else
+                         "input smaller than L2 (stays L2-resident between steps; no flush)",
+            "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"]}),
+        "templates_per_s": world * n_templates / (ms_step * 1e-3),
+        "inband_lookups_per_s": world * inband / (ms_step * 1e-3),
+        "inband_fraction": inband / nominal,
+        "stage_ms": {"tables": stage_ms[0], "sum": stage_ms[1], "best": stage_ms[2], "search": stage_ms[3],
+                     "searches_averaged": n_timed, "host_wall_ms_per_step": 1e3 * t_host / args.steps},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic[0] if traffic else None, "peak_source": peak_src,
+                     "kernel": f"sum_{info['kernel']}_kernel", "algorithmic_bytes_per_launch": b_comp,
+                     "kernel_ms": sum_ms,
+                     "bytes_per_inband_lookup": b_comp / inband if inband else None},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
+                "path": "tcw_create(pinned HOST spectrogram) + tcw_search_host(pinned HOST out_stat, out_best) + tcw_destroy"},
+        "gpu_launches": info["launches"] * args.steps,
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cb = time_oracle(w, args.cpu_seconds)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"]["templates_per_s"] = cb["templates"] / cb["seconds"]
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--format", default=None, choices=["f32", "u8", "bits"])
+    ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged"])
+    ap.add_argument("--f0-per-lane", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

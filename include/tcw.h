@@ -153,10 +153,14 @@ enum {
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 
-/* tcw_get_timing -- device time of the stages of the last tcw_search, in milliseconds:
+/* tcw_get_timing -- device time of the stages of tcw_search, in milliseconds, AVERAGED over the
+ * searches enqueued on this handle since TCW_OPT_TIMING was set or tcw_get_timing was last
+ * called (at most 4096 are kept; later ones are not recorded):
  *  ms[0] Doppler + spin-down tables, ms[1] gather-accumulate kernel, ms[2] candidate reduction,
- *  ms[3] whole call.  Needs TCW_OPT_TIMING = 1; synchronises the search's stream. */
-int tcw_get_timing(tcw_handle *h, float ms[4]);
+ *  ms[3] whole call.  *n_searches (may be NULL) receives how many searches were averaged.
+ * The events are recorded on the search's own stream without synchronising it; this call
+ * waits for the last of them. */
+int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
 
 /* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,

@@ -79,7 +79,7 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_set_option.restype = ci
     L.tcw_set_option.argtypes = [vp, ci, cl]
     L.tcw_get_timing.restype = ci
-    L.tcw_get_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.tcw_get_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ci)]
     L.tcw_get_info.restype = ci
     L.tcw_get_info.argtypes = [vp, ctypes.POINTER(cl)]
     _lib = L
@@ -250,10 +250,12 @@ class Handle:
         _check(load_library().tcw_set_option(self._h, int(key), int(value)))
 
     def timing(self):
-        """Device milliseconds of the last search: (tables, sum kernel, best kernel, whole call)."""
+        """Average device milliseconds per search since timing was enabled or last read:
+        ((tables, sum kernel, best kernel, whole call), searches averaged)."""
         ms = (ctypes.c_float * 4)()
-        _check(load_library().tcw_get_timing(self._h, ms))
-        return tuple(float(x) for x in ms)
+        n = ctypes.c_int(0)
+        _check(load_library().tcw_get_timing(self._h, ms, ctypes.byref(n)))
+        return tuple(float(x) for x in ms), int(n.value)
 
     def info(self) -> dict:
         v = (ctypes.c_long * 6)()

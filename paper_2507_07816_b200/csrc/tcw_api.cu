@@ -42,6 +42,7 @@ int fail(int code, const char *fmt, ...)
 
 constexpr double C_LIGHT = 299792458.0;
 constexpr size_t SMEM_MAX = 227 * 1024;
+constexpr size_t TIMING_MAX = 4096;  // timed searches kept between two tcw_get_timing calls
 
 template <typename T> struct DevBuf {
     T *p = nullptr;
@@ -101,8 +102,8 @@ struct tcw_handle {
     cudaEvent_t ev_stage = nullptr;
     // options
     int opt_kernel = 0, opt_timing = 0, opt_r = 0;
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    bool timing_valid = false;
+    std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
+    size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
     long info[6] = {0, 0, 0, 0, 0, 0};
     // last tables
@@ -363,7 +364,6 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     CREATE_TRY(cudaMalloc((void **)&h->d_vel, sizeof(double) * 3 * (size_t)n_sft));
     CREATE_TRY(cudaMalloc((void **)&h->d_status, sizeof(int)));
     CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
-    for (auto &e : h->ev) CREATE_TRY(cudaEventCreate(&e));
     CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     if ((size_t)h->pitch != row_bytes(format, n_bins))
         CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));
@@ -412,6 +412,7 @@ int tcw_set_option(tcw_handle *h, int key, long value)
     case TCW_OPT_TIMING:
         if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_TIMING must be 0 or 1");
         h->opt_timing = (int)value;
+        h->timing_n = 0;
         return TCW_OK;
     case TCW_OPT_F0_PER_LANE:
         if (value != 0 && value != 4 && value != 8) return fail(TCW_EINVAL, "TCW_OPT_F0_PER_LANE must be 0, 4 or 8");
@@ -465,18 +466,26 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     p.partial = h->d_partial.p;
     p.out_stat = out_stat;
 
-    const bool tm = h->opt_timing != 0;
-    h->timing_valid = false;
-    if (tm) CUDA_TRY(cudaEventRecord(h->ev[0], st));
+    const bool tm = h->opt_timing != 0 && h->timing_n < TIMING_MAX;
+    cudaEvent_t *ev = nullptr;
+    if (tm) {
+        while (h->ev.size() < 4 * (h->timing_n + 1)) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreate(&e));
+            h->ev.push_back(e);
+        }
+        ev = h->ev.data() + 4 * h->timing_n;
+        CUDA_TRY(cudaEventRecord(ev[0], st));
+    }
     if ((rc = prepare(h, grid, 0, nullptr, st)) != TCW_OK) return rc;
     p.f0 = h->a_f0;
     p.gtab = h->d_g.p;
     p.dtab = h->d_d.p;
-    if (tm) CUDA_TRY(cudaEventRecord(h->ev[1], st));
+    if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
     if (kernel == 2) rc = launch_staged(h->format, r, h->t_pow2, p, n_ctas, smem, st);
     else rc = launch_gather(h->format, h->t_pow2, p, n_ctas, st);
     if (rc != TCW_OK) return rc;
-    if (tm) CUDA_TRY(cudaEventRecord(h->ev[2], st));
+    if (tm) CUDA_TRY(cudaEventRecord(ev[2], st));
     void *best_dst = out_best ? out_best : (void *)h->d_best.p;
     if (h->format == TCW_F32_POWER)
         tcw::best_kernel<float><<<(unsigned)((n_groups + 127) / 128), 128, 0, st>>>(
@@ -486,8 +495,8 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             (const tcw::Best<int> *)h->d_partial.p, n_groups, p.n_tiles, (tcw::Best<int> *)best_dst);
     CUDA_TRY(cudaGetLastError());
     if (tm) {
-        CUDA_TRY(cudaEventRecord(h->ev[3], st));
-        h->timing_valid = true;
+        CUDA_TRY(cudaEventRecord(ev[3], st));
+        h->timing_n++;
     }
     h->info[0] = kernel;
     h->info[1] = p.tile;
@@ -555,15 +564,25 @@ int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream)
     return TCW_OK;
 }
 
-int tcw_get_timing(tcw_handle *h, float ms[4])
+int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches)
 {
     if (!h || !ms) return fail(TCW_EINVAL, "NULL argument");
-    if (!h->timing_valid) return fail(TCW_EINVAL, "no timed search: set TCW_OPT_TIMING = 1 before tcw_search");
-    CUDA_TRY(cudaEventSynchronize(h->ev[3]));
-    CUDA_TRY(cudaEventElapsedTime(&ms[0], h->ev[0], h->ev[1]));
-    CUDA_TRY(cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]));
-    CUDA_TRY(cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]));
-    CUDA_TRY(cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]));
+    if (!h->timing_n) return fail(TCW_EINVAL, "no timed search: set TCW_OPT_TIMING = 1 before tcw_search");
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaEventSynchronize(h->ev[4 * h->timing_n - 1]));
+    double acc[4] = {0, 0, 0, 0};
+    for (size_t q = 0; q < h->timing_n; ++q) {
+        const cudaEvent_t *e = h->ev.data() + 4 * q;
+        float t[4];
+        CUDA_TRY(cudaEventElapsedTime(&t[0], e[0], e[1]));
+        CUDA_TRY(cudaEventElapsedTime(&t[1], e[1], e[2]));
+        CUDA_TRY(cudaEventElapsedTime(&t[2], e[2], e[3]));
+        CUDA_TRY(cudaEventElapsedTime(&t[3], e[0], e[3]));
+        for (int c = 0; c < 4; ++c) acc[c] += t[c];
+    }
+    for (int c = 0; c < 4; ++c) ms[c] = (float)(acc[c] / (double)h->timing_n);
+    if (n_searches) *n_searches = (int)h->timing_n;
+    h->timing_n = 0;
     return TCW_OK;
 }
 

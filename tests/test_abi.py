@@ -105,7 +105,7 @@ def test_null_handle_calls(lib):
     assert lib.tcw_search(None, None, None, None, None) == tcw.TCW_EINVAL
     assert lib.tcw_search_host(None, None, None, None, None) == tcw.TCW_EINVAL
     assert lib.tcw_set_option(None, 0, 0) == tcw.TCW_EINVAL
-    assert lib.tcw_get_timing(None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_get_timing(None, None, None) == tcw.TCW_EINVAL
     assert lib.tcw_get_info(None, None) == tcw.TCW_EINVAL
     assert lib.tcw_tables(None, None, None, None) == tcw.TCW_EINVAL
     assert lib.tcw_track_indices(None, None, 0, None, None, None) == tcw.TCW_EINVAL
