@@ -58,8 +58,9 @@ enum {
  *  out             receives the handle.
  *  spectrogram     SFT-major rows, row j at byte offset j*row_pitch_bytes.  DEVICE pointer, or
  *                  HOST pointer (pageable or pinned): the library copies it with
- *                  cudaMemcpyDefault into its own 16-byte-aligned, zero-padded pitch, so the
- *                  caller may free or overwrite it as soon as tcw_create returns.
+ *                  cudaMemcpyDefault into its own layout (16-byte-aligned rows with zero bins on
+ *                  both sides; bit-packed counts expanded to one byte per bin), so the caller
+ *                  may free or overwrite it as soon as tcw_create returns.
  *  format          one of TCW_F32_POWER / TCW_U8_COUNT / TCW_BIT_COUNT.
  *  row_pitch_bytes >= the bytes of one row (4*n_bins, n_bins, 4*ceil(n_bins/32)).
  *  n_sft, n_bins   > 0.  SFTs that are missing are simply absent from the list (reading Q16).
@@ -147,9 +148,10 @@ int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
 enum {
     TCW_OPT_KERNEL = 0,     /* 0 auto (default), 1 force the global-memory gather kernel,
                                2 force the TMA-staged kernel (TCW_EUNSUPPORTED at search if the
-                               f0 spacing makes the window exceed shared memory)              */
+                               f0 spacing makes a tile's window exceed the row padding)       */
     TCW_OPT_TIMING = 1,     /* 1: record CUDA events around each stage of tcw_search           */
-    TCW_OPT_F0_PER_LANE = 2 /* staged kernel: templates per lane, 4 or 8 (tile = 32x that); 0 auto */
+    TCW_OPT_F0_PER_LANE = 2,/* staged kernel: templates per lane, 4, 8 or 16 (tile = 32x that); 0 auto */
+    TCW_OPT_STAGES = 3      /* staged kernel: upper limit of the per-warp ring depth, 2..16; 0 auto  */
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 
@@ -165,8 +167,9 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
 /* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
- * info[5] kernels launched by the call.  Synchronises the search's stream. */
-int tcw_get_info(tcw_handle *h, long info[6]);
+ * info[5] kernels launched by the call, info[6] ring depth per warp, info[7] reserved.
+ * Synchronises the search's stream. */
+int tcw_get_info(tcw_handle *h, long info[8]);
 
 #ifdef __cplusplus
 }

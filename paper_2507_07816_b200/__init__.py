@@ -22,7 +22,7 @@ __all__ = [
 
 TCW_OK, TCW_EINVAL, TCW_ENOMEM, TCW_ECUDA, TCW_EUNSUPPORTED = 0, -1, -2, -3, -4
 TCW_F32_POWER, TCW_U8_COUNT, TCW_BIT_COUNT = 0, 1, 2
-TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE = 0, 1, 2
+TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE, TCW_OPT_STAGES = 0, 1, 2, 3
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
@@ -258,10 +258,10 @@ class Handle:
         return tuple(float(x) for x in ms), int(n.value)
 
     def info(self) -> dict:
-        v = (ctypes.c_long * 6)()
+        v = (ctypes.c_long * 8)()
         _check(load_library().tcw_get_info(self._h, v))
         return dict(kernel={1: "gather", 2: "staged"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
-                    smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]))
+                    smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -1,7 +1,8 @@
 // tcw_api.cu -- host runtime and C ABI of libtcw.so (declared in include/tcw.h).
 //
 // The host side validates arguments, owns the device copies (spectrogram re-laid to a 16-byte
-// aligned zero-padded pitch, timestamps, velocities), the grow-only scratch (tables, grid axes,
+// aligned pitch with PAD_BINS zero bins on both sides of every row, bit-packed counts expanded
+// to one byte per bin; timestamps; velocities), the grow-only scratch (tables, grid axes,
 // per-tile candidates) and the launch plan.  Every step of the path runs in the kernels of
 // tcw_tables.cuh and tcw_sum.cuh; there is no CPU fallback.
 #include "../../include/tcw.h"
@@ -85,7 +86,9 @@ bool is_pow2(double x)
 struct tcw_handle {
     int device = 0;
     int format = 0, n_sft = 0, n_bins = 0, k_min = 0;
-    long pitch = 0;
+    int fmt_dev = 0;   // device format of the library's copy: tcw::FMT_F32 or tcw::FMT_U8
+    long pitch = 0;    // its row pitch in bytes, padding included
+    long pad_bytes = 0;
     double f_min = 0, T = 0;
     bool t_pow2 = false;
     double vmax = 0;  // max |v_j|
@@ -101,11 +104,11 @@ struct tcw_handle {
     size_t h_stage_cap = 0;     // bytes
     cudaEvent_t ev_stage = nullptr;
     // options
-    int opt_kernel = 0, opt_timing = 0, opt_r = 0;
+    int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0;
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
-    long info[6] = {0, 0, 0, 0, 0, 0};
+    long info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     // last tables
     int tab_tau = 0, tab_brk = 0, tab_sky = 0;
     // device axis pointers of the last prepared grid
@@ -208,7 +211,7 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
 {
     tcw::SumParams p;
     std::memset(&p, 0, sizeof p);
-    p.spec = h->d_spec;
+    p.spec = h->d_spec + h->pad_bytes;
     p.pitch = h->pitch;
     p.n_sft = h->n_sft;
     p.n_bins = h->n_bins;
@@ -240,9 +243,10 @@ long max_window_bins(const tcw_grid *g, int tile, double dmaxT)
     return w > 1e9 ? (long)1e9 : (long)w;
 }
 
-int slab_pitch(int format, long w_bins)
+// Bytes of one ring slot: the window's bins plus the 16-byte alignment slack at both ends.
+int slot_bytes_for(int fmt_dev, long w_bins)
 {
-    long b = format == TCW_F32_POWER ? 4 * w_bins + 32 : (format == TCW_U8_COUNT ? w_bins + 32 : (w_bins + 7) / 8 + 48);
+    long b = (fmt_dev == tcw::FMT_F32 ? 4 * w_bins : w_bins) + 32;
     b = (b + 15) & ~15L;
     return b > (1L << 30) ? (1 << 30) : (int)b;
 }
@@ -260,22 +264,20 @@ int launch_staged_t(const tcw::SumParams &p, long n_ctas, size_t smem, cudaStrea
 template <int FMT, bool P2>
 int launch_staged_r(int r, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    return r == 8 ? launch_staged_t<FMT, 8, P2>(p, n_ctas, smem, st) : launch_staged_t<FMT, 4, P2>(p, n_ctas, smem, st);
+    switch (r) {
+    case 16: return launch_staged_t<FMT, 16, P2>(p, n_ctas, smem, st);
+    case 8: return launch_staged_t<FMT, 8, P2>(p, n_ctas, smem, st);
+    default: return launch_staged_t<FMT, 4, P2>(p, n_ctas, smem, st);
+    }
 }
 
 int launch_staged(int fmt, int r, bool p2, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    switch (fmt) {
-    case TCW_F32_POWER:
+    if (fmt == tcw::FMT_F32)
         return p2 ? launch_staged_r<tcw::FMT_F32, true>(r, p, n_ctas, smem, st)
                   : launch_staged_r<tcw::FMT_F32, false>(r, p, n_ctas, smem, st);
-    case TCW_U8_COUNT:
-        return p2 ? launch_staged_r<tcw::FMT_U8, true>(r, p, n_ctas, smem, st)
-                  : launch_staged_r<tcw::FMT_U8, false>(r, p, n_ctas, smem, st);
-    default:
-        return p2 ? launch_staged_r<tcw::FMT_BITS, true>(r, p, n_ctas, smem, st)
-                  : launch_staged_r<tcw::FMT_BITS, false>(r, p, n_ctas, smem, st);
-    }
+    return p2 ? launch_staged_r<tcw::FMT_U8, true>(r, p, n_ctas, smem, st)
+              : launch_staged_r<tcw::FMT_U8, false>(r, p, n_ctas, smem, st);
 }
 
 template <int FMT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
@@ -288,11 +290,8 @@ template <int FMT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_
 
 int launch_gather(int fmt, bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
 {
-    switch (fmt) {
-    case TCW_F32_POWER: return launch_gather_t<tcw::FMT_F32>(p2, p, n_ctas, st);
-    case TCW_U8_COUNT: return launch_gather_t<tcw::FMT_U8>(p2, p, n_ctas, st);
-    default: return launch_gather_t<tcw::FMT_BITS>(p2, p, n_ctas, st);
-    }
+    return fmt == tcw::FMT_F32 ? launch_gather_t<tcw::FMT_F32>(p2, p, n_ctas, st)
+                               : launch_gather_t<tcw::FMT_U8>(p2, p, n_ctas, st);
 }
 
 }  // namespace
@@ -345,8 +344,13 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     h->k_min = (int)km;
     h->vmax = vmax;
     h->ts.assign(timestamps, timestamps + n_sft);
-    h->pitch = (long)((row_bytes(format, n_bins) + 15) & ~(size_t)15);
+    h->fmt_dev = format == TCW_F32_POWER ? tcw::FMT_F32 : tcw::FMT_U8;
+    const size_t bpb = h->fmt_dev == tcw::FMT_F32 ? 4 : 1;
+    const size_t dev_row = bpb * (size_t)n_bins;           // bytes of one row in the device format
+    h->pad_bytes = (long)(bpb * tcw::PAD_BINS);            // multiple of 16
+    h->pitch = (long)(2 * (size_t)h->pad_bytes + ((dev_row + 15) & ~(size_t)15));
     cudaStream_t st = (cudaStream_t)stream;
+    void *d_words = nullptr;
 
 #define CREATE_TRY(call)                                                                       \
     do {                                                                                       \
@@ -354,6 +358,7 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
         if (e_ != cudaSuccess) {                                                               \
             int rc_ = fail(e_ == cudaErrorMemoryAllocation ? TCW_ENOMEM : TCW_ECUDA, "%s: %s", #call, \
                            cudaGetErrorString(e_));                                            \
+            if (d_words) cudaFree(d_words);                                                    \
             tcw_destroy(h);                                                                    \
             return rc_;                                                                        \
         }                                                                                      \
@@ -365,15 +370,28 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     CREATE_TRY(cudaMalloc((void **)&h->d_status, sizeof(int)));
     CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
     CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
-    if ((size_t)h->pitch != row_bytes(format, n_bins))
-        CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));
-    CREATE_TRY(cudaMemcpy2DAsync(h->d_spec, (size_t)h->pitch, spectrogram, (size_t)row_pitch_bytes,
-                                 row_bytes(format, n_bins), (size_t)n_sft, cudaMemcpyDefault, st));
+    CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));   // the padding must read as zero
+    if (format == TCW_BIT_COUNT) {
+        // bit-packed input: stage the words on the device, then expand to one byte per bin
+        const size_t wrow = row_bytes(format, n_bins);
+        CREATE_TRY(cudaMalloc((void **)&d_words, wrow * n_sft));
+        CREATE_TRY(cudaMemcpy2DAsync(d_words, wrow, spectrogram, (size_t)row_pitch_bytes, wrow, (size_t)n_sft,
+                                     cudaMemcpyDefault, st));
+        const long total = (long)n_sft * n_bins;
+        const unsigned blocks = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
+        tcw::expand_bits_kernel<<<blocks, 256, 0, st>>>((const uint32_t *)d_words, (long)(wrow / 4), n_sft, n_bins,
+                                                        h->d_spec + h->pad_bytes, h->pitch);
+        CREATE_TRY(cudaGetLastError());
+    } else {
+        CREATE_TRY(cudaMemcpy2DAsync(h->d_spec + h->pad_bytes, (size_t)h->pitch, spectrogram, (size_t)row_pitch_bytes,
+                                     dev_row, (size_t)n_sft, cudaMemcpyDefault, st));
+    }
     CREATE_TRY(cudaMemcpyAsync(h->d_ts, timestamps, sizeof(double) * n_sft, cudaMemcpyHostToDevice, st));
     CREATE_TRY(cudaMemcpyAsync(h->d_vel, velocities, sizeof(double) * 3 * (size_t)n_sft, cudaMemcpyHostToDevice, st));
     CREATE_TRY(cudaEventRecord(h->ev_stage, st));
     CREATE_TRY(cudaStreamSynchronize(st));
 #undef CREATE_TRY
+    if (d_words) cudaFree(d_words);
     *out = h;
     return TCW_OK;
 }
@@ -415,8 +433,13 @@ int tcw_set_option(tcw_handle *h, int key, long value)
         h->timing_n = 0;
         return TCW_OK;
     case TCW_OPT_F0_PER_LANE:
-        if (value != 0 && value != 4 && value != 8) return fail(TCW_EINVAL, "TCW_OPT_F0_PER_LANE must be 0, 4 or 8");
+        if (value != 0 && value != 4 && value != 8 && value != 16)
+            return fail(TCW_EINVAL, "TCW_OPT_F0_PER_LANE must be 0, 4, 8 or 16");
         h->opt_r = (int)value;
+        return TCW_OK;
+    case TCW_OPT_STAGES:
+        if (value != 0 && (value < 2 || value > 16)) return fail(TCW_EINVAL, "TCW_OPT_STAGES must be 0 or 2..16");
+        h->opt_stages = (int)value;
         return TCW_OK;
     default: return fail(TCW_EINVAL, "unknown option %d", key);
     }
@@ -432,31 +455,33 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
 
     tcw::SumParams p = base_params(h, grid);
-    // ---- launch plan: staged kernel with the largest tile whose window fits shared memory
-    int kernel = 0, r = 0, stages = 0, pitch_s = 0;
+    // ---- launch plan: staged kernel with the largest tile whose window fits the row padding and
+    // whose ring (as deep as possible, up to opt_stages) still lets two CTAs share an SM
+    int kernel = 0, r = 0, stages = 0, slot = 0;
     size_t smem = 0;
     if (h->opt_kernel != 1) {
-        const int cand[2] = {h->opt_r ? h->opt_r : 8, 4};
-        for (int c = 0; c < (h->opt_r ? 1 : 2) && !kernel; ++c) {
-            int ps = slab_pitch(h->format, max_window_bins(grid, 32 * cand[c], p.dmaxT));
-            size_t need_red = (size_t)tcw::NCW * 32 * cand[c] * 4;
-            for (int s = 4; s >= 2; --s) {
-                size_t b = tcw::staged_smem_bytes(s, ps);
+        const int all[3] = {16, 8, 4};
+        for (int c = 0; c < 3 && !kernel; ++c) {
+            if (h->opt_r && all[c] != h->opt_r) continue;
+            const long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
+            if (w_bins > tcw::PAD_BINS) continue;
+            const int sb = slot_bytes_for(h->fmt_dev, w_bins);
+            for (int s = h->opt_stages ? h->opt_stages : 8; s >= 2; --s) {
+                const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c]);
                 if (b <= SMEM_MAX / 2 - 1024 || (s == 2 && b <= SMEM_MAX)) {
-                    if ((size_t)s * tcw::ROWS * ps < need_red) continue;
-                    kernel = 2; r = cand[c]; stages = s; pitch_s = ps; smem = b;
+                    kernel = 2; r = all[c]; stages = s; slot = sb; smem = b;
                     break;
                 }
             }
         }
         if (!kernel && h->opt_kernel == 2)
-            return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the staged kernel (window exceeds shared memory)");
+            return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the staged kernel (window exceeds the row padding)");
     }
     if (!kernel) kernel = 1;
     p.tile = kernel == 2 ? 32 * r : 128;
     p.n_tiles = (grid->n_f0 + p.tile - 1) / p.tile;
     p.stages = stages;
-    p.pitch_s = pitch_s;
+    p.slot_bytes = slot;
     const long n_ctas = n_groups * p.n_tiles;
     if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "grid needs more than 2^31-1 CTAs; split the search");
 
@@ -482,8 +507,8 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     p.gtab = h->d_g.p;
     p.dtab = h->d_d.p;
     if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
-    if (kernel == 2) rc = launch_staged(h->format, r, h->t_pow2, p, n_ctas, smem, st);
-    else rc = launch_gather(h->format, h->t_pow2, p, n_ctas, st);
+    if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, p, n_ctas, smem, st);
+    else rc = launch_gather(h->fmt_dev, h->t_pow2, p, n_ctas, st);
     if (rc != TCW_OK) return rc;
     if (tm) CUDA_TRY(cudaEventRecord(ev[2], st));
     void *best_dst = out_best ? out_best : (void *)h->d_best.p;
@@ -502,6 +527,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     h->info[1] = p.tile;
     h->info[2] = n_ctas;
     h->info[3] = (long)smem;
+    h->info[6] = stages;
     h->info[5] = 4;  // doppler table, spin-down table, sum, best
     return TCW_OK;
 }
@@ -586,7 +612,7 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches)
     return TCW_OK;
 }
 
-int tcw_get_info(tcw_handle *h, long info[6])
+int tcw_get_info(tcw_handle *h, long info[8])
 {
     if (!h || !info) return fail(TCW_EINVAL, "NULL argument");
     if (!h->info[0]) return fail(TCW_EINVAL, "no search has been run on this handle");

@@ -5,21 +5,31 @@
 //     x = ((f0_i * g[a][b][j]) * D[s][j]) * T_sft ,  k = rint(x) - k_min         (eq. (1)-(2))
 //     stat_i += spectrogram[j][k]  if 0 <= k < n_bins .
 // Two kernels compute it:
-//   * sum_staged_kernel -- the product path.  One CTA owns (group, tile of consecutive f0).
-//     Consecutive f0 of one group select a narrow contiguous bin window per SFT (g <= 1), so a
-//     producer warp stages the [32 SFT x window] slab into shared memory with one TMA bulk copy
-//     (cp.async.bulk, mbarrier complete_tx) per SFT row through a multi-stage ring, and eight
-//     consumer warps gather from shared memory, each lane carrying R templates.
+//   * sum_staged_kernel -- the product path.  One CTA owns (group, tile of 32*R consecutive f0).
+//     Consecutive f0 of one group select a narrow contiguous bin window per SFT (g <= 1).  Every
+//     warp owns the SFT rows j = j_begin + warp + NW*n and runs its own software pipeline: it
+//     computes the window [k(f_first, j), k(f_last, j)] of a row a few rows ahead, one lane
+//     issues ONE TMA bulk copy (cp.async.bulk, mbarrier complete_tx) of exactly that window
+//     into the warp's private shared-memory ring, and all lanes gather row n from shared memory,
+//     each lane carrying R templates in registers.  The library's spectrogram copy carries
+//     PAD_BINS zero bins on both sides of every row, so a window that is partly out of band is
+//     still copied whole and no per-lookup bounds test is needed (out-of-band bins add 0).
 //   * sum_gather_kernel -- one thread per template gathering from global memory.  It serves f0
-//     axes so sparse that the window of a 32-template tile does not fit shared memory, and it is
-//     the simple kernel the staged one is checked against.
+//     axes so sparse that the window of a 128-template tile does not fit the row padding, and it
+//     is the simple kernel the staged one is checked against.
+// Device formats: float32 power or uint8 counts (a bit-packed input is expanded to uint8 by
+// tcw_create: with the index arithmetic fixed at 3 FP64 operations per lookup the count paths are
+// bound by instruction issue, and a byte load + add is cheaper than word load + shift + mask).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace tcw {
 
-enum { FMT_F32 = 0, FMT_U8 = 1, FMT_BITS = 2 };
+enum { FMT_F32 = 0, FMT_U8 = 1 };
+
+// zero bins on each side of every spectrogram row in the library's copy
+constexpr int PAD_BINS = 1056;
 
 // 1.5 * 2^52: adding it rounds x to the nearest integer (ties to even) in the low mantissa bits,
 // so the low word of the sum is rint(x) for |x| < 2^31.
@@ -36,8 +46,8 @@ __device__ __forceinline__ int bin_lo(double f0, double g, double Dp, double T)
 }
 
 struct SumParams {
-    const unsigned char *spec;  // library copy of the spectrogram, rows 16-byte aligned
-    long pitch;                 // its row pitch in bytes (multiple of 16)
+    const unsigned char *spec;  // bin 0 of row 0 of the library's copy (PAD_BINS zero bins before it)
+    long pitch;                 // row pitch in bytes (multiple of 16), padding included
     int n_sft, n_bins, k_min;
     double T;
     const double *gtab;         // [n_tau*n_brk][n_sft]
@@ -49,7 +59,7 @@ struct SumParams {
     void *out_stat;             // float32 / int32 [n_groups][n_f0] or NULL
     void *partial;              // {stat, f0_index} [n_groups][n_tiles]
     int n_tiles, tile;          // tiles per group, templates per tile
-    int stages, pitch_s;        // staged kernel: ring depth, shared-memory row pitch (bytes)
+    int stages, slot_bytes;     // staged kernel: ring depth per warp, bytes per ring slot
     int *status;                // device status word
 };
 
@@ -110,8 +120,7 @@ sum_gather_kernel(const SumParams p)
         if ((unsigned)k < (unsigned)p.n_bins) {
             const unsigned char *row = p.spec + (long)j * p.pitch;
             if (FMT == FMT_F32) acc += ((const float *)row)[k];
-            else if (FMT == FMT_U8) acc += (V)row[k];
-            else acc += (V)((((const uint32_t *)row)[k >> 5] >> (k & 31)) & 1u);
+            else acc += (V)row[k];
         }
     }
     if (valid && p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = acc;
@@ -125,10 +134,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)_
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
 {
@@ -165,192 +170,166 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
     asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ uint32_t lds_u32(uint32_t a)
-{
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
-}
 
 // --------------------------------------------------------------------------- staged kernel
-constexpr int ROWS = 32;      // SFT rows per stage (one per producer lane)
-constexpr int NCW = 8;        // consumer warps
-constexpr int STAGED_THREADS = 32 * (NCW + 1);
+constexpr int NW = 8;  // warps per CTA; warp w owns the rows j = j_begin + w + NW*n
+constexpr int STAGED_THREADS = 32 * NW;
 
-// Per staged row: what a consumer lane needs to turn rint(x) into a shared-memory address.
+// What the lanes need to turn rint(x) into a shared-memory address of a staged row.
 struct __align__(16) RowMeta {
     double g, Dp;   // spin-down factor and Doppler factor (times T_sft when it is a power of two)
-    uint32_t rb;    // f32: addr = rb + 4*lo   u8: addr = rb + lo   bits: word addr = rb + 4*((u + d0) >> 5)
-    int lo0;        // k_min + first in-band bin of the row window
-    int span;       // last - first in-band bin of the window; < 0: nothing to do in this row
-    int d0;         // bits: offset of bin lo0 from the first staged bit
+    uint32_t rb;    // f32: addr = rb + 4*rint(x)   u8: addr = rb + rint(x)
+    int live;       // 1 staged row, 0 row with no in-band bin (nothing staged), -1 no further rows
+    int pad[2];
 };
 
-// dynamic shared memory: [full[S] | empty[S] | ctrl[S] (pad to 16)] [meta S*ROWS] [slab S*ROWS*pitch_s]
-__host__ __device__ inline size_t staged_header_bytes(int stages) { return ((size_t)stages * 20 + 15) & ~(size_t)15; }
-__host__ __device__ inline size_t staged_smem_bytes(int stages, int pitch_s)
+// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*D] [slot NW*D*slot_bytes].  The slot region is
+// reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has completed; the
+// mbarrier words are never reused as data (they are updated through the async proxy, and a generic
+// store to the same bytes is not ordered against that without a proxy fence).
+__host__ __device__ inline size_t staged_header_bytes(int stages) { return (size_t)NW * stages * (8 + sizeof(RowMeta)); }
+__host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile)
 {
-    return staged_header_bytes(stages) + (size_t)stages * ROWS * (sizeof(RowMeta) + pitch_s);
-}
-
-template <int FMT> __device__ __forceinline__ int byte_of_bin(int k)
-{
-    return FMT == FMT_F32 ? 4 * k : (FMT == FMT_U8 ? k : (k >> 5) * 4);
+    size_t ring = (size_t)NW * stages * (size_t)slot_bytes;
+    size_t red = (size_t)NW * tile * 4 + 128;
+    return staged_header_bytes(stages) + (ring > red ? ring : red);
 }
 
 template <int FMT, int R, bool TPOW2>
-__global__ void __launch_bounds__(STAGED_THREADS)
+__global__ void __launch_bounds__(STAGED_THREADS, 2)
 sum_staged_kernel(const SumParams p)
 {
     typedef typename Acc<FMT>::type V;
-    constexpr int F = 32 * R;  // templates per tile
-    extern __shared__ __align__(16) unsigned char smem[];
-    const int S = p.stages;
-    uint64_t *full = (uint64_t *)smem;
-    uint64_t *empty = full + S;
-    volatile int *ctrl = (volatile int *)(empty + S);
-    RowMeta *meta = (RowMeta *)(smem + staged_header_bytes(S));
-    unsigned char *slab = (unsigned char *)(meta + S * ROWS);
-
+    constexpr int F = 32 * R;                      // templates per tile
+    constexpr int BPB = FMT == FMT_F32 ? 4 : 1;    // bytes per bin
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int D = p.stages;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint64_t *bars = (uint64_t *)smem + warp * D;
+    RowMeta *metas = (RowMeta *)(smem + (size_t)NW * D * 8) + warp * D;
+    unsigned char *slots = smem + staged_header_bytes(D);
+    const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D * p.slot_bytes);
+    const uint32_t bars_s = smem_u32(bars);
+
     // heavy tiles (high f0 stays in band longest) are launched first
     const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);
     const long grp = blockIdx.x / p.n_tiles;
     const int i0 = tile * F;
     const int i_last = min(i0 + F, p.n_f0) - 1;
 
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < S; ++s) {
-            mbar_init(smem_u32(full + s), 32);
-            mbar_init(smem_u32(empty + s), NCW);
-            ctrl[s] = 0;
-        }
+    if (lane == 0) {
+        for (int s = 0; s < D; ++s) mbar_init(bars_s + 8u * s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    __syncwarp();
 
     V acc[R];
+    double f0r[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) acc[r] = 0;
+    for (int r = 0; r < R; ++r) {
+        acc[r] = 0;
+        f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
+    }
+    const double f_first = p.f0[i0], f_last = p.f0[i_last];
+    const double below = (double)p.k_min - 1.0;
+    const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
+    const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
+    const int jw = p.j_begin + warp;
+    const int n_rows = jw < p.n_sft ? (p.n_sft - jw + NW - 1) / NW : 0;
+    const unsigned char *spec_w = p.spec + (long)jw * p.pitch;
+    const long pitch_w = (long)NW * p.pitch;
 
-    if (warp == NCW) {
-        // ---------------- producer warp: lane = SFT row of the stage
-        const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
-        const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
-        const double f_first = p.f0[i0], f_last = p.f0[i_last];
-        const double below = (double)p.k_min - 1.0;
-        int st = 0;
-        uint32_t ph = 0;
-        for (int jt = p.j_begin;; jt += ROWS) {
-            const int j = jt + lane;
-            const bool in_list = j < p.n_sft;
-            const double gj = in_list ? g[j] : 0.0;
-            const double dj = in_list ? d[j] : 1.0;
-            // g decreases with j, so once the highest template of the tile is below the band
-            // for the largest possible Doppler factor, no later SFT can contribute.
-            const bool row_dead = !in_list || (f_last * gj * p.dmaxT < below);
-            const bool tile_dead = __shfl_sync(0xffffffffu, row_dead, 0);
-            mbar_wait(smem_u32(empty + st), ph ^ 1);
-            if (tile_dead) {
-                if (lane == 0) ctrl[st] = 1;
-                __syncwarp();
-                mbar_arrive(smem_u32(full + st));
-                break;
-            }
-            RowMeta m;
-            m.g = gj;
-            m.Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
-            m.rb = 0; m.lo0 = 0; m.span = -1; m.d0 = 0;
-            uint32_t bytes = 0;
-            const unsigned char *src = nullptr;
-            const uint32_t row_s = smem_u32(slab + (size_t)(st * ROWS + lane) * p.pitch_s);
-            if (in_list) {
-                int kf = bin_lo<TPOW2>(f_first, gj, m.Dp, p.T) - p.k_min;
-                int kl = bin_lo<TPOW2>(f_last, gj, m.Dp, p.T) - p.k_min;
-                int kfc = max(kf, 0), klc = min(kl, p.n_bins - 1);
-                if (kfc <= klc) {
-                    int a_byte = byte_of_bin<FMT>(kfc) & ~15;
-                    int e_byte = (byte_of_bin<FMT>(klc) + (FMT == FMT_U8 ? 1 : 4) + 15) & ~15;
-                    if (e_byte - a_byte > p.pitch_s) {
-                        atomicOr(p.status, 1);  // host-side window bound violated: never expected
-                    } else {
-                        bytes = (uint32_t)(e_byte - a_byte);
-                        src = p.spec + (long)j * p.pitch + a_byte;
-                        m.lo0 = p.k_min + kfc;
-                        m.span = klc - kfc;
-                        if (FMT == FMT_F32) m.rb = row_s - 4u * (uint32_t)(p.k_min + a_byte / 4);
-                        else if (FMT == FMT_U8) m.rb = row_s - (uint32_t)(p.k_min + a_byte);
-                        else { m.rb = row_s; m.d0 = kfc - a_byte * 8; }
-                    }
+    // (g, D) of the next two rows to stage, loaded ahead of use
+    double ga = 0, da = 1, gb = 0, db = 1;
+    if (0 < n_rows) { ga = __ldg(g + jw); da = __ldg(d + jw); }
+    if (1 < n_rows) { gb = __ldg(g + jw + NW); db = __ldg(d + jw + NW); }
+
+    int ni = 0, si = 0;   // next row to stage and its ring slot
+    // Stage row ni into slot si (or mark it skipped / final) and advance.
+    auto stage_next = [&]() {
+        const double gj = ga, dj = da;
+        ga = gb; da = db;
+        if (ni + 2 < n_rows) { gb = __ldg(g + jw + NW * (ni + 2)); db = __ldg(d + jw + NW * (ni + 2)); }
+        RowMeta m;
+        m.g = gj;
+        m.Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
+        m.rb = 0; m.live = -1; m.pad[0] = m.pad[1] = 0;
+        uint32_t bytes = 0;
+        const unsigned char *src = nullptr;
+        const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
+        // g decreases with j, so once the highest template of the tile is below the band for the
+        // largest possible Doppler factor, no later SFT can contribute.
+        if (ni < n_rows && !(f_last * gj * p.dmaxT < below)) {
+            const int kf = bin_lo<TPOW2>(f_first, gj, m.Dp, p.T) - p.k_min;
+            const int kl = bin_lo<TPOW2>(f_last, gj, m.Dp, p.T) - p.k_min;
+            m.live = 0;
+            if (kl >= 0 && kf < p.n_bins) {
+                const int a_byte = (BPB * kf) & ~15;                 // rounds towards -inf: may reach into the left padding
+                const int e_byte = (BPB * (kl + 1) + 15) & ~15;
+                if (e_byte - a_byte > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                    atomicOr(p.status, 1);  // host-side window bound violated: never expected
+                } else {
+                    bytes = (uint32_t)(e_byte - a_byte);
+                    src = spec_w + (long)ni * pitch_w + a_byte;
+                    m.rb = slot_s - (uint32_t)(BPB * p.k_min + a_byte);
+                    m.live = 1;
                 }
             }
-            meta[st * ROWS + lane] = m;
+        }
+        if (lane == 0) {
+            metas[si] = m;
             if (bytes) {
-                mbar_arrive_expect_tx(smem_u32(full + st), bytes);
-                bulk_g2s(row_s, src, bytes, smem_u32(full + st));
-            } else {
-                mbar_arrive(smem_u32(full + st));
+                mbar_arrive_expect_tx(bars_s + 8u * si, bytes);
+                bulk_g2s(slot_s, src, bytes, bars_s + 8u * si);
             }
-            if (++st == S) { st = 0; ph ^= 1; }
         }
-    } else {
-        // ---------------- consumer warps: lane carries templates i0 + r*32 + lane
-        double f0r[R];
+        __syncwarp();
+        ++ni;
+        if (++si == D) si = 0;
+    };
+
+    for (int q = 0; q < D - 1; ++q) stage_next();
+
+    uint32_t phase = 0;   // bit s: parity of the next completion of slot s
+    int sc = 0;
+    for (;;) {
+        stage_next();     // refills the slot consumed in the previous iteration
+        const RowMeta m = metas[sc];
+        if (m.live < 0) break;
+        if (m.live > 0) {
+            mbar_wait(bars_s + 8u * sc, (phase >> sc) & 1u);
+            phase ^= 1u << sc;
 #pragma unroll
-        for (int r = 0; r < R; ++r) f0r[r] = p.f0[min(i0 + r * 32 + lane, p.n_f0 - 1)];
-        int st = 0;
-        uint32_t ph = 0;
-        for (;;) {
-            mbar_wait(smem_u32(full + st), ph);
-            if (ctrl[st]) break;
-            const RowMeta *ms = meta + st * ROWS;
-#pragma unroll 1
-            for (int rr = warp; rr < ROWS; rr += NCW) {
-                const RowMeta m = ms[rr];
-                if (m.span < 0) continue;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const int lo = bin_lo<TPOW2>(f0r[r], m.g, m.Dp, p.T);
-                    const uint32_t u = (uint32_t)(lo - m.lo0);
-                    if (u <= (uint32_t)m.span) {
-                        if (FMT == FMT_F32) acc[r] += lds_f32(m.rb + 4u * (uint32_t)lo);
-                        else if (FMT == FMT_U8) acc[r] += (V)lds_u8(m.rb + (uint32_t)lo);
-                        else {
-                            const uint32_t rel = u + (uint32_t)m.d0;
-                            acc[r] += (V)((lds_u32(m.rb + 4u * (rel >> 5)) >> (rel & 31u)) & 1u);
-                        }
-                    }
-                }
+            for (int r = 0; r < R; ++r) {
+                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], m.g, m.Dp, p.T);
+                if (FMT == FMT_F32) acc[r] += lds_f32(m.rb + 4u * lo);
+                else acc[r] += (V)lds_u8(m.rb + lo);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(empty + st));
-            if (++st == S) { st = 0; ph ^= 1; }
         }
+        __syncwarp();     // every lane has read slot sc before the next iteration refills it
+        if (++sc == D) sc = 0;
     }
 
-    // ---------------- fixed-order combine of the consumer warps' partial sums
-    __syncthreads();  // every staged copy has been consumed: the slab can be reused
-    V *red = (V *)slab;
-    if (warp < NCW) {
+    // ---------------- fixed-order combine of the warps' partial sums
+    __syncthreads();      // every staged copy has been consumed: the slot region can be reused
+    V *red = (V *)slots;
 #pragma unroll
-        for (int r = 0; r < R; ++r) red[warp * F + r * 32 + lane] = acc[r];
-    }
+    for (int r = 0; r < R; ++r) red[warp * F + r * 32 + lane] = acc[r];
     __syncthreads();
-    V tot = lowest<V>();
-    int idx = INT32_MAX;
-    if (threadIdx.x < F) {
-        const int i = i0 + threadIdx.x;
+    V best_v = lowest<V>();
+    int best_i = INT32_MAX;
+    for (int t = threadIdx.x; t < F; t += STAGED_THREADS) {
+        const int i = i0 + t;
         if (i < p.n_f0) {
-            V s = red[threadIdx.x];
+            V s = red[t];
 #pragma unroll
-            for (int w = 1; w < NCW; ++w) s += red[w * F + threadIdx.x];
+            for (int w = 1; w < NW; ++w) s += red[w * F + t];
             if (p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = s;
-            tot = s;
-            idx = i;
+            argmax_step(best_v, best_i, s, i);
         }
     }
     __syncthreads();
-    block_best<V>(tot, idx, (Best<V> *)meta, (Best<V> *)p.partial + grp * p.n_tiles + tile);
+    block_best<V>(best_v, best_i, (Best<V> *)slots, (Best<V> *)p.partial + grp * p.n_tiles + tile);
 }
 
 // --------------------------------------------------------------------------- candidate reduction
@@ -393,6 +372,20 @@ track_index_kernel(const SumParams p, const long *__restrict__ sel, long n_sel, 
     double d = p.dtab[(grp / p.n_ab) * (long)p.n_sft + j];
     double Dp = TPOW2 ? __dmul_rn(d, p.T) : d;
     out_k[q] = bin_lo<TPOW2>(p.f0[i], g, Dp, p.T) - p.k_min;
+}
+
+// --------------------------------------------------------------------------- layout
+// Bit-packed number counts (uint32 words, LSB first) -> one byte per bin, rows at `pitch`.
+__global__ void __launch_bounds__(256)
+expand_bits_kernel(const uint32_t *__restrict__ words, long words_pitch, int n_sft, int n_bins,
+                   unsigned char *__restrict__ dst, long pitch)
+{
+    const long total = (long)n_sft * n_bins;
+    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x) {
+        const int j = (int)(q / n_bins), k = (int)(q % n_bins);
+        const uint32_t w = words[j * words_pitch + (k >> 5)];
+        dst[j * pitch + k] = (unsigned char)((w >> (k & 31)) & 1u);
+    }
 }
 
 }  // namespace tcw
