@@ -135,6 +135,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -239,48 +243,60 @@ sum_staged_kernel(const SumParams p)
     const unsigned char *spec_w = p.spec + (long)jw * p.pitch;
     const long pitch_w = (long)NW * p.pitch;
 
-    // (g, D) of the next two rows to stage, loaded ahead of use
-    double ga = 0, da = 1, gb = 0, db = 1;
-    if (0 < n_rows) { ga = __ldg(g + jw); da = __ldg(d + jw); }
-    if (1 < n_rows) { gb = __ldg(g + jw + NW); db = __ldg(d + jw + NW); }
+    // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp),
+    // and kept in the lane's registers until that lane stages its row.
+    double b_g = 0, b_Dp = 0;          // spin-down and Doppler factor of the lane's row
+    const unsigned char *b_src = nullptr;
+    uint32_t b_rb = 0;                 // -(BPB*k_min + first staged byte): added to the slot address
+    int b_bytes = 0;                   // bytes to stage
+    int b_live = -1;                   // 1 staged, 0 no in-band bin, -1 no further rows
+    double gn = 0, dn = 1;             // (g, D) of the lane's row in the NEXT batch, loaded ahead of use
+    if (lane < n_rows) { gn = __ldg(g + jw + NW * lane); dn = __ldg(d + jw + NW * lane); }
 
-    int ni = 0, si = 0;   // next row to stage and its ring slot
-    // Stage row ni into slot si (or mark it skipped / final) and advance.
-    auto stage_next = [&]() {
-        const double gj = ga, dj = da;
-        ga = gb; da = db;
-        if (ni + 2 < n_rows) { gb = __ldg(g + jw + NW * (ni + 2)); db = __ldg(d + jw + NW * (ni + 2)); }
-        RowMeta m;
-        m.g = gj;
-        m.Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
-        m.rb = 0; m.live = -1; m.pad[0] = m.pad[1] = 0;
-        uint32_t bytes = 0;
-        const unsigned char *src = nullptr;
-        const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
+    auto compute_batch = [&](int m) {
+        const int n = 32 * m + lane;
+        const double gj = gn, dj = dn;
+        if (n + 32 < n_rows) { gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32)); }
+        b_g = gj;
+        b_Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
+        b_live = -1;
+        b_bytes = 0;
         // g decreases with j, so once the highest template of the tile is below the band for the
         // largest possible Doppler factor, no later SFT can contribute.
-        if (ni < n_rows && !(f_last * gj * p.dmaxT < below)) {
-            const int kf = bin_lo<TPOW2>(f_first, gj, m.Dp, p.T) - p.k_min;
-            const int kl = bin_lo<TPOW2>(f_last, gj, m.Dp, p.T) - p.k_min;
-            m.live = 0;
+        if (n < n_rows && !(f_last * gj * p.dmaxT < below)) {
+            const int kf = bin_lo<TPOW2>(f_first, gj, b_Dp, p.T) - p.k_min;
+            const int kl = bin_lo<TPOW2>(f_last, gj, b_Dp, p.T) - p.k_min;
+            b_live = 0;
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = (BPB * kf) & ~15;                 // rounds towards -inf: may reach into the left padding
                 const int e_byte = (BPB * (kl + 1) + 15) & ~15;
                 if (e_byte - a_byte > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
                     atomicOr(p.status, 1);  // host-side window bound violated: never expected
                 } else {
-                    bytes = (uint32_t)(e_byte - a_byte);
-                    src = spec_w + (long)ni * pitch_w + a_byte;
-                    m.rb = slot_s - (uint32_t)(BPB * p.k_min + a_byte);
-                    m.live = 1;
+                    b_bytes = e_byte - a_byte;
+                    b_src = spec_w + (long)n * pitch_w + a_byte;
+                    b_rb = 0u - (uint32_t)(BPB * p.k_min + a_byte);
+                    b_live = 1;
                 }
             }
         }
-        if (lane == 0) {
+    };
+
+    int ni = 0, si = 0;   // next row to stage and its ring slot
+    // Stage row ni into slot si (or mark it skipped / final) and advance.  The lane that holds the
+    // row's metadata publishes it and issues the copy.
+    auto stage_next = [&]() {
+        if ((ni & 31) == 0) compute_batch(ni >> 5);
+        if (lane == (ni & 31)) {
+            const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
+            RowMeta m;
+            m.g = b_g; m.Dp = b_Dp; m.rb = slot_s + b_rb; m.live = b_live; m.pad[0] = m.pad[1] = 0;
             metas[si] = m;
-            if (bytes) {
-                mbar_arrive_expect_tx(bars_s + 8u * si, bytes);
-                bulk_g2s(slot_s, src, bytes, bars_s + 8u * si);
+            if (b_live > 0) {
+                mbar_arrive_expect_tx(bars_s + 8u * si, (uint32_t)b_bytes);
+                bulk_g2s(slot_s, b_src, (uint32_t)b_bytes, bars_s + 8u * si);
+            } else if (b_live == 0) {
+                mbar_arrive(bars_s + 8u * si);   // every use of a slot completes one phase of its barrier
             }
         }
         __syncwarp();
@@ -290,15 +306,15 @@ sum_staged_kernel(const SumParams p)
 
     for (int q = 0; q < D - 1; ++q) stage_next();
 
-    uint32_t phase = 0;   // bit s: parity of the next completion of slot s
+    uint32_t ph = 0;      // parity of the phase the slots complete in this pass over the ring
     int sc = 0;
     for (;;) {
         stage_next();     // refills the slot consumed in the previous iteration
         const RowMeta m = metas[sc];
-        if (m.live < 0) break;
-        if (m.live > 0) {
-            mbar_wait(bars_s + 8u * sc, (phase >> sc) & 1u);
-            phase ^= 1u << sc;
+        if (m.live <= 0) {
+            if (m.live < 0) break;
+        } else {
+            mbar_wait(bars_s + 8u * sc, ph);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], m.g, m.Dp, p.T);
@@ -307,7 +323,7 @@ sum_staged_kernel(const SumParams p)
             }
         }
         __syncwarp();     // every lane has read slot sc before the next iteration refills it
-        if (++sc == D) sc = 0;
+        if (++sc == D) { sc = 0; ph ^= 1u; }
     }
 
     // ---------------- fixed-order combine of the warps' partial sums
