@@ -43,7 +43,10 @@ C_LIGHT = 299792458.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the gather-accumulate kernel,
 # from the committed `ncu --set full` capture named beside each entry (None = not captured).
 NCU_TRAFFIC_BYTES = {
-    # "cfg2": (bytes, "profiles/r1_cfg2_sum_staged_full.md"),
+    "cfg2": (3275861000 + 6621440, "profiles/r1b_cfg2_sum_staged_full.md"),
+    "cfg2:f32": (3275861000 + 6621440, "profiles/r1b_cfg2_sum_staged_full.md"),
+    "cfg4": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
+    "cfg4:f32": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
 }
 
 
@@ -237,7 +240,9 @@ def run_ours(args):
 
     h = tcw.Handle.from_workload(w, device=dev)
     if args.kernel:
-        h.set_option(tcw.TCW_OPT_KERNEL, {"auto": 0, "gather": 1, "staged": 2}[args.kernel])
+        h.set_option(tcw.TCW_OPT_KERNEL, tcw.KERNELS[args.kernel])
+    if args.sky_block:
+        h.set_option(tcw.TCW_OPT_SKY_BLOCK, args.sky_block)
     if args.f0_per_lane:
         h.set_option(tcw.TCW_OPT_F0_PER_LANE, args.f0_per_lane)
     out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
@@ -331,14 +336,16 @@ def run_ours(args):
             "parallelism": f"dp{world} (templates sharded by sky point, spectrogram replicated, no collective)",
             "l2_policy": "inputs larger than L2 (no flush)" if w.spectrogram.nbytes > 126e6 else
                          "input smaller than L2 (stays L2-resident between steps; no flush)",
-            "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"]}),
+            "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"],
+            "sky_block": info["sky_block"]}),
         "templates_per_s": world * n_templates / (ms_step * 1e-3),
         "inband_lookups_per_s": world * inband / (ms_step * 1e-3),
         "inband_fraction": inband / nominal,
         "stage_ms": {"tables": stage_ms[0], "sum": stage_ms[1], "best": stage_ms[2], "search": stage_ms[3],
                      "searches_averaged": n_timed, "host_wall_ms_per_step": 1e3 * t_host / args.steps},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic[0] if traffic else None, "peak_source": peak_src,
+                     "traffic": traffic[0] if traffic else None,
+                     "traffic_source": traffic[1] if traffic else None, "peak_source": peak_src,
                      "kernel": f"sum_{info['kernel']}_kernel", "algorithmic_bytes_per_launch": b_comp,
                      "kernel_ms": sum_ms,
                      "bytes_per_inband_lookup": b_comp / inband if inband else None},
@@ -366,7 +373,8 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--format", default=None, choices=["f32", "u8", "bits"])
-    ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged"])
+    ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged", "skyblock"])
+    ap.add_argument("--sky-block", type=int, default=0, choices=[0, 64, 128])
     ap.add_argument("--f0-per-lane", type=int, default=0)
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)

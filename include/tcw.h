@@ -148,10 +148,14 @@ int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
 enum {
     TCW_OPT_KERNEL = 0,     /* 0 auto (default), 1 force the global-memory gather kernel,
                                2 force the TMA-staged kernel (TCW_EUNSUPPORTED at search if the
-                               f0 spacing makes a tile's window exceed the row padding)       */
+                               f0 spacing makes a tile's window exceed the row padding),
+                               3 force the sky-block kernel (count formats only; exact sharing
+                               of lookups between neighbouring sky points, auto for >= 16 sky
+                               points; TCW_EUNSUPPORTED for the power format)                 */
     TCW_OPT_TIMING = 1,     /* 1: record CUDA events around each stage of tcw_search           */
     TCW_OPT_F0_PER_LANE = 2,/* staged kernel: templates per lane, 4, 8 or 16 (tile = 32x that); 0 auto */
-    TCW_OPT_STAGES = 3      /* staged kernel: upper limit of the per-warp ring depth, 2..16; 0 auto  */
+    TCW_OPT_STAGES = 3,     /* staged kernel: upper limit of the per-warp ring depth, 2..16; 0 auto  */
+    TCW_OPT_SKY_BLOCK = 4   /* sky-block kernel: sky points per block, 64 or 128; 0 auto             */
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 
@@ -164,10 +168,12 @@ int tcw_set_option(tcw_handle *h, int key, long value);
  * waits for the last of them. */
 int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
 
-/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged),
+/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged,
+ * 3 sky-block),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
- * info[5] kernels launched by the call, info[6] ring depth per warp, info[7] reserved.
+ * info[5] kernels launched by the call, info[6] ring depth per warp, info[7] sky points per
+ * block (sky-block kernel, else 0).
  * Synchronises the search's stream. */
 int tcw_get_info(tcw_handle *h, long info[8]);
 

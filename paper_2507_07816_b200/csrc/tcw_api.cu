@@ -19,6 +19,7 @@
 
 #include "tcw_sum.cuh"
 #include "tcw_tables.cuh"
+#include "tcw_skyblock.cuh"
 
 namespace {
 
@@ -92,6 +93,7 @@ struct tcw_handle {
     double f_min = 0, T = 0;
     bool t_pow2 = false;
     double vmax = 0;  // max |v_j|
+    double vmid[3] = {0, 0, 0};  // velocity at the middle SFT: sort key of the sky-block kernel
     std::vector<double> ts;
     unsigned char *d_spec = nullptr;
     double *d_ts = nullptr, *d_vel = nullptr;
@@ -99,12 +101,15 @@ struct tcw_handle {
     DevBuf<double> d_g, d_d, d_axes;
     DevBuf<unsigned char> d_partial, d_stat, d_best;
     DevBuf<long> d_sel;
+    DevBuf<double> d_dts, d_dmm;  // sky-block kernel: per-block Doppler rows and their {min, max}
+    DevBuf<int> d_slot;           // sky index of each block slot
+    std::vector<int> slot_host;
     int *d_status = nullptr;
     double *h_stage = nullptr;  // pinned staging for the grid axes / selections
     size_t h_stage_cap = 0;     // bytes
     cudaEvent_t ev_stage = nullptr;
     // options
-    int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0;
+    int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0, opt_sky = 0;
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
@@ -158,11 +163,14 @@ int ensure_stage(tcw_handle *h, size_t bytes)
 
 // Copy the grid axes (and an optional selection list) to the device through pinned staging,
 // then build both tables on `st`.
-int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaStream_t st)
+int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaStream_t st,
+            const std::vector<int> *slots = nullptr)
 {
     CUDA_TRY(cudaSetDevice(h->device));
     const size_t n_axes = (size_t)g->n_f0 + g->n_tau + g->n_brk + 3 * (size_t)g->n_sky;
-    const size_t stage_bytes = n_axes * sizeof(double) + (size_t)std::max<long>(n_sel, 0) * sizeof(long);
+    const size_t n_slots = slots ? slots->size() : 0;
+    const size_t stage_bytes = n_axes * sizeof(double) + (size_t)std::max<long>(n_sel, 0) * sizeof(long) +
+                               n_slots * sizeof(int);
     // the staging buffer may still feed the previous call's copy
     CUDA_TRY(cudaEventSynchronize(h->ev_stage));
     int rc;
@@ -171,6 +179,7 @@ int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaS
     if ((rc = h->d_g.reserve((size_t)g->n_tau * g->n_brk * h->n_sft)) != TCW_OK) return rc;
     if ((rc = h->d_d.reserve((size_t)g->n_sky * h->n_sft)) != TCW_OK) return rc;
     if (n_sel > 0 && (rc = h->d_sel.reserve((size_t)n_sel)) != TCW_OK) return rc;
+    if (n_slots && (rc = h->d_slot.reserve(n_slots)) != TCW_OK) return rc;
 
     double *w = h->h_stage;
     std::memcpy(w, g->f0, sizeof(double) * g->n_f0);
@@ -181,6 +190,11 @@ int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaS
     if (n_sel > 0) {
         std::memcpy(w + n_axes, sel, sizeof(long) * (size_t)n_sel);
         CUDA_TRY(cudaMemcpyAsync(h->d_sel.p, w + n_axes, sizeof(long) * (size_t)n_sel, cudaMemcpyHostToDevice, st));
+    }
+    if (n_slots) {
+        int *ws = (int *)((char *)w + n_axes * sizeof(double) + (size_t)std::max<long>(n_sel, 0) * sizeof(long));
+        std::memcpy(ws, slots->data(), n_slots * sizeof(int));
+        CUDA_TRY(cudaMemcpyAsync(h->d_slot.p, ws, n_slots * sizeof(int), cudaMemcpyHostToDevice, st));
     }
     CUDA_TRY(cudaEventRecord(h->ev_stage, st));
     h->a_f0 = h->d_axes.p;
@@ -294,6 +308,37 @@ int launch_gather(int fmt, bool p2, const tcw::SumParams &p, long n_ctas, cudaSt
                                : launch_gather_t<tcw::FMT_U8>(p2, p, n_ctas, st);
 }
 
+template <int R, int SC, bool P2>
+int launch_sky_t(const tcw::SumParams &p, const tcw::SkyParams &q, long n_ctas, size_t smem, cudaStream_t st)
+{
+    auto kern = tcw::sum_skyblock_kernel<R, SC, P2>;
+    CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)n_ctas, tcw::SKY_THREADS, smem, st>>>(p, q);
+    CUDA_TRY(cudaGetLastError());
+    return TCW_OK;
+}
+
+int launch_sky(int sc, bool p2, const tcw::SumParams &p, const tcw::SkyParams &q, long n_ctas, size_t smem,
+               cudaStream_t st)
+{
+    if (sc == 2) return p2 ? launch_sky_t<16, 2, true>(p, q, n_ctas, smem, st) : launch_sky_t<16, 2, false>(p, q, n_ctas, smem, st);
+    return p2 ? launch_sky_t<8, 4, true>(p, q, n_ctas, smem, st) : launch_sky_t<8, 4, false>(p, q, n_ctas, smem, st);
+}
+
+int launch_sky_table(int sc, bool p2, const tcw_handle *h, const double *sky, int n_blocks, cudaStream_t st)
+{
+    const long warps = (long)n_blocks * h->n_sft;
+    const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
+#define TCW_SKY_TABLE(SC, P2)                                                                              \
+    tcw::skyblock_table_kernel<SC, P2><<<blocks, 256, 0, st>>>(h->d_vel, h->n_sft, sky, h->d_slot.p, n_blocks, \
+                                                               h->T, h->d_dts.p, h->d_dmm.p)
+    if (sc == 2) { if (p2) TCW_SKY_TABLE(2, true); else TCW_SKY_TABLE(2, false); }
+    else { if (p2) TCW_SKY_TABLE(4, true); else TCW_SKY_TABLE(4, false); }
+#undef TCW_SKY_TABLE
+    CUDA_TRY(cudaGetLastError());
+    return TCW_OK;
+}
+
 }  // namespace
 
 // =============================================================================== C ABI
@@ -343,6 +388,7 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     h->t_pow2 = is_pow2(T_sft);
     h->k_min = (int)km;
     h->vmax = vmax;
+    for (int c = 0; c < 3; ++c) h->vmid[c] = velocities[3 * (size_t)(n_sft / 2) + c];
     h->ts.assign(timestamps, timestamps + n_sft);
     h->fmt_dev = format == TCW_F32_POWER ? tcw::FMT_F32 : tcw::FMT_U8;
     const size_t bpb = h->fmt_dev == tcw::FMT_F32 ? 4 : 1;
@@ -411,6 +457,9 @@ int tcw_destroy(tcw_handle *h)
     h->d_stat.release();
     h->d_best.release();
     h->d_sel.release();
+    h->d_dts.release();
+    h->d_dmm.release();
+    h->d_slot.release();
     if (h->h_stage) cudaFreeHost(h->h_stage);
     if (h->ev_stage) cudaEventDestroy(h->ev_stage);
     for (auto &e : h->ev)
@@ -424,7 +473,7 @@ int tcw_set_option(tcw_handle *h, int key, long value)
     if (!h) return fail(TCW_EINVAL, "handle is NULL");
     switch (key) {
     case TCW_OPT_KERNEL:
-        if (value < 0 || value > 2) return fail(TCW_EINVAL, "TCW_OPT_KERNEL must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(TCW_EINVAL, "TCW_OPT_KERNEL must be 0, 1, 2 or 3");
         h->opt_kernel = (int)value;
         return TCW_OK;
     case TCW_OPT_TIMING:
@@ -441,6 +490,10 @@ int tcw_set_option(tcw_handle *h, int key, long value)
         if (value != 0 && (value < 2 || value > 16)) return fail(TCW_EINVAL, "TCW_OPT_STAGES must be 0 or 2..16");
         h->opt_stages = (int)value;
         return TCW_OK;
+    case TCW_OPT_SKY_BLOCK:
+        if (value != 0 && value != 64 && value != 128) return fail(TCW_EINVAL, "TCW_OPT_SKY_BLOCK must be 0, 64 or 128");
+        h->opt_sky = (int)value;
+        return TCW_OK;
     default: return fail(TCW_EINVAL, "unknown option %d", key);
     }
 }
@@ -455,11 +508,34 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
 
     tcw::SumParams p = base_params(h, grid);
-    // ---- launch plan: staged kernel with the largest tile whose window fits the row padding and
-    // whose ring (as deep as possible, up to opt_stages) still lets two CTAs share an SM
-    int kernel = 0, r = 0, stages = 0, slot = 0;
+    tcw::SkyParams q;
+    std::memset(&q, 0, sizeof q);
+    int kernel = 0, r = 0, stages = 0, slot = 0, sky_sc = 0, n_blocks = 0;
     size_t smem = 0;
-    if (h->opt_kernel != 1) {
+    // ---- launch plan, count formats with many sky points: the sky-block kernel (tcw_skyblock.cuh)
+    if (h->opt_kernel == 3 && h->fmt_dev != tcw::FMT_U8)
+        return fail(TCW_EUNSUPPORTED, "the sky-block kernel serves the count formats only");
+    if (h->fmt_dev == tcw::FMT_U8 && (h->opt_kernel == 3 || (h->opt_kernel == 0 && grid->n_sky >= 16))) {
+        const int sc = h->opt_sky == 128 ? 4 : 2, rr = sc == 2 ? 16 : 8, S = 32 * sc;
+        // two sky points differ by |D_s - D_s'| <= 2 vmax / c whatever the block holds
+        const double spread = grid->f0[grid->n_f0 - 1] * h->T * 2.0 * (h->vmax / C_LIGHT) * (1.0 + 1e-5);
+        const long w_bins = max_window_bins(grid, 32 * rr, p.dmaxT) + (long)std::ceil(spread) + 2;
+        if (w_bins <= tcw::PAD_BINS) {
+            const int sb = 8 * S + (int)((w_bins + 32 + 15) & ~15L);
+            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 4; s >= 2; --s) {
+                const size_t b = tcw::sky_smem_bytes(s, sb, 32 * rr, S);
+                if (b <= SMEM_MAX) {
+                    kernel = 3; r = rr; sky_sc = sc; stages = s; slot = sb; smem = b;
+                    break;
+                }
+            }
+        }
+        if (!kernel && h->opt_kernel == 3)
+            return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the sky-block kernel (window exceeds the row padding)");
+    }
+    // ---- otherwise: staged kernel with the largest tile whose window fits the row padding and
+    // whose ring (as deep as possible, up to opt_stages) still lets two CTAs share an SM
+    if (!kernel && h->opt_kernel != 1) {
         const int all[3] = {16, 8, 4};
         for (int c = 0; c < 3 && !kernel; ++c) {
             if (h->opt_r && all[c] != h->opt_r) continue;
@@ -478,16 +554,37 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the staged kernel (window exceeds the row padding)");
     }
     if (!kernel) kernel = 1;
-    p.tile = kernel == 2 ? 32 * r : 128;
+    p.tile = kernel >= 2 ? 32 * r : 128;
     p.n_tiles = (grid->n_f0 + p.tile - 1) / p.tile;
     p.stages = stages;
     p.slot_bytes = slot;
-    const long n_ctas = n_groups * p.n_tiles;
+    const long n_partial = n_groups * p.n_tiles;
+    long n_ctas = n_partial;
+    if (kernel == 3) {
+        // sky points sorted by their Doppler shift at the middle SFT, cut into blocks of S
+        const int S = 32 * sky_sc;
+        n_blocks = (grid->n_sky + S - 1) / S;
+        n_ctas = (long)n_blocks * p.n_ab * p.n_tiles;
+        std::vector<std::pair<double, int>> key((size_t)grid->n_sky);
+        for (int s = 0; s < grid->n_sky; ++s) {
+            const double *n = grid->sky + 3 * (size_t)s;
+            key[s] = {n[0] * h->vmid[0] + n[1] * h->vmid[1] + n[2] * h->vmid[2], s};
+        }
+        std::sort(key.begin(), key.end());
+        h->slot_host.resize((size_t)n_blocks * S);
+        for (size_t t = 0; t < h->slot_host.size(); ++t)
+            h->slot_host[t] = key[std::min(t, (size_t)grid->n_sky - 1)].second;
+    }
     if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "grid needs more than 2^31-1 CTAs; split the search");
 
     CUDA_TRY(cudaSetDevice(h->device));
-    if ((rc = h->d_partial.reserve((size_t)n_ctas * 8)) != TCW_OK) return rc;
+    if ((rc = h->d_partial.reserve((size_t)n_partial * 8)) != TCW_OK) return rc;
     if (!out_best && (rc = h->d_best.reserve((size_t)n_groups * 8)) != TCW_OK) return rc;
+    if (kernel == 3) {
+        const size_t rows = (size_t)n_blocks * h->n_sft;
+        if ((rc = h->d_dts.reserve(rows * 32 * sky_sc)) != TCW_OK) return rc;
+        if ((rc = h->d_dmm.reserve(rows * 2)) != TCW_OK) return rc;
+    }
     p.partial = h->d_partial.p;
     p.out_stat = out_stat;
 
@@ -502,12 +599,21 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
         ev = h->ev.data() + 4 * h->timing_n;
         CUDA_TRY(cudaEventRecord(ev[0], st));
     }
-    if ((rc = prepare(h, grid, 0, nullptr, st)) != TCW_OK) return rc;
+    if ((rc = prepare(h, grid, 0, nullptr, st, kernel == 3 ? &h->slot_host : nullptr)) != TCW_OK) return rc;
     p.f0 = h->a_f0;
     p.gtab = h->d_g.p;
     p.dtab = h->d_d.p;
+    if (kernel == 3) {
+        if ((rc = launch_sky_table(sky_sc, h->t_pow2, h, h->a_sky, n_blocks, st)) != TCW_OK) return rc;
+        q.dts = h->d_dts.p;
+        q.dmm = h->d_dmm.p;
+        q.slot_sky = h->d_slot.p;
+        q.n_sky = grid->n_sky;
+        q.n_blocks = n_blocks;
+    }
     if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
-    if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, p, n_ctas, smem, st);
+    if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
+    else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, p, n_ctas, smem, st);
     else rc = launch_gather(h->fmt_dev, h->t_pow2, p, n_ctas, st);
     if (rc != TCW_OK) return rc;
     if (tm) CUDA_TRY(cudaEventRecord(ev[2], st));
@@ -528,7 +634,8 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     h->info[2] = n_ctas;
     h->info[3] = (long)smem;
     h->info[6] = stages;
-    h->info[5] = 4;  // doppler table, spin-down table, sum, best
+    h->info[7] = 32 * sky_sc;
+    h->info[5] = kernel == 3 ? 5 : 4;  // doppler table, spin-down table, (sky-block table,) sum, best
     return TCW_OK;
 }
 

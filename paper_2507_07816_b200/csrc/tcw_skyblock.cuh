@@ -1,0 +1,312 @@
+// tcw_skyblock.cuh -- exact sky-shared gather-accumulate for number counts (sm_100a).
+//
+// The statistic of template (f0, tau, n, n-hat_s) is "summed across the data bins selected by the
+// track" with the bin k = rint((f0*g)*(D_s*T)) - k_min of eqs. (1)-(2)
+// (PAPER.md:25, 32).  Only the Doppler factor D_s depends on the sky point, and it moves the track
+// by a fraction of a bin across neighbouring sky points, so most sky points of a patch select the
+// SAME bin for a given (f0, tau, n, SFT).  This kernel uses that without approximating anything:
+//
+//   * IEEE multiplication by a positive number, the magic-add rounding and hence rint(a*d) are
+//     monotone non-decreasing in d.  For a block B of sky points and one SFT j, with
+//     d_min = min_{s in B} D_s(j)*T and d_max = max_{s in B} D_s(j)*T (taken over the very doubles
+//     the per-sky path multiplies by), every s in B has lo(a*d_min) <= lo(a*D_s*T) <= lo(a*d_max).
+//   * If the two ends agree, all sky points of the block select that bin: one lookup serves the
+//     whole block (it is added to a per-template base sum).  If they are adjacent bins holding the
+//     same value, likewise.  Otherwise the lookup is resolved per sky point (lanes = sky points)
+//     and the difference to the base value goes to a per-(template, sky) correction in shared
+//     memory.  stat[s] = base + corr[s] in exact integer arithmetic, so the result is bit-identical
+//     to the per-sky evaluation whatever the order of the additions.
+//
+// The host sorts the sky points by their Doppler shift at the middle SFT and cuts the sorted list
+// into blocks of S = 32*SC points, which keeps d_max - d_min (and so the fraction of lookups that
+// must be resolved) small for any sky grid, ordered or not.  Integer accumulation only: the
+// float32 power format keeps the per-sky staged kernel (a fixed summation order is part of its
+// contract).
+//
+// One CTA owns (sky block, (tau, n), tile of 32*R consecutive f0).  As in sum_staged_kernel every
+// warp owns the SFT rows j = j_begin + warp + NWS*n and runs a private TMA ring; a ring slot holds
+// the block's S Doppler factors of the row followed by the spectrogram window of the row.
+#pragma once
+#include "tcw_sum.cuh"
+#include "tcw_tables.cuh"
+
+namespace tcw {
+
+constexpr int NWS = 16;                 // warps per CTA
+constexpr int SKY_THREADS = 32 * NWS;
+
+struct SkyParams {
+    const double *dts;     // [n_blocks][n_sft][S]  D_s(j) (times T_sft when it is a power of two), block order
+    const double *dmm;     // [n_blocks][n_sft][2]  {min, max} of the row above
+    const int *slot_sky;   // [n_blocks*S] sky index of each slot; slots >= n_sky repeat the last sky point
+    int n_sky, n_blocks;
+};
+
+// ---------------------------------------------------------------------------- block tables
+// One warp per (block, SFT): lanes run over the block's sky points.
+template <int SC, bool TPOW2>
+__global__ void __launch_bounds__(256)
+skyblock_table_kernel(const double *__restrict__ vel, int n_sft, const double *__restrict__ sky,
+                      const int *__restrict__ slot_sky, int n_blocks, double T,
+                      double *__restrict__ dts, double *__restrict__ dmm)
+{
+    constexpr int S = 32 * SC;
+    const long wq = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (wq >= (long)n_blocks * n_sft) return;
+    const int j = (int)(wq % n_sft);
+    const int b = (int)(wq / n_sft);
+    const double *v = vel + 3 * (long)j;
+    double lo = 0, hi = 0;
+#pragma unroll
+    for (int c = 0; c < SC; ++c) {
+        const int s = slot_sky[b * S + c * 32 + lane];
+        double d = doppler_factor(v, sky + 3 * (long)s);
+        if (TPOW2) d = __dmul_rn(d, T);
+        dts[wq * S + c * 32 + lane] = d;
+        lo = c ? fmin(lo, d) : d;
+        hi = c ? fmax(hi, d) : d;
+    }
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if (lane == 0) {
+        dmm[2 * wq] = lo;
+        dmm[2 * wq + 1] = hi;
+    }
+}
+
+// ---------------------------------------------------------------------------- sum kernel
+__device__ __forceinline__ double lds_f64(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void red_shared_add(uint32_t a, int v)
+{
+    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
+struct __align__(16) SkyRowMeta {
+    double g, d0, d1;   // spin-down factor; min and max Doppler factor of the block in this row
+    uint32_t rb;        // shared address of bin (0 - k_min) of the staged window: addr = rb + rint(x)
+    int live;           // 1 staged row, 0 row with no in-band bin, -1 no further rows
+    int pad[2];
+};
+
+// dynamic shared memory: [mbarrier NWS*D][SkyRowMeta NWS*D][corr F*(S+1) int][slots NWS*D*slot_bytes]
+__host__ __device__ inline size_t sky_header_bytes(int stages) { return (size_t)NWS * stages * (8 + sizeof(SkyRowMeta)); }
+__host__ __device__ inline size_t sky_corr_bytes(int tile, int S) { return (((size_t)tile * (S + 1) * 4) + 127) & ~(size_t)127; }
+__host__ __device__ inline size_t sky_smem_bytes(int stages, int slot_bytes, int tile, int S)
+{
+    size_t ring = (size_t)NWS * stages * (size_t)slot_bytes;
+    size_t red = (size_t)NWS * tile * 4 + 128;
+    return ((sky_header_bytes(stages) + 127) & ~(size_t)127) + sky_corr_bytes(tile, S) + (ring > red ? ring : red);
+}
+
+template <bool TPOW2>
+__device__ __forceinline__ int lo_of(double a, double d, double T)
+{
+    double x = __dmul_rn(a, d);
+    if (!TPOW2) x = __dmul_rn(x, T);
+    return __double2loint(__dadd_rn(x, TCW_MAGIC));
+}
+
+template <int R, int SC, bool TPOW2>
+__global__ void __launch_bounds__(SKY_THREADS, 1)
+sum_skyblock_kernel(const SumParams p, const SkyParams q)
+{
+    constexpr int F = 32 * R;       // templates per tile
+    constexpr int S = 32 * SC;      // sky points per block
+    constexpr int CS = S + 1;       // corr row stride in words: odd, so both access patterns are conflict-free
+    constexpr uint32_t FULL = 0xffffffffu;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int D = p.stages;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint64_t *bars = (uint64_t *)smem + warp * D;
+    SkyRowMeta *metas = (SkyRowMeta *)(smem + (size_t)NWS * D * 8) + warp * D;
+    int *corr = (int *)(smem + ((sky_header_bytes(D) + 127) & ~(size_t)127));
+    unsigned char *slots = (unsigned char *)corr + sky_corr_bytes(F, S);
+    const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D * p.slot_bytes);
+    const uint32_t bars_s = smem_u32(bars);
+    const uint32_t corr_s = smem_u32(corr);
+
+    // heavy tiles (high f0 stays in band longest) are launched first
+    const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);
+    const int ab = (int)((blockIdx.x / p.n_tiles) % p.n_ab);
+    const int blk = (int)(blockIdx.x / ((long)p.n_tiles * p.n_ab));
+    const int i0 = tile * F;
+    const int i_last = min(i0 + F, p.n_f0) - 1;
+
+    if (lane == 0) {
+        for (int s = 0; s < D; ++s) mbar_init(bars_s + 8u * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int t = threadIdx.x; t < F * CS; t += SKY_THREADS) corr[t] = 0;
+    __syncthreads();
+
+    int acc[R];
+    double f0r[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        acc[r] = 0;
+        f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
+    }
+    const double f_first = p.f0[i0], f_last = p.f0[i_last];
+    const double below = (double)p.k_min - 1.0;
+    const double *g = p.gtab + (long)ab * p.n_sft;
+    const double *mm = q.dmm + 2 * (long)blk * p.n_sft;
+    const double *dts = q.dts + (long)blk * p.n_sft * S;
+    const int jw = p.j_begin + warp;
+    const int n_rows = jw < p.n_sft ? (p.n_sft - jw + NWS - 1) / NWS : 0;
+    const unsigned char *spec_w = p.spec + (long)jw * p.pitch;
+    const long pitch_w = (long)NWS * p.pitch;
+
+    // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp).
+    double b_g = 0, b_d0 = 0, b_d1 = 0;
+    const unsigned char *b_src = nullptr;
+    const double *b_dts = nullptr;
+    uint32_t b_rb = 0;
+    int b_bytes = 0, b_live = -1;
+    double gn = 0, d0n = 1, d1n = 1;
+    if (lane < n_rows) {
+        const int j = jw + NWS * lane;
+        gn = __ldg(g + j); d0n = __ldg(mm + 2 * j); d1n = __ldg(mm + 2 * j + 1);
+    }
+
+    auto compute_batch = [&](int m) {
+        const int n = 32 * m + lane;
+        b_g = gn; b_d0 = d0n; b_d1 = d1n;
+        if (n + 32 < n_rows) {
+            const int j = jw + NWS * (n + 32);
+            gn = __ldg(g + j); d0n = __ldg(mm + 2 * j); d1n = __ldg(mm + 2 * j + 1);
+        }
+        b_live = -1;
+        b_bytes = 0;
+        // g decreases with j: once the tile's highest template is below the band for the largest
+        // possible Doppler factor, no later SFT can contribute.
+        if (n < n_rows && !(f_last * b_g * p.dmaxT < below)) {
+            const int kf = lo_of<TPOW2>(__dmul_rn(f_first, b_g), b_d0, p.T) - p.k_min;
+            const int kl = lo_of<TPOW2>(__dmul_rn(f_last, b_g), b_d1, p.T) - p.k_min;
+            b_live = 0;
+            if (kl >= 0 && kf < p.n_bins) {
+                const int a_byte = kf & ~15;                      // rounds towards -inf: may reach into the left padding
+                const int e_byte = (kl + 1 + 15) & ~15;
+                if (e_byte - a_byte + 8 * S > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                    atomicOr(p.status, 1);  // host-side window bound violated: never expected
+                } else {
+                    b_bytes = e_byte - a_byte;
+                    b_src = spec_w + (long)n * pitch_w + a_byte;
+                    b_dts = dts + (long)(jw + NWS * n) * S;
+                    b_rb = (uint32_t)(8 * S) - (uint32_t)(p.k_min + a_byte);
+                    b_live = 1;
+                }
+            }
+        }
+    };
+
+    int ni = 0, si = 0;   // next row to stage and its ring slot
+    auto stage_next = [&]() {
+        if ((ni & 31) == 0) compute_batch(ni >> 5);
+        if (lane == (ni & 31)) {
+            const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
+            SkyRowMeta m;
+            m.g = b_g; m.d0 = b_d0; m.d1 = b_d1; m.rb = slot_s + b_rb; m.live = b_live; m.pad[0] = m.pad[1] = 0;
+            metas[si] = m;
+            if (b_live > 0) {
+                mbar_arrive_expect_tx(bars_s + 8u * si, (uint32_t)(b_bytes + 8 * S));
+                bulk_g2s(slot_s, b_dts, (uint32_t)(8 * S), bars_s + 8u * si);
+                bulk_g2s(slot_s + 8u * S, b_src, (uint32_t)b_bytes, bars_s + 8u * si);
+            } else if (b_live == 0) {
+                mbar_arrive(bars_s + 8u * si);
+            }
+        }
+        __syncwarp();
+        ++ni;
+        if (++si == D) si = 0;
+    };
+
+    for (int s = 0; s < D - 1; ++s) stage_next();
+
+    uint32_t ph = 0;
+    int sc = 0;
+    for (;;) {
+        stage_next();
+        const SkyRowMeta m = metas[sc];
+        if (m.live <= 0) {
+            if (m.live < 0) break;
+        } else {
+            mbar_wait(bars_s + 8u * sc, ph);
+            const uint32_t dt_s = slots_s + (uint32_t)(sc * p.slot_bytes) + 8u * lane;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double a = __dmul_rn(f0r[r], m.g);
+                const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
+                const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
+                const int v0 = (int)lds_u8(m.rb + (uint32_t)lo0);
+                acc[r] += v0;
+                bool need = lo1 != lo0;
+                if (need) need = (lo1 != lo0 + 1) || ((int)lds_u8(m.rb + (uint32_t)lo1) != v0);
+                unsigned mask = __ballot_sync(FULL, need);
+                while (mask) {
+                    const int L = __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    const double a_b = __shfl_sync(FULL, a, L);
+                    const int v0_b = __shfl_sync(FULL, v0, L);
+                    const uint32_t c_s = corr_s + 4u * (uint32_t)((r * 32 + L) * CS + lane);
+#pragma unroll
+                    for (int c = 0; c < SC; ++c) {
+                        const double dt = lds_f64(dt_s + 256u * c);
+                        const int lo = lo_of<TPOW2>(a_b, dt, p.T);
+                        const int dv = (int)lds_u8(m.rb + (uint32_t)lo) - v0_b;
+                        if (dv) red_shared_add(c_s + 128u * c, dv);
+                    }
+                }
+            }
+        }
+        __syncwarp();     // every lane has read slot sc before the next iteration refills it
+        if (++sc == D) { sc = 0; ph ^= 1u; }
+    }
+
+    // ---------------- combine: base[t] = sum over warps (integers: any order is exact)
+    __syncthreads();      // every staged copy has been consumed and every correction has landed
+    int *red = (int *)slots;
+#pragma unroll
+    for (int r = 0; r < R; ++r) red[warp * F + r * 32 + lane] = acc[r];
+    __syncthreads();
+    for (int t = threadIdx.x; t < F; t += SKY_THREADS) {
+        int s = red[t];
+        for (int w = 1; w < NWS; ++w) s += red[w * F + t];
+        red[t] = s;
+    }
+    __syncthreads();
+    // ---------------- stat[s][t] = base[t] + corr[t][s]; warp w serves the block's slots w, w + NWS, ...
+    for (int sl = warp; sl < S; sl += NWS) {
+        const int slot = blk * S + sl;
+        if (slot >= q.n_sky) break;           // padding slots repeat the last sky point; no output
+        const long grp = (long)q.slot_sky[slot] * p.n_ab + ab;
+        int best_v = INT32_MIN, best_i = INT32_MAX;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int t = r * 32 + lane;
+            const int i = i0 + t;
+            if (i < p.n_f0) {
+                const int s = red[t] + corr[t * CS + sl];
+                if (p.out_stat) ((int *)p.out_stat)[grp * p.n_f0 + i] = s;
+                argmax_step(best_v, best_i, s, i);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            const int ov = __shfl_xor_sync(FULL, best_v, o);
+            const int oi = __shfl_xor_sync(FULL, best_i, o);
+            argmax_step(best_v, best_i, ov, oi);
+        }
+        if (lane == 0) ((Best<int> *)p.partial)[grp * p.n_tiles + tile] = {best_v, best_i == INT32_MAX ? 0 : best_i};
+    }
+}
+
+}  // namespace tcw

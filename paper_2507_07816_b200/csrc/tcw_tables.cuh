@@ -159,6 +159,13 @@ spindown_table_kernel(const double *__restrict__ ts, int n_sft, double T0,
     g_out[q] = pow_rn(base, e);
 }
 
+// D = 1 + ((vx*nx + vy*ny) + vz*nz)/c, eq. (2): five single binary64 operations, never fused.
+__device__ __forceinline__ double doppler_factor(const double *__restrict__ v, const double *__restrict__ n)
+{
+    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], n[0]), __dmul_rn(v[1], n[1])), __dmul_rn(v[2], n[2]));
+    return __dadd_rn(1.0, __ddiv_rn(dot, 299792458.0));
+}
+
 // D[s][j], one thread per entry.
 __global__ void __launch_bounds__(256)
 doppler_table_kernel(const double *__restrict__ vel, int n_sft, const double *__restrict__ sky,
@@ -169,11 +176,7 @@ doppler_table_kernel(const double *__restrict__ vel, int n_sft, const double *__
     if (q >= total) return;
     int j = (int)(q % n_sft);
     int s = (int)(q / n_sft);
-    const double *v = vel + 3 * (long)j;
-    const double *n = sky + 3 * (long)s;
-    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], n[0]), __dmul_rn(v[1], n[1])), __dmul_rn(v[2], n[2]));
-    double beta = __ddiv_rn(dot, 299792458.0);
-    d_out[q] = __dadd_rn(1.0, beta);
+    d_out[q] = doppler_factor(vel + 3 * (long)j, sky + 3 * (long)s);
 }
 
 }  // namespace tcw

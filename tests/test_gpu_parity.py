@@ -19,7 +19,7 @@ from tcw_inputs import Workload, detector_velocity, sky_vector
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-4
-KERNELS = {"auto": 0, "gather": 1, "staged": 2}
+KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 
 
 @pytest.fixture(scope="module")
@@ -31,11 +31,12 @@ def tcw():
     return pkg
 
 
-def gpu_search(tcw, w, kernel="auto", f0_per_lane=0, host=False):
+def gpu_search(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0):
     import torch
     with tcw.Handle.from_workload(w, host=host) as h:
         h.set_option(tcw.TCW_OPT_KERNEL, KERNELS[kernel])
         h.set_option(tcw.TCW_OPT_F0_PER_LANE, f0_per_lane)
+        h.set_option(tcw.TCW_OPT_SKY_BLOCK, sky_block)
         grid = tcw.Grid.of(w)
         stat, best = h.search(grid)
         torch.cuda.synchronize()
@@ -75,8 +76,8 @@ def assert_best_parity(w, n_f0, bs, bi, want_stat):
         assert np.array_equal(bi, idx)
 
 
-def full_parity(tcw, w, kernel="auto", f0_per_lane=0, host=False):
-    got, bs, bi, info = gpu_search(tcw, w, kernel, f0_per_lane, host)
+def full_parity(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0):
+    got, bs, bi, info = gpu_search(tcw, w, kernel, f0_per_lane, host, sky_block)
     ref = oracle.evaluate(w)
     assert_stat_parity(w, got, ref.stat)
     assert_best_parity(w, len(w.f0), bs, bi, ref.stat)
