@@ -85,9 +85,11 @@ __device__ __forceinline__ double lds_f64(uint32_t a)
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ void red_shared_add(uint32_t a, int v)
+// shared[a] += v where cond != 0 (a predicated reduction, no branch)
+__device__ __forceinline__ void red_shared_add_if(uint32_t a, int v, uint32_t cond)
 {
-    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p red.shared.add.s32 [%0], %1;\n}"
+                 ::"r"(a), "r"(v), "r"(cond) : "memory");
 }
 
 struct __align__(16) SkyRowMeta {
@@ -167,10 +169,7 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
 
     // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp).
     double b_g = 0, b_d0 = 0, b_d1 = 0;
-    const unsigned char *b_src = nullptr;
-    const double *b_dts = nullptr;
-    uint32_t b_rb = 0;
-    int b_bytes = 0, b_live = -1;
+    int b_abyte = 0, b_bytes = 0, b_live = -1;   // first staged byte of the row's window, bytes staged
     double gn = 0, d0n = 1, d1n = 1;
     if (lane < n_rows) {
         const int j = jw + NWS * lane;
@@ -199,9 +198,7 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
                     atomicOr(p.status, 1);  // host-side window bound violated: never expected
                 } else {
                     b_bytes = e_byte - a_byte;
-                    b_src = spec_w + (long)n * pitch_w + a_byte;
-                    b_dts = dts + (long)(jw + NWS * n) * S;
-                    b_rb = (uint32_t)(8 * S) - (uint32_t)(p.k_min + a_byte);
+                    b_abyte = a_byte;
                     b_live = 1;
                 }
             }
@@ -214,12 +211,13 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
         if (lane == (ni & 31)) {
             const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
             SkyRowMeta m;
-            m.g = b_g; m.d0 = b_d0; m.d1 = b_d1; m.rb = slot_s + b_rb; m.live = b_live; m.pad[0] = m.pad[1] = 0;
+            m.g = b_g; m.d0 = b_d0; m.d1 = b_d1; m.live = b_live; m.pad[0] = m.pad[1] = 0;
+            m.rb = slot_s + (uint32_t)(8 * S) - (uint32_t)(p.k_min + b_abyte);
             metas[si] = m;
             if (b_live > 0) {
                 mbar_arrive_expect_tx(bars_s + 8u * si, (uint32_t)(b_bytes + 8 * S));
-                bulk_g2s(slot_s, b_dts, (uint32_t)(8 * S), bars_s + 8u * si);
-                bulk_g2s(slot_s + 8u * S, b_src, (uint32_t)b_bytes, bars_s + 8u * si);
+                bulk_g2s(slot_s, dts + (long)(jw + NWS * ni) * S, (uint32_t)(8 * S), bars_s + 8u * si);
+                bulk_g2s(slot_s + 8u * S, spec_w + (long)ni * pitch_w + b_abyte, (uint32_t)b_bytes, bars_s + 8u * si);
             } else if (b_live == 0) {
                 mbar_arrive(bars_s + 8u * si);
             }
@@ -241,30 +239,63 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
         } else {
             mbar_wait(bars_s + 8u * sc, ph);
             const uint32_t dt_s = slots_s + (uint32_t)(sc * p.slot_bytes) + 8u * lane;
+            // Phase A (lanes = templates): every template against the two ends of the block.  All R
+            // chains are independent, so they are issued back to back; the votes are kept.
+            constexpr int RB = R < 8 ? R : 8;    // templates per lane handled between two phase switches
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
+            for (int rh = 0; rh < R; rh += RB) {
+            unsigned masks[RB];
+#pragma unroll
+            for (int rr = 0; rr < RB; ++rr) {
+                const int r = rh + rr;
                 const double a = __dmul_rn(f0r[r], m.g);
                 const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
                 const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
                 const int v0 = (int)lds_u8(m.rb + (uint32_t)lo0);
+                const int v1 = (int)lds_u8(m.rb + (uint32_t)lo1);
                 acc[r] += v0;
-                bool need = lo1 != lo0;
-                if (need) need = (lo1 != lo0 + 1) || ((int)lds_u8(m.rb + (uint32_t)lo1) != v0);
-                unsigned mask = __ballot_sync(FULL, need);
-                while (mask) {
+                // resolved per sky point unless both ends agree, or are adjacent bins of equal value
+                masks[rr] = __ballot_sync(FULL, (lo1 != lo0) & ((lo1 != lo0 + 1) | (v1 != v0)));
+            }
+            // Phase B (lanes = sky points): the few lookups the block does not agree on
+#pragma unroll
+            for (int rr = 0; rr < RB; ++rr) {
+                const int r = rh + rr;
+                unsigned mask = masks[rr];
+                if (mask == 0) continue;
+                const double a = __dmul_rn(f0r[r], m.g);
+                const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
+                const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
+                const uint32_t v0 = lds_u8(m.rb + (uint32_t)lo0);
+                const uint32_t v1 = lds_u8(m.rb + (uint32_t)lo1);
+                // value at the low end, value at the high end, "ends are adjacent bins", parity of the low bin
+                const uint32_t packed = v0 | (v1 << 8) | ((lo1 == lo0 + 1) ? 0x10000u : 0u) | (((uint32_t)lo0 & 1u) << 17);
+                do {
                     const int L = __ffs(mask) - 1;
                     mask &= mask - 1;
                     const double a_b = __shfl_sync(FULL, a, L);
-                    const int v0_b = __shfl_sync(FULL, v0, L);
+                    const uint32_t pk = __shfl_sync(FULL, packed, L);
+                    const int v0_b = (int)(pk & 0xffu);
                     const uint32_t c_s = corr_s + 4u * (uint32_t)((r * 32 + L) * CS + lane);
+                    if (pk & 0x10000u) {
+                        // two candidate bins: a sky point reads the high one iff its bin parity differs
+                        const int dv = (int)((pk >> 8) & 0xffu) - v0_b;
+                        const uint32_t par = pk >> 17;
 #pragma unroll
-                    for (int c = 0; c < SC; ++c) {
-                        const double dt = lds_f64(dt_s + 256u * c);
-                        const int lo = lo_of<TPOW2>(a_b, dt, p.T);
-                        const int dv = (int)lds_u8(m.rb + (uint32_t)lo) - v0_b;
-                        if (dv) red_shared_add(c_s + 128u * c, dv);
+                        for (int c = 0; c < SC; ++c) {
+                            const uint32_t lo = (uint32_t)lo_of<TPOW2>(a_b, lds_f64(dt_s + 256u * c), p.T);
+                            red_shared_add_if(c_s + 128u * c, dv, (lo ^ par) & 1u);
+                        }
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < SC; ++c) {
+                            const uint32_t lo = (uint32_t)lo_of<TPOW2>(a_b, lds_f64(dt_s + 256u * c), p.T);
+                            const int dv = (int)lds_u8(m.rb + lo) - v0_b;
+                            red_shared_add_if(c_s + 128u * c, dv, (uint32_t)dv);
+                        }
                     }
-                }
+                } while (mask);
+            }
             }
         }
         __syncwarp();     // every lane has read slot sc before the next iteration refills it
