@@ -85,11 +85,23 @@ __device__ __forceinline__ double lds_f64(uint32_t a)
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
     return v;
 }
-// shared[a] += v where cond != 0 (a predicated reduction, no branch)
-__device__ __forceinline__ void red_shared_add_if(uint32_t a, int v, uint32_t cond)
+__device__ __forceinline__ void red_shared_add(uint32_t a, int v)
 {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@p red.shared.add.s32 [%0], %1;\n}"
-                 ::"r"(a), "r"(v), "r"(cond) : "memory");
+    asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
+constexpr int ITEM_GENERIC = 0x10000;   // item.pk >= this: generic resolve, pk - ITEM_GENERIC is the base value
+// one unresolved lookup: a = f0*g, pk, shared address of the template's correction row
+__device__ __forceinline__ void sts_item(uint32_t addr, double a, int pk, uint32_t c_s)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(__double2loint(a)), "r"(__double2hiint(a)),
+                 "r"(pk), "r"(c_s) : "memory");
+}
+__device__ __forceinline__ void lds_item(uint32_t addr, double &a, int &pk, uint32_t &c_s)
+{
+    int lo, hi;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(lo), "=r"(hi), "=r"(pk), "=r"(c_s) : "r"(addr));
+    a = __hiloint2double(hi, lo);
 }
 
 struct __align__(16) SkyRowMeta {
@@ -99,14 +111,17 @@ struct __align__(16) SkyRowMeta {
     int pad[2];
 };
 
-// dynamic shared memory: [mbarrier NWS*D][SkyRowMeta NWS*D][corr F*(S+1) int][slots NWS*D*slot_bytes]
+// dynamic shared memory: [mbarrier NWS*D][SkyRowMeta NWS*D][item lists NWS*32*16 B][f0 tile F double]
+//                        [corr F*(S+1) int][slots NWS*D*slot_bytes]
 __host__ __device__ inline size_t sky_header_bytes(int stages) { return (size_t)NWS * stages * (8 + sizeof(SkyRowMeta)); }
 __host__ __device__ inline size_t sky_corr_bytes(int tile, int S) { return (((size_t)tile * (S + 1) * 4) + 127) & ~(size_t)127; }
+__host__ __device__ inline size_t sky_items_off(int stages) { return (sky_header_bytes(stages) + 127) & ~(size_t)127; }
+__host__ __device__ inline size_t sky_f0_off(int stages) { return sky_items_off(stages) + (size_t)NWS * 32 * 16; }
 __host__ __device__ inline size_t sky_smem_bytes(int stages, int slot_bytes, int tile, int S)
 {
     size_t ring = (size_t)NWS * stages * (size_t)slot_bytes;
     size_t red = (size_t)NWS * tile * 4 + 128;
-    return ((sky_header_bytes(stages) + 127) & ~(size_t)127) + sky_corr_bytes(tile, S) + (ring > red ? ring : red);
+    return sky_f0_off(stages) + (size_t)tile * 8 + sky_corr_bytes(tile, S) + (ring > red ? ring : red);
 }
 
 template <bool TPOW2>
@@ -130,11 +145,14 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint64_t *bars = (uint64_t *)smem + warp * D;
     SkyRowMeta *metas = (SkyRowMeta *)(smem + (size_t)NWS * D * 8) + warp * D;
-    int *corr = (int *)(smem + ((sky_header_bytes(D) + 127) & ~(size_t)127));
+    double *f0t = (double *)(smem + sky_f0_off(D));          // the tile's f0, lane-interleaved: f0t[r*32 + lane]
+    int *corr = (int *)(f0t + F);
     unsigned char *slots = (unsigned char *)corr + sky_corr_bytes(F, S);
     const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D * p.slot_bytes);
     const uint32_t bars_s = smem_u32(bars);
     const uint32_t corr_s = smem_u32(corr);
+    const uint32_t f0_s = smem_u32(f0t) + 8u * lane;
+    const uint32_t items_s = smem_u32(smem + sky_items_off(D)) + (uint32_t)(warp * 32 * 16);
 
     // heavy tiles (high f0 stays in band longest) are launched first
     const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);
@@ -148,15 +166,12 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int t = threadIdx.x; t < F * CS; t += SKY_THREADS) corr[t] = 0;
+    for (int t = threadIdx.x; t < F; t += SKY_THREADS) f0t[t] = p.f0[min(i0 + t, i_last)];
     __syncthreads();
 
     int acc[R];
-    double f0r[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        acc[r] = 0;
-        f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
-    }
+    for (int r = 0; r < R; ++r) acc[r] = 0;
     const double f_first = p.f0[i0], f_last = p.f0[i_last];
     const double below = (double)p.k_min - 1.0;
     const double *g = p.gtab + (long)ab * p.n_sft;
@@ -239,63 +254,67 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
         } else {
             mbar_wait(bars_s + 8u * sc, ph);
             const uint32_t dt_s = slots_s + (uint32_t)(sc * p.slot_bytes) + 8u * lane;
-            // Phase A (lanes = templates): every template against the two ends of the block.  All R
-            // chains are independent, so they are issued back to back; the votes are kept.
-            constexpr int RB = R < 8 ? R : 8;    // templates per lane handled between two phase switches
+            // Phase A (lanes = templates): every template against the two ends of the block.  The R
+            // chains are independent and issue back to back; a lane notes which of its templates
+            // the block does not agree on.
+            uint32_t bits = 0;
 #pragma unroll
-            for (int rh = 0; rh < R; rh += RB) {
-            unsigned masks[RB];
-#pragma unroll
-            for (int rr = 0; rr < RB; ++rr) {
-                const int r = rh + rr;
-                const double a = __dmul_rn(f0r[r], m.g);
+            for (int r = 0; r < R; ++r) {
+                const double a = __dmul_rn(lds_f64(f0_s + 256u * r), m.g);
                 const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
                 const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
                 const int v0 = (int)lds_u8(m.rb + (uint32_t)lo0);
                 const int v1 = (int)lds_u8(m.rb + (uint32_t)lo1);
                 acc[r] += v0;
-                // resolved per sky point unless both ends agree, or are adjacent bins of equal value
-                masks[rr] = __ballot_sync(FULL, (lo1 != lo0) & ((lo1 != lo0 + 1) | (v1 != v0)));
+                // unanimous if both ends agree (then v1 is v0 read twice) or are adjacent bins of equal value
+                if ((v1 != v0) | ((uint32_t)(lo1 - lo0) > 1u)) bits |= 1u << r;
             }
-            // Phase B (lanes = sky points): the few lookups the block does not agree on
-#pragma unroll
-            for (int rr = 0; rr < RB; ++rr) {
-                const int r = rh + rr;
-                unsigned mask = masks[rr];
-                if (mask == 0) continue;
-                const double a = __dmul_rn(f0r[r], m.g);
-                const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
-                const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
-                const uint32_t v0 = lds_u8(m.rb + (uint32_t)lo0);
-                const uint32_t v1 = lds_u8(m.rb + (uint32_t)lo1);
-                // value at the low end, value at the high end, "ends are adjacent bins", parity of the low bin
-                const uint32_t packed = v0 | (v1 << 8) | ((lo1 == lo0 + 1) ? 0x10000u : 0u) | (((uint32_t)lo0 & 1u) << 17);
-                do {
-                    const int L = __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    const double a_b = __shfl_sync(FULL, a, L);
-                    const uint32_t pk = __shfl_sync(FULL, packed, L);
-                    const int v0_b = (int)(pk & 0xffu);
-                    const uint32_t c_s = corr_s + 4u * (uint32_t)((r * 32 + L) * CS + lane);
-                    if (pk & 0x10000u) {
-                        // two candidate bins: a sky point reads the high one iff its bin parity differs
-                        const int dv = (int)((pk >> 8) & 0xffu) - v0_b;
-                        const uint32_t par = pk >> 17;
+            // Phase B: the few lookups the block does not agree on.  Owners publish one lookup each
+            // (a, what to add, where) in the warp's item list; then lanes = sky points resolve the
+            // listed lookups one after the other.  Usually one round of a handful of items.
+            for (;;) {
+                const unsigned own = __ballot_sync(FULL, bits != 0);
+                if (own == 0) break;
+                if (bits) {
+                    const int r = __ffs(bits) - 1;
+                    bits &= bits - 1;
+                    const double a = __dmul_rn(lds_f64(f0_s + 256u * r), m.g);
+                    const int lo0 = lo_of<TPOW2>(a, m.d0, p.T);
+                    const int lo1 = lo_of<TPOW2>(a, m.d1, p.T);
+                    const int v0 = (int)lds_u8(m.rb + (uint32_t)lo0);
+                    // two candidate bins: (value difference, parity of the low bin); else: the base value
+                    const int pk = lo1 - lo0 == 1 ? 2 * ((int)lds_u8(m.rb + (uint32_t)lo1) - v0) + (lo0 & 1) : ITEM_GENERIC + v0;
+                    sts_item(items_s + 16u * __popc(own & ((1u << lane) - 1u)), a, pk,
+                             corr_s + 4u * (uint32_t)((r * 32 + lane) * CS));
+                }
+                __syncwarp();
+                const int n_items = __popc(own);
+#pragma unroll 2
+                for (int i = 0; i < n_items; ++i) {
+                    double a;
+                    int pk;
+                    uint32_t c_s;
+                    lds_item(items_s + 16u * i, a, pk, c_s);
+                    c_s += 4u * lane;
+                    if (pk < ITEM_GENERIC) {
+                        // a sky point reads the high bin iff its bin's parity differs from the low bin's
+                        const int dv = pk >> 1;
 #pragma unroll
                         for (int c = 0; c < SC; ++c) {
-                            const uint32_t lo = (uint32_t)lo_of<TPOW2>(a_b, lds_f64(dt_s + 256u * c), p.T);
-                            red_shared_add_if(c_s + 128u * c, dv, (lo ^ par) & 1u);
+                            const int lo = lo_of<TPOW2>(a, lds_f64(dt_s + 256u * c), p.T);
+                            red_shared_add(c_s + 128u * c, ((lo ^ pk) & 1) * dv);
                         }
                     } else {
+                        // ends several bins apart (wide sky blocks, high bands): every sky point looks its bin up
+                        const int v0 = pk - ITEM_GENERIC;
 #pragma unroll
                         for (int c = 0; c < SC; ++c) {
-                            const uint32_t lo = (uint32_t)lo_of<TPOW2>(a_b, lds_f64(dt_s + 256u * c), p.T);
-                            const int dv = (int)lds_u8(m.rb + lo) - v0_b;
-                            red_shared_add_if(c_s + 128u * c, dv, (uint32_t)dv);
+                            const uint32_t lo = (uint32_t)lo_of<TPOW2>(a, lds_f64(dt_s + 256u * c), p.T);
+                            red_shared_add(c_s + 128u * c, (int)lds_u8(m.rb + lo) - v0);
                         }
                     }
-                } while (mask);
-            }
+                }
+                __syncwarp();     // the list is rewritten by the next round
             }
         }
         __syncwarp();     // every lane has read slot sc before the next iteration refills it
