@@ -47,6 +47,7 @@ NCU_TRAFFIC_BYTES = {
     "cfg2:f32": (3275861000 + 6621440, "profiles/r1b_cfg2_sum_staged_full.md"),
     "cfg4": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
     "cfg4:f32": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
+    "cfg3:u8": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
 }
 
 
