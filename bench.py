@@ -246,6 +246,10 @@ def run_ours(args):
         h.set_option(tcw.TCW_OPT_SKY_BLOCK, args.sky_block)
     if args.f0_per_lane:
         h.set_option(tcw.TCW_OPT_F0_PER_LANE, args.f0_per_lane)
+    if args.chunk_rows:
+        h.set_option(tcw.TCW_OPT_CHUNK_ROWS, args.chunk_rows)
+    if args.stages:
+        h.set_option(tcw.TCW_OPT_STAGES, args.stages)
     out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
     out_best = torch.empty((n_groups, 2), dtype=torch.int32, device=dev)
 
@@ -338,7 +342,8 @@ def run_ours(args):
             "l2_policy": "inputs larger than L2 (no flush)" if w.spectrogram.nbytes > 126e6 else
                          "input smaller than L2 (stays L2-resident between steps; no flush)",
             "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"],
-            "sky_block": info["sky_block"]}),
+            "sky_block": info["sky_block"], "sft_chunks": info["chunks"], "chunk_rows": info["chunk_rows"],
+            "ring_stages": info["stages"]}),
         "templates_per_s": world * n_templates / (ms_step * 1e-3),
         "inband_lookups_per_s": world * inband / (ms_step * 1e-3),
         "inband_fraction": inband / nominal,
@@ -377,6 +382,8 @@ def main():
     ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged", "skyblock"])
     ap.add_argument("--sky-block", type=int, default=0, choices=[0, 64, 128])
     ap.add_argument("--f0-per-lane", type=int, default=0)
+    ap.add_argument("--chunk-rows", type=int, default=0, help="staged kernel: SFT rows per chunk (0 auto, -1 never)")
+    ap.add_argument("--stages", type=int, default=0, help="staged kernel: ring depth limit (0 auto)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -155,7 +155,12 @@ enum {
     TCW_OPT_TIMING = 1,     /* 1: record CUDA events around each stage of tcw_search           */
     TCW_OPT_F0_PER_LANE = 2,/* staged kernel: templates per lane, 4, 8 or 16 (tile = 32x that); 0 auto */
     TCW_OPT_STAGES = 3,     /* staged kernel: upper limit of the per-warp ring depth, 2..16; 0 auto  */
-    TCW_OPT_SKY_BLOCK = 4   /* sky-block kernel: sky points per block, 64 or 128; 0 auto             */
+    TCW_OPT_SKY_BLOCK = 4,  /* sky-block kernel: sky points per block, 64 or 128; 0 auto             */
+    TCW_OPT_CHUNK_ROWS = 5  /* staged kernel: SFT rows per chunk (rounded up to a multiple of 64).  A
+                               chunked search runs every (group, f0 tile) over one chunk of SFTs
+                               before any over the next, so the rows in use stay in L2; per-chunk
+                               partial sums are then added in ascending chunk order (fixed order).
+                               0 auto (chunk only spectrograms larger than L2), -1 never chunk    */
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 
@@ -172,10 +177,11 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
  * 3 sky-block),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
- * info[5] kernels launched by the call, info[6] ring depth per warp, info[7] sky points per
- * block (sky-block kernel, else 0).
+ * info[5] kernels launched by the call, info[6] ring depth per warp (slots of two SFT rows in the staged kernel), info[7] sky points per
+ * block (sky-block kernel, else 0), info[8] SFT chunks of the staged kernel (1 = not chunked),
+ * info[9] SFT rows per chunk.
  * Synchronises the search's stream. */
-int tcw_get_info(tcw_handle *h, long info[8]);
+int tcw_get_info(tcw_handle *h, long info[10]);
 
 #ifdef __cplusplus
 }

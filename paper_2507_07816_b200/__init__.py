@@ -23,6 +23,7 @@ __all__ = [
 TCW_OK, TCW_EINVAL, TCW_ENOMEM, TCW_ECUDA, TCW_EUNSUPPORTED = 0, -1, -2, -3, -4
 TCW_F32_POWER, TCW_U8_COUNT, TCW_BIT_COUNT = 0, 1, 2
 TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE, TCW_OPT_STAGES, TCW_OPT_SKY_BLOCK = 0, 1, 2, 3, 4
+TCW_OPT_CHUNK_ROWS = 5
 KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
@@ -259,11 +260,11 @@ class Handle:
         return tuple(float(x) for x in ms), int(n.value)
 
     def info(self) -> dict:
-        v = (ctypes.c_long * 8)()
+        v = (ctypes.c_long * 10)()
         _check(load_library().tcw_get_info(self._h, v))
         return dict(kernel={1: "gather", 2: "staged", 3: "skyblock"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
                     smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]),
-                    sky_block=int(v[7]))
+                    sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

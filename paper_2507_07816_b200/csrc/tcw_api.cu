@@ -45,6 +45,9 @@ int fail(int code, const char *fmt, ...)
 constexpr double C_LIGHT = 299792458.0;
 constexpr size_t SMEM_MAX = 227 * 1024;
 constexpr size_t TIMING_MAX = 4096;  // timed searches kept between two tcw_get_timing calls
+// staged kernel, SFT chunking: used when the spectrogram rows of the span exceed CHUNK_MIN_BYTES;
+// a chunk then holds about CHUNK_TARGET_BYTES of rows (well inside the 126 MB L2)
+constexpr double CHUNK_MIN_BYTES = 96e6, CHUNK_TARGET_BYTES = 48e6, CHUNK_SCRATCH_MAX = 16e9;
 
 template <typename T> struct DevBuf {
     T *p = nullptr;
@@ -100,6 +103,7 @@ struct tcw_handle {
     // grow-only scratch
     DevBuf<double> d_g, d_d, d_axes;
     DevBuf<unsigned char> d_partial, d_stat, d_best;
+    DevBuf<unsigned char> d_cpart, d_clive;  // chunked staged searches: per-chunk partial sums, live flags
     DevBuf<long> d_sel;
     DevBuf<double> d_dts, d_dmm;  // sky-block kernel: per-block Doppler rows and their {min, max}
     DevBuf<int> d_slot;           // sky index of each block slot
@@ -110,10 +114,11 @@ struct tcw_handle {
     cudaEvent_t ev_stage = nullptr;
     // options
     int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0, opt_sky = 0;
+    long opt_chunk = 0;  // SFT rows per chunk of the staged kernel: 0 auto, -1 never chunk
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
-    long info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 0};
     // last tables
     int tab_tau = 0, tab_brk = 0, tab_sky = 0;
     // device axis pointers of the last prepared grid
@@ -226,6 +231,8 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
     tcw::SumParams p;
     std::memset(&p, 0, sizeof p);
     p.spec = h->d_spec + h->pad_bytes;
+    p.spec_pad = h->d_spec;
+    p.pad16 = (int)(h->pad_bytes >> 4);
     p.pitch = h->pitch;
     p.n_sft = h->n_sft;
     p.n_bins = h->n_bins;
@@ -236,6 +243,9 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
     p.f0 = h->a_f0;
     p.n_f0 = g->n_f0;
     p.n_ab = g->n_tau * g->n_brk;
+    p.n_groups = (long)g->n_sky * g->n_tau * g->n_brk;
+    p.chunk_rows = h->n_sft;
+    p.n_chunks = 1;
     p.j_begin = (int)(std::lower_bound(h->ts.begin(), h->ts.end(), g->T0) - h->ts.begin());
     // |beta| <= |v| |n-hat| / c with | |n-hat| - 1 | <= 1e-6; a relative 1e-5 on beta is ample
     const double dmax = 1.0 + (h->vmax / C_LIGHT) * (1.0 + 1e-5) + 1e-15;
@@ -456,6 +466,8 @@ int tcw_destroy(tcw_handle *h)
     h->d_partial.release();
     h->d_stat.release();
     h->d_best.release();
+    h->d_cpart.release();
+    h->d_clive.release();
     h->d_sel.release();
     h->d_dts.release();
     h->d_dmm.release();
@@ -493,6 +505,10 @@ int tcw_set_option(tcw_handle *h, int key, long value)
     case TCW_OPT_SKY_BLOCK:
         if (value != 0 && value != 64 && value != 128) return fail(TCW_EINVAL, "TCW_OPT_SKY_BLOCK must be 0, 64 or 128");
         h->opt_sky = (int)value;
+        return TCW_OK;
+    case TCW_OPT_CHUNK_ROWS:
+        if (value < -1 || value > (1L << 30)) return fail(TCW_EINVAL, "TCW_OPT_CHUNK_ROWS must be -1, 0 or a row count");
+        h->opt_chunk = value;
         return TCW_OK;
     default: return fail(TCW_EINVAL, "unknown option %d", key);
     }
@@ -542,7 +558,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             const long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
             if (w_bins > tcw::PAD_BINS) continue;
             const int sb = slot_bytes_for(h->fmt_dev, w_bins);
-            for (int s = h->opt_stages ? h->opt_stages : 8; s >= 2; --s) {
+            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 4; s >= 2; --s) {
                 const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c]);
                 if (b <= SMEM_MAX / 2 - 1024 || (s == 2 && b <= SMEM_MAX)) {
                     kernel = 2; r = all[c]; stages = s; slot = sb; smem = b;
@@ -560,6 +576,25 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     p.slot_bytes = slot;
     const long n_partial = n_groups * p.n_tiles;
     long n_ctas = n_partial;
+    if (kernel == 2) {
+        // SFT chunks (slowest block index): the CTAs in flight then share a set of rows small enough
+        // to stay in L2 while every group reads it.  Only worth it when the rows do not fit anyway.
+        const long rows = h->n_sft - p.j_begin;
+        const double row_b = (double)(h->fmt_dev == tcw::FMT_F32 ? 4 : 1) * h->n_bins;
+        long c_rows = 0;
+        if (h->opt_chunk > 0) c_rows = h->opt_chunk;
+        else if (h->opt_chunk == 0 && rows * row_b > CHUNK_MIN_BYTES) c_rows = (long)(CHUNK_TARGET_BYTES / row_b);
+        if (c_rows > 0) {
+            c_rows = std::max<long>(64, (c_rows + 63) / 64 * 64);
+            long nc = (rows + c_rows - 1) / c_rows;
+            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * 4.0;
+            if (nc > 1 && nc <= 255 && scratch <= CHUNK_SCRATCH_MAX && nc * n_partial <= 2147483647L) {
+                p.chunk_rows = (int)c_rows;
+                p.n_chunks = (int)nc;
+                n_ctas = nc * n_partial;
+            }
+        }
+    }
     if (kernel == 3) {
         // sky points sorted by their Doppler shift at the middle SFT, cut into blocks of S
         const int S = 32 * sky_sc;
@@ -584,6 +619,12 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
         const size_t rows = (size_t)n_blocks * h->n_sft;
         if ((rc = h->d_dts.reserve(rows * 32 * sky_sc)) != TCW_OK) return rc;
         if ((rc = h->d_dmm.reserve(rows * 2)) != TCW_OK) return rc;
+    }
+    if (p.n_chunks > 1) {
+        if ((rc = h->d_cpart.reserve((size_t)p.n_chunks * n_groups * grid->n_f0 * 4)) != TCW_OK) return rc;
+        if ((rc = h->d_clive.reserve((size_t)p.n_chunks * n_partial)) != TCW_OK) return rc;
+        p.cpart = h->d_cpart.p;
+        p.clive = h->d_clive.p;
     }
     p.partial = h->d_partial.p;
     p.out_stat = out_stat;
@@ -616,6 +657,11 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, p, n_ctas, smem, st);
     else rc = launch_gather(h->fmt_dev, h->t_pow2, p, n_ctas, st);
     if (rc != TCW_OK) return rc;
+    if (p.n_chunks > 1) {
+        if (h->format == TCW_F32_POWER) tcw::chunk_reduce_kernel<float><<<(unsigned)n_partial, 256, 0, st>>>(p);
+        else tcw::chunk_reduce_kernel<int><<<(unsigned)n_partial, 256, 0, st>>>(p);
+        CUDA_TRY(cudaGetLastError());
+    }
     if (tm) CUDA_TRY(cudaEventRecord(ev[2], st));
     void *best_dst = out_best ? out_best : (void *)h->d_best.p;
     if (h->format == TCW_F32_POWER)
@@ -635,7 +681,9 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     h->info[3] = (long)smem;
     h->info[6] = stages;
     h->info[7] = 32 * sky_sc;
-    h->info[5] = kernel == 3 ? 5 : 4;  // doppler table, spin-down table, (sky-block table,) sum, best
+    h->info[5] = (kernel == 3 ? 5 : 4) + (p.n_chunks > 1 ? 1 : 0);  // doppler table, spin-down table, (sky-block table,) sum, (chunk reduce,) best
+    h->info[8] = p.n_chunks;
+    h->info[9] = p.chunk_rows;
     return TCW_OK;
 }
 
@@ -719,7 +767,7 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches)
     return TCW_OK;
 }
 
-int tcw_get_info(tcw_handle *h, long info[8])
+int tcw_get_info(tcw_handle *h, long info[10])
 {
     if (!h || !info) return fail(TCW_EINVAL, "NULL argument");
     if (!h->info[0]) return fail(TCW_EINVAL, "no search has been run on this handle");

@@ -47,6 +47,8 @@ __device__ __forceinline__ int bin_lo(double f0, double g, double Dp, double T)
 
 struct SumParams {
     const unsigned char *spec;  // bin 0 of row 0 of the library's copy (PAD_BINS zero bins before it)
+    const unsigned char *spec_pad;  // first byte of row 0 of that copy, left padding included (16-byte aligned)
+    int pad16;                  // bytes of the left padding / 16
     long pitch;                 // row pitch in bytes (multiple of 16), padding included
     int n_sft, n_bins, k_min;
     double T;
@@ -59,7 +61,11 @@ struct SumParams {
     void *out_stat;             // float32 / int32 [n_groups][n_f0] or NULL
     void *partial;              // {stat, f0_index} [n_groups][n_tiles]
     int n_tiles, tile;          // tiles per group, templates per tile
-    int stages, slot_bytes;     // staged kernel: ring depth per warp, bytes per ring slot
+    int stages, slot_bytes;     // staged kernel: ring depth per warp (slots of RB rows), bytes per staged row
+    long n_groups;              // n_sky * n_tau * n_brk
+    int chunk_rows, n_chunks;   // staged kernel: SFT rows per chunk, number of chunks (1 = whole span per CTA)
+    void *cpart;                // chunked: float32 / int32 [n_chunks][n_groups][n_f0] partial sums
+    unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
 };
 
@@ -176,27 +182,64 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 }
 
 // --------------------------------------------------------------------------- staged kernel
-constexpr int NW = 8;  // warps per CTA; warp w owns the rows j = j_begin + w + NW*n
+#ifndef TCW_NW
+#define TCW_NW 8
+#endif
+#ifndef TCW_RB
+#define TCW_RB 2
+#endif
+constexpr int NW = TCW_NW;      // warps per CTA; warp w owns the rows j = j0 + w + NW*n of the CTA's SFT chunk
 constexpr int STAGED_THREADS = 32 * NW;
+constexpr int RB = TCW_RB;      // SFT rows per ring slot (one mbarrier phase, one wait, one refill per RB rows)
+constexpr int META_ROWS = 64;   // per-warp ring of row metadata: two batches of 32 rows
+static_assert(RB == 1 || RB == 2 || RB == 4, "RB must divide the 32-row metadata batch");
 
-// What the lanes need to turn rint(x) into a shared-memory address of a staged row.
-struct __align__(16) RowMeta {
-    double g, Dp;   // spin-down factor and Doppler factor (times T_sft when it is a power of two)
-    uint32_t rb;    // f32: addr = rb + 4*rint(x)   u8: addr = rb + rint(x)
-    int live;       // 1 staged row, 0 row with no in-band bin (nothing staged), -1 no further rows
-    int pad[2];
+// What a warp needs to stage a row and to turn rint(x) into a shared-memory address of it.
+struct __align__(8) RowMeta {
+    double g, Dp;    // spin-down factor and Doppler factor (times T_sft when it is a power of two)
+    uint32_t off16;  // first staged byte of the row's window, in 16-byte units from SumParams::spec
+    int ab;          // low half: that byte relative to bin 0 of the row, in 16-byte units (signed);
+                     // high half: 16-byte units staged (> 0), 0 row with no in-band bin, -1 no further rows
 };
+constexpr int META_BYTES = (int)sizeof(RowMeta);
+static_assert(META_BYTES == 24, "RowMeta layout");
 
-// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*D] [slot NW*D*slot_bytes].  The slot region is
-// reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has completed; the
-// mbarrier words are never reused as data (they are updated through the async proxy, and a generic
-// store to the same bytes is not ordered against that without a proxy fence).
-__host__ __device__ inline size_t staged_header_bytes(int stages) { return (size_t)NW * stages * (8 + sizeof(RowMeta)); }
+// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*META_ROWS] [slot NW*D*RB*slot_bytes].  The slot
+// region is reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has
+// completed; the mbarrier words are never reused as data (they are updated through the async proxy,
+// and a generic store to the same bytes is not ordered against that without a proxy fence).
+__host__ __device__ inline size_t staged_header_bytes(int stages)
+{
+    return ((size_t)NW * stages * 8 + (size_t)NW * META_ROWS * sizeof(RowMeta) + 127) & ~(size_t)127;
+}
 __host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile)
 {
-    size_t ring = (size_t)NW * stages * (size_t)slot_bytes;
+    size_t ring = (size_t)NW * stages * RB * (size_t)slot_bytes;
     size_t red = (size_t)NW * tile * 4 + 128;
     return staged_header_bytes(stages) + (ring > red ? ring : red);
+}
+
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t p;
+    asm volatile("{ .reg .pred P; elect.sync _|P, 0xffffffff; selp.u32 %0, 1, 0, P; }" : "=r"(p));
+    return p != 0;
+}
+__device__ __forceinline__ void lds_v2(uint32_t a, uint32_t &x, uint32_t &y)
+{
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x), "=r"(y) : "r"(a));
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_f64s(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
 }
 
 template <int FMT, int R, bool TPOW2>
@@ -206,20 +249,43 @@ sum_staged_kernel(const SumParams p)
     typedef typename Acc<FMT>::type V;
     constexpr int F = 32 * R;                      // templates per tile
     constexpr int BPB = FMT == FMT_F32 ? 4 : 1;    // bytes per bin
+    constexpr uint32_t FULL = 0xffffffffu;
     extern __shared__ __align__(128) unsigned char smem[];
     const int D = p.stages;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint64_t *bars = (uint64_t *)smem + warp * D;
-    RowMeta *metas = (RowMeta *)(smem + (size_t)NW * D * 8) + warp * D;
+    RowMeta *meta = (RowMeta *)(smem + (size_t)NW * D * 8) + warp * META_ROWS;
     unsigned char *slots = smem + staged_header_bytes(D);
-    const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D * p.slot_bytes);
+    const uint32_t slot_stride = (uint32_t)(RB * p.slot_bytes);
+    const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D) * slot_stride;
+    const uint32_t slots_e = slots_s + (uint32_t)D * slot_stride;
     const uint32_t bars_s = smem_u32(bars);
+    const uint32_t meta_s = smem_u32(meta), meta_e = meta_s + META_ROWS * META_BYTES;
 
-    // heavy tiles (high f0 stays in band longest) are launched first
-    const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);
-    const long grp = blockIdx.x / p.n_tiles;
+    // block -> (SFT chunk, group, f0 tile).  Chunks are the slowest index: the CTAs in flight work
+    // on the same few hundred SFT rows, which therefore stay in L2 while every group reads them.
+    // Within a group heavy tiles (high f0 stays in band longest) are launched first.
+    long bq = blockIdx.x;
+    const int tile = p.n_tiles - 1 - (int)(bq % p.n_tiles);
+    bq /= p.n_tiles;
+    const long grp = bq % p.n_groups;
+    const int chunk = (int)(bq / p.n_groups);
     const int i0 = tile * F;
     const int i_last = min(i0 + F, p.n_f0) - 1;
+    const int j0 = p.j_begin + chunk * p.chunk_rows;
+    const int j1 = min(p.n_sft, j0 + p.chunk_rows);
+    const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
+    const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
+    const double f_first = p.f0[i0], f_last = p.f0[i_last];
+    const double below = (double)p.k_min - 1.0;
+
+    if (p.n_chunks > 1) {
+        // g decreases with j: a tile whose highest template is below the band at the chunk's first
+        // row, for the largest possible Doppler factor, has nothing to add in this chunk
+        const bool dead = f_last * __ldg(g + j0) * p.dmaxT < below;
+        if (threadIdx.x == 0) p.clive[((long)chunk * p.n_groups + grp) * p.n_tiles + tile] = dead ? 0 : 1;
+        if (dead) return;
+    }
 
     if (lane == 0) {
         for (int s = 0; s < D; ++s) mbar_init(bars_s + 8u * s, 1);
@@ -234,96 +300,116 @@ sum_staged_kernel(const SumParams p)
         acc[r] = 0;
         f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
     }
-    const double f_first = p.f0[i0], f_last = p.f0[i_last];
-    const double below = (double)p.k_min - 1.0;
-    const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
-    const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
-    const int jw = p.j_begin + warp;
-    const int n_rows = jw < p.n_sft ? (p.n_sft - jw + NW - 1) / NW : 0;
-    const unsigned char *spec_w = p.spec + (long)jw * p.pitch;
-    const long pitch_w = (long)NW * p.pitch;
+    const int jw = j0 + warp;
+    const int n_rows = jw < j1 ? (j1 - jw + NW - 1) / NW : 0;
+    const uint32_t pitch16 = (uint32_t)(p.pitch >> 4);
 
     // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp),
-    // and kept in the lane's registers until that lane stages its row.
-    double b_g = 0, b_Dp = 0;          // spin-down and Doppler factor of the lane's row
-    const unsigned char *b_src = nullptr;
-    uint32_t b_rb = 0;                 // -(BPB*k_min + first staged byte): added to the slot address
-    int b_bytes = 0;                   // bytes to stage
-    int b_live = -1;                   // 1 staged, 0 no in-band bin, -1 no further rows
-    double gn = 0, dn = 1;             // (g, D) of the lane's row in the NEXT batch, loaded ahead of use
+    // and written to the warp's metadata ring; (g, D) of the next batch are loaded ahead of use.
+    double gn = 0, dn = 1;
     if (lane < n_rows) { gn = __ldg(g + jw + NW * lane); dn = __ldg(d + jw + NW * lane); }
 
     auto compute_batch = [&](int m) {
         const int n = 32 * m + lane;
-        const double gj = gn, dj = dn;
+        RowMeta mt;
+        mt.g = gn;
+        mt.Dp = TPOW2 ? __dmul_rn(dn, p.T) : dn;
+        mt.off16 = 0;
+        mt.ab = -65536;
         if (n + 32 < n_rows) { gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32)); }
-        b_g = gj;
-        b_Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
-        b_live = -1;
-        b_bytes = 0;
-        // g decreases with j, so once the highest template of the tile is below the band for the
-        // largest possible Doppler factor, no later SFT can contribute.
-        if (n < n_rows && !(f_last * gj * p.dmaxT < below)) {
-            const int kf = bin_lo<TPOW2>(f_first, gj, b_Dp, p.T) - p.k_min;
-            const int kl = bin_lo<TPOW2>(f_last, gj, b_Dp, p.T) - p.k_min;
-            b_live = 0;
+        // once the highest template of the tile is below the band for the largest possible Doppler
+        // factor, no later SFT can contribute
+        if (n < n_rows && !(f_last * mt.g * p.dmaxT < below)) {
+            const int kf = bin_lo<TPOW2>(f_first, mt.g, mt.Dp, p.T) - p.k_min;
+            const int kl = bin_lo<TPOW2>(f_last, mt.g, mt.Dp, p.T) - p.k_min;
+            mt.ab = 0;
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = (BPB * kf) & ~15;                 // rounds towards -inf: may reach into the left padding
                 const int e_byte = (BPB * (kl + 1) + 15) & ~15;
                 if (e_byte - a_byte > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
                     atomicOr(p.status, 1);  // host-side window bound violated: never expected
                 } else {
-                    b_bytes = e_byte - a_byte;
-                    b_src = spec_w + (long)n * pitch_w + a_byte;
-                    b_rb = 0u - (uint32_t)(BPB * p.k_min + a_byte);
-                    b_live = 1;
+                    mt.off16 = (uint32_t)(jw + NW * n) * pitch16 + (uint32_t)(p.pad16 + (a_byte >> 4));
+                    mt.ab = (((e_byte - a_byte) >> 4) << 16) | ((a_byte >> 4) & 0xffff);
                 }
             }
         }
+        meta[n & (META_ROWS - 1)] = mt;
+        __syncwarp();
     };
 
-    int ni = 0, si = 0;   // next row to stage and its ring slot
-    // Stage row ni into slot si (or mark it skipped / final) and advance.  The lane that holds the
-    // row's metadata publishes it and issues the copy.
+    int ni = 0;                                  // next slot (RB rows) to stage
+    uint32_t bar_i = bars_s, slot_i = slots_s, meta_i = meta_s + 16u;
+    // Stage the rows RB*ni .. RB*ni + RB-1.  Every lane reads the rows' metadata and a warp-wide OR
+    // makes the copy operands warp-uniform (uniform registers); one elected lane then issues one TMA
+    // bulk copy per staged row, all counted on the slot's mbarrier.
     auto stage_next = [&]() {
-        if ((ni & 31) == 0) compute_batch(ni >> 5);
-        if (lane == (ni & 31)) {
-            const uint32_t slot_s = slots_s + (uint32_t)(si * p.slot_bytes);
-            RowMeta m;
-            m.g = b_g; m.Dp = b_Dp; m.rb = slot_s + b_rb; m.live = b_live; m.pad[0] = m.pad[1] = 0;
-            metas[si] = m;
-            if (b_live > 0) {
-                mbar_arrive_expect_tx(bars_s + 8u * si, (uint32_t)b_bytes);
-                bulk_g2s(slot_s, b_src, (uint32_t)b_bytes, bars_s + 8u * si);
-            } else if (b_live == 0) {
-                mbar_arrive(bars_s + 8u * si);   // every use of a slot completes one phase of its barrier
+        if ((ni & (32 / RB - 1)) == 0) compute_batch(ni / (32 / RB));
+        uint32_t off[RB];
+        int by[RB], tot = 0;
+#pragma unroll
+        for (int q = 0; q < RB; ++q) {
+            uint32_t o, ab;
+            lds_v2(meta_i + (uint32_t)(q * META_BYTES), o, ab);
+            off[q] = __reduce_or_sync(FULL, o);
+            by[q] = (int)__reduce_or_sync(FULL, ab) >> 16;
+            tot += max(by[q], 0);
+        }
+        if (elect_one()) {
+            if (tot > 0) {
+                mbar_arrive_expect_tx(bar_i, (uint32_t)tot << 4);
+#pragma unroll
+                for (int q = 0; q < RB; ++q)
+                    if (by[q] > 0)
+                        bulk_g2s(slot_i + (uint32_t)(q * p.slot_bytes), p.spec_pad + ((size_t)off[q] << 4),
+                                 (uint32_t)by[q] << 4, bar_i);
+            } else if (by[0] >= 0) {
+                mbar_arrive(bar_i);   // every use of a slot completes one phase of its barrier
             }
         }
-        __syncwarp();
         ++ni;
-        if (++si == D) si = 0;
+        bar_i += 8u; slot_i += slot_stride; meta_i += RB * META_BYTES;
+        if (slot_i == slots_e) { slot_i = slots_s; bar_i = bars_s; }
+        if (meta_i == meta_e + 16u) meta_i = meta_s + 16u;
     };
 
     for (int q = 0; q < D - 1; ++q) stage_next();
 
     uint32_t ph = 0;      // parity of the phase the slots complete in this pass over the ring
-    int sc = 0;
+    uint32_t bar_c = bars_s, slot_c = slots_s - (uint32_t)(BPB * p.k_min), meta_c = meta_s;
+    const uint32_t slots_ce = slots_e - (uint32_t)(BPB * p.k_min);
     for (;;) {
         stage_next();     // refills the slot consumed in the previous iteration
-        const RowMeta m = metas[sc];
-        if (m.live <= 0) {
-            if (m.live < 0) break;
-        } else {
-            mbar_wait(bars_s + 8u * sc, ph);
+        int ab[RB];
+        bool any = false;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], m.g, m.Dp, p.T);
-                if (FMT == FMT_F32) acc[r] += lds_f32(m.rb + 4u * lo);
-                else acc[r] += (V)lds_u8(m.rb + lo);
+        for (int q = 0; q < RB; ++q) {
+            ab[q] = (int)lds_u32(meta_c + (uint32_t)(q * META_BYTES) + 20u);
+            any |= ab[q] >= 65536;
+        }
+        if (ab[0] < 0) break;
+        if (any) {
+            mbar_wait(bar_c, ph);
+#pragma unroll
+            for (int q = 0; q < RB; ++q) {
+                if (ab[q] >= 65536) {
+                    const uint32_t mq = meta_c + (uint32_t)(q * META_BYTES);
+                    const double gj = lds_f64s(mq), Dp = lds_f64s(mq + 8u);
+                    // shared address of bin (0 - k_min) of the staged window
+                    const uint32_t rb = slot_c + (uint32_t)(q * p.slot_bytes) - (uint32_t)((int)((uint32_t)ab[q] << 16) >> 12);
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
+                        if (FMT == FMT_F32) acc[r] += lds_f32(rb + 4u * lo);
+                        else acc[r] += (V)lds_u8(rb + lo);
+                    }
+                }
             }
         }
-        __syncwarp();     // every lane has read slot sc before the next iteration refills it
-        if (++sc == D) { sc = 0; ph ^= 1u; }
+        __syncwarp();     // every lane has read the slot before the next iteration refills it
+        bar_c += 8u; slot_c += slot_stride; meta_c += RB * META_BYTES;
+        if (slot_c == slots_ce) { slot_c = slots_s - (uint32_t)(BPB * p.k_min); bar_c = bars_s; ph ^= 1u; }
+        if (meta_c == meta_e) meta_c = meta_s;
     }
 
     // ---------------- fixed-order combine of the warps' partial sums
@@ -334,18 +420,51 @@ sum_staged_kernel(const SumParams p)
     __syncthreads();
     V best_v = lowest<V>();
     int best_i = INT32_MAX;
+    V *dst = p.n_chunks > 1 ? (V *)p.cpart + ((long)chunk * p.n_groups + grp) * p.n_f0
+                            : (p.out_stat ? (V *)p.out_stat + grp * p.n_f0 : nullptr);
     for (int t = threadIdx.x; t < F; t += STAGED_THREADS) {
         const int i = i0 + t;
         if (i < p.n_f0) {
             V s = red[t];
 #pragma unroll
             for (int w = 1; w < NW; ++w) s += red[w * F + t];
+            if (dst) dst[i] = s;
+            argmax_step(best_v, best_i, s, i);
+        }
+    }
+    if (p.n_chunks > 1) return;   // chunk_reduce_kernel adds the chunks and finds the tile's best
+    __syncthreads();
+    block_best<V>(best_v, best_i, (Best<V> *)slots, (Best<V> *)p.partial + grp * p.n_tiles + tile);
+}
+
+// Chunked searches: out_stat[i] = sum over the live SFT chunks, in ascending chunk order, of the
+// chunk's partial sum; then the tile's (max, lowest index).  One block per (group, f0 tile).
+template <typename V>
+__global__ void __launch_bounds__(256)
+chunk_reduce_kernel(const SumParams p)
+{
+    __shared__ Best<V> red[8];
+    __shared__ unsigned char live[256];
+    const int tile = (int)(blockIdx.x % p.n_tiles);
+    const long grp = blockIdx.x / p.n_tiles;
+    for (int c = threadIdx.x; c < p.n_chunks; c += blockDim.x)
+        live[c] = p.clive[((long)c * p.n_groups + grp) * p.n_tiles + tile];
+    __syncthreads();
+    V best_v = lowest<V>();
+    int best_i = INT32_MAX;
+    const long stride = p.n_groups * (long)p.n_f0;
+    const V *src = (const V *)p.cpart + grp * p.n_f0;
+    for (int t = threadIdx.x; t < p.tile; t += blockDim.x) {
+        const int i = tile * p.tile + t;
+        if (i < p.n_f0) {
+            V s = 0;
+            for (int c = 0; c < p.n_chunks; ++c)
+                if (live[c]) s += src[c * stride + i];
             if (p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = s;
             argmax_step(best_v, best_i, s, i);
         }
     }
-    __syncthreads();
-    block_best<V>(best_v, best_i, (Best<V> *)slots, (Best<V> *)p.partial + grp * p.n_tiles + tile);
+    block_best<V>(best_v, best_i, red, (Best<V> *)p.partial + grp * p.n_tiles + tile);
 }
 
 // --------------------------------------------------------------------------- candidate reduction

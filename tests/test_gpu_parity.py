@@ -31,10 +31,11 @@ def tcw():
     return pkg
 
 
-def gpu_search(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0):
+def gpu_search(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0, chunk_rows=0):
     import torch
     with tcw.Handle.from_workload(w, host=host) as h:
         h.set_option(tcw.TCW_OPT_KERNEL, KERNELS[kernel])
+        h.set_option(tcw.TCW_OPT_CHUNK_ROWS, chunk_rows)
         h.set_option(tcw.TCW_OPT_F0_PER_LANE, f0_per_lane)
         h.set_option(tcw.TCW_OPT_SKY_BLOCK, sky_block)
         grid = tcw.Grid.of(w)
@@ -76,8 +77,8 @@ def assert_best_parity(w, n_f0, bs, bi, want_stat):
         assert np.array_equal(bi, idx)
 
 
-def full_parity(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0):
-    got, bs, bi, info = gpu_search(tcw, w, kernel, f0_per_lane, host, sky_block)
+def full_parity(tcw, w, kernel="auto", f0_per_lane=0, host=False, sky_block=0, chunk_rows=0):
+    got, bs, bi, info = gpu_search(tcw, w, kernel, f0_per_lane, host, sky_block, chunk_rows)
     ref = oracle.evaluate(w)
     assert_stat_parity(w, got, ref.stat)
     assert_best_parity(w, len(w.f0), bs, bi, ref.stat)
@@ -208,6 +209,34 @@ def test_ragged_edges_parity(tcw, fmt, kernel, r):
     assert (ref.n_inband == 0).any() and (ref.n_inband > 500).any()
     if kernel == "staged":
         assert info["tile"] == 32 * r and info["ctas"] == w.n_groups * -(-len(w.f0) // (32 * r))
+
+
+@pytest.mark.parametrize("fmt", ["f32", "u8", "bits"])
+@pytest.mark.parametrize("chunk_rows,r", [(64, 8), (128, 4), (320, 16), (4096, 8)])
+def test_sft_chunked_staged_parity(tcw, fmt, chunk_rows, r):
+    """TCW_OPT_CHUNK_ROWS: (chunk, group, tile) CTAs + chunk_reduce_kernel.  The ragged workload has
+    tiles that leave the band after a few chunks (dead CTAs), tiles never in band, a last chunk
+    shorter than the others, and T0 > 0."""
+    w = ragged_workload(fmt)
+    got, ref, info = full_parity(tcw, w, "staged", r, chunk_rows=chunk_rows)
+    rows = w.n_sft - int(np.searchsorted(w.timestamps, w.T0))
+    want_chunks = -(-rows // chunk_rows) if chunk_rows < rows else 1
+    assert info["chunks"] == want_chunks and info["ctas"] == want_chunks * w.n_groups * -(-len(w.f0) // (32 * r))
+    assert info["launches"] == (5 if want_chunks > 1 else 4)
+    # counts do not depend on the chunking at all; chunked power sums are run-to-run identical
+    again, _, _, _ = gpu_search(tcw, w, "staged", r, chunk_rows=chunk_rows)
+    assert np.array_equal(got, again)
+    if fmt != "f32":
+        plain, _, _, _ = gpu_search(tcw, w, "staged", r, chunk_rows=-1)
+        assert np.array_equal(got, plain)
+
+
+def test_sft_chunking_auto_only_for_large_spectrograms(tcw, cfg1):
+    _, _, _, info = gpu_search(tcw, cfg1, "staged")
+    assert info["chunks"] == 1
+    with tcw.Handle.from_workload(cfg1) as h:
+        with pytest.raises(tcw.TcwError):
+            h.set_option(tcw.TCW_OPT_CHUNK_ROWS, -2)
 
 
 def test_odd_band_start_and_tiny_sizes(tcw):
