@@ -46,8 +46,11 @@ constexpr double C_LIGHT = 299792458.0;
 constexpr size_t SMEM_MAX = 227 * 1024;
 constexpr size_t TIMING_MAX = 4096;  // timed searches kept between two tcw_get_timing calls
 // staged kernel, SFT chunking: used when the spectrogram rows of the span exceed CHUNK_MIN_BYTES;
-// a chunk then holds about CHUNK_TARGET_BYTES of rows (well inside the 126 MB L2)
-constexpr double CHUNK_MIN_BYTES = 96e6, CHUNK_TARGET_BYTES = 48e6, CHUNK_SCRATCH_MAX = 16e9;
+// a chunk then holds about CHUNK_TARGET_BYTES of rows (inside the 126 MB L2) and at most
+// CHUNK_MAX_ROWS rows (measured on B200: cfg4 is fastest at 1024-1280 rows of 80 KB, cfg2 at 2048
+// rows of 16 KB; _work sweeps of round 1d)
+constexpr double CHUNK_MIN_BYTES = 96e6, CHUNK_TARGET_BYTES = 80e6, CHUNK_SCRATCH_MAX = 16e9;
+constexpr long CHUNK_MAX_ROWS = 2048;
 
 template <typename T> struct DevBuf {
     T *p = nullptr;
@@ -550,7 +553,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             return fail(TCW_EUNSUPPORTED, "f0 spacing too wide for the sky-block kernel (window exceeds the row padding)");
     }
     // ---- otherwise: staged kernel with the largest tile whose window fits the row padding and
-    // whose ring (as deep as possible, up to opt_stages) still lets two CTAs share an SM
+    // whose ring still lets 12 warps share an SM
     if (!kernel && h->opt_kernel != 1) {
         const int all[3] = {16, 8, 4};
         for (int c = 0; c < 3 && !kernel; ++c) {
@@ -558,9 +561,11 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             const long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
             if (w_bins > tcw::PAD_BINS) continue;
             const int sb = slot_bytes_for(h->fmt_dev, w_bins);
-            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 4; s >= 2; --s) {
+            // rings two slots deep (a slot is RB rows) hide the L2 latency; three CTAs of four warps per SM
+            const int per_sm = 12 / tcw::NW;
+            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 2; s >= 2; --s) {
                 const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c]);
-                if (b <= SMEM_MAX / 2 - 1024 || (s == 2 && b <= SMEM_MAX)) {
+                if (b <= SMEM_MAX / per_sm - 1024 || (s == 2 && b <= SMEM_MAX)) {
                     kernel = 2; r = all[c]; stages = s; slot = sb; smem = b;
                     break;
                 }
@@ -583,7 +588,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
         const double row_b = (double)(h->fmt_dev == tcw::FMT_F32 ? 4 : 1) * h->n_bins;
         long c_rows = 0;
         if (h->opt_chunk > 0) c_rows = h->opt_chunk;
-        else if (h->opt_chunk == 0 && rows * row_b > CHUNK_MIN_BYTES) c_rows = (long)(CHUNK_TARGET_BYTES / row_b);
+        else if (h->opt_chunk == 0 && rows * row_b > CHUNK_MIN_BYTES) c_rows = std::min(CHUNK_MAX_ROWS, (long)(CHUNK_TARGET_BYTES / row_b));
         if (c_rows > 0) {
             c_rows = std::max<long>(64, (c_rows + 63) / 64 * 64);
             long nc = (rows + c_rows - 1) / c_rows;

@@ -183,10 +183,10 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 
 // --------------------------------------------------------------------------- staged kernel
 #ifndef TCW_NW
-#define TCW_NW 8
+#define TCW_NW 4
 #endif
 #ifndef TCW_RB
-#define TCW_RB 2
+#define TCW_RB 4
 #endif
 constexpr int NW = TCW_NW;      // warps per CTA; warp w owns the rows j = j0 + w + NW*n of the CTA's SFT chunk
 constexpr int STAGED_THREADS = 32 * NW;
@@ -243,7 +243,7 @@ __device__ __forceinline__ double lds_f64s(uint32_t a)
 }
 
 template <int FMT, int R, bool TPOW2>
-__global__ void __launch_bounds__(STAGED_THREADS, 2)
+__global__ void __launch_bounds__(STAGED_THREADS, 12 / NW)
 sum_staged_kernel(const SumParams p)
 {
     typedef typename Acc<FMT>::type V;
