@@ -217,7 +217,7 @@ int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaS
         CUDA_TRY(cudaGetLastError());
     }
     {
-        long total = (long)g->n_tau * g->n_brk * h->n_sft;
+        long total = (long)g->n_tau * h->n_sft;
         tcw::spindown_table_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(
             h->d_ts, h->n_sft, g->T0, h->a_tau, g->n_tau, h->a_brk, g->n_brk, h->d_g.p);
         CUDA_TRY(cudaGetLastError());

@@ -77,46 +77,35 @@ __device__ __forceinline__ dd dd_mul_d(dd a, double b)
 
 __device__ __forceinline__ dd dd_neg(dd a) { return {-a.hi, -a.lo}; }
 
-// exp of a double-double, |a| < 64.  a = k*ln2 + 512*r; exp(r) - 1 by its Taylor series
-// (|r| < 6.8e-4, nine terms reach 1e-34); nine squarings (1+s)^2 - 1 = 2s + s^2; scale by 2^k.
+#include "tcw_exp_tables.inc"
+
+// exp of a double-double.  a = k*ln2 + i1/64 + i2/4096 + r with |r| <= 2^-13:
+// exp(a) = 2^k * T1[i1] * T2[i2] * (1 + s), s = exp(r) - 1 = r + r^2/2 + r^3/6 + tail.  The three
+// leading terms are formed in double-double; the tail r^4/24 + ... + r^7/5040 is below 1e-17 and
+// plain binary64 carries it to 1e-33.  Tables: exp(i/64), exp(i/4096), i = -32..32, as hi + lo
+// (tcw_exp_tables.inc, written by gen_exp_tables.py).  Relative error about 2^-100.
 __device__ dd dd_exp(dd a)
 {
-    const dd LN2 = {0.6931471805599453, 2.3190468138462996e-17};
-    const dd INV_FACT[9] = {
-        {0.16666666666666666, 9.25185853854297e-18},     // 1/3!
-        {0.041666666666666664, 2.3129646346357427e-18},  // 1/4!
-        {0.008333333333333333, 1.1564823173178714e-19},  // 1/5!
-        {0.001388888888888889, -5.300543954373577e-20},  // 1/6!
-        {0.0001984126984126984, 1.7209558293420705e-22}, // 1/7!
-        {2.48015873015873e-05, 2.1511947866775882e-23},  // 1/8!
-        {2.7557319223985893e-06, -1.858393274046472e-22},// 1/9!
-        {2.755731922398589e-07, 2.3767714622250297e-23}, // 1/10!
-        {2.505210838544172e-08, -1.448814070935912e-24}, // 1/11!
-    };
-    double kd = rint(__dmul_rn(a.hi, 1.4426950408889634));
-    dd r = dd_add(a, dd_neg(dd_mul_d(LN2, kd)));
-    r.hi = __dmul_rn(r.hi, 0.001953125);  // exact: 1/512
-    r.lo = __dmul_rn(r.lo, 0.001953125);
-
-    dd p = dd_mul(r, r);                       // r^2
-    dd s = dd_add(r, {__dmul_rn(p.hi, 0.5), __dmul_rn(p.lo, 0.5)});
-    p = dd_mul(p, r);                          // r^3
-    dd t = dd_mul(p, INV_FACT[0]);
-#pragma unroll 1
-    for (int i = 1; i < 9; ++i) {
-        s = dd_add(s, t);
-        p = dd_mul(p, r);
-        t = dd_mul(p, INV_FACT[i]);
-    }
-    s = dd_add(s, t);
-#pragma unroll 1
-    for (int i = 0; i < 9; ++i) {
-        dd s2 = dd_mul(s, s);
-        s = dd_add({__dmul_rn(s.hi, 2.0), __dmul_rn(s.lo, 2.0)}, s2);
-    }
-    s = dd_add_d(s, 1.0);
-    int k = (int)kd;
-    return {ldexp(s.hi, k), ldexp(s.lo, k)};
+    const double kd = rint(__dmul_rn(a.hi, 1.4426950408889634));
+    dd r = dd_add(a, dd_neg(dd_mul_d(DD_LN2, kd)));          // |r| <= 0.347
+    const double i1 = rint(__dmul_rn(r.hi, 64.0));
+    r = dd_add_d(r, -__dmul_rn(i1, 0.015625));                // exact products: i/64, i/4096
+    const double i2 = rint(__dmul_rn(r.hi, 4096.0));
+    r = dd_add_d(r, -__dmul_rn(i2, 0.000244140625));
+    const dd r2 = dd_mul(r, r);
+    const dd r3 = dd_mul(r2, r);
+    const double x = r.hi;
+    // r^4/24 (1 + r/5 (1 + r/6 (1 + r/7))) with fused multiply-adds: accuracy, not a defined rounding, matters here
+    double tail = __fma_rn(x, 1.0 / 7.0, 1.0);
+    tail = __fma_rn(__dmul_rn(x, 1.0 / 6.0), tail, 1.0);
+    tail = __fma_rn(__dmul_rn(x, 0.2), tail, 1.0);
+    tail = __dmul_rn(__dmul_rn(__dmul_rn(r2.hi, r2.hi), 1.0 / 24.0), tail);
+    dd s = dd_add(r, {__dmul_rn(r2.hi, 0.5), __dmul_rn(r2.lo, 0.5)});
+    s = dd_add(s, dd_add_d(dd_mul(r3, DD_SIXTH), tail));
+    const dd m = dd_mul(EXP_T1[(int)i1 + 32], EXP_T2[(int)i2 + 32]);
+    const dd v = dd_add(m, dd_mul(m, s));
+    const int k = (int)kd;
+    return {ldexp(v.hi, k), ldexp(v.lo, k)};
 }
 
 // log of a positive double b: y0 = log(b) in binary64, then one Newton step on exp(y) = b in
@@ -129,34 +118,31 @@ __device__ dd dd_log_d(double b)
     return dd_add_d(c, y0);
 }
 
-// RN(b^e) for b >= 1 (the base of eq. (1) for t >= T0) and finite e.
-__device__ double pow_rn(double b, double e)
-{
-    dd l = dd_log_d(b);
-    dd r = dd_exp(dd_mul_d(l, e));
-    return r.hi;  // normalised: |lo| <= ulp(hi)/2, so hi is the nearest double of hi + lo
-}
-
-// g[a][b][j], one thread per entry.  Entries with t_j < T0 are 0 (outside the span, reading Q2).
+// g[a][b][j] = RN(base^e): one thread per (tau_a, SFT j) evaluates log(base) once in double-double
+// and one exp per braking index.  exp returns a normalised pair (|lo| <= ulp(hi)/2), so hi is the
+// nearest double of hi + lo.  Entries with t_j < T0 are 0 (outside the span, reading Q2).
 __global__ void __launch_bounds__(128)
 spindown_table_kernel(const double *__restrict__ ts, int n_sft, double T0,
                       const double *__restrict__ tau, int n_tau,
                       const double *__restrict__ brk, int n_brk, double *__restrict__ g_out)
 {
     long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    long total = (long)n_tau * n_brk * n_sft;
+    long total = (long)n_tau * n_sft;
     if (q >= total) return;
-    int j = (int)(q % n_sft);
-    int b = (int)((q / n_sft) % n_brk);
-    int a = (int)(q / ((long)n_sft * n_brk));
-    double t = ts[j];
+    const int j = (int)(q % n_sft);
+    const int a = (int)(q / n_sft);
+    double *out = g_out + (long)a * n_brk * n_sft + j;
+    const double t = ts[j];
     if (t < T0) {
-        g_out[q] = 0.0;
+        for (int b = 0; b < n_brk; ++b) out[(long)b * n_sft] = 0.0;
         return;
     }
-    double base = __dadd_rn(__ddiv_rn(__dsub_rn(t, T0), tau[a]), 1.0);
-    double e = __ddiv_rn(1.0, __dsub_rn(1.0, brk[b]));
-    g_out[q] = pow_rn(base, e);
+    const double base = __dadd_rn(__ddiv_rn(__dsub_rn(t, T0), tau[a]), 1.0);
+    const dd l = dd_log_d(base);
+    for (int b = 0; b < n_brk; ++b) {
+        const double e = __ddiv_rn(1.0, __dsub_rn(1.0, brk[b]));
+        out[(long)b * n_sft] = dd_exp(dd_mul_d(l, e)).hi;
+    }
 }
 
 // D = 1 + ((vx*nx + vy*ny) + vz*nz)/c, eq. (2): five single binary64 operations, never fused.
