@@ -61,6 +61,14 @@ def lib() -> ctypes.CDLL:
                                 ctypes.c_long, ctypes.c_void_p,
                                 ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                 ctypes.c_void_p, ctypes.c_int]
+        L.tcwo_eval_weighted.restype = ctypes.c_int
+        L.tcwo_eval_weighted.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_long, ctypes.c_int, ctypes.c_int,
+                                         ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_double,
+                                         ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int, dp,
+                                         ctypes.c_void_p, ctypes.c_double, ctypes.c_double,
+                                         ctypes.c_long, ctypes.c_void_p,
+                                         ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                         ctypes.c_int]
         L.tcwo_best_f64.restype = None
         L.tcwo_best_f64.argtypes = [dp, ctypes.c_long, ctypes.c_int, dp, ctypes.c_void_p]
         L.tcwo_best_i64.restype = None
@@ -158,6 +166,43 @@ def evaluate(w, sel=None, want_k: bool = False, literal: bool = False) -> Oracle
     if rc != 0:
         raise ValueError("tcwo_eval: bad arguments")
     return OracleResult(stat_i if stat_i is not None else stat_f, n_in, n_amb, k)
+
+
+@dataclass
+class WeightedResult:
+    s: np.ndarray      # float64 [n_sel]  weighted statistic  sum_j w_j * spectrogram[j][k_j]
+    w1: np.ndarray     # float64 [n_sel]  sum of the weights of the in-band SFTs
+    w2: np.ndarray     # float64 [n_sel]  sum of their squares
+    psi: np.ndarray    # float64 [n_sel]  critical ratio, eq. (4)
+
+
+def evaluate_weighted(w, weights, mean1: float, var1: float, sel=None, literal: bool = False) -> WeightedResult:
+    """Weighted statistic and critical ratio (eq. (4)) of workload `w` with
+    float32 weights [n_sky][n_sft] (None = all ones) and per-bin noise moments (mean1, var1)."""
+    spec = np.ascontiguousarray(w.spectrogram)
+    fmt = FORMATS[w.fmt]
+    pitch = spec.strides[0]
+    ts, vel = _f64(w.timestamps), _f64(w.velocities)
+    f0, tau, brk, sky = _f64(w.f0), _f64(w.tau), _f64(w.brk), _f64(w.sky)
+    n_templates = len(sky) * len(tau) * len(brk) * len(f0)
+    if weights is not None:
+        weights = np.ascontiguousarray(weights, dtype=np.float32)
+        assert weights.shape == (len(sky), w.n_sft), weights.shape
+    if sel is None:
+        n_sel, sel_arr, sel_ptr = n_templates, None, None
+    else:
+        sel_arr = np.ascontiguousarray(sel, dtype=np.int64)
+        n_sel, sel_ptr = len(sel_arr), sel_arr.ctypes.data
+    out = [np.empty(n_sel, dtype=np.float64) for _ in range(4)]
+    rc = lib().tcwo_eval_weighted(spec.ctypes.data, fmt, pitch, int(w.n_sft), int(w.n_bins),
+                                  float(w.f_min), float(w.T_sft), _dp(ts), _dp(vel), float(w.T0),
+                                  len(f0), _dp(f0), len(tau), _dp(tau), len(brk), _dp(brk), len(sky), _dp(sky),
+                                  weights.ctypes.data if weights is not None else None,
+                                  float(mean1), float(var1), n_sel, sel_ptr,
+                                  *[o.ctypes.data for o in out], int(bool(literal)))
+    if rc != 0:
+        raise ValueError("tcwo_eval_weighted: bad arguments")
+    return WeightedResult(*out)
 
 
 def best(stat: np.ndarray, n_f0: int):

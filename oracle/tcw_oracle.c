@@ -215,6 +215,86 @@ int tcwo_eval(const void *spectrogram, int format, long pitch_bytes, int n_sft, 
     return bad ? -1 : 0;
 }
 
+/* ---- NEXT-1: weighted statistic and critical ratio ------------------
+ *
+ * "The power and number count statistics are weighed taking into account the antenna patterns
+ * and changing noise floors ... summed across the data bins selected by the track"
+ * and the critical ratio of eq. (4):  Psi_s = (s - <s>) / sigma_s.
+ * The weight formula is in the paper's ref. [14], which is not available: weights are an INPUT,
+ * w[s][j] >= 0 per (sky point, SFT) (reading Q21).  Per template, over the SFTs j
+ * with t_j >= T0 whose bin k_j (steps 1-9 above) is in band:
+ *
+ *  11  s   += (double) w[s][j] * (double) spectrogram[j][k_j]
+ *  12  W1  += (double) w[s][j]
+ *  13  W2  += (double) w[s][j] * (double) w[s][j]
+ *  14  <s>      = mean1 * W1          mean of a weighted sum of independent bins of mean mean1
+ *  15  sigma_s  = sqrt(var1 * W2)     its standard deviation (reading Q14: sigma_s is the
+ *                                     standard deviation), bins of variance var1
+ *  16  Psi      = (s - <s>) / sigma_s,  0 when W2 == 0 (no in-band SFT carries weight)
+ *
+ * (mean1, var1) are the per-bin noise moments of the spectrogram: (1, 1) for normalised power
+ * rho ~ Exp(1); (p, p(1-p)) with p = exp(-threshold) for the number count nu.  weights == NULL
+ * means w = 1.  Outputs (any may be NULL): s_out, w1_out, w2_out, psi_out, each [n_sel].
+ * `literal` as in tcwo_eval.
+ * Parity status: pinned (tests/test_oracle_pins.py, section "weighted"). */
+int tcwo_eval_weighted(const void *spectrogram, int format, long pitch_bytes, int n_sft, int n_bins,
+                       double f_min, double T_sft, const double *ts, const double *vel, double T0,
+                       int n_f0, const double *f0, int n_tau, const double *tau, int n_brk,
+                       const double *brk, int n_sky, const double *sky, const float *weights,
+                       double mean1, double var1, long n_sel, const long *sel, double *s_out,
+                       double *w1_out, double *w2_out, double *psi_out, int literal)
+{
+    if (!spectrogram || !ts || !vel || !f0 || !tau || !brk || !sky) return -1;
+    if (format < 0 || format > 2 || n_sft <= 0 || n_bins <= 0) return -1;
+    const unsigned char *spec = (const unsigned char *)spectrogram;
+    const long k_min = tcwo_kmin(f_min, T_sft);
+    const long n_templates = (long)n_sky * n_tau * n_brk * n_f0;
+    double *gtab = NULL;
+    if (!literal) { /* as in tcwo_eval: the same tcwo_spindown, evaluated once per (tau, n, j) */
+        gtab = (double *)malloc(sizeof(double) * (size_t)n_tau * n_brk * n_sft);
+        if (!gtab) return -1;
+        tcwo_spindown_table(n_sft, ts, T0, n_tau, tau, n_brk, brk, gtab, NULL);
+    }
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (long q = 0; q < n_sel; ++q) {
+        long lin = sel ? sel[q] : q;
+        if (lin < 0 || lin >= n_templates) {
+#pragma omp atomic write
+            bad = 1;
+            continue;
+        }
+        int i = (int)(lin % n_f0);
+        long grp = lin / n_f0;
+        int b = (int)(grp % n_brk);
+        int a = (int)((grp / n_brk) % n_tau);
+        int s = (int)(grp / ((long)n_brk * n_tau));
+        double sum = 0.0, W1 = 0.0, W2 = 0.0;
+        for (int j = 0; j < n_sft; ++j) {
+            if (ts[j] < T0) continue;
+            double g = literal ? tcwo_spindown(ts[j], T0, tau[a], brk[b])
+                               : gtab[((long)a * n_brk + b) * n_sft + j];
+            double D = tcwo_doppler(vel + 3 * (long)j, sky + 3 * (long)s);
+            double x = tcwo_track_x(f0[i], g, D, T_sft);
+            long k = tcwo_bin(x, k_min);
+            if (k >= 0 && k < n_bins) {
+                double w = weights ? (double)weights[(long)s * n_sft + j] : 1.0;
+                sum += w * spec_value(spec, format, pitch_bytes, j, k);
+                W1 += w;
+                W2 += w * w;
+            }
+        }
+        double mean = mean1 * W1;
+        double sigma = sqrt(var1 * W2);
+        if (s_out) s_out[q] = sum;
+        if (w1_out) w1_out[q] = W1;
+        if (w2_out) w2_out[q] = W2;
+        if (psi_out) psi_out[q] = W2 > 0.0 ? (sum - mean) / sigma : 0.0;
+    }
+    free(gtab);
+    return bad ? -1 : 0;
+}
+
 /* Candidate reduction (north_star (d)): per group of n_f0 consecutive entries,
  * the maximum and the lowest f0 index attaining it. */
 void tcwo_best_f64(const double *stat, long n_groups, int n_f0, double *best_val, int32_t *best_idx)

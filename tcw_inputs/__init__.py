@@ -15,4 +15,5 @@ from .configs import (  # noqa: F401
     make_workload,
     pack_bits,
     sky_vector,
+    synthetic_weights,
 )

@@ -98,6 +98,28 @@ def pack_bits(nu: np.ndarray) -> np.ndarray:
     return np.ascontiguousarray(by).view("<u4").reshape(n_sft, n_words)
 
 
+def synthetic_weights(sky: np.ndarray, timestamps: np.ndarray, seed: int) -> np.ndarray:
+    """Stand-in for the weights of the paper's ref. [14] ("antenna patterns and changing noise
+    floors"): float32 [n_sky][n_sft], positive, mean 1 along each row.
+
+    w[s][j] = F_s(t_j) / S_j with a smooth sidereal-day antenna-pattern-like modulation
+    F_s(t) = 0.55 + 0.35 cos(theta(t) - alpha_s) cos(delta_s) + 0.10 sin(2 (theta(t) - alpha_s)),
+    theta(t) = 2 pi t / 86164.0905 s, (alpha_s, delta_s) the sky point's right ascension and
+    declination, and a seeded per-SFT noise-floor factor S_j ~ U[0.7, 1.3]^2.  Input synthesis
+    only: the search treats the weights as given numbers."""
+    sky = np.asarray(sky, dtype=np.float64)
+    t = np.asarray(timestamps, dtype=np.float64)
+    rng = np.random.Generator(np.random.PCG64(seed + 7919))
+    alpha = np.arctan2(sky[:, 1], sky[:, 0])[:, None]
+    cdel = np.sqrt(np.maximum(0.0, 1.0 - sky[:, 2] ** 2))[:, None]
+    th = (2.0 * np.pi / 86164.0905) * t[None, :] - alpha
+    F = 0.55 + 0.35 * np.cos(th) * cdel + 0.10 * np.sin(2.0 * th)
+    S = rng.uniform(0.7, 1.3, size=len(t)) ** 2
+    w = F / S[None, :]
+    w /= w.mean(axis=1, keepdims=True)
+    return np.ascontiguousarray(w, dtype=np.float32)
+
+
 # --------------------------------------------------------------------------- workload
 @dataclass
 class Workload:
