@@ -43,11 +43,15 @@ C_LIGHT = 299792458.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the gather-accumulate kernel,
 # from the committed `ncu --set full` capture named beside each entry (None = not captured).
 NCU_TRAFFIC_BYTES = {
-    "cfg2": (3275861000 + 6621440, "profiles/r1b_cfg2_sum_staged_full.md"),
-    "cfg2:f32": (3275861000 + 6621440, "profiles/r1b_cfg2_sum_staged_full.md"),
-    "cfg4": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
-    "cfg4:f32": (467270546000 + 55483136, "profiles/r1b_cfg4_sum_staged_full.md"),
+    "cfg2": (164000256 + 10949120, "profiles/r1d_cfg2_sum_full.md"),
+    "cfg2:f32": (164000256 + 10949120, "profiles/r1d_cfg2_sum_full.md"),
+    "cfg4": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
+    "cfg4:f32": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
+    "cfg3": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
     "cfg3:u8": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
+    "cfg3:bits": (145765888 + 305440256, "profiles/r1d_cfg3bits_sky_full.md"),
+    "cfg5": (803163136 + 1557699000, "profiles/r1d_cfg5_sky_full.md"),
+    "cfg5:bits": (803163136 + 1557699000, "profiles/r1d_cfg5_sky_full.md"),
 }
 
 
