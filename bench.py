@@ -24,6 +24,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -257,9 +258,25 @@ def run_ours(args):
     out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
     out_best = torch.empty((n_groups, 2), dtype=torch.int32, device=dev)
 
+    weighted = None
+    if args.weighted:
+        # NEXT-1: the weighted statistic + critical ratio (tcw_search_weighted) on the same workload,
+        # device-resident weights; the step then produces Psi, s and the per-group best Psi
+        mean1, var1 = (1.0, 1.0) if w.fmt == "f32" else (math.exp(-1.6), math.exp(-1.6) * (1 - math.exp(-1.6)))
+        wts = torch.from_numpy(tcw_inputs.synthetic_weights(w.sky, w.timestamps, w.seed)).to(dev)
+        out_psi = torch.empty(out_stat.shape, dtype=torch.float32, device=dev)
+        out_stat = torch.empty(out_stat.shape, dtype=torch.float32, device=dev)
+        weighted = dict(mean1=mean1, var1=var1)
+
+    def step():
+        if weighted:
+            h.search_weighted(grid, wts, mean1, var1, out_psi, out_stat, out_best)
+        else:
+            h.search(grid, out_stat, out_best)
+
     sampler = ClockSampler(local)
     for _ in range(args.warmup):
-        h.search(grid, out_stat, out_best)
+        step()
     h.set_option(tcw.TCW_OPT_TIMING, 1)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -268,7 +285,7 @@ def run_ours(args):
     t_host0 = time.perf_counter()
     ev0.record(stream)
     for _ in range(args.steps):
-        h.search(grid, out_stat, out_best)
+        step()
     ev1.record(stream)
     barrier()
     t_host = time.perf_counter() - t_host0
@@ -347,7 +364,9 @@ def run_ours(args):
                          "input smaller than L2 (stays L2-resident between steps; no flush)",
             "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"],
             "sky_block": info["sky_block"], "sft_chunks": info["chunks"], "chunk_rows": info["chunk_rows"],
-            "ring_stages": info["stages"]}),
+            "ring_stages": info["stages"],
+            **({"statistic": "weighted s + critical ratio Psi (tcw_search_weighted), device-resident weights; "
+                             "the e2e leg below times the unweighted tcw_search_host"} if weighted else {})}),
         "templates_per_s": world * n_templates / (ms_step * 1e-3),
         "inband_lookups_per_s": world * inband / (ms_step * 1e-3),
         "inband_fraction": inband / nominal,
@@ -391,6 +410,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--weighted", action="store_true",
+                    help="time tcw_search_weighted (weighted statistic + critical ratio, NEXT-1) instead of tcw_search")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps

@@ -123,6 +123,50 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host,
                     void *stream);
 
+/* ---- weighted statistic and critical ratio -------------------
+ *
+ * "The power and number count statistics are weighed taking into account the antenna patterns
+ *  and changing noise floors that modulate the signal amplitude.  The statistics are then summed
+ *  across the data bins selected by the track. ... we compute the critical ratio
+ *  Psi_s = (s - <s>)/sigma_s"  (eq. (4)).
+ * The weight formula is in the paper's ref. [14] and is not restated there, so weights are an
+ * input (reading Q21).  Over the SFTs j with t_j >= T0 whose bin k_j is in band:
+ *
+ *     s   = sum_j w[s][j] * spectrogram[j][k_j]        W1 = sum_j w[s][j]      W2 = sum_j w[s][j]^2
+ *     <s> = mean1 * W1      sigma_s = sqrt(var1 * W2)      Psi = (s - <s>)/sigma_s,  0 if W2 == 0
+ *
+ * (the mean and the standard deviation of a weighted sum of independent bins of mean mean1 and
+ * variance var1; reading Q14: sigma_s is the standard deviation).
+ *
+ *  weights   [n_sky][n_sft] float32, row s for sky point s of the grid; HOST or DEVICE pointer
+ *            (copied with cudaMemcpyDefault on `stream`: a pageable host array may be freed when
+ *            the call returns, a pinned or device array once the stream has passed the call).
+ *            NULL = all ones.  Values are not checked: negative or non-finite weights propagate.
+ *  mean1     per-bin noise mean of the spectrogram elements: 1 for normalised power rho ~ Exp(1),
+ *            p = exp(-threshold) for number counts nu = (rho > threshold).
+ *  var1      per-bin noise variance: 1 for rho, p(1-p) for nu.  TCW_EINVAL unless finite and > 0.
+ */
+typedef struct {
+    const float *weights;
+    double mean1, var1;
+} tcw_weighting;
+
+/* tcw_search_weighted -- weighted statistic, critical ratio and the per-group best critical ratio.
+ *
+ *  out_psi   DEVICE, float32 [n_sky][n_tau][n_brk][n_f0], Psi per template; may be NULL.
+ *  out_stat  DEVICE, float32 (for every spectrogram format), the weighted statistic s; may be NULL.
+ *  out_best  DEVICE, [n_sky*n_tau*n_brk] tcw_best_f32 = { max over f0 of Psi, lowest f0 index
+ *            attaining it }; may be NULL (not all three NULL).
+ *  stream    as for tcw_search (asynchronous).
+ *
+ * s accumulates in float32 (fused multiply-add of weight and element) in the fixed order of
+ * tcw_search; W1 and W2 in float64, except over the SFTs in which a 32*R-template tile straddles
+ * a band edge, where they are counted per template in float32.  Runs on the TMA-staged or the
+ * gather kernel (one sky point at a time: weights differ between sky points, so the sky-block
+ * kernel does not apply; forcing that kernel through tcw_set_option gives TCW_EUNSUPPORTED). */
+int tcw_search_weighted(tcw_handle *h, const tcw_grid *grid, const tcw_weighting *weighting,
+                        float *out_psi, float *out_stat, tcw_best_f32 *out_best, void *stream);
+
 /* tcw_destroy -- free the handle and everything it owns.  NULL is a no-op returning TCW_OK. */
 int tcw_destroy(tcw_handle *h);
 

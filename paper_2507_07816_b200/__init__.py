@@ -28,7 +28,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_search", "tcw_search_host", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -47,6 +47,10 @@ class _CGrid(ctypes.Structure):
         ("n_brk", ctypes.c_int), ("brk", ctypes.POINTER(ctypes.c_double)),
         ("n_sky", ctypes.c_int), ("sky", ctypes.POINTER(ctypes.c_double)),
     ]
+
+
+class _CWeighting(ctypes.Structure):
+    _fields_ = [("weights", ctypes.c_void_p), ("mean1", ctypes.c_double), ("var1", ctypes.c_double)]
 
 
 _lib = None
@@ -70,6 +74,8 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_search.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
     L.tcw_search_host.restype = ci
     L.tcw_search_host.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
+    L.tcw_search_weighted.restype = ci
+    L.tcw_search_weighted.argtypes = [vp, ctypes.POINTER(_CGrid), ctypes.POINTER(_CWeighting), vp, vp, vp, vp]
     L.tcw_destroy.restype = ci
     L.tcw_destroy.argtypes = [vp]
     L.tcw_last_error.restype = ctypes.c_char_p
@@ -203,6 +209,43 @@ class Handle:
                             out_stat.data_ptr() if out_stat is not None else None,
                             out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
         return out_stat, out_best
+
+    def search_weighted(self, grid: Grid, weights, mean1: float, var1: float, out_psi=None, out_stat=None,
+                        out_best=None, want_psi: bool = True, want_stat: bool = True, want_best: bool = True,
+                        stream=None):
+        """tcw_search_weighted.  `weights`: None (all ones), a host numpy float32 array or a CUDA
+        float32 tensor, [n_sky][n_sft].  Returns (psi, stat, best): float32 CUDA tensors
+        [n_sky][n_tau][n_brk][n_f0] and an int32 tensor [n_groups][2] (column 0: bits of the float32
+        maximum of Psi, column 1: f0 index).  Asynchronous."""
+        import torch
+        L = load_library()
+        dev = torch.device("cuda", torch.cuda.current_device())
+        shape = (len(grid.sky), len(grid.tau), len(grid.brk), len(grid.f0))
+        if out_psi is None and want_psi:
+            out_psi = torch.empty(shape, dtype=torch.float32, device=dev)
+        if out_stat is None and want_stat:
+            out_stat = torch.empty(shape, dtype=torch.float32, device=dev)
+        if out_best is None and want_best:
+            out_best = torch.empty((grid.n_groups, 2), dtype=torch.int32, device=dev)
+        if weights is None:
+            wptr = None
+        elif isinstance(weights, np.ndarray):
+            weights = np.ascontiguousarray(weights, dtype=np.float32)
+            wptr = weights.ctypes.data
+        else:
+            weights = weights.contiguous()
+            if weights.dtype != torch.float32:
+                raise ValueError("weights must be float32")
+            wptr = weights.data_ptr()
+        if weights is not None and tuple(weights.shape) != (len(grid.sky), self.n_sft):
+            raise ValueError("weights must be [n_sky][n_sft]")
+        cg = grid._c()
+        cw = _CWeighting(wptr, float(mean1), float(var1))
+        _check(L.tcw_search_weighted(self._h, ctypes.byref(cg), ctypes.byref(cw),
+                                     out_psi.data_ptr() if out_psi is not None else None,
+                                     out_stat.data_ptr() if out_stat is not None else None,
+                                     out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
+        return out_psi, out_stat, out_best
 
     def search_host(self, grid: Grid, out_stat: np.ndarray | None = None, out_best: np.ndarray | None = None,
                     want_stat: bool = True, stream=None):

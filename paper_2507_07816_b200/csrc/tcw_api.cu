@@ -107,6 +107,7 @@ struct tcw_handle {
     DevBuf<double> d_g, d_d, d_axes;
     DevBuf<unsigned char> d_partial, d_stat, d_best;
     DevBuf<unsigned char> d_cpart, d_clive;  // chunked staged searches: per-chunk partial sums, live flags
+    DevBuf<float> d_w, d_cw;                 // weighted searches: weights [n_sky][n_sft]; per-chunk sums of w and w^2
     DevBuf<long> d_sel;
     DevBuf<double> d_dts, d_dmm;  // sky-block kernel: per-block Doppler rows and their {min, max}
     DevBuf<int> d_slot;           // sky index of each block slot
@@ -278,47 +279,57 @@ int slot_bytes_for(int fmt_dev, long w_bins)
     return b > (1L << 30) ? (1 << 30) : (int)b;
 }
 
-template <int FMT, int R, bool P2>
+template <int FMT, int R, bool P2, bool WGT>
 int launch_staged_t(const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    auto kern = tcw::sum_staged_kernel<FMT, R, P2>;
+    auto kern = tcw::sum_staged_kernel<FMT, R, P2, WGT>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)n_ctas, tcw::STAGED_THREADS, smem, st>>>(p);
     CUDA_TRY(cudaGetLastError());
     return TCW_OK;
 }
 
-template <int FMT, bool P2>
+template <int FMT, bool P2, bool WGT>
 int launch_staged_r(int r, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
     switch (r) {
-    case 16: return launch_staged_t<FMT, 16, P2>(p, n_ctas, smem, st);
-    case 8: return launch_staged_t<FMT, 8, P2>(p, n_ctas, smem, st);
-    default: return launch_staged_t<FMT, 4, P2>(p, n_ctas, smem, st);
+    case 16: return launch_staged_t<FMT, 16, P2, WGT>(p, n_ctas, smem, st);
+    case 8: return launch_staged_t<FMT, 8, P2, WGT>(p, n_ctas, smem, st);
+    default: return launch_staged_t<FMT, 4, P2, WGT>(p, n_ctas, smem, st);
     }
 }
 
-int launch_staged(int fmt, int r, bool p2, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
+template <bool WGT>
+int launch_staged_w(int fmt, int r, bool p2, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
     if (fmt == tcw::FMT_F32)
-        return p2 ? launch_staged_r<tcw::FMT_F32, true>(r, p, n_ctas, smem, st)
-                  : launch_staged_r<tcw::FMT_F32, false>(r, p, n_ctas, smem, st);
-    return p2 ? launch_staged_r<tcw::FMT_U8, true>(r, p, n_ctas, smem, st)
-              : launch_staged_r<tcw::FMT_U8, false>(r, p, n_ctas, smem, st);
+        return p2 ? launch_staged_r<tcw::FMT_F32, true, WGT>(r, p, n_ctas, smem, st)
+                  : launch_staged_r<tcw::FMT_F32, false, WGT>(r, p, n_ctas, smem, st);
+    return p2 ? launch_staged_r<tcw::FMT_U8, true, WGT>(r, p, n_ctas, smem, st)
+              : launch_staged_r<tcw::FMT_U8, false, WGT>(r, p, n_ctas, smem, st);
 }
 
-template <int FMT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
+int launch_staged(int fmt, int r, bool p2, bool wgt, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    if (p2) tcw::sum_gather_kernel<FMT, true><<<(unsigned)n_ctas, 128, 0, st>>>(p);
-    else tcw::sum_gather_kernel<FMT, false><<<(unsigned)n_ctas, 128, 0, st>>>(p);
+    return wgt ? launch_staged_w<true>(fmt, r, p2, p, n_ctas, smem, st)
+               : launch_staged_w<false>(fmt, r, p2, p, n_ctas, smem, st);
+}
+
+template <int FMT, bool WGT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
+{
+    if (p2) tcw::sum_gather_kernel<FMT, true, WGT><<<(unsigned)n_ctas, 128, 0, st>>>(p);
+    else tcw::sum_gather_kernel<FMT, false, WGT><<<(unsigned)n_ctas, 128, 0, st>>>(p);
     CUDA_TRY(cudaGetLastError());
     return TCW_OK;
 }
 
-int launch_gather(int fmt, bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
+int launch_gather(int fmt, bool p2, bool wgt, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
 {
-    return fmt == tcw::FMT_F32 ? launch_gather_t<tcw::FMT_F32>(p2, p, n_ctas, st)
-                               : launch_gather_t<tcw::FMT_U8>(p2, p, n_ctas, st);
+    if (wgt)
+        return fmt == tcw::FMT_F32 ? launch_gather_t<tcw::FMT_F32, true>(p2, p, n_ctas, st)
+                                   : launch_gather_t<tcw::FMT_U8, true>(p2, p, n_ctas, st);
+    return fmt == tcw::FMT_F32 ? launch_gather_t<tcw::FMT_F32, false>(p2, p, n_ctas, st)
+                               : launch_gather_t<tcw::FMT_U8, false>(p2, p, n_ctas, st);
 }
 
 template <int R, int SC, bool P2>
@@ -471,6 +482,8 @@ int tcw_destroy(tcw_handle *h)
     h->d_best.release();
     h->d_cpart.release();
     h->d_clive.release();
+    h->d_w.release();
+    h->d_cw.release();
     h->d_sel.release();
     h->d_dts.release();
     h->d_dmm.release();
@@ -517,12 +530,20 @@ int tcw_set_option(tcw_handle *h, int key, long value)
     }
 }
 
-int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_best, void *stream)
+// The search proper.  wt == NULL: the plain track sum (tcw_search).  Otherwise the weighted statistic,
+// its critical ratio and the per-group maximum of the critical ratio (tcw_search_weighted).
+static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting *wt, void *out_stat, float *out_psi,
+                       void *out_best, void *stream)
 {
     if (!h) return fail(TCW_EINVAL, "handle is NULL");
     int rc = validate_grid(h, grid);
     if (rc != TCW_OK) return rc;
-    if (!out_stat && !out_best) return fail(TCW_EINVAL, "out_stat and out_best are both NULL");
+    const bool wgt = wt != nullptr;
+    if (!out_stat && !out_best && !out_psi) return fail(TCW_EINVAL, "every output pointer is NULL");
+    if (wgt && (!std::isfinite(wt->mean1) || !(wt->var1 > 0) || !std::isfinite(wt->var1)))
+        return fail(TCW_EINVAL, "weighting needs a finite mean1 and a finite var1 > 0");
+    if (wgt && h->opt_kernel == 3)
+        return fail(TCW_EUNSUPPORTED, "the sky-block kernel does not serve weighted searches (weights depend on the sky point)");
     cudaStream_t st = (cudaStream_t)stream;
     const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
 
@@ -534,7 +555,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     // ---- launch plan, count formats with many sky points: the sky-block kernel (tcw_skyblock.cuh)
     if (h->opt_kernel == 3 && h->fmt_dev != tcw::FMT_U8)
         return fail(TCW_EUNSUPPORTED, "the sky-block kernel serves the count formats only");
-    if (h->fmt_dev == tcw::FMT_U8 && (h->opt_kernel == 3 || (h->opt_kernel == 0 && grid->n_sky >= 16))) {
+    if (!wgt && h->fmt_dev == tcw::FMT_U8 && (h->opt_kernel == 3 || (h->opt_kernel == 0 && grid->n_sky >= 16))) {
         const int sc = h->opt_sky == 128 ? 4 : 2, rr = sc == 2 ? 16 : 8, S = 32 * sc;
         // two sky points differ by |D_s - D_s'| <= 2 vmax / c whatever the block holds
         const double spread = grid->f0[grid->n_f0 - 1] * h->T * 2.0 * (h->vmax / C_LIGHT) * (1.0 + 1e-5);
@@ -564,7 +585,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
             // rings two slots deep (a slot is RB rows) hide the L2 latency; three CTAs of four warps per SM
             const int per_sm = 12 / tcw::NW;
             for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 2; s >= 2; --s) {
-                const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c]);
+                const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c], wgt);
                 if (b <= SMEM_MAX / per_sm - 1024 || (s == 2 && b <= SMEM_MAX)) {
                     kernel = 2; r = all[c]; stages = s; slot = sb; smem = b;
                     break;
@@ -592,7 +613,7 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
         if (c_rows > 0) {
             c_rows = std::max<long>(64, (c_rows + 63) / 64 * 64);
             long nc = (rows + c_rows - 1) / c_rows;
-            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * 4.0;
+            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * (wgt ? 12.0 : 4.0);
             if (nc > 1 && nc <= 255 && scratch <= CHUNK_SCRATCH_MAX && nc * n_partial <= 2147483647L) {
                 p.chunk_rows = (int)c_rows;
                 p.n_chunks = (int)nc;
@@ -630,9 +651,26 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
         if ((rc = h->d_clive.reserve((size_t)p.n_chunks * n_partial)) != TCW_OK) return rc;
         p.cpart = h->d_cpart.p;
         p.clive = h->d_clive.p;
+        if (wgt) {
+            const size_t plane = (size_t)p.n_chunks * n_groups * grid->n_f0;
+            if ((rc = h->d_cw.reserve(2 * plane)) != TCW_OK) return rc;
+            p.cw1 = h->d_cw.p;
+            p.cw2 = h->d_cw.p + plane;
+        }
     }
     p.partial = h->d_partial.p;
     p.out_stat = out_stat;
+    if (wgt) {
+        p.mean1 = wt->mean1;
+        p.var1 = wt->var1;
+        p.out_psi = out_psi;
+        if (wt->weights) {
+            const size_t n_w = (size_t)grid->n_sky * h->n_sft;
+            if ((rc = h->d_w.reserve(n_w)) != TCW_OK) return rc;
+            CUDA_TRY(cudaMemcpyAsync(h->d_w.p, wt->weights, n_w * sizeof(float), cudaMemcpyDefault, st));
+            p.wtab = h->d_w.p;
+        }
+    }
 
     const bool tm = h->opt_timing != 0 && h->timing_n < TIMING_MAX;
     cudaEvent_t *ev = nullptr;
@@ -659,17 +697,18 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     }
     if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
     if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
-    else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, p, n_ctas, smem, st);
-    else rc = launch_gather(h->fmt_dev, h->t_pow2, p, n_ctas, st);
+    else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, wgt, p, n_ctas, smem, st);
+    else rc = launch_gather(h->fmt_dev, h->t_pow2, wgt, p, n_ctas, st);
     if (rc != TCW_OK) return rc;
     if (p.n_chunks > 1) {
-        if (h->format == TCW_F32_POWER) tcw::chunk_reduce_kernel<float><<<(unsigned)n_partial, 256, 0, st>>>(p);
-        else tcw::chunk_reduce_kernel<int><<<(unsigned)n_partial, 256, 0, st>>>(p);
+        if (wgt) tcw::chunk_reduce_kernel<float, true><<<(unsigned)n_partial, 256, 0, st>>>(p);
+        else if (h->format == TCW_F32_POWER) tcw::chunk_reduce_kernel<float, false><<<(unsigned)n_partial, 256, 0, st>>>(p);
+        else tcw::chunk_reduce_kernel<int, false><<<(unsigned)n_partial, 256, 0, st>>>(p);
         CUDA_TRY(cudaGetLastError());
     }
     if (tm) CUDA_TRY(cudaEventRecord(ev[2], st));
     void *best_dst = out_best ? out_best : (void *)h->d_best.p;
-    if (h->format == TCW_F32_POWER)
+    if (wgt || h->format == TCW_F32_POWER)
         tcw::best_kernel<float><<<(unsigned)((n_groups + 127) / 128), 128, 0, st>>>(
             (const tcw::Best<float> *)h->d_partial.p, n_groups, p.n_tiles, (tcw::Best<float> *)best_dst);
     else
@@ -690,6 +729,19 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
     h->info[8] = p.n_chunks;
     h->info[9] = p.chunk_rows;
     return TCW_OK;
+}
+
+int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_best, void *stream)
+{
+    if (h && grid && !out_stat && !out_best) return fail(TCW_EINVAL, "out_stat and out_best are both NULL");
+    return search_impl(h, grid, nullptr, out_stat, nullptr, out_best, stream);
+}
+
+int tcw_search_weighted(tcw_handle *h, const tcw_grid *grid, const tcw_weighting *weighting, float *out_psi,
+                        float *out_stat, tcw_best_f32 *out_best, void *stream)
+{
+    if (h && !weighting) return fail(TCW_EINVAL, "weighting is NULL");
+    return search_impl(h, grid, weighting, out_stat, out_psi, out_best, stream);
 }
 
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host, void *stream)

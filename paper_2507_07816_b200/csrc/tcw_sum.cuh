@@ -67,10 +67,25 @@ struct SumParams {
     void *cpart;                // chunked: float32 / int32 [n_chunks][n_groups][n_f0] partial sums
     unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
+    // weighted search (tcw_search_weighted; eq. (4)): s = sum w_j * spectrogram[j][k_j]
+    const float *wtab;          // [n_sky][n_sft] weights, or NULL (all ones)
+    double mean1, var1;         // per-bin noise mean and variance of the spectrogram elements
+    float *out_psi;             // critical ratio [n_groups][n_f0]
+    float *cw1, *cw2;           // chunked: per-chunk sums of w and w^2 over the in-band SFTs, laid out like cpart
 };
 
 template <int FMT> struct Acc { typedef int type; };
 template <> struct Acc<FMT_F32> { typedef float type; };
+// accumulator of a search: weighted sums are float32 whatever the spectrogram format
+template <int FMT, bool WGT> struct AccW { typedef typename Acc<FMT>::type type; };
+template <int FMT> struct AccW<FMT, true> { typedef float type; };
+
+// Psi = (s - <s>)/sigma_s with <s> = mean1*W1, sigma_s^2 = var1*W2 (eq. (4)); 0 when W2 = 0.
+__device__ __forceinline__ float critical_ratio(float s, double W1, double W2, double mean1, double var1)
+{
+    if (!(W2 > 0.0)) return 0.0f;
+    return (float)(((double)s - mean1 * W1) / sqrt(var1 * W2));
+}
 
 template <typename V> __device__ __forceinline__ V lowest();
 template <> __device__ __forceinline__ float lowest<float>() { return -__int_as_float(0x7f800000); }
@@ -106,11 +121,11 @@ __device__ __forceinline__ void block_best(V v, int i, Best<V> *red, Best<V> *ds
 }
 
 // --------------------------------------------------------------------------- gather kernel
-template <int FMT, bool TPOW2>
+template <int FMT, bool TPOW2, bool WGT>
 __global__ void __launch_bounds__(128)
 sum_gather_kernel(const SumParams p)
 {
-    typedef typename Acc<FMT>::type V;
+    typedef typename AccW<FMT, WGT>::type V;
     __shared__ Best<V> red[4];
     const int tile = blockIdx.x % p.n_tiles;
     const long grp = blockIdx.x / p.n_tiles;
@@ -119,17 +134,30 @@ sum_gather_kernel(const SumParams p)
     const double f0 = p.f0[valid ? i : p.n_f0 - 1];
     const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
     const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
+    const float *wr = WGT && p.wtab ? p.wtab + (grp / p.n_ab) * (long)p.n_sft : nullptr;
     V acc = 0;
+    double W1 = 0, W2 = 0;
     for (int j = p.j_begin; j < p.n_sft; ++j) {
         double Dp = TPOW2 ? __dmul_rn(d[j], p.T) : d[j];
         int k = bin_lo<TPOW2>(f0, g[j], Dp, p.T) - p.k_min;
         if ((unsigned)k < (unsigned)p.n_bins) {
             const unsigned char *row = p.spec + (long)j * p.pitch;
-            if (FMT == FMT_F32) acc += ((const float *)row)[k];
+            if (WGT) {
+                const float w = wr ? wr[j] : 1.0f;
+                const float v = FMT == FMT_F32 ? ((const float *)row)[k] : (float)row[k];
+                acc = __fmaf_rn(w, v, acc);
+                W1 += (double)w;
+                W2 += (double)w * (double)w;
+            } else if (FMT == FMT_F32) acc += ((const float *)row)[k];
             else acc += (V)row[k];
         }
     }
-    if (valid && p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = acc;
+    if (WGT) {
+        const float psi = critical_ratio(acc, W1, W2, p.mean1, p.var1);
+        if (valid && p.out_stat) ((float *)p.out_stat)[grp * p.n_f0 + i] = acc;
+        if (valid && p.out_psi) p.out_psi[grp * p.n_f0 + i] = psi;
+        acc = psi;
+    } else if (valid && p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = acc;
     block_best<V>(valid ? acc : lowest<V>(), valid ? i : INT32_MAX, red,
                   (Best<V> *)p.partial + grp * p.n_tiles + tile);
 }
@@ -201,22 +229,32 @@ struct __align__(8) RowMeta {
     int ab;          // low half: that byte relative to bin 0 of the row, in 16-byte units (signed);
                      // high half: 16-byte units staged (> 0), 0 row with no in-band bin, -1 no further rows
 };
-constexpr int META_BYTES = (int)sizeof(RowMeta);
-static_assert(META_BYTES == 24, "RowMeta layout");
+// weighted search: the row's weight, and whether every template of the tile is in band in this row
+// (then the weight sums W1, W2 advance by the same amount for the whole tile: one warp-uniform add)
+struct __align__(8) RowMetaW {
+    double g, Dp;
+    uint32_t off16;
+    int ab;
+    float w;
+    int full;
+};
+template <bool WGT> struct MetaT { typedef RowMeta type; };
+template <> struct MetaT<true> { typedef RowMetaW type; };
+static_assert(sizeof(RowMeta) == 24 && sizeof(RowMetaW) == 32, "RowMeta layout");
 
 // dynamic shared memory: [mbarrier NW*D] [RowMeta NW*META_ROWS] [slot NW*D*RB*slot_bytes].  The slot
 // region is reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has
 // completed; the mbarrier words are never reused as data (they are updated through the async proxy,
 // and a generic store to the same bytes is not ordered against that without a proxy fence).
-__host__ __device__ inline size_t staged_header_bytes(int stages)
+__host__ __device__ inline size_t staged_header_bytes(int stages, bool wgt)
 {
-    return ((size_t)NW * stages * 8 + (size_t)NW * META_ROWS * sizeof(RowMeta) + 127) & ~(size_t)127;
+    return ((size_t)NW * stages * 8 + (size_t)NW * META_ROWS * (wgt ? sizeof(RowMetaW) : sizeof(RowMeta)) + 127) & ~(size_t)127;
 }
-__host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile)
+__host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile, bool wgt)
 {
     size_t ring = (size_t)NW * stages * RB * (size_t)slot_bytes;
-    size_t red = (size_t)NW * tile * 4 + 128;
-    return staged_header_bytes(stages) + (ring > red ? ring : red);
+    size_t red = (size_t)NW * tile * 4 * (wgt ? 3 : 1) + (size_t)NW * 16 + 128;
+    return staged_header_bytes(stages, wgt) + (ring > red ? ring : red);
 }
 
 __device__ __forceinline__ bool elect_one()
@@ -242,11 +280,13 @@ __device__ __forceinline__ double lds_f64s(uint32_t a)
     return v;
 }
 
-template <int FMT, int R, bool TPOW2>
+template <int FMT, int R, bool TPOW2, bool WGT>
 __global__ void __launch_bounds__(STAGED_THREADS, 12 / NW)
 sum_staged_kernel(const SumParams p)
 {
-    typedef typename Acc<FMT>::type V;
+    typedef typename AccW<FMT, WGT>::type V;
+    typedef typename MetaT<WGT>::type RowMeta;     // shadows tcw::RowMeta
+    constexpr int META_BYTES = (int)sizeof(RowMeta);
     constexpr int F = 32 * R;                      // templates per tile
     constexpr int BPB = FMT == FMT_F32 ? 4 : 1;    // bytes per bin
     constexpr uint32_t FULL = 0xffffffffu;
@@ -255,7 +295,7 @@ sum_staged_kernel(const SumParams p)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint64_t *bars = (uint64_t *)smem + warp * D;
     RowMeta *meta = (RowMeta *)(smem + (size_t)NW * D * 8) + warp * META_ROWS;
-    unsigned char *slots = smem + staged_header_bytes(D);
+    unsigned char *slots = smem + staged_header_bytes(D, WGT);
     const uint32_t slot_stride = (uint32_t)(RB * p.slot_bytes);
     const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D) * slot_stride;
     const uint32_t slots_e = slots_s + (uint32_t)D * slot_stride;
@@ -276,6 +316,7 @@ sum_staged_kernel(const SumParams p)
     const int j1 = min(p.n_sft, j0 + p.chunk_rows);
     const double *g = p.gtab + (grp % p.n_ab) * (long)p.n_sft;
     const double *d = p.dtab + (grp / p.n_ab) * (long)p.n_sft;
+    const float *wr = WGT && p.wtab ? p.wtab + (grp / p.n_ab) * (long)p.n_sft : nullptr;
     const double f_first = p.f0[i0], f_last = p.f0[i_last];
     const double below = (double)p.k_min - 1.0;
 
@@ -295,10 +336,15 @@ sum_staged_kernel(const SumParams p)
 
     V acc[R];
     double f0r[R];
+    // weighted: sums of w and w^2 over the in-band SFTs.  Rows in which the whole tile is in band
+    // advance a warp-uniform float64 pair; only rows that straddle a band edge are counted per lane.
+    float w1p[WGT ? R : 1], w2p[WGT ? R : 1];
+    double W1u = 0, W2u = 0;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         acc[r] = 0;
         f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
+        if (WGT) w1p[r] = w2p[r] = 0.0f;
     }
     const int jw = j0 + warp;
     const int n_rows = jw < j1 ? (j1 - jw + NW - 1) / NW : 0;
@@ -307,7 +353,11 @@ sum_staged_kernel(const SumParams p)
     // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp),
     // and written to the warp's metadata ring; (g, D) of the next batch are loaded ahead of use.
     double gn = 0, dn = 1;
-    if (lane < n_rows) { gn = __ldg(g + jw + NW * lane); dn = __ldg(d + jw + NW * lane); }
+    float wn = 1.0f;
+    if (lane < n_rows) {
+        gn = __ldg(g + jw + NW * lane); dn = __ldg(d + jw + NW * lane);
+        if (WGT && wr) wn = __ldg(wr + jw + NW * lane);
+    }
 
     auto compute_batch = [&](int m) {
         const int n = 32 * m + lane;
@@ -316,7 +366,11 @@ sum_staged_kernel(const SumParams p)
         mt.Dp = TPOW2 ? __dmul_rn(dn, p.T) : dn;
         mt.off16 = 0;
         mt.ab = -65536;
-        if (n + 32 < n_rows) { gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32)); }
+        if constexpr (WGT) { mt.w = wn; mt.full = 0; }
+        if (n + 32 < n_rows) {
+            gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32));
+            if (WGT && wr) wn = __ldg(wr + jw + NW * (n + 32));
+        }
         // once the highest template of the tile is below the band for the largest possible Doppler
         // factor, no later SFT can contribute
         if (n < n_rows && !(f_last * mt.g * p.dmaxT < below)) {
@@ -331,6 +385,7 @@ sum_staged_kernel(const SumParams p)
                 } else {
                     mt.off16 = (uint32_t)(jw + NW * n) * pitch16 + (uint32_t)(p.pad16 + (a_byte >> 4));
                     mt.ab = (((e_byte - a_byte) >> 4) << 16) | ((a_byte >> 4) & 0xffff);
+                    if constexpr (WGT) mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
                 }
             }
         }
@@ -397,11 +452,38 @@ sum_staged_kernel(const SumParams p)
                     const double gj = lds_f64s(mq), Dp = lds_f64s(mq + 8u);
                     // shared address of bin (0 - k_min) of the staged window
                     const uint32_t rb = slot_c + (uint32_t)(q * p.slot_bytes) - (uint32_t)((int)((uint32_t)ab[q] << 16) >> 12);
+                    if constexpr (WGT) {
+                        const float wj = lds_f32(mq + 24u);
+                        if (lds_u32(mq + 28u)) {          // warp-uniform: the whole tile is in band
+                            const double wd = (double)wj;
+                            W1u = __dadd_rn(W1u, wd);
+                            W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
-                        if (FMT == FMT_F32) acc[r] += lds_f32(rb + 4u * lo);
-                        else acc[r] += (V)lds_u8(rb + lo);
+                            for (int r = 0; r < R; ++r) {
+                                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
+                                const float v = FMT == FMT_F32 ? lds_f32(rb + 4u * lo) : (float)lds_u8(rb + lo);
+                                acc[r] = __fmaf_rn(wj, v, acc[r]);
+                            }
+                        } else {
+                            const float wj2 = __fmul_rn(wj, wj);
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
+                                const float v = FMT == FMT_F32 ? lds_f32(rb + 4u * lo) : (float)lds_u8(rb + lo);
+                                acc[r] = __fmaf_rn(wj, v, acc[r]);
+                                if (lo - (uint32_t)p.k_min < (uint32_t)p.n_bins) {
+                                    w1p[r] = __fadd_rn(w1p[r], wj);
+                                    w2p[r] = __fadd_rn(w2p[r], wj2);
+                                }
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
+                            if (FMT == FMT_F32) acc[r] += lds_f32(rb + 4u * lo);
+                            else acc[r] += (V)lds_u8(rb + lo);
+                        }
                     }
                 }
             }
@@ -417,11 +499,21 @@ sum_staged_kernel(const SumParams p)
     V *red = (V *)slots;
 #pragma unroll
     for (int r = 0; r < R; ++r) red[warp * F + r * 32 + lane] = acc[r];
+    if constexpr (WGT) {
+        float *rw = (float *)slots + NW * F;          // [2][NW][F] per-lane sums, then [NW][2] float64 uniform sums
+        double *wu = (double *)((float *)slots + 3 * NW * F);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            rw[warp * F + r * 32 + lane] = w1p[r];
+            rw[(NW + warp) * F + r * 32 + lane] = w2p[r];
+        }
+        if (lane == 0) { wu[2 * warp] = W1u; wu[2 * warp + 1] = W2u; }
+    }
     __syncthreads();
     V best_v = lowest<V>();
     int best_i = INT32_MAX;
-    V *dst = p.n_chunks > 1 ? (V *)p.cpart + ((long)chunk * p.n_groups + grp) * p.n_f0
-                            : (p.out_stat ? (V *)p.out_stat + grp * p.n_f0 : nullptr);
+    const long cbase = ((long)chunk * p.n_groups + grp) * p.n_f0;
+    V *dst = p.n_chunks > 1 ? (V *)p.cpart + cbase : (p.out_stat ? (V *)p.out_stat + grp * p.n_f0 : nullptr);
     for (int t = threadIdx.x; t < F; t += STAGED_THREADS) {
         const int i = i0 + t;
         if (i < p.n_f0) {
@@ -429,6 +521,23 @@ sum_staged_kernel(const SumParams p)
 #pragma unroll
             for (int w = 1; w < NW; ++w) s += red[w * F + t];
             if (dst) dst[i] = s;
+            if constexpr (WGT) {
+                const float *rw = (const float *)slots + NW * F;
+                const double *wu = (const double *)((const float *)slots + 3 * NW * F);
+                double W1 = 0, W2 = 0;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) {
+                    W1 += wu[2 * w] + (double)rw[w * F + t];
+                    W2 += wu[2 * w + 1] + (double)rw[(NW + w) * F + t];
+                }
+                if (p.n_chunks > 1) {
+                    p.cw1[cbase + i] = (float)W1;
+                    p.cw2[cbase + i] = (float)W2;
+                } else {
+                    s = critical_ratio(s, W1, W2, p.mean1, p.var1);
+                    if (p.out_psi) p.out_psi[grp * p.n_f0 + i] = s;
+                }
+            }
             argmax_step(best_v, best_i, s, i);
         }
     }
@@ -439,7 +548,7 @@ sum_staged_kernel(const SumParams p)
 
 // Chunked searches: out_stat[i] = sum over the live SFT chunks, in ascending chunk order, of the
 // chunk's partial sum; then the tile's (max, lowest index).  One block per (group, f0 tile).
-template <typename V>
+template <typename V, bool WGT>
 __global__ void __launch_bounds__(256)
 chunk_reduce_kernel(const SumParams p)
 {
@@ -461,6 +570,16 @@ chunk_reduce_kernel(const SumParams p)
             for (int c = 0; c < p.n_chunks; ++c)
                 if (live[c]) s += src[c * stride + i];
             if (p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = s;
+            if constexpr (WGT) {
+                double W1 = 0, W2 = 0;
+                for (int c = 0; c < p.n_chunks; ++c)
+                    if (live[c]) {
+                        W1 += (double)p.cw1[c * stride + grp * p.n_f0 + i];
+                        W2 += (double)p.cw2[c * stride + grp * p.n_f0 + i];
+                    }
+                s = critical_ratio(s, W1, W2, p.mean1, p.var1);
+                if (p.out_psi) p.out_psi[grp * p.n_f0 + i] = s;
+            }
             argmax_step(best_v, best_i, s, i);
         }
     }

@@ -50,11 +50,15 @@ def test_library_is_sm100a_and_has_tma_bulk_copies():
         pytest.skip("cuobjdump not available")
     elf = subprocess.run([cuobjdump, "-lelf", tcw.library_path()], capture_output=True, text=True).stdout
     assert "sm_100a" in elf
-    sass = subprocess.run([cuobjdump, "-sass", "-fun", "_ZN3tcw17sum_staged_kernelILi0ELi8ELb1EEEvNS_9SumParamsE",
-                           tcw.library_path()], capture_output=True, text=True).stdout
-    assert "UBLKCP" in sass and "SYNCS" in sass
-    assert "DFMA" not in sass            # the index chain is never contracted
-    assert "DMUL" in sass and "DADD" in sass
+    for wgt in ("0", "1"):               # plain and weighted instantiations
+        sass = subprocess.run([cuobjdump, "-sass", "-fun", f"_ZN3tcw17sum_staged_kernelILi0ELi8ELb1ELb{wgt}EEEvNS_9SumParamsE",
+                               tcw.library_path()], capture_output=True, text=True).stdout
+        assert "UBLKCP" in sass and "SYNCS" in sass
+        # the index chain is never contracted; the weighted kernel's epilogue holds the IEEE division
+        # and square root of eq. (4), whose correctly rounded library sequences are built from DFMA
+        assert ("DFMA" in sass) == (wgt == "1")
+        assert "DMUL" in sass and "DADD" in sass
+        assert ("FFMA" in sass) == (wgt == "1")   # only the weighted sum fuses weight * element + acc
 
 
 def _create_args(n_sft=4, n_bins=8):
