@@ -69,6 +69,11 @@ def lib() -> ctypes.CDLL:
                                          ctypes.c_long, ctypes.c_void_p,
                                          ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                          ctypes.c_int]
+        L.tcwo_eval_bank.restype = ctypes.c_int
+        L.tcwo_eval_bank.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_long, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_double,
+                                     ctypes.c_long, dp, dp, dp, dp, ctypes.c_int,
+                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.tcwo_best_f64.restype = None
         L.tcwo_best_f64.argtypes = [dp, ctypes.c_long, ctypes.c_int, dp, ctypes.c_void_p]
         L.tcwo_best_i64.restype = None
@@ -203,6 +208,33 @@ def evaluate_weighted(w, weights, mean1: float, var1: float, sel=None, literal: 
     if rc != 0:
         raise ValueError("tcwo_eval_weighted: bad arguments")
     return WeightedResult(*out)
+
+
+def evaluate_bank(w, f0, tau, brk, sky, want_k: bool = False) -> OracleResult:
+    """Track sums of a template bank (PAPER.md:63 (ii)): per-template f0, tau, brk [n] and sky
+    [n][3], or one shared sky vector [3] / [1][3].  Data (spectrogram, timestamps, velocities,
+    band, T0) come from the workload-like object `w`."""
+    spec = np.ascontiguousarray(w.spectrogram)
+    fmt = FORMATS[w.fmt]
+    ts, vel = _f64(w.timestamps), _f64(w.velocities)
+    f0, tau, brk = _f64(f0), _f64(tau), _f64(brk)
+    sky = _f64(sky).reshape(-1, 3)
+    n = len(f0)
+    assert len(tau) == n and len(brk) == n and len(sky) in (1, n)
+    shared = len(sky) == 1
+    stat_f = np.empty(n, dtype=np.float64)
+    stat_i = np.empty(n, dtype=np.int64) if fmt != 0 else None
+    n_in = np.empty(n, dtype=np.int32)
+    n_amb = np.empty(n, dtype=np.int32)
+    k = np.empty((n, w.n_sft), dtype=np.int32) if want_k else None
+    rc = lib().tcwo_eval_bank(spec.ctypes.data, fmt, spec.strides[0], int(w.n_sft), int(w.n_bins),
+                              float(w.f_min), float(w.T_sft), _dp(ts), _dp(vel), float(w.T0),
+                              n, _dp(f0), _dp(tau), _dp(brk), _dp(sky), int(shared),
+                              stat_f.ctypes.data, stat_i.ctypes.data if stat_i is not None else None,
+                              k.ctypes.data if k is not None else None, n_in.ctypes.data, n_amb.ctypes.data)
+    if rc != 0:
+        raise ValueError("tcwo_eval_bank: bad arguments")
+    return OracleResult(stat_i if stat_i is not None else stat_f, n_in, n_amb, k)
 
 
 def best(stat: np.ndarray, n_f0: int):

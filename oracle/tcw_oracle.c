@@ -295,6 +295,60 @@ int tcwo_eval_weighted(const void *spectrogram, int format, long pitch_bytes, in
     return bad ? -1 : 0;
 }
 
+/* ---- NEXT-2: uniform random template bank --------------------------
+ *
+ * "(ii) the uniform random template bank that samples templates from a uniform prior over the
+ * parameter space".  Every template q carries its own (f0, tau, n) and, unless
+ * sky_shared, its own n-hat; with sky_shared all templates use sky[0..2] ("each template used the
+ * T0, and sky position values of the injection being searched for").  The statistic
+ * is the same ten steps as tcwo_eval, evaluated literally per (template, SFT): nothing is hoisted,
+ * g is the correctly rounded power evaluated for every lookup.
+ * Outputs as in tcwo_eval (any may be NULL).  Parity status: pinned (tests/test_oracle_bank_pins.py). */
+int tcwo_eval_bank(const void *spectrogram, int format, long pitch_bytes, int n_sft, int n_bins,
+                   double f_min, double T_sft, const double *ts, const double *vel, double T0,
+                   long n_tpl, const double *f0, const double *tau, const double *brk,
+                   const double *sky, int sky_shared, double *stat_f64, long long *stat_i64,
+                   int32_t *k_out, int32_t *n_inband, int32_t *n_ambig)
+{
+    if (!spectrogram || !ts || !vel || !f0 || !tau || !brk || !sky) return -1;
+    if (format < 0 || format > 2 || n_sft <= 0 || n_bins <= 0 || n_tpl < 0) return -1;
+    const unsigned char *spec = (const unsigned char *)spectrogram;
+    const long k_min = tcwo_kmin(f_min, T_sft);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (long q = 0; q < n_tpl; ++q) {
+        const double *nhat = sky + (sky_shared ? 0 : 3 * q);
+        double sum = 0.0;
+        long long cnt = 0;
+        int32_t inband = 0, ambig = 0;
+        for (int j = 0; j < n_sft; ++j) {
+            if (ts[j] < T0) {
+                if (k_out) k_out[q * n_sft + j] = INT32_MIN;
+                continue;
+            }
+            double g = tcwo_spindown(ts[j], T0, tau[q], brk[q]);
+            double D = tcwo_doppler(vel + 3 * (long)j, nhat);
+            double x = tcwo_track_x(f0[q], g, D, T_sft);
+            long k = tcwo_bin(x, k_min);
+            if (k_out) k_out[q * n_sft + j] = (int32_t)k;
+            double fr = x - floor(x);
+            if (fabs(fr - 0.5) < 1e-9) ambig++;
+            if (k >= 0 && k < n_bins) {
+                inband++;
+                if (format == TCWO_F32_POWER)
+                    sum += spec_value(spec, format, pitch_bytes, j, k);
+                else
+                    cnt += (long long)spec_value(spec, format, pitch_bytes, j, k);
+            }
+        }
+        if (format != TCWO_F32_POWER) sum = (double)cnt;
+        if (stat_f64) stat_f64[q] = sum;
+        if (stat_i64) stat_i64[q] = cnt;
+        if (n_inband) n_inband[q] = inband;
+        if (n_ambig) n_ambig[q] = ambig;
+    }
+    return 0;
+}
+
 /* Candidate reduction (north_star (d)): per group of n_f0 consecutive entries,
  * the maximum and the lowest f0 index attaining it. */
 void tcwo_best_f64(const double *stat, long n_groups, int n_f0, double *best_val, int32_t *best_idx)

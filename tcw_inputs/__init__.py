@@ -14,6 +14,7 @@ from .configs import (  # noqa: F401
     fibonacci_sphere,
     make_workload,
     pack_bits,
+    random_bank,
     sky_vector,
     synthetic_weights,
 )

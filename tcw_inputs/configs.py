@@ -98,6 +98,24 @@ def pack_bits(nu: np.ndarray) -> np.ndarray:
     return np.ascontiguousarray(by).view("<u4").reshape(n_sft, n_words)
 
 
+def random_bank(n: int, f_lo: float, f_hi: float, seed: int, sky=None):
+    """Uniform random template bank (PAPER.md:63 (ii)): f0 ~ U[f_lo, f_hi], tau ~ U[3500, 35000] s,
+    n ~ U[3, 7] ("the full theoretical ranges").  sky = None draws isotropic
+    unit vectors per template; otherwise the given vector is shared by all templates.
+    Returns float64 arrays (f0, tau, brk, sky) with sky [n][3] or [1][3]."""
+    rng = np.random.Generator(np.random.PCG64(seed + 104729))
+    f0 = rng.uniform(f_lo, f_hi, size=n)
+    tau = rng.uniform(3500.0, 35000.0, size=n)
+    brk = rng.uniform(3.0, 7.0, size=n)
+    if sky is None:
+        v = rng.standard_normal((n, 3))
+        sky = _renormalise(v)
+    else:
+        sky = np.asarray(sky, dtype=np.float64).reshape(1, 3)
+    return (np.ascontiguousarray(f0), np.ascontiguousarray(tau), np.ascontiguousarray(brk),
+            np.ascontiguousarray(sky, dtype=np.float64))
+
+
 def synthetic_weights(sky: np.ndarray, timestamps: np.ndarray, seed: int) -> np.ndarray:
     """Stand-in for the weights of the paper's ref. [14] ("antenna patterns and changing noise
     floors"): float32 [n_sky][n_sft], positive, mean 1 along each row.
