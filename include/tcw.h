@@ -167,6 +167,44 @@ typedef struct {
 int tcw_search_weighted(tcw_handle *h, const tcw_grid *grid, const tcw_weighting *weighting,
                         float *out_psi, float *out_stat, tcw_best_f32 *out_best, void *stream);
 
+/* ---- uniform random template bank ---------------------------
+ *
+ * "(ii) the uniform random template bank that samples templates from a uniform prior over the
+ *  parameter space"; "Each template used the T0, and sky position values of the
+ *  injection being searched for".  Template q has its own (f0[q], tau[q], brk[q])
+ * and either its own unit vector sky[3q..3q+2] or, with sky_shared != 0, the one vector sky[0..2].
+ * The statistic of a template is the one tcw_search computes (same bin indices: the kernel decides
+ * each bin with a fast binary64 evaluation of eq. (1)-(2) and falls back to the defining chain
+ * with the correctly rounded power wherever the fast value lies within x*2^-40 of a rounding
+ * boundary).
+ * All pointers are HOST arrays, validated and copied with cudaMemcpyAsync during the call
+ * (pageable arrays may be freed on return; pinned arrays once the stream has passed the call). */
+typedef struct {
+    double T0;          /* signal start time; SFTs with t_j < T0 are skipped                  */
+    long n;             /* number of templates, > 0                                           */
+    const double *f0;   /* [n] Hz, > 0 (any order)                                            */
+    const double *tau;  /* [n] s, > 0                                                         */
+    const double *brk;  /* [n] braking index, > 1                                             */
+    const double *sky;  /* [n][3] unit vectors, or [3] when sky_shared != 0                   */
+    int sky_shared;
+} tcw_bank;
+
+/* tcw_search_bank -- track sums of a template bank.
+ *  out_stat    DEVICE, [n] float32 (power) or int32 (counts); required.
+ *  out_inband  DEVICE, [n] int32 number of in-band SFTs of each template (the N of the noise
+ *              moments: for unit weights Psi = (s - mean1*N)/sqrt(var1*N)); may be NULL.
+ *  out_k       DEVICE, int32 [n][n_sft] bin indices (INT32_MIN where t_j < T0); inspection output
+ *              for parity tests, may be NULL (and should be for large banks).
+ * Power sums accumulate in float32 in ascending SFT order (deterministic); counts exactly.
+ * Asynchronous like tcw_search. */
+int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *out_inband, int *out_k,
+                    void *stream);
+
+/* tcw_get_counter -- diagnostic counters of the last search on this handle (synchronises its
+ * stream).  which = 0: lookups of the last tcw_search_bank that were decided by the defining
+ * chain (correctly rounded power) instead of the fast evaluation. */
+int tcw_get_counter(tcw_handle *h, int which, long long *value);
+
 /* tcw_destroy -- free the handle and everything it owns.  NULL is a no-op returning TCW_OK. */
 int tcw_destroy(tcw_handle *h);
 
@@ -217,7 +255,7 @@ int tcw_set_option(tcw_handle *h, int key, long value);
  * waits for the last of them. */
 int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
 
-/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged,
+/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged, 4 bank,
  * 3 sky-block),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),

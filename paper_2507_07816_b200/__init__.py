@@ -28,7 +28,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -47,6 +47,13 @@ class _CGrid(ctypes.Structure):
         ("n_brk", ctypes.c_int), ("brk", ctypes.POINTER(ctypes.c_double)),
         ("n_sky", ctypes.c_int), ("sky", ctypes.POINTER(ctypes.c_double)),
     ]
+
+
+class _CBank(ctypes.Structure):
+    _fields_ = [("T0", ctypes.c_double), ("n", ctypes.c_long),
+                ("f0", ctypes.POINTER(ctypes.c_double)), ("tau", ctypes.POINTER(ctypes.c_double)),
+                ("brk", ctypes.POINTER(ctypes.c_double)), ("sky", ctypes.POINTER(ctypes.c_double)),
+                ("sky_shared", ctypes.c_int)]
 
 
 class _CWeighting(ctypes.Structure):
@@ -76,6 +83,10 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_search_host.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
     L.tcw_search_weighted.restype = ci
     L.tcw_search_weighted.argtypes = [vp, ctypes.POINTER(_CGrid), ctypes.POINTER(_CWeighting), vp, vp, vp, vp]
+    L.tcw_search_bank.restype = ci
+    L.tcw_search_bank.argtypes = [vp, ctypes.POINTER(_CBank), vp, vp, vp, vp]
+    L.tcw_get_counter.restype = ci
+    L.tcw_get_counter.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_longlong)]
     L.tcw_destroy.restype = ci
     L.tcw_destroy.argtypes = [vp]
     L.tcw_last_error.restype = ctypes.c_char_p
@@ -247,6 +258,36 @@ class Handle:
                                      out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
         return out_psi, out_stat, out_best
 
+    def search_bank(self, f0, tau, brk, sky, T0: float = 0.0, out_stat=None, want_inband: bool = True,
+                    want_k: bool = False, stream=None):
+        """tcw_search_bank: per-template f0, tau, brk [n] and sky [n][3], or one shared vector
+        ([3] / [1][3]).  Returns (stat [n], n_inband [n] or None, k [n][n_sft] or None) as CUDA
+        tensors.  Asynchronous."""
+        import torch
+        L = load_library()
+        f0, tau, brk = _f64(f0), _f64(tau), _f64(brk)
+        sky = _f64(sky).reshape(-1, 3)
+        n = len(f0)
+        if len(tau) != n or len(brk) != n or len(sky) not in (1, n):
+            raise ValueError("bank arrays must have equal lengths (sky: [n][3] or one vector)")
+        shared = len(sky) == 1
+        dev = torch.device("cuda", torch.cuda.current_device())
+        if out_stat is None:
+            out_stat = torch.empty(n, dtype=self.stat_dtype, device=dev)
+        inband = torch.empty(n, dtype=torch.int32, device=dev) if want_inband else None
+        k = torch.empty((n, self.n_sft), dtype=torch.int32, device=dev) if want_k else None
+        cb = _CBank(float(T0), n, _dp(f0), _dp(tau), _dp(brk), _dp(sky), int(shared))
+        _check(L.tcw_search_bank(self._h, ctypes.byref(cb), out_stat.data_ptr(),
+                                 inband.data_ptr() if inband is not None else None,
+                                 k.data_ptr() if k is not None else None, _stream_ptr(stream)))
+        return out_stat, inband, k
+
+    def counter(self, which: int = 0) -> int:
+        """tcw_get_counter (0: bank lookups decided by the defining chain in the last bank search)."""
+        v = ctypes.c_longlong(0)
+        _check(load_library().tcw_get_counter(self._h, int(which), ctypes.byref(v)))
+        return int(v.value)
+
     def search_host(self, grid: Grid, out_stat: np.ndarray | None = None, out_best: np.ndarray | None = None,
                     want_stat: bool = True, stream=None):
         """tcw_search_host: results land in host numpy arrays; synchronous."""
@@ -305,7 +346,7 @@ class Handle:
     def info(self) -> dict:
         v = (ctypes.c_long * 10)()
         _check(load_library().tcw_get_info(self._h, v))
-        return dict(kernel={1: "gather", 2: "staged", 3: "skyblock"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
+        return dict(kernel={1: "gather", 2: "staged", 3: "skyblock", 4: "bank"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
                     smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]),
                     sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]))
 

@@ -20,6 +20,7 @@
 #include "tcw_sum.cuh"
 #include "tcw_tables.cuh"
 #include "tcw_skyblock.cuh"
+#include "tcw_bank.cuh"
 
 namespace {
 
@@ -107,6 +108,8 @@ struct tcw_handle {
     DevBuf<double> d_g, d_d, d_axes;
     DevBuf<unsigned char> d_partial, d_stat, d_best;
     DevBuf<unsigned char> d_cpart, d_clive;  // chunked staged searches: per-chunk partial sums, live flags
+    DevBuf<double> d_bank;                   // bank searches: f0, tau, brk [n] and sky [n][3] or [3]
+    unsigned long long *d_counter = nullptr; // bank searches: lookups decided by the defining chain
     DevBuf<float> d_w, d_cw;                 // weighted searches: weights [n_sky][n_sft]; per-chunk sums of w and w^2
     DevBuf<long> d_sel;
     DevBuf<double> d_dts, d_dmm;  // sky-block kernel: per-block Doppler rows and their {min, max}
@@ -438,6 +441,8 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     CREATE_TRY(cudaMalloc((void **)&h->d_ts, sizeof(double) * n_sft));
     CREATE_TRY(cudaMalloc((void **)&h->d_vel, sizeof(double) * 3 * (size_t)n_sft));
     CREATE_TRY(cudaMalloc((void **)&h->d_status, sizeof(int)));
+    CREATE_TRY(cudaMalloc((void **)&h->d_counter, sizeof(unsigned long long)));
+    CREATE_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned long long), st));
     CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
     CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));   // the padding must read as zero
@@ -483,6 +488,8 @@ int tcw_destroy(tcw_handle *h)
     h->d_cpart.release();
     h->d_clive.release();
     h->d_w.release();
+    h->d_bank.release();
+    if (h->d_counter) cudaFree(h->d_counter);
     h->d_cw.release();
     h->d_sel.release();
     h->d_dts.release();
@@ -742,6 +749,120 @@ int tcw_search_weighted(tcw_handle *h, const tcw_grid *grid, const tcw_weighting
 {
     if (h && !weighting) return fail(TCW_EINVAL, "weighting is NULL");
     return search_impl(h, grid, weighting, out_stat, out_psi, out_best, stream);
+}
+
+int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *out_inband, int *out_k, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    if (!bank) return fail(TCW_EINVAL, "bank is NULL");
+    if (bank->n <= 0) return fail(TCW_EINVAL, "bank size must be positive");
+    if (!bank->f0 || !bank->tau || !bank->brk || !bank->sky) return fail(TCW_EINVAL, "bank array pointer is NULL");
+    if (!std::isfinite(bank->T0)) return fail(TCW_EINVAL, "T0 is not finite");
+    if (!out_stat) return fail(TCW_EINVAL, "out_stat is NULL");
+    const long n = bank->n;
+    const double f_cap = (2147483648.0 - 1048576.0) / h->T;
+    for (long q = 0; q < n; ++q) {
+        if (!(bank->f0[q] > 0) || !(bank->f0[q] < f_cap)) return fail(TCW_EINVAL, "f0[%ld] must be > 0 and f0*T_sft < 2^31 - 2^20", q);
+        if (!(bank->tau[q] > 0) || !std::isfinite(bank->tau[q])) return fail(TCW_EINVAL, "tau[%ld] must be > 0", q);
+        if (!(bank->brk[q] > 1) || !std::isfinite(bank->brk[q])) return fail(TCW_EINVAL, "braking index brk[%ld] must be > 1", q);
+    }
+    const long n_vec = bank->sky_shared ? 1 : n;
+    for (long q = 0; q < n_vec; ++q) {
+        const double *v = bank->sky + 3 * q;
+        const double nrm = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        if (!(std::fabs(nrm - 1.0) <= 1e-6)) return fail(TCW_EINVAL, "sky[%ld] is not a unit vector", q);
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(cudaSetDevice(h->device));
+    int rc;
+    if ((rc = h->d_bank.reserve((size_t)(3 * n + 3 * n_vec))) != TCW_OK) return rc;
+    if (bank->sky_shared && (rc = h->d_d.reserve((size_t)h->n_sft)) != TCW_OK) return rc;
+    double *d_f0 = h->d_bank.p, *d_tau = d_f0 + n, *d_brk = d_tau + n, *d_sky = d_brk + n;
+    CUDA_TRY(cudaMemcpyAsync(d_f0, bank->f0, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_tau, bank->tau, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_brk, bank->brk, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_sky, bank->sky, sizeof(double) * 3 * n_vec, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned long long), st));
+
+    const bool tm = h->opt_timing != 0 && h->timing_n < TIMING_MAX;
+    cudaEvent_t *ev = nullptr;
+    if (tm) {
+        while (h->ev.size() < 4 * (h->timing_n + 1)) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreate(&e));
+            h->ev.push_back(e);
+        }
+        ev = h->ev.data() + 4 * h->timing_n;
+        CUDA_TRY(cudaEventRecord(ev[0], st));
+    }
+    if (bank->sky_shared) {
+        // the exact Doppler factor of the shared sky point, one entry per SFT (eq. (2))
+        tcw::doppler_table_kernel<<<(unsigned)((h->n_sft + 255) / 256), 256, 0, st>>>(h->d_vel, h->n_sft, d_sky, 1, h->d_d.p);
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
+    tcw::BankParams p;
+    std::memset(&p, 0, sizeof p);
+    p.spec = h->d_spec + h->pad_bytes;
+    p.pitch = h->pitch;
+    p.n_sft = h->n_sft;
+    p.n_bins = h->n_bins;
+    p.k_min = h->k_min;
+    p.j_begin = (int)(std::lower_bound(h->ts.begin(), h->ts.end(), bank->T0) - h->ts.begin());
+    p.T = h->T;
+    p.T0 = bank->T0;
+    p.ts = h->d_ts;
+    p.vel = h->d_vel;
+    p.dshared = bank->sky_shared ? h->d_d.p : nullptr;
+    p.n_tpl = n;
+    p.f0 = d_f0;
+    p.tau = d_tau;
+    p.brk = d_brk;
+    p.sky = d_sky;
+    p.dmax = (1.0 + (h->vmax / C_LIGHT) * (1.0 + 1e-5) + 1e-15) * (1.0 + 1e-9);
+    p.out_stat = out_stat;
+    p.out_inband = out_inband;
+    p.out_k = out_k;
+    p.n_exact = h->d_counter;
+    const long n_ctas = (n + tcw::BANK_THREADS - 1) / tcw::BANK_THREADS;
+    if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "bank needs more than 2^31-1 CTAs; split the search");
+    if (h->fmt_dev == tcw::FMT_F32) {
+        if (h->t_pow2) tcw::sum_bank_kernel<tcw::FMT_F32, true><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);
+        else tcw::sum_bank_kernel<tcw::FMT_F32, false><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);
+    } else {
+        if (h->t_pow2) tcw::sum_bank_kernel<tcw::FMT_U8, true><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);
+        else tcw::sum_bank_kernel<tcw::FMT_U8, false><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);
+    }
+    CUDA_TRY(cudaGetLastError());
+    if (tm) {
+        CUDA_TRY(cudaEventRecord(ev[2], st));
+        CUDA_TRY(cudaEventRecord(ev[3], st));
+        h->timing_n++;
+    }
+    h->last_stream = st;
+    h->tab_tau = 0;   // the grid tables of an earlier search are gone (d_d is reused)
+    h->info[0] = 4;
+    h->info[1] = tcw::BANK_THREADS;
+    h->info[2] = n_ctas;
+    h->info[3] = 0;
+    h->info[5] = bank->sky_shared ? 2 : 1;
+    h->info[6] = 0;
+    h->info[7] = 0;
+    h->info[8] = 1;
+    h->info[9] = h->n_sft;
+    return TCW_OK;
+}
+
+int tcw_get_counter(tcw_handle *h, int which, long long *value)
+{
+    if (!h || !value) return fail(TCW_EINVAL, "NULL argument");
+    if (which != 0) return fail(TCW_EINVAL, "unknown counter %d", which);
+    CUDA_TRY(cudaSetDevice(h->device));
+    if (h->last_stream || h->info[0]) CUDA_TRY(cudaStreamSynchronize(h->last_stream));
+    unsigned long long v = 0;
+    CUDA_TRY(cudaMemcpy(&v, h->d_counter, sizeof v, cudaMemcpyDeviceToHost));
+    *value = (long long)v;
+    return TCW_OK;
 }
 
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host, void *stream)
