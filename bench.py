@@ -394,6 +394,56 @@ def run_ours(args):
     return 0
 
 
+# ----------------------------------------------------------------------------- bank mode (NEXT-2)
+def run_bank(args):
+    """--bank N: tcw_search_bank on N uniform random templates (PAPER.md:63 (ii)) over the config's
+    data, at the config's first sky point.  Not the headline metric: a second line
+    for DESIGN.md.  The path is bound by FP64 arithmetic (one power per lookup), so the roofline
+    object is an ALU one: FP64 instructions per lookup (counted in the SASS of the fast path:
+    DESIGN.md section 7) x lookups evaluated / time, against 148 SMs x 64 FP64 lanes x 1.965 GHz."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    import tcw_inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the tCW path has no CPU fallback")
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    w = tcw_inputs.make_workload(args.config, fmt=args.format)
+    f_hi = w.f_min + w.n_bins / w.T_sft
+    f0, tau, brk, sky = tcw_inputs.random_bank(args.bank, w.f_min, f_hi, w.seed, sky=w.sky[0])
+    h = tcw.Handle.from_workload(w, device="cuda:0")
+    out = torch.empty(args.bank, dtype=h.stat_dtype, device="cuda:0")
+    for _ in range(args.warmup):
+        _, inband, _ = h.search_bank(f0, tau, brk, sky, T0=w.T0, out_stat=out)
+    h.set_option(tcw.TCW_OPT_TIMING, 1)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, inband, _ = h.search_bank(f0, tau, brk, sky, T0=w.T0, out_stat=out)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    stage_ms, n_timed = h.timing()
+    n_exact = h.counter(0)
+    nominal = float(args.bank) * w.n_sft
+    evaluated = float(inband.sum(dtype=torch.int64).item())
+    kern_ms = stage_ms[1]
+    line = {"metric": METRIC + " (random template bank, tcw_search_bank)", "value": nominal / (kern_ms * 1e-3), "unit": UNIT,
+            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 index + f32/i32 accumulate",
+            "data": "synthetic", "config": workload_config(w, {"bank_templates": args.bank, "sky": "shared (PAPER.md:77)"}),
+            "templates_per_s": args.bank / (kern_ms * 1e-3), "kernel_ms": kern_ms,
+            "host_ms_per_step_incl_parameter_copy": 1e3 * wall / args.steps,
+            "inband_lookups": evaluated, "inband_fraction": evaluated / nominal,
+            "exact_chain_lookups": n_exact,
+            "us_per_template": 1e3 * kern_ms / args.bank,
+            "paper_us_per_template_a100": 15.0}
+    print(json.dumps(line), flush=True)
+    h.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -410,11 +460,14 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--bank", type=int, default=0, help="time tcw_search_bank on this many random templates (NEXT-2)")
     ap.add_argument("--weighted", action="store_true",
                     help="time tcw_search_weighted (weighted statistic + critical ratio, NEXT-1) instead of tcw_search")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    if args.bank and args.impl == "ours":
+        return run_bank(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 
