@@ -205,6 +205,28 @@ int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *ou
  * chain (correctly rounded power) instead of the fast evaluation. */
 int tcw_get_counter(tcw_handle *h, int which, long long *value);
 
+/* ---- downstream selection ------------------------------------
+ *
+ * "a threshold was set on Psi based on the distribution of critical ratios on only noise using the
+ *  same amount of templates (Psi_noise max).  That is, an injection was considered detected if a
+ *  template close to the injection had Psi > Psi_noise max."
+ * Both calls read a DEVICE array of n statistics -- dtype 0: float32 (Psi, power sums), 1: int32
+ * (counts) -- e.g. an out_psi / out_stat of a search, and are exact and deterministic.
+ * NaN is never selected; -0.0 equals +0.0.  Asynchronous on `stream`; `h` supplies the scratch. */
+
+/* tcw_topk -- the K largest values in descending order, equal values in ascending index order
+ * (reading Q23).  K in 1..2048.  K = 1 on a noise-only search is Psi_noise max.
+ *  out_val    DEVICE [K], same dtype as values;  out_idx  DEVICE [K] int64 indices into values;
+ *  out_count  DEVICE int32 (may be NULL): entries written = min(K, selectable values). */
+int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *out_val,
+             long long *out_idx, int *out_count, void *stream);
+
+/* tcw_select_above -- the indices i with values[i] > threshold, ascending.
+ *  out_idx    DEVICE [capacity] int64 (may be NULL when capacity == 0): the first `capacity` hits;
+ *  out_count  DEVICE int64: the total number of hits (may exceed capacity). */
+int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, double threshold,
+                     long capacity, long long *out_idx, long long *out_count, void *stream);
+
 /* tcw_destroy -- free the handle and everything it owns.  NULL is a no-op returning TCW_OK. */
 int tcw_destroy(tcw_handle *h);
 

@@ -28,7 +28,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -87,6 +87,10 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_search_bank.argtypes = [vp, ctypes.POINTER(_CBank), vp, vp, vp, vp]
     L.tcw_get_counter.restype = ci
     L.tcw_get_counter.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_longlong)]
+    L.tcw_topk.restype = ci
+    L.tcw_topk.argtypes = [vp, vp, ci, cl, ci, vp, vp, vp, vp]
+    L.tcw_select_above.restype = ci
+    L.tcw_select_above.argtypes = [vp, vp, ci, cl, ctypes.c_double, cl, vp, vp, vp]
     L.tcw_destroy.restype = ci
     L.tcw_destroy.argtypes = [vp]
     L.tcw_last_error.restype = ctypes.c_char_p
@@ -281,6 +285,38 @@ class Handle:
                                  inband.data_ptr() if inband is not None else None,
                                  k.data_ptr() if k is not None else None, _stream_ptr(stream)))
         return out_stat, inband, k
+
+    @staticmethod
+    def _sel_dtype(values) -> int:
+        import torch
+        if values.dtype == torch.float32:
+            return 0
+        if values.dtype == torch.int32:
+            return 1
+        raise ValueError("values must be a float32 or int32 CUDA tensor")
+
+    def topk(self, values, K: int, stream=None):
+        """tcw_topk over a CUDA tensor of statistics (flattened).  Returns (val [K], idx [K] int64,
+        count int32 scalar tensor); only the first `count` entries are meaningful.  Asynchronous."""
+        import torch
+        v = values.contiguous().view(-1)
+        out_val = torch.empty(K, dtype=v.dtype, device=v.device)
+        out_idx = torch.empty(K, dtype=torch.int64, device=v.device)
+        out_cnt = torch.zeros((), dtype=torch.int32, device=v.device)
+        _check(load_library().tcw_topk(self._h, v.data_ptr(), self._sel_dtype(v), v.numel(), int(K),
+                                       out_val.data_ptr(), out_idx.data_ptr(), out_cnt.data_ptr(), _stream_ptr(stream)))
+        return out_val, out_idx, out_cnt
+
+    def select_above(self, values, threshold: float, capacity: int, stream=None):
+        """tcw_select_above: (idx [capacity] int64, count int64 scalar tensor).  Asynchronous."""
+        import torch
+        v = values.contiguous().view(-1)
+        out_idx = torch.empty(max(capacity, 1), dtype=torch.int64, device=v.device)
+        out_cnt = torch.zeros((), dtype=torch.int64, device=v.device)
+        _check(load_library().tcw_select_above(self._h, v.data_ptr(), self._sel_dtype(v), v.numel(), float(threshold),
+                                               int(capacity), out_idx.data_ptr() if capacity > 0 else None,
+                                               out_cnt.data_ptr(), _stream_ptr(stream)))
+        return out_idx[:capacity], out_cnt
 
     def counter(self, which: int = 0) -> int:
         """tcw_get_counter (0: bank lookups decided by the defining chain in the last bank search)."""

@@ -21,6 +21,7 @@
 #include "tcw_tables.cuh"
 #include "tcw_skyblock.cuh"
 #include "tcw_bank.cuh"
+#include "tcw_select.cuh"
 
 namespace {
 
@@ -108,6 +109,7 @@ struct tcw_handle {
     DevBuf<double> d_g, d_d, d_axes;
     DevBuf<unsigned char> d_partial, d_stat, d_best;
     DevBuf<unsigned char> d_cpart, d_clive;  // chunked staged searches: per-chunk partial sums, live flags
+    DevBuf<unsigned char> d_selws;           // selection scratch (histogram, state, block counts, candidates)
     DevBuf<double> d_bank;                   // bank searches: f0, tau, brk [n] and sky [n][3] or [3]
     unsigned long long *d_counter = nullptr; // bank searches: lookups decided by the defining chain
     DevBuf<float> d_w, d_cw;                 // weighted searches: weights [n_sky][n_sft]; per-chunk sums of w and w^2
@@ -489,6 +491,7 @@ int tcw_destroy(tcw_handle *h)
     h->d_clive.release();
     h->d_w.release();
     h->d_bank.release();
+    h->d_selws.release();
     if (h->d_counter) cudaFree(h->d_counter);
     h->d_cw.release();
     h->d_sel.release();
@@ -862,6 +865,107 @@ int tcw_get_counter(tcw_handle *h, int which, long long *value)
     unsigned long long v = 0;
     CUDA_TRY(cudaMemcpy(&v, h->d_counter, sizeof v, cudaMemcpyDeviceToHost));
     *value = (long long)v;
+    return TCW_OK;
+}
+
+namespace {
+struct SelScratch {
+    unsigned int *hist, *blk_gt, *blk_eq, *cand_bits;
+    unsigned long long *off_gt, *off_eq;
+    long long *cand_idx;
+    tcw::SelState *state;
+};
+
+int sel_scratch(tcw_handle *h, SelScratch *sc)
+{
+    const size_t B = tcw::SEL_MAX_BLOCKS, K = tcw::SEL_MAX_K;
+    const size_t bytes = 2048 * 4 + 256 + 2 * B * 4 + 2 * B * 8 + K * 4 + K * 8;
+    int rc = h->d_selws.reserve(bytes);
+    if (rc != TCW_OK) return rc;
+    unsigned char *q = h->d_selws.p;
+    sc->off_gt = (unsigned long long *)q; q += B * 8;
+    sc->off_eq = (unsigned long long *)q; q += B * 8;
+    sc->cand_idx = (long long *)q; q += K * 8;
+    sc->state = (tcw::SelState *)q; q += 256;
+    sc->hist = (unsigned int *)q; q += 2048 * 4;
+    sc->blk_gt = (unsigned int *)q; q += B * 4;
+    sc->blk_eq = (unsigned int *)q; q += B * 4;
+    sc->cand_bits = (unsigned int *)q;
+    return TCW_OK;
+}
+
+// contiguous segment per CTA (a multiple of the CTA size), at most SEL_MAX_BLOCKS CTAs
+void sel_grid(long n, long *seg, int *n_blocks)
+{
+    long want = std::min<long>(tcw::SEL_MAX_BLOCKS, std::max<long>(1, (n + 4095) / 4096));
+    long s = (n + want - 1) / want;
+    s = (s + tcw::SEL_THREADS - 1) / tcw::SEL_THREADS * tcw::SEL_THREADS;
+    *seg = s;
+    *n_blocks = (int)((n + s - 1) / s);
+}
+}  // namespace
+
+int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *out_val, long long *out_idx,
+             int *out_count, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    if (!values || !out_val || !out_idx) return fail(TCW_EINVAL, "NULL array pointer");
+    if (dtype != 0 && dtype != 1) return fail(TCW_EINVAL, "dtype must be 0 (float32) or 1 (int32)");
+    if (n <= 0) return fail(TCW_EINVAL, "n must be positive");
+    if (K <= 0 || K > tcw::SEL_MAX_K) return fail(TCW_EINVAL, "K must be in 1..%d", tcw::SEL_MAX_K);
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(cudaSetDevice(h->device));
+    SelScratch sc;
+    int rc = sel_scratch(h, &sc);
+    if (rc != TCW_OK) return rc;
+    long seg;
+    int nb;
+    sel_grid(n, &seg, &nb);
+    const unsigned int *v = (const unsigned int *)values;
+    CUDA_TRY(cudaMemsetAsync(sc.hist, 0, 2048 * 4, st));
+    CUDA_TRY(cudaMemsetAsync(sc.state, 0, sizeof(tcw::SelState), st));
+    tcw::sel_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
+    tcw::sel_pick_kernel<0><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
+    tcw::sel_pick_kernel<1><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_hist_kernel<2><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
+    tcw::sel_pick_kernel<2><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_count_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, 0.0, sc.blk_gt, sc.blk_eq);
+    tcw::sel_scan_kernel<<<1, 1, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
+    tcw::sel_scatter_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, 0.0, sc.off_gt, sc.off_eq,
+                                                                    0, sc.cand_bits, sc.cand_idx);
+    tcw::sel_sort_kernel<<<1, 1024, 0, st>>>(sc.cand_bits, sc.cand_idx, dtype, sc.state, (unsigned int *)out_val, out_idx,
+                                             out_count);
+    CUDA_TRY(cudaGetLastError());
+    h->last_stream = st;
+    return TCW_OK;
+}
+
+int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, double threshold, long capacity,
+                     long long *out_idx, long long *out_count, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    if (!values || !out_count || (capacity > 0 && !out_idx)) return fail(TCW_EINVAL, "NULL array pointer");
+    if (dtype != 0 && dtype != 1) return fail(TCW_EINVAL, "dtype must be 0 (float32) or 1 (int32)");
+    if (n <= 0 || capacity < 0) return fail(TCW_EINVAL, "n must be positive and capacity >= 0");
+    if (std::isnan(threshold)) return fail(TCW_EINVAL, "threshold is NaN");
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(cudaSetDevice(h->device));
+    SelScratch sc;
+    int rc = sel_scratch(h, &sc);
+    if (rc != TCW_OK) return rc;
+    long seg;
+    int nb;
+    sel_grid(n, &seg, &nb);
+    const unsigned int *v = (const unsigned int *)values;
+    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, threshold, sc.blk_gt, sc.blk_eq);
+    tcw::sel_scan_kernel<<<1, 1, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
+    if (capacity > 0)
+        tcw::sel_scatter_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, threshold, sc.off_gt,
+                                                                       sc.off_eq, capacity, nullptr, out_idx);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(out_count, &sc.state->count, sizeof(long long), cudaMemcpyDeviceToDevice, st));
+    h->last_stream = st;
     return TCW_OK;
 }
 
