@@ -444,6 +444,46 @@ def run_bank(args):
     return 0
 
 
+# ----------------------------------------------------------------------------- selection mode (NEXT-4)
+def run_select(args):
+    """--select N: tcw_topk (K = 1000) and tcw_select_above over N float32 statistics ~ N(0, 1)
+    (the shape of a Psi array; cfg5's out_stat has 393 M entries).  HBM-bound streaming passes: the
+    algorithmic bytes are ONE read of the array (4 N bytes); top-K makes five passes (three
+    histogram passes, count, scatter), threshold selection two."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    import tcw_inputs
+
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    w = tcw_inputs.make_workload("cfg1")
+    h = tcw.Handle.from_workload(w, device="cuda:0")
+    n = args.select
+    g = torch.Generator(device="cuda").manual_seed(1)
+    v = torch.randn(n, generator=g, device="cuda", dtype=torch.float32)
+    peak, peak_src = load_peaks()
+    res = {}
+    for name, fn in (("topk_K1000", lambda: h.topk(v, 1000)), ("select_above_4.5", lambda: h.select_above(v, 4.5, 1 << 20))):
+        for _ in range(max(3, args.warmup)):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        res[name] = {"ms": ms, "values_per_s": n / (ms * 1e-3),
+                     "roofline": {"bound": "hbm", "achieved": 4.0 * n / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                                  "frac": 4.0 * n / (ms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src}}
+    print(json.dumps({"metric": "statistics selected per second (tcw_topk / tcw_select_above)", "n": n,
+                      "steps": args.steps, "data": "synthetic", "results": res}), flush=True)
+    h.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -461,11 +501,14 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bank", type=int, default=0, help="time tcw_search_bank on this many random templates (NEXT-2)")
+    ap.add_argument("--select", type=int, default=0, help="time tcw_topk / tcw_select_above over this many float32 values (NEXT-4)")
     ap.add_argument("--weighted", action="store_true",
                     help="time tcw_search_weighted (weighted statistic + critical ratio, NEXT-1) instead of tcw_search")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    if args.select and args.impl == "ours":
+        return run_select(args)
     if args.bank and args.impl == "ours":
         return run_bank(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)

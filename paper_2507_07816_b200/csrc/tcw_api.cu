@@ -897,9 +897,9 @@ int sel_scratch(tcw_handle *h, SelScratch *sc)
 // contiguous segment per CTA (a multiple of the CTA size), at most SEL_MAX_BLOCKS CTAs
 void sel_grid(long n, long *seg, int *n_blocks)
 {
-    long want = std::min<long>(tcw::SEL_MAX_BLOCKS, std::max<long>(1, (n + 4095) / 4096));
+    long want = std::min<long>(tcw::SEL_MAX_BLOCKS, std::max<long>(1, (n + 8191) / 8192));
     long s = (n + want - 1) / want;
-    s = (s + tcw::SEL_THREADS - 1) / tcw::SEL_THREADS * tcw::SEL_THREADS;
+    s = (s + 2 * tcw::SEL_TILE - 1) / (2 * tcw::SEL_TILE) * (2 * tcw::SEL_TILE);   // whole tile pairs: 16-byte aligned starts
     *seg = s;
     *n_blocks = (int)((n + s - 1) / s);
 }
@@ -922,18 +922,19 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
     int nb;
     sel_grid(n, &seg, &nb);
     const unsigned int *v = (const unsigned int *)values;
+    const int vec = ((uintptr_t)values & 15) == 0;
     CUDA_TRY(cudaMemsetAsync(sc.hist, 0, 2048 * 4, st));
     CUDA_TRY(cudaMemsetAsync(sc.state, 0, sizeof(tcw::SelState), st));
-    tcw::sel_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
-    tcw::sel_pick_kernel<0><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
-    tcw::sel_pick_kernel<1><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_hist_kernel<2><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, sc.hist);
-    tcw::sel_pick_kernel<2><<<1, 1, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_count_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, 0.0, sc.blk_gt, sc.blk_eq);
-    tcw::sel_scan_kernel<<<1, 1, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
-    tcw::sel_scatter_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, 0.0, sc.off_gt, sc.off_eq,
-                                                                    0, sc.cand_bits, sc.cand_idx);
+    tcw::sel_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
+    tcw::sel_pick_kernel<0><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
+    tcw::sel_pick_kernel<1><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_hist_kernel<2><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
+    tcw::sel_pick_kernel<2><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
+    tcw::sel_count_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq);
+    tcw::sel_scan_kernel<<<1, 256, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
+    tcw::sel_scatter_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq,
+                                                                    sc.off_gt, sc.off_eq, 0, sc.cand_bits, sc.cand_idx);
     tcw::sel_sort_kernel<<<1, 1024, 0, st>>>(sc.cand_bits, sc.cand_idx, dtype, sc.state, (unsigned int *)out_val, out_idx,
                                              out_count);
     CUDA_TRY(cudaGetLastError());
@@ -958,11 +959,12 @@ int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, doubl
     int nb;
     sel_grid(n, &seg, &nb);
     const unsigned int *v = (const unsigned int *)values;
-    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, threshold, sc.blk_gt, sc.blk_eq);
-    tcw::sel_scan_kernel<<<1, 1, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
+    const int vec = ((uintptr_t)values & 15) == 0;
+    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, threshold, sc.blk_gt, sc.blk_eq);
+    tcw::sel_scan_kernel<<<1, 256, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
     if (capacity > 0)
-        tcw::sel_scatter_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, sc.state, threshold, sc.off_gt,
-                                                                       sc.off_eq, capacity, nullptr, out_idx);
+        tcw::sel_scatter_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, threshold, sc.blk_gt,
+                                                                       sc.blk_eq, sc.off_gt, sc.off_eq, capacity, nullptr, out_idx);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(out_count, &sc.state->count, sizeof(long long), cudaMemcpyDeviceToDevice, st));
     h->last_stream = st;

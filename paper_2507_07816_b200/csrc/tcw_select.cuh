@@ -54,57 +54,105 @@ __device__ __forceinline__ SelSeg sel_segment(long n, long seg)
     return {b, e};
 }
 
+// Streaming access: a CTA walks its segment in tiles of 4 * SEL_THREADS elements, thread t owning the
+// four consecutive elements tile + 4t .. tile + 4t + 3 (one 16-byte load when the array is 16-byte
+// aligned; segments start on multiples of 1024 elements).  nv = how many of the four are in range.
+constexpr int SEL_TILE = 4 * SEL_THREADS;
+__device__ __forceinline__ void sel_load4(const unsigned int *__restrict__ vals, long i, long end, bool vec,
+                                          unsigned int (&b)[4], int &nv)
+{
+    nv = end - i >= 4 ? 4 : (end > i ? (int)(end - i) : 0);
+    if (vec && nv == 4) {
+        const uint4 q = __ldg((const uint4 *)(vals + i));
+        b[0] = q.x; b[1] = q.y; b[2] = q.z; b[3] = q.w;
+    } else {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) b[c] = c < nv ? __ldg(vals + i + c) : 0u;
+    }
+}
+
 // histogram of one radix digit over the keys whose higher bits equal state->prefix
 //   pass 0: bits 31..21 (2048 bins), pass 1: bits 20..10 (2048), pass 2: bits 9..0 (1024)
+// Pass 0 sees every key and statistics cluster in a few dozen digits, so it keeps four copies of
+// the histogram, picked by the lane, which cuts same-address atomic conflicts fourfold.
 template <int PASS>
 __global__ void __launch_bounds__(SEL_THREADS)
-sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int,
+sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
                 const SelState *__restrict__ state, unsigned int *__restrict__ hist)
 {
-    __shared__ unsigned int h[2048];
-    for (int t = threadIdx.x; t < 2048; t += SEL_THREADS) h[t] = 0;
+    constexpr int COPIES = PASS == 0 ? 4 : 1;
+    __shared__ unsigned int h[COPIES * 2048];
+    for (int t = threadIdx.x; t < COPIES * 2048; t += SEL_THREADS) h[t] = 0;
     __syncthreads();
     const unsigned int prefix = PASS ? state->prefix : 0u;
     const SelSeg sg = sel_segment(n, seg);
-    for (long i = sg.begin + threadIdx.x; i < sg.end; i += SEL_THREADS) {
-        const unsigned int bits = vals[i];
-        if (!sel_valid(bits, is_int)) continue;
-        const unsigned int key = sel_key(bits, is_int);
-        if (PASS == 0) atomicAdd(&h[key >> 21], 1u);
-        else if (PASS == 1) { if ((key >> 21) == (prefix >> 21)) atomicAdd(&h[(key >> 10) & 2047u], 1u); }
-        else { if ((key >> 10) == (prefix >> 10)) atomicAdd(&h[key & 1023u], 1u); }
+    unsigned int *hc = h + (threadIdx.x & (COPIES - 1)) * 2048;
+    for (long t0 = sg.begin; t0 < sg.end; t0 += SEL_TILE) {
+        unsigned int b[4];
+        int nv;
+        sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b, nv);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const bool ok = c < nv && sel_valid(b[c], is_int);
+            const unsigned int key = sel_key(b[c], is_int);
+            if (PASS == 0) {
+                if (ok) atomicAdd(&hc[key >> 21], 1u);
+            } else if (PASS == 1) {
+                if (ok && (key >> 21) == (prefix >> 21)) atomicAdd(&h[(key >> 10) & 2047u], 1u);
+            } else {
+                if (ok && (key >> 10) == (prefix >> 10)) atomicAdd(&h[key & 1023u], 1u);
+            }
+        }
     }
     __syncthreads();
-    for (int t = threadIdx.x; t < 2048; t += SEL_THREADS)
-        if (h[t]) atomicAdd(&hist[t], h[t]);
+    for (int t = threadIdx.x; t < 2048; t += SEL_THREADS) {
+        unsigned int c = h[t];
+        for (int q = 1; q < COPIES; ++q) c += h[q * 2048 + t];
+        if (c) atomicAdd(&hist[t], c);
+    }
 }
 
 // one CTA: walk the digit histogram from the top until the cumulative count reaches k_rem
+// (thread t sums the 8 bins [8t, 8t + 8); thread 0 walks the 256 partial sums, then the 8 bins)
 template <int PASS>
-__global__ void __launch_bounds__(1)
+__global__ void __launch_bounds__(256)
 sel_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, unsigned int K)
 {
-    const int bins = PASS == 2 ? 1024 : 2048;
-    unsigned int k_rem = state->k_rem;
-    if (PASS == 0) {
-        unsigned long long total = 0;
-        for (int b = 0; b < bins; ++b) total += hist[b];
-        k_rem = (unsigned int)(total < K ? total : K);
-        state->k_eff = k_rem;
-        state->prefix = 0;
-    }
-    unsigned int above = 0;
-    int d = bins - 1;
-    if (k_rem > 0)
-        for (; d > 0; --d) {
-            if (above + hist[d] >= k_rem) break;
-            above += hist[d];
+    constexpr int bins = PASS == 2 ? 1024 : 2048;
+    __shared__ unsigned int part[256];
+    unsigned int mine = 0;
+    for (int b = 0; b < 8; ++b) { const int q = 8 * threadIdx.x + b; mine += q < bins ? hist[q] : 0u; }
+    part[threadIdx.x] = mine;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int k_rem = state->k_rem;
+        if (PASS == 0) {
+            unsigned long long total = 0;
+            for (int t = 0; t < 256; ++t) total += part[t];
+            k_rem = (unsigned int)(total < K ? total : K);
+            state->k_eff = k_rem;
+            state->prefix = 0;
         }
-    const int shift = PASS == 0 ? 21 : (PASS == 1 ? 10 : 0);
-    state->prefix |= (unsigned int)d << shift;
-    state->k_rem = k_rem - above;          // still to take among the keys with this digit
-    if (PASS == 2) state->n_greater = state->k_eff - state->k_rem;
-    for (int b = 0; b < bins; ++b) hist[b] = 0;   // ready for the next pass
+        unsigned int above = 0;
+        int d = 0;
+        if (k_rem > 0) {
+            int t = bins / 8 - 1;
+            for (; t > 0; --t) {
+                if (above + part[t] >= k_rem) break;
+                above += part[t];
+            }
+            for (d = 8 * t + 7; d > 8 * t; --d) {
+                if (above + hist[d] >= k_rem) break;
+                above += hist[d];
+            }
+        }
+        constexpr int shift = PASS == 0 ? 21 : (PASS == 1 ? 10 : 0);
+        state->prefix |= (unsigned int)d << shift;
+        state->k_rem = k_rem - above;          // still to take among the keys with this digit
+        if (PASS == 2) state->n_greater = state->k_eff - state->k_rem;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < bins; b += 256) hist[b] = 0;   // ready for the next pass
 }
 
 // ---- ordered compaction -------------------------------------------------------------------
@@ -117,14 +165,19 @@ __device__ __forceinline__ int sel_class(unsigned int bits, int is_int, unsigned
         const double v = is_int ? (double)(int)bits : (double)__uint_as_float(bits);
         return v > thr ? 2 : 0;                       // NaN compares false
     }
-    if (!sel_valid(bits, is_int)) return 0;
-    const unsigned int key = sel_key(bits, is_int);
-    return key > kth ? 2 : (key == kth ? 1 : 0);
+    if (is_int) {
+        const int v = (int)bits, kv = (int)(kth ^ 0x80000000u);
+        return v > kv ? 2 : (v == kv ? 1 : 0);
+    }
+    // float32: comparing the values is comparing the keys (NaN compares false; -0.0 == +0.0 as in sel_key)
+    const float kf = __uint_as_float((kth & 0x80000000u) ? (kth & 0x7fffffffu) : ~kth);
+    const float v = __uint_as_float(bits);
+    return v > kf ? 2 : (v == kf ? 1 : 0);
 }
 
 template <bool THR>
 __global__ void __launch_bounds__(SEL_THREADS)
-sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int,
+sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
                  const SelState *__restrict__ state, double thr,
                  unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq)
 {
@@ -134,10 +187,18 @@ sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is
     const unsigned int kth = THR ? 0u : state->prefix;
     const SelSeg sg = sel_segment(n, seg);
     unsigned int gt = 0, eq = 0;
-    for (long i = sg.begin + threadIdx.x; i < sg.end; i += SEL_THREADS) {
-        const int c = sel_class<THR>(vals[i], is_int, kth, thr);
-        gt += c == 2;
-        eq += c == 1;
+    for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
+        unsigned int b0[4], b1[4];
+        int n0, n1;
+        sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, n0);
+        sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, n1);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int c0 = c < n0 ? sel_class<THR>(b0[c], is_int, kth, thr) : 0;
+            const int c1 = c < n1 ? sel_class<THR>(b1[c], is_int, kth, thr) : 0;
+            gt += (c0 == 2) + (c1 == 2);
+            eq += (c0 == 1) + (c1 == 1);
+        }
     }
     for (int o = 16; o; o >>= 1) {
         gt += __shfl_xor_sync(0xffffffffu, gt, o);
@@ -148,28 +209,49 @@ sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is
     if (threadIdx.x == 0) { blk_gt[blockIdx.x] = s_gt; blk_eq[blockIdx.x] = s_eq; }
 }
 
-// exclusive scan of the per-block counts (one thread: at most SEL_MAX_BLOCKS entries)
-__global__ void __launch_bounds__(1)
+// exclusive scan of the per-block counts (at most SEL_MAX_BLOCKS = 8 * 256 entries: thread t owns 8)
+__global__ void __launch_bounds__(256)
 sel_scan_kernel(unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq, int n_blocks,
                 unsigned long long *__restrict__ off_gt, unsigned long long *__restrict__ off_eq,
                 SelState *__restrict__ state)
 {
+    __shared__ unsigned long long pa[256], pb[256];
     unsigned long long a = 0, b = 0;
-    for (int q = 0; q < n_blocks; ++q) {
-        off_gt[q] = a;
-        off_eq[q] = b;
-        a += blk_gt[q];
-        b += blk_eq[q];
+    for (int c = 0; c < 8; ++c) {
+        const int q = 8 * threadIdx.x + c;
+        if (q < n_blocks) { a += blk_gt[q]; b += blk_eq[q]; }
     }
-    state->count = a;
+    pa[threadIdx.x] = a;
+    pb[threadIdx.x] = b;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long sa = 0, sb = 0;
+        for (int t = 0; t < 256; ++t) {
+            const unsigned long long ta = pa[t], tb = pb[t];
+            pa[t] = sa; pb[t] = sb;
+            sa += ta; sb += tb;
+        }
+        state->count = sa;
+    }
+    __syncthreads();
+    a = pa[threadIdx.x];
+    b = pb[threadIdx.x];
+    for (int c = 0; c < 8; ++c) {
+        const int q = 8 * threadIdx.x + c;
+        if (q < n_blocks) { off_gt[q] = a; off_eq[q] = b; a += blk_gt[q]; b += blk_eq[q]; }
+    }
 }
 
-// block-wide exclusive scan of a 0/1 flag; returns this thread's rank and the block total
-__device__ __forceinline__ unsigned int sel_block_rank(bool flag, unsigned int *warp_tot, unsigned int &total)
+// block-wide exclusive scan of a small per-thread count; returns this thread's offset and the block total
+__device__ __forceinline__ unsigned int sel_block_scan(unsigned int cnt, unsigned int *warp_tot, unsigned int &total)
 {
     const unsigned int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned int m = __ballot_sync(0xffffffffu, flag);
-    if (lane == 0) warp_tot[warp] = __popc(m);
+    unsigned int inc = cnt;
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int up = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= (unsigned int)o) inc += up;
+    }
+    if (lane == 31) warp_tot[warp] = inc;
     __syncthreads();
     unsigned int base = 0, tot = 0;
     for (unsigned int w = 0; w < SEL_THREADS / 32; ++w) {
@@ -179,16 +261,19 @@ __device__ __forceinline__ unsigned int sel_block_rank(bool flag, unsigned int *
     }
     __syncthreads();
     total = tot;
-    return base + __popc(m & ((1u << lane) - 1u));
+    return base + inc - cnt;
 }
 
 // THR: out_idx[rank] = i for the values above the threshold, ascending i, up to `capacity`.
 // top-K: candidates (raw bits, index) -> cand_bits / cand_idx [k_eff]: the keys above the K-th
-// first (any order: they are sorted afterwards), then the lowest-index keys equal to it.
+// first (in index order; they are sorted afterwards), then the lowest-index keys equal to it.
+// A CTA whose segment holds no candidate (known from the count pass) reads nothing; a tile with no
+// candidate costs one vector load and one barrier.
 template <bool THR>
 __global__ void __launch_bounds__(SEL_THREADS)
-sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int,
+sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
                    const SelState *__restrict__ state, double thr,
+                   const unsigned int *__restrict__ blk_gt, const unsigned int *__restrict__ blk_eq,
                    const unsigned long long *__restrict__ off_gt, const unsigned long long *__restrict__ off_eq,
                    long capacity, unsigned int *__restrict__ cand_bits, long long *__restrict__ out_idx)
 {
@@ -197,28 +282,41 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
     const unsigned long long n_greater = THR ? 0ull : state->n_greater;
     const unsigned long long eq_budget = THR ? 0ull : state->k_rem;
     unsigned long long base_gt = off_gt[blockIdx.x], base_eq = off_eq[blockIdx.x];
+    const bool want_eq = !THR && blk_eq[blockIdx.x] != 0 && base_eq < eq_budget;
+    if (blk_gt[blockIdx.x] == 0 && !want_eq) return;
+    if (THR && (long)base_gt >= capacity) return;
     const SelSeg sg = sel_segment(n, seg);
-    for (long i0 = sg.begin; i0 < sg.end; i0 += SEL_THREADS) {
-        const long i = i0 + threadIdx.x;
-        const unsigned int bits = i < sg.end ? vals[i] : 0u;
-        const int c = i < sg.end ? sel_class<THR>(bits, is_int, kth, thr) : 0;
+    for (long t0 = sg.begin; t0 < sg.end; t0 += SEL_TILE) {
+        const long i = t0 + 4 * threadIdx.x;
+        unsigned int b[4];
+        int nv, cls[4];
+        sel_load4(vals, i, sg.end, vec != 0, b, nv);
+        unsigned int c2 = 0, c1 = 0;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            cls[c] = c < nv ? sel_class<THR>(b[c], is_int, kth, thr) : 0;
+            c2 += cls[c] == 2;
+            c1 += cls[c] == 1;
+        }
+        if (!__syncthreads_or((int)(c2 | c1))) continue;
         unsigned int tot;
-        const unsigned int r2 = sel_block_rank(c == 2, wt, tot);
-        if (c == 2) {
-            const unsigned long long pos = base_gt + r2;
-            if (THR) { if ((long)pos < capacity) out_idx[pos] = i; }
-            else { cand_bits[pos] = bits; out_idx[pos] = i; }
-        }
-        base_gt += tot;
-        if (!THR) {
-            const unsigned int r1 = sel_block_rank(c == 1, wt, tot);
-            if (c == 1 && base_eq + r1 < eq_budget) {
-                const unsigned long long pos = n_greater + base_eq + r1;
-                cand_bits[pos] = bits;
-                out_idx[pos] = i;
+        unsigned int r2 = sel_block_scan(c2, wt, tot);
+        const unsigned int tot2 = tot;
+        unsigned int r1 = 0, tot1 = 0;
+        if (!THR) { r1 = sel_block_scan(c1, wt, tot); tot1 = tot; }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            if (cls[c] == 2) {
+                const unsigned long long pos = base_gt + r2++;
+                if (THR) { if ((long)pos < capacity) out_idx[pos] = i + c; }
+                else { cand_bits[pos] = b[c]; out_idx[pos] = i + c; }
+            } else if (!THR && cls[c] == 1) {
+                const unsigned long long q = base_eq + r1++;
+                if (q < eq_budget) { cand_bits[n_greater + q] = b[c]; out_idx[n_greater + q] = i + c; }
             }
-            base_eq += tot;
         }
+        base_gt += tot2;
+        base_eq += tot1;
     }
 }
 

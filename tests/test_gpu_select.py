@@ -50,6 +50,22 @@ def test_topk_special_values(handle):
     _check_topk(handle, np.full(5000, 2.5, dtype=np.float32), 7)               # all equal: indices 0..6
 
 
+def test_unaligned_array_start(handle):
+    """An array that starts 4 bytes into a 16-byte line takes the scalar-load path."""
+    import torch
+    rng = np.random.default_rng(9)
+    v = rng.standard_normal(50_001).astype(np.float32)
+    d = torch.from_numpy(v).cuda()[1:]
+    assert d.data_ptr() % 16 == 4
+    val, idx, cnt = handle.topk(d, 33)
+    sidx, scnt = handle.select_above(d, 1.0, 50_000)
+    torch.cuda.synchronize()
+    rv, ri = select.topk(v[1:], 33)
+    assert np.array_equal(idx.cpu().numpy(), ri) and np.array_equal(val.cpu().numpy(), rv)
+    ref = select.select_above(v[1:], 1.0)
+    assert int(scnt.item()) == ref.size and np.array_equal(sidx.cpu().numpy()[:ref.size], ref)
+
+
 def test_topk_int32(handle):
     rng = np.random.default_rng(3)
     v = rng.integers(-50, 50, size=200_001).astype(np.int32)
