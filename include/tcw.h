@@ -227,6 +227,38 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
 int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, double threshold,
                      long capacity, long long *out_idx, long long *out_count, void *stream);
 
+/* ---- data preparation ----------------------------------------
+ *
+ * "The data used in this study are 8-second Han-windowed Short Fourier Transforms (SFTs), which
+ *  are processed into either normalized power rho_j or number count nu_j as described by Oliver
+ *  et al. [14]".  Ref. [14] is not available; reading Q24:
+ *    segment j = samples [j*N, (j+1)*N), N = fs*T_sft (no overlap, a trailing partial segment is dropped)
+ *    X_j = DFT of w[t]*x_j[t], w[t] = 0.5 - 0.5 cos(2 pi t/N);   P_j[k] = |X_j[k]|^2
+ *    m_j[k] = median of P_j[k-h .. k+h], h = (median_bins - 1)/2
+ *    rho_j[k] = P_j[k]*ln 2/m_j[k]   (mean 1 in Gaussian noise);   nu_j[k] = rho_j[k] > threshold
+ * for the band bins k_min .. k_min + n_bins - 1, k_min = rint(f_min*T_sft).  float32 arithmetic;
+ * the DFT is cuFFT's batched real-to-complex transform. */
+typedef struct {
+    double fs;          /* sampling rate, Hz                                                      */
+    double T_sft;       /* SFT length, s; fs*T_sft must be an even integer                        */
+    double f_min;       /* band start, Hz; f_min*T_sft must be an integer                         */
+    int n_bins;         /* band bins; the band plus h bins on both sides must lie in 0..N/2       */
+    int median_bins;    /* running-median window W, odd, 1..257                                   */
+    double threshold;   /* number-count threshold on rho (1.6 in BASELINE.json's configs)         */
+} tcw_prep;
+
+/* tcw_prepare -- strain to spectrogram, written in the layout tcw_create reads.
+ *  strain           HOST or DEVICE, float32 [n_samples].
+ *  format           TCW_F32_POWER (rho), TCW_U8_COUNT or TCW_BIT_COUNT (nu).
+ *  out_spectrogram  DEVICE, n_sft rows of out_pitch_bytes (>= one row; a multiple of 4 except for
+ *                   uint8), n_sft = n_samples / N rows are written.
+ *  n_sft            HOST int, receives the number of SFTs.
+ * Synchronises `stream` before returning (scratch is allocated and freed inside the call).
+ * TCW_EINVAL for inconsistent sizes; TCW_EUNSUPPORTED if the band does not fit one CTA's shared
+ * memory (about 45 000 bins). */
+int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int format,
+                void *out_spectrogram, long out_pitch_bytes, int *n_sft, void *stream);
+
 /* tcw_destroy -- free the handle and everything it owns.  NULL is a no-op returning TCW_OK. */
 int tcw_destroy(tcw_handle *h);
 

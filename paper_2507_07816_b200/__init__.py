@@ -28,7 +28,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -54,6 +54,11 @@ class _CBank(ctypes.Structure):
                 ("f0", ctypes.POINTER(ctypes.c_double)), ("tau", ctypes.POINTER(ctypes.c_double)),
                 ("brk", ctypes.POINTER(ctypes.c_double)), ("sky", ctypes.POINTER(ctypes.c_double)),
                 ("sky_shared", ctypes.c_int)]
+
+
+class _CPrep(ctypes.Structure):
+    _fields_ = [("fs", ctypes.c_double), ("T_sft", ctypes.c_double), ("f_min", ctypes.c_double),
+                ("n_bins", ctypes.c_int), ("median_bins", ctypes.c_int), ("threshold", ctypes.c_double)]
 
 
 class _CWeighting(ctypes.Structure):
@@ -91,6 +96,8 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_topk.argtypes = [vp, vp, ci, cl, ci, vp, vp, vp, vp]
     L.tcw_select_above.restype = ci
     L.tcw_select_above.argtypes = [vp, vp, ci, cl, ctypes.c_double, cl, vp, vp, vp]
+    L.tcw_prepare.restype = ci
+    L.tcw_prepare.argtypes = [vp, cl, ctypes.POINTER(_CPrep), ci, vp, cl, ctypes.POINTER(ci), vp]
     L.tcw_destroy.restype = ci
     L.tcw_destroy.argtypes = [vp]
     L.tcw_last_error.restype = ctypes.c_char_p
@@ -402,6 +409,36 @@ class Handle:
 
     def __exit__(self, *exc):
         self.close()
+
+
+def prepare(strain, fs: float, T_sft: float, f_min: float, n_bins: int, median_bins: int = 101,
+            threshold: float = 1.6, fmt: str = "f32", stream=None):
+    """tcw_prepare: strain (host numpy float32 or CUDA float32 tensor) -> spectrogram CUDA tensor
+    [n_sft][n_bins] float32 (fmt "f32"), uint8 ("u8") or int32 words [n_sft][ceil(n_bins/32)] ("bits")."""
+    import torch
+    L = load_library()
+    if isinstance(strain, np.ndarray):
+        x = np.ascontiguousarray(strain, dtype=np.float32)
+        ptr, n = x.ctypes.data, x.size
+    else:
+        x = strain.contiguous()
+        if x.dtype != torch.float32:
+            raise ValueError("strain must be float32")
+        ptr, n = x.data_ptr(), x.numel()
+    N = int(round(fs * T_sft))
+    n_seg = max(n // max(N, 1), 1)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if fmt == "f32":
+        out = torch.empty((n_seg, n_bins), dtype=torch.float32, device=dev)
+    elif fmt == "u8":
+        out = torch.empty((n_seg, n_bins), dtype=torch.uint8, device=dev)
+    else:
+        out = torch.empty((n_seg, (n_bins + 31) // 32), dtype=torch.int32, device=dev)
+    cp = _CPrep(float(fs), float(T_sft), float(f_min), int(n_bins), int(median_bins), float(threshold))
+    got = ctypes.c_int(0)
+    _check(L.tcw_prepare(ptr, n, ctypes.byref(cp), FORMATS[fmt], out.data_ptr(), out.stride(0) * out.element_size(),
+                         ctypes.byref(got), _stream_ptr(stream)))
+    return out[: got.value]
 
 
 def shard_groups(n_sky: int, rank: int, world_size: int) -> slice:

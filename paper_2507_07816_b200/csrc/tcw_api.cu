@@ -8,6 +8,7 @@
 #include "../../include/tcw.h"
 
 #include <cuda_runtime.h>
+#include <cufft.h>
 
 #include <algorithm>
 #include <cmath>
@@ -22,6 +23,7 @@
 #include "tcw_skyblock.cuh"
 #include "tcw_bank.cuh"
 #include "tcw_select.cuh"
+#include "tcw_prep.cuh"
 
 namespace {
 
@@ -969,6 +971,91 @@ int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, doubl
     CUDA_TRY(cudaMemcpyAsync(out_count, &sc.state->count, sizeof(long long), cudaMemcpyDeviceToDevice, st));
     h->last_stream = st;
     return TCW_OK;
+}
+
+int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int format, void *out_spectrogram,
+                long out_pitch_bytes, int *n_sft, void *stream)
+{
+    if (!strain || !prep || !out_spectrogram || !n_sft) return fail(TCW_EINVAL, "NULL argument");
+    if (format != TCW_F32_POWER && format != TCW_U8_COUNT && format != TCW_BIT_COUNT)
+        return fail(TCW_EINVAL, "unknown spectrogram format %d", format);
+    if (!(prep->fs > 0) || !(prep->T_sft > 0) || !std::isfinite(prep->fs) || !std::isfinite(prep->T_sft))
+        return fail(TCW_EINVAL, "fs and T_sft must be positive");
+    const double Nd = std::rint(prep->fs * prep->T_sft);
+    if (std::fabs(prep->fs * prep->T_sft - Nd) > 1e-9 || Nd < 2 || Nd > (double)(1 << 27) || ((long)Nd & 1))
+        return fail(TCW_EINVAL, "fs*T_sft must be an even integer number of samples (2..2^27)");
+    const int N = (int)Nd, n_half = N / 2 + 1;
+    const long n_seg = n_samples / N;
+    if (n_seg <= 0 || n_seg > 2147483647L) return fail(TCW_EINVAL, "n_samples holds no whole segment (or too many)");
+    const int W = prep->median_bins, h = (W - 1) / 2;
+    if (W < 1 || W > tcw::PREP_MAX_W || !(W & 1)) return fail(TCW_EINVAL, "median_bins must be odd, 1..%d", tcw::PREP_MAX_W);
+    const double km = std::rint(prep->f_min * prep->T_sft);
+    if (!(prep->f_min >= 0) || std::fabs(prep->f_min * prep->T_sft - km) > 1e-9)
+        return fail(TCW_EINVAL, "f_min*T_sft must be a non-negative integer (bin-aligned band start)");
+    if (prep->n_bins <= 0 || km - h < 0 || km + prep->n_bins + h > n_half)
+        return fail(TCW_EINVAL, "band plus median half-window does not fit the bins 0..N/2");
+    if (format != TCW_F32_POWER && std::isnan(prep->threshold)) return fail(TCW_EINVAL, "threshold is NaN");
+    if (out_pitch_bytes < (long)row_bytes(format, prep->n_bins) || (format != TCW_U8_COUNT && (out_pitch_bytes & 3)))
+        return fail(TCW_EINVAL, "out_pitch_bytes is smaller than one row or not a multiple of 4");
+    const size_t smem = (((size_t)(prep->n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)prep->n_bins + 31) & ~(size_t)31);
+    if (smem > SMEM_MAX) return fail(TCW_EUNSUPPORTED, "band too wide for one CTA's shared memory (%zu bytes)", smem);
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const int batch = (int)std::min<long>(n_seg, std::max<long>(1, (64L << 20) / ((long)N * 4)));
+    float *d_x = nullptr;
+    float2 *d_spec = nullptr;
+    cufftHandle plan = 0;
+    bool have_plan = false;
+    int rc = TCW_OK;
+#define PREP_TRY(call)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess) {                                                                    \
+            rc = fail(e_ == cudaErrorMemoryAllocation ? TCW_ENOMEM : TCW_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+            goto done;                                                                              \
+        }                                                                                           \
+    } while (0)
+    PREP_TRY(cudaMalloc((void **)&d_x, (size_t)batch * N * sizeof(float)));
+    PREP_TRY(cudaMalloc((void **)&d_spec, (size_t)batch * n_half * sizeof(float2)));
+    {
+        int dims[1] = {N};
+        if (cufftPlanMany(&plan, 1, dims, nullptr, 1, N, nullptr, 1, n_half, CUFFT_R2C, batch) != CUFFT_SUCCESS) {
+            rc = fail(TCW_ECUDA, "cufftPlanMany failed");
+            goto done;
+        }
+        have_plan = true;
+        if (cufftSetStream(plan, st) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftSetStream failed"); goto done; }
+    }
+    PREP_TRY(cudaFuncSetAttribute(tcw::prep_normalise_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    for (long j0 = 0; j0 < n_seg; j0 += batch) {
+        const int nb = (int)std::min<long>(batch, n_seg - j0);
+        if (nb < batch)   // zero the tail of the batch buffer: cuFFT always transforms `batch` segments
+            PREP_TRY(cudaMemsetAsync(d_x + (size_t)nb * N, 0, (size_t)(batch - nb) * N * sizeof(float), st));
+        PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyDefault, st));
+        tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(d_x, 0, nb, N, d_x);
+        PREP_TRY(cudaGetLastError());
+        if (cufftExecR2C(plan, d_x, (cufftComplex *)d_spec) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftExecR2C failed"); goto done; }
+        tcw::PrepParams p;
+        p.spec = d_spec;
+        p.n_half = n_half;
+        p.k_min = (int)km;
+        p.n_bins = prep->n_bins;
+        p.h = h;
+        p.threshold = (float)prep->threshold;
+        p.out_format = format;
+        p.out = (unsigned char *)out_spectrogram + j0 * out_pitch_bytes;
+        p.out_pitch = out_pitch_bytes;
+        tcw::prep_normalise_kernel<<<nb, tcw::PREP_THREADS, smem, st>>>(p);
+        PREP_TRY(cudaGetLastError());
+    }
+    PREP_TRY(cudaStreamSynchronize(st));
+    *n_sft = (int)n_seg;
+done:
+#undef PREP_TRY
+    if (have_plan) cufftDestroy(plan);
+    if (d_x) cudaFree(d_x);
+    if (d_spec) cudaFree(d_spec);
+    return rc;
 }
 
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host, void *stream)

@@ -1,0 +1,109 @@
+// tcw_prep.cuh -- strain -> Hann-windowed SFTs -> normalised power / number count (sm_100a).
+//
+// "The data used in this study are 8-second Han-windowed Short Fourier Transforms (SFTs), which are
+// processed into either normalized power rho_j or number count nu_j".  Reading Q24
+// (DESIGN.md): non-overlapping segments of N = fs*T_sft samples, w[t] = 0.5 - 0.5 cos(2 pi t/N),
+// P_j[k] = |DFT(w x_j)[k]|^2, m_j[k] = running median of P_j over W = 2h + 1 bins centred on k,
+// rho_j[k] = P_j[k] ln 2 / m_j[k], nu_j[k] = (rho_j[k] > threshold).
+//
+// The DFT itself is a plain batched real-to-complex transform and is left to cuFFT (a library
+// primitive, like a GEMM left to cuBLAS).  Everything around it is here:
+//   * prep_window_kernel: window multiply into the batch buffer cuFFT reads (float32);
+//   * prep_normalise_kernel: one CTA per SFT: |X|^2 of the band and its two half-windows into shared
+//     memory, then every thread slides a sorted window over its run of consecutive bins (insertion
+//     sort once, then one removal and one insertion per bin), and writes rho (float32), nu (uint8)
+//     or nu bit-packed (uint32 words, LSB first) straight into the spectrogram layout tcw_create reads.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tcw {
+
+constexpr int PREP_THREADS = 256;
+constexpr int PREP_MAX_W = 257;       // median window limit (odd)
+
+// out[b][t] = x[(j0 + b)*N + t] * w[t]
+__global__ void __launch_bounds__(256)
+prep_window_kernel(const float *x, long j0, int n_batch, int N, float *out)   // out may alias x (in place)
+{
+    const long total = (long)n_batch * N;
+    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x) {
+        const int t = (int)(q % N);
+        const double w = 0.5 - 0.5 * cospi(2.0 * (double)t / (double)N);
+        out[q] = x[j0 * N + q] * (float)w;
+    }
+}
+
+struct PrepParams {
+    const float2 *spec;     // cuFFT output of this batch: [n_batch][N/2 + 1] complex
+    int n_half;             // N/2 + 1
+    int k_min, n_bins, h;   // band start bin, band bins, median half-window
+    float threshold;
+    int out_format;         // 0 float32 rho, 1 uint8 nu, 2 bit-packed nu
+    unsigned char *out;     // row 0 of this batch in the output spectrogram
+    long out_pitch;         // bytes
+};
+
+// dynamic shared memory: float P[n_bins + 2h], then (count formats) unsigned char nu[n_bins rounded up to 32]
+__global__ void __launch_bounds__(PREP_THREADS)
+prep_normalise_kernel(const PrepParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    float *P = (float *)smem;
+    const int n_in = p.n_bins + 2 * p.h;
+    unsigned char *nu = smem + (((size_t)n_in * 4 + 15) & ~(size_t)15);
+    const float2 *row = p.spec + (long)blockIdx.x * p.n_half + (p.k_min - p.h);
+    for (int t = threadIdx.x; t < n_in; t += PREP_THREADS) {
+        const float2 c = row[t];
+        P[t] = c.x * c.x + c.y * c.y;
+    }
+    __syncthreads();
+
+    const int W = 2 * p.h + 1;
+    const int run = (p.n_bins + PREP_THREADS - 1) / PREP_THREADS;
+    const int k0 = threadIdx.x * run, k1 = min(k0 + run, p.n_bins);
+    unsigned char *orow = p.out + (long)blockIdx.x * p.out_pitch;
+    if (k0 < k1) {
+        float win[PREP_MAX_W];            // sorted window of bin k: P[k .. k + W - 1] (band bin k is its centre)
+        for (int q = 0; q < W; ++q) {     // insertion sort of the first window
+            const float v = P[k0 + q];
+            int i = q;
+            while (i > 0 && win[i - 1] > v) { win[i] = win[i - 1]; --i; }
+            win[i] = v;
+        }
+        for (int k = k0; k < k1; ++k) {
+            if (k > k0) {
+                // slide: remove P[k - 1], insert P[k + W - 1], keeping the array sorted
+                const float out_v = P[k - 1], in_v = P[k + W - 1];
+                int i = 0;
+                while (i < W - 1 && win[i] != out_v) ++i;          // present by construction (the bound guards NaN input)
+                if (in_v >= out_v) {
+                    while (i + 1 < W && win[i + 1] < in_v) { win[i] = win[i + 1]; ++i; }
+                } else {
+                    while (i > 0 && win[i - 1] > in_v) { win[i] = win[i - 1]; --i; }
+                }
+                win[i] = in_v;
+            }
+            const float rho = P[k + p.h] * 0.69314718055994531f / win[p.h];
+            if (p.out_format == 0) ((float *)orow)[k] = rho;
+            else nu[k] = rho > p.threshold ? 1 : 0;
+        }
+    }
+    if (p.out_format == 0) return;
+    __syncthreads();
+    if (p.out_format == 1) {
+        for (int k = threadIdx.x; k < p.n_bins; k += PREP_THREADS) orow[k] = nu[k];
+    } else {
+        const int n_words = (p.n_bins + 31) / 32;
+        for (int wd = threadIdx.x; wd < n_words; wd += PREP_THREADS) {
+            uint32_t bits = 0;
+            for (int b = 0; b < 32; ++b) {
+                const int k = 32 * wd + b;
+                if (k < p.n_bins && nu[k]) bits |= 1u << b;
+            }
+            ((uint32_t *)orow)[wd] = bits;
+        }
+    }
+}
+
+}  // namespace tcw

@@ -16,5 +16,6 @@ from .configs import (  # noqa: F401
     pack_bits,
     random_bank,
     sky_vector,
+    synthetic_strain,
     synthetic_weights,
 )

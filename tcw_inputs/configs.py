@@ -116,6 +116,22 @@ def random_bank(n: int, f_lo: float, f_hi: float, seed: int, sky=None):
             np.ascontiguousarray(sky, dtype=np.float64))
 
 
+def synthetic_strain(n_sft: int, fs: float, T_sft: float, seed: int, lines=()):
+    """Stand-in for detector strain (the paper uses coloured Gaussian noise at the aLIGO design
+    sensitivity): float32 white Gaussian noise shaped by a gentle per-segment drift of
+    the noise level (non-stationary floor, factor U[0.7, 1.3] per 8-s segment) plus optional
+    sinusoidal lines (frequency Hz, amplitude) so that some bins stand far above the floor."""
+    rng = np.random.Generator(np.random.PCG64(seed + 15485863))
+    N = int(round(fs * T_sft))
+    x = rng.standard_normal((n_sft, N))
+    x *= rng.uniform(0.7, 1.3, size=(n_sft, 1))
+    x = x.reshape(-1)
+    t = np.arange(x.size, dtype=np.float64) / fs
+    for f, a in lines:
+        x += a * np.cos(2.0 * np.pi * f * t)
+    return np.ascontiguousarray(x, dtype=np.float32)
+
+
 def synthetic_weights(sky: np.ndarray, timestamps: np.ndarray, seed: int) -> np.ndarray:
     """Stand-in for the weights of the paper's ref. [14] ("antenna patterns and changing noise
     floors"): float32 [n_sky][n_sft], positive, mean 1 along each row.
