@@ -484,6 +484,43 @@ def run_select(args):
     return 0
 
 
+# ----------------------------------------------------------------------------- data preparation mode (NEXT-3)
+def run_prep(args):
+    """--prep N_SFT: tcw_prepare on N_SFT 8-s segments of synthetic strain at 4096 Hz (device-resident),
+    band 500-1000 Hz (4000 bins), running median over 101 bins, bit-packed number count output: the
+    step that produces cfg3's input.  HBM model: one read of the strain (4 B/sample)."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    import tcw_inputs
+
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    fs, T = 4096.0, 8.0
+    n_sft = args.prep
+    g = torch.Generator(device="cuda").manual_seed(2)
+    x = torch.randn(n_sft * int(fs * T), generator=g, device="cuda", dtype=torch.float32)
+    peak, peak_src = load_peaks()
+    res = {}
+    for fmt in ("f32", "bits"):
+        for _ in range(max(2, min(args.warmup, 3))):
+            tcw.prepare(x, fs, T, 500.0, 4000, 101, 1.6, fmt)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            tcw.prepare(x, fs, T, 500.0, 4000, 101, 1.6, fmt)      # synchronises its stream
+        ms = 1e3 * (time.perf_counter() - t0) / args.steps
+        gbs = 4.0 * x.numel() / (ms * 1e-3) / 1e9
+        res[fmt] = {"ms": ms, "sfts_per_s": n_sft / (ms * 1e-3), "samples_per_s": x.numel() / (ms * 1e-3),
+                    "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                                 "traffic": None, "peak_source": peak_src}}
+    print(json.dumps({"metric": "SFTs prepared per second (tcw_prepare: window, cuFFT R2C, running median, normalise, threshold)",
+                      "n_sft": n_sft, "fs": fs, "T_sft": T, "band_bins": 4000, "median_bins": 101, "steps": args.steps,
+                      "data": "synthetic", "timing": "host wall clock around the synchronous call (includes plan creation and scratch allocation)",
+                      "results": res}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -502,11 +539,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bank", type=int, default=0, help="time tcw_search_bank on this many random templates (NEXT-2)")
     ap.add_argument("--select", type=int, default=0, help="time tcw_topk / tcw_select_above over this many float32 values (NEXT-4)")
+    ap.add_argument("--prep", type=int, default=0, help="time tcw_prepare on this many 8-s SFTs of synthetic strain (NEXT-3)")
     ap.add_argument("--weighted", action="store_true",
                     help="time tcw_search_weighted (weighted statistic + critical ratio, NEXT-1) instead of tcw_search")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    if args.prep and args.impl == "ours":
+        return run_prep(args)
     if args.select and args.impl == "ours":
         return run_select(args)
     if args.bank and args.impl == "ours":

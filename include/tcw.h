@@ -243,7 +243,7 @@ typedef struct {
     double T_sft;       /* SFT length, s; fs*T_sft must be an even integer                        */
     double f_min;       /* band start, Hz; f_min*T_sft must be an integer                         */
     int n_bins;         /* band bins; the band plus h bins on both sides must lie in 0..N/2       */
-    int median_bins;    /* running-median window W, odd, 1..257                                   */
+    int median_bins;    /* running-median window W, odd, 1..1025                                  */
     double threshold;   /* number-count threshold on rho (1.6 in BASELINE.json's configs)         */
 } tcw_prep;
 

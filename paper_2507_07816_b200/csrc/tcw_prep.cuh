@@ -10,9 +10,9 @@
 // primitive, like a GEMM left to cuBLAS).  Everything around it is here:
 //   * prep_window_kernel: window multiply into the batch buffer cuFFT reads (float32);
 //   * prep_normalise_kernel: one CTA per SFT: |X|^2 of the band and its two half-windows into shared
-//     memory, then every thread slides a sorted window over its run of consecutive bins (insertion
-//     sort once, then one removal and one insertion per bin), and writes rho (float32), nu (uint8)
-//     or nu bit-packed (uint32 words, LSB first) straight into the spectrogram layout tcw_create reads.
+//     memory, then every thread walks a run of consecutive bins keeping the running median by
+//     counting (see the kernel), and writes rho (float32), nu (uint8) or nu bit-packed (uint32
+//     words, LSB first) straight into the spectrogram layout tcw_create reads.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -20,7 +20,7 @@
 namespace tcw {
 
 constexpr int PREP_THREADS = 256;
-constexpr int PREP_MAX_W = 257;       // median window limit (odd)
+constexpr int PREP_MAX_W = 1025;      // median window limit (odd)
 
 // out[b][t] = x[(j0 + b)*N + t] * w[t]
 __global__ void __launch_bounds__(256)
@@ -45,7 +45,7 @@ struct PrepParams {
 };
 
 // dynamic shared memory: float P[n_bins + 2h], then (count formats) unsigned char nu[n_bins rounded up to 32]
-__global__ void __launch_bounds__(PREP_THREADS)
+__global__ void __launch_bounds__(256)
 prep_normalise_kernel(const PrepParams p)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -53,38 +53,49 @@ prep_normalise_kernel(const PrepParams p)
     const int n_in = p.n_bins + 2 * p.h;
     unsigned char *nu = smem + (((size_t)n_in * 4 + 15) & ~(size_t)15);
     const float2 *row = p.spec + (long)blockIdx.x * p.n_half + (p.k_min - p.h);
-    for (int t = threadIdx.x; t < n_in; t += PREP_THREADS) {
+    for (int t = threadIdx.x; t < n_in; t += (int)blockDim.x) {
         const float2 c = row[t];
         P[t] = c.x * c.x + c.y * c.y;
     }
     __syncthreads();
 
-    const int W = 2 * p.h + 1;
-    const int run = (p.n_bins + PREP_THREADS - 1) / PREP_THREADS;
-    const int k0 = threadIdx.x * run, k1 = min(k0 + run, p.n_bins);
+    // Running median without per-thread sorted arrays (those live in local memory and serialise):
+    // the first bin of a thread's run selects the rank-h value of its window by a bitwise binary
+    // search on the float bits (P >= 0, so the bits order like the values); every further bin
+    // re-counts the slid window against the previous median m.  One element left and one entered,
+    // so #(x < m) <= h + 1 and #(x <= m) >= h: the new median is m, or the largest element below it,
+    // or the smallest element above it.  All reads are conflict-free shared-memory loads.
+    const int W = 2 * p.h + 1, h = p.h;
+    // an odd run length: lanes then start 'run' words apart, which visits all 32 banks (no conflicts)
+    const int run = ((p.n_bins + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
+    const int k0 = min((int)threadIdx.x * run, p.n_bins), k1 = min(k0 + run, p.n_bins);
     unsigned char *orow = p.out + (long)blockIdx.x * p.out_pitch;
     if (k0 < k1) {
-        float win[PREP_MAX_W];            // sorted window of bin k: P[k .. k + W - 1] (band bin k is its centre)
-        for (int q = 0; q < W; ++q) {     // insertion sort of the first window
-            const float v = P[k0 + q];
-            int i = q;
-            while (i > 0 && win[i - 1] > v) { win[i] = win[i - 1]; --i; }
-            win[i] = v;
+        const unsigned int *Pu = (const unsigned int *)P;
+        unsigned int key = 0;
+        for (int bit = 30; bit >= 0; --bit) {
+            const unsigned int cand = key | (1u << bit);
+            int c = 0;
+            for (int q = 0; q < W; ++q) c += Pu[k0 + q] < cand;
+            if (c <= h) key = cand;
         }
+        float m = __uint_as_float(key);
         for (int k = k0; k < k1; ++k) {
             if (k > k0) {
-                // slide: remove P[k - 1], insert P[k + W - 1], keeping the array sorted
-                const float out_v = P[k - 1], in_v = P[k + W - 1];
-                int i = 0;
-                while (i < W - 1 && win[i] != out_v) ++i;          // present by construction (the bound guards NaN input)
-                if (in_v >= out_v) {
-                    while (i + 1 < W && win[i + 1] < in_v) { win[i] = win[i + 1]; ++i; }
-                } else {
-                    while (i > 0 && win[i - 1] > in_v) { win[i] = win[i - 1]; --i; }
+                int c_less = 0, c_leq = 0;
+                float pred = -__int_as_float(0x7f800000), succ = __int_as_float(0x7f800000);
+                for (int q = 0; q < W; ++q) {
+                    const float x = P[k + q];
+                    const bool lt = x < m, gt = x > m;
+                    c_less += lt;
+                    c_leq += !gt;
+                    pred = fmaxf(pred, lt ? x : pred);
+                    succ = fminf(succ, gt ? x : succ);
                 }
-                win[i] = in_v;
+                if (c_less > h) m = pred;
+                else if (c_leq <= h) m = succ;
             }
-            const float rho = P[k + p.h] * 0.69314718055994531f / win[p.h];
+            const float rho = P[k + h] * 0.69314718055994531f / m;
             if (p.out_format == 0) ((float *)orow)[k] = rho;
             else nu[k] = rho > p.threshold ? 1 : 0;
         }
@@ -92,10 +103,10 @@ prep_normalise_kernel(const PrepParams p)
     if (p.out_format == 0) return;
     __syncthreads();
     if (p.out_format == 1) {
-        for (int k = threadIdx.x; k < p.n_bins; k += PREP_THREADS) orow[k] = nu[k];
+        for (int k = threadIdx.x; k < p.n_bins; k += (int)blockDim.x) orow[k] = nu[k];
     } else {
         const int n_words = (p.n_bins + 31) / 32;
-        for (int wd = threadIdx.x; wd < n_words; wd += PREP_THREADS) {
+        for (int wd = threadIdx.x; wd < n_words; wd += (int)blockDim.x) {
             uint32_t bits = 0;
             for (int b = 0; b < 32; ++b) {
                 const int k = 32 * wd + b;

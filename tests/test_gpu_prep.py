@@ -99,7 +99,7 @@ def test_prepared_spectrogram_feeds_the_search(tcw):
 
 def test_prepare_argument_errors(tcw):
     x = np.zeros(4096, dtype=np.float32)
-    bad = [dict(fs=63.9), dict(n_bins=0), dict(median_bins=4), dict(median_bins=301), dict(f_min=0.05),
+    bad = [dict(fs=63.9), dict(n_bins=0), dict(median_bins=4), dict(median_bins=2001), dict(f_min=0.05),
            dict(f_min=31.0, n_bins=40), dict(f_min=0.0, median_bins=9)]
     for kw in bad:
         args = dict(fs=64.0, T_sft=8.0, f_min=8.0, n_bins=64, median_bins=9, threshold=1.6)
