@@ -1003,9 +1003,14 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
 
     cudaStream_t st = (cudaStream_t)stream;
     const int batch = (int)std::min<long>(n_seg, std::max<long>(1, (64L << 20) / ((long)N * 4)));
-    float *d_x = nullptr;
+    float *d_x = nullptr, *d_win = nullptr;
     float2 *d_spec = nullptr;
     cufftHandle plan = 0;
+    // a device-resident strain is windowed straight out of the caller's buffer; a host one is staged
+    cudaPointerAttributes attr;
+    const bool on_device = cudaPointerGetAttributes(&attr, strain) == cudaSuccess &&
+                           (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
+    cudaGetLastError();   // a plain host pointer may leave an error state on older runtimes
     bool have_plan = false;
     int rc = TCW_OK;
 #define PREP_TRY(call)                                                                              \
@@ -1018,6 +1023,9 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     } while (0)
     PREP_TRY(cudaMalloc((void **)&d_x, (size_t)batch * N * sizeof(float)));
     PREP_TRY(cudaMalloc((void **)&d_spec, (size_t)batch * n_half * sizeof(float2)));
+    PREP_TRY(cudaMalloc((void **)&d_win, (size_t)N * sizeof(float)));
+    tcw::prep_window_table_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, d_win);
+    PREP_TRY(cudaGetLastError());
     {
         int dims[1] = {N};
         if (cufftPlanMany(&plan, 1, dims, nullptr, 1, N, nullptr, 1, n_half, CUFFT_R2C, batch) != CUFFT_SUCCESS) {
@@ -1032,8 +1040,9 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         const int nb = (int)std::min<long>(batch, n_seg - j0);
         if (nb < batch)   // zero the tail of the batch buffer: cuFFT always transforms `batch` segments
             PREP_TRY(cudaMemsetAsync(d_x + (size_t)nb * N, 0, (size_t)(batch - nb) * N * sizeof(float), st));
-        PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyDefault, st));
-        tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(d_x, 0, nb, N, d_x);
+        if (!on_device)
+            PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyHostToDevice, st));
+        tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(on_device ? strain + j0 * N : d_x, d_win, nb, N, d_x);
         PREP_TRY(cudaGetLastError());
         if (cufftExecR2C(plan, d_x, (cufftComplex *)d_spec) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftExecR2C failed"); goto done; }
         tcw::PrepParams p;
@@ -1055,6 +1064,7 @@ done:
 #undef PREP_TRY
     if (have_plan) cufftDestroy(plan);
     if (d_x) cudaFree(d_x);
+    if (d_win) cudaFree(d_win);
     if (d_spec) cudaFree(d_spec);
     return rc;
 }

@@ -22,16 +22,21 @@ namespace tcw {
 constexpr int PREP_THREADS = 256;
 constexpr int PREP_MAX_W = 1025;      // median window limit (odd)
 
-// out[b][t] = x[(j0 + b)*N + t] * w[t]
+// w[t] = 0.5 - 0.5 cos(2 pi t / N), evaluated once per call in binary64 and stored as float32
 __global__ void __launch_bounds__(256)
-prep_window_kernel(const float *x, long j0, int n_batch, int N, float *out)   // out may alias x (in place)
+prep_window_table_kernel(int N, float *__restrict__ w)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < N) w[t] = (float)(0.5 - 0.5 * cospi(2.0 * (double)t / (double)N));
+}
+
+// out[b][t] = x[b*N + t] * w[t]   (out may alias x: each element is read and written by one thread)
+__global__ void __launch_bounds__(256)
+prep_window_kernel(const float *x, const float *__restrict__ w, int n_batch, int N, float *out)
 {
     const long total = (long)n_batch * N;
-    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x) {
-        const int t = (int)(q % N);
-        const double w = 0.5 - 0.5 * cospi(2.0 * (double)t / (double)N);
-        out[q] = x[j0 * N + q] * (float)w;
-    }
+    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x)
+        out[q] = x[q] * __ldg(w + (int)(q % N));
 }
 
 struct PrepParams {
