@@ -345,3 +345,26 @@ def test_strided_device_spectrogram(tcw, cfg1):
         stat, _ = h.search(tcw.Grid.of(cfg1))
         torch.cuda.synchronize()
     assert_stat_parity(cfg1, stat.cpu().numpy().reshape(-1), oracle.evaluate(cfg1).stat)
+
+
+@pytest.mark.parametrize("fmt", ["f32", "u8"])
+def test_T0_after_the_last_sft_gives_empty_spans(tcw, cfg1, fmt):
+    """Degenerate span: every SFT is before T0 (reading Q2), so every statistic is 0, the best index 0,
+    Psi 0 and every bank template has no in-band SFT -- for each entry point and kernel."""
+    import torch
+    w = dataclasses.replace(cfg1.with_format(fmt), T0=float(cfg1.timestamps[-1]) + 1.0)
+    ref = oracle.evaluate(w)
+    assert not ref.stat.any() and not ref.n_inband.any()
+    for kernel in ("staged", "gather"):
+        got, bs, bi, _ = gpu_search(tcw, w, kernel=kernel)
+        assert not got.any() and not bs.any() and not bi.any()
+    many = dataclasses.replace(w, sky=tcw_inputs.fibonacci_cap(20, 1.0, 0.3, 5.0))
+    if fmt == "u8":
+        got, bs, bi, info = gpu_search(tcw, many)
+        assert info["kernel"] == "skyblock" and not got.any() and not bi.any()
+    with tcw.Handle.from_workload(w) as h:
+        psi, stat, best = h.search_weighted(tcw.Grid.of(w), None, 1.0, 1.0)
+        bstat, inband, _ = h.search_bank(w.f0, np.full(len(w.f0), 5000.0), np.full(len(w.f0), 5.0), w.sky[0], T0=w.T0)
+        torch.cuda.synchronize()
+        assert not psi.any().item() and not stat.any().item() and not best[:, 1].any().item()
+        assert not bstat.any().item() and not inband.any().item()
