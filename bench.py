@@ -388,6 +388,13 @@ def run_ours(args):
         cb = time_oracle(w, args.cpu_seconds)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
         line["cpu_baseline"]["templates_per_s"] = cb["templates"] / cb["seconds"]
+        # the same oracle on one thread (all cores and one core), a smaller sample
+        import oracle
+        all_threads = oracle.num_threads()
+        oracle.set_num_threads(1)
+        c1 = time_oracle(w, min(4.0, args.cpu_seconds))
+        oracle.set_num_threads(all_threads)
+        line["cpu_baseline"]["one_thread"] = {"value": c1["value"], "unit": UNIT, "cores": 1, "sample": c1["sample"]}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

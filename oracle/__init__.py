@@ -49,6 +49,8 @@ def lib() -> ctypes.CDLL:
         L.tcwo_kmin.restype = ctypes.c_long
         L.tcwo_kmin.argtypes = [ctypes.c_double, ctypes.c_double]
         L.tcwo_num_threads.restype = ctypes.c_int
+        L.tcwo_set_num_threads.restype = None
+        L.tcwo_set_num_threads.argtypes = [ctypes.c_int]
         L.tcwo_spindown_table.restype = None
         L.tcwo_spindown_table.argtypes = [ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp,
                                           ctypes.c_int, dp, dp, ctypes.c_void_p]
@@ -92,6 +94,10 @@ def _f64(a) -> np.ndarray:
 
 def num_threads() -> int:
     return int(lib().tcwo_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().tcwo_set_num_threads(int(n))
 
 
 def spindown(t: float, T0: float, tau: float, n: float) -> float:

@@ -79,6 +79,16 @@ long tcwo_kmin(double f_min, double T_sft)
     return (long)rint(f_min * T_sft);
 }
 
+/* OpenMP thread count of the following calls (bench.py times the oracle with all cores and with one) */
+void tcwo_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int tcwo_num_threads(void)
 {
 #ifdef _OPENMP
