@@ -71,6 +71,13 @@ enum {
  *  velocities      HOST, [n_sft][3], detector velocity wrt the SSB in m/s, equatorial frame.
  *  stream          cudaStream_t (NULL = default stream).  The stream is synchronised before
  *                  tcw_create returns.
+ *
+ * Device memory of the library (the spectrogram copy, tables, scratch) comes from a library-owned
+ * CUDA memory pool per device (stream-ordered allocation on the call's stream); the pool keeps up
+ * to 8 GiB of freed blocks for reuse by the next handle, so a create / search / destroy cycle
+ * does not pay cudaMalloc / cudaFree.  A contiguous HOST spectrogram is sent in one copy and
+ * re-laid on the device.  If a later call on the same handle uses a different stream, the library
+ * first waits for the handle's previous stream.
  */
 int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes,
                int n_sft, int n_bins, double f_min, double T_sft, const double *timestamps,
