@@ -87,13 +87,20 @@ sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_
     const unsigned int prefix = PASS ? state->prefix : 0u;
     const SelSeg sg = sel_segment(n, seg);
     unsigned int *hc = h + (threadIdx.x & (COPIES - 1)) * 2048;
-    for (long t0 = sg.begin; t0 < sg.end; t0 += SEL_TILE) {
-        unsigned int b[4];
-        int nv;
-        sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b, nv);
+    // two tiles per iteration: 32 bytes in flight per thread keep the HBM pipe full
+    for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
+        unsigned int b[8];
+        int nv[2];
+        {
+            unsigned int b0[4], b1[4];
+            sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, nv[0]);
+            sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, nv[1]);
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const bool ok = c < nv && sel_valid(b[c], is_int);
+            for (int c = 0; c < 4; ++c) { b[c] = b0[c]; b[4 + c] = b1[c]; }
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const bool ok = (c & 3) < nv[c >> 2] && sel_valid(b[c], is_int);
             const unsigned int key = sel_key(b[c], is_int);
             if (PASS == 0) {
                 if (ok) atomicAdd(&hc[key >> 21], 1u);
