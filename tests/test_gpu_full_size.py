@@ -121,3 +121,61 @@ def test_cfg5_all_sky_subset_bits(tcw):
     groups = np.array([0, 100, 333, 500, w.n_groups - 1])
     ref = sampled_group_parity(tcw, w, groups, stat.cpu().numpy(), bs, bi)
     assert ref.stat.max() > 100
+
+
+def _device_group_parity(tcw, w, groups, stat, best, h):
+    """Sampled whole groups of a search whose outputs stay on the device (too large to copy whole)."""
+    import torch
+    n_f0 = len(w.f0)
+    g = torch.as_tensor(groups, device=stat.device)
+    got = stat.reshape(-1, n_f0)[g].cpu().numpy().reshape(-1)
+    b = best[g].cpu().numpy()
+    bs, bi = h.best_fields(b)
+    ref = oracle.evaluate(w, sel=oracle.group_templates(w, groups))
+    assert_stat_parity(w, got, ref.stat)
+    assert_best_parity(w, n_f0, bs, bi, ref.stat)
+    return ref
+
+
+def test_cfg4_full_size_sampled_groups(tcw):
+    """cfg4 exactly as bench.py --config cfg4 runs it: 11.52 M templates x 20 843 SFTs of 20 000 bins
+    (1.67 GB, timestamps with holes), chunked staged kernel; the oracle recomputes three whole groups."""
+    import torch
+    w = tcw_inputs.make_workload("cfg4")
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == "staged" and info["chunks"] > 1 and info["status"] == 0
+        ref = _device_group_parity(tcw, w, np.array([0, 287, 575]), stat, best, h)
+        st = stat.reshape(-1, len(w.f0))
+        bmax = st.max(dim=1)
+        b = best.cpu().numpy()
+        bs, bi = h.best_fields(b)
+        assert np.array_equal(bs, bmax.values.cpu().numpy())
+        assert torch.isfinite(stat).all().item() and (stat >= 0).all().item()
+    assert ref.n_inband.max() == w.n_sft
+
+
+def test_cfg5_full_size_sampled_groups(tcw):
+    """cfg5 exactly as bench.py --config cfg5 runs it: 393.2 M templates (4096 sky points), bit-packed
+    counts, sky-block kernel; counts of sampled whole groups bit-exact, best per group exact."""
+    import torch
+    w = tcw_inputs.make_workload("cfg5")
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == "skyblock" and info["status"] == 0
+        n_ab = len(w.tau) * len(w.brk)
+        groups = np.array([0, 1, 777 * n_ab + 5, 2048 * n_ab + 11, 4095 * n_ab + n_ab - 1])
+        _device_group_parity(tcw, w, groups, stat, best, h)
+        st = stat.reshape(-1, len(w.f0))
+        bmax = st.max(dim=1)
+        b = best.cpu().numpy()
+        assert np.array_equal(b[:, 0], bmax.values.cpu().numpy())
+        # the reported index attains the maximum and no lower index does (lowest f0 index on ties)
+        idx = torch.as_tensor(b[:, 1], device=st.device).long()
+        assert torch.equal(st[torch.arange(st.shape[0], device=st.device), idx], bmax.values)
+        first = (st == bmax.values[:, None]).int().argmax(dim=1)
+        assert torch.equal(first, idx)
