@@ -87,6 +87,21 @@ sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_
     const unsigned int prefix = PASS ? state->prefix : 0u;
     const SelSeg sg = sel_segment(n, seg);
     unsigned int *hc = h + (threadIdx.x & (COPIES - 1)) * 2048;
+    // Passes 1 and 2 only count the keys that share the prefix found so far, a small minority: a
+    // cheap value-range test (a superset of the matching keys) skips the key arithmetic for the rest.
+    const unsigned int kmask = PASS == 1 ? 0x001fffffu : 0x000003ffu;
+    const unsigned int klo = PASS == 1 ? (prefix & ~kmask) : (prefix & ~kmask), khi = klo | kmask;
+    float flo = 0.f, fhi = 0.f;
+    int ilo = 0, ihi = 0;
+    if (PASS) {
+        if (is_int) { ilo = (int)(klo ^ 0x80000000u); ihi = (int)(khi ^ 0x80000000u); }
+        else {
+            // clamp the key range to the keys of -inf .. +inf, then map both ends back to float32
+            const unsigned int a = klo < 0x007fffffu ? 0x007fffffu : klo, b = khi > 0xff800000u ? 0xff800000u : khi;
+            flo = __uint_as_float((a & 0x80000000u) ? (a & 0x7fffffffu) : ~a);
+            fhi = __uint_as_float((b & 0x80000000u) ? (b & 0x7fffffffu) : ~b);
+        }
+    }
     // two tiles per iteration: 32 bytes in flight per thread keep the HBM pipe full
     for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
         unsigned int b[8];
@@ -100,6 +115,11 @@ sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_
         }
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
+            if (PASS) {
+                const bool maybe = is_int ? ((int)b[c] >= ilo && (int)b[c] <= ihi)
+                                          : (__uint_as_float(b[c]) >= flo && __uint_as_float(b[c]) <= fhi);
+                if (!maybe) continue;
+            }
             const bool ok = (c & 3) < nv[c >> 2] && sel_valid(b[c], is_int);
             const unsigned int key = sel_key(b[c], is_int);
             if (PASS == 0) {
