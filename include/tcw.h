@@ -83,6 +83,23 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
                int n_sft, int n_bins, double f_min, double T_sft, const double *timestamps,
                const double *velocities, void *stream);
 
+/* tcw_create_async -- tcw_create for a contiguous HOST spectrogram (row_pitch_bytes = bytes of one
+ * row; float32 or uint8) that lets the transfer overlap the first search: the rows are sent in
+ * pieces on a copy stream owned by the handle, the call returns without waiting for them, and the
+ * first search on the handle launches SFT chunk by SFT chunk, each behind the piece that completes
+ * its rows.  The caller must keep the host spectrogram valid and unchanged until that first search
+ * has completed on its stream, or until tcw_upload_wait returns.  Pinned host memory is needed for
+ * the overlap (a pageable array is staged synchronously by the driver).  For any other input
+ * (device pointer, padded rows, bit-packed counts) it behaves exactly like tcw_create.  Results are
+ * identical to those of a handle made by tcw_create. */
+int tcw_create_async(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes,
+                     int n_sft, int n_bins, double f_min, double T_sft, const double *timestamps,
+                     const double *velocities, void *stream);
+
+/* tcw_upload_wait -- block until every piece of a tcw_create_async upload has arrived (a no-op for
+ * other handles). */
+int tcw_upload_wait(tcw_handle *h);
+
 /* The cubic-lattice template bank: explicit axes, HOST pointers, copied during
  * the call.  Spacing is the caller's business; only f0 must be ascending. */
 typedef struct {

@@ -28,7 +28,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_create_async", "tcw_upload_wait", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -82,6 +82,10 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     vp, dp, ci, cl = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_long
     L.tcw_create.restype = ci
     L.tcw_create.argtypes = [ctypes.POINTER(vp), vp, ci, cl, ci, ci, ctypes.c_double, ctypes.c_double, dp, dp, vp]
+    L.tcw_create_async.restype = ci
+    L.tcw_create_async.argtypes = L.tcw_create.argtypes
+    L.tcw_upload_wait.restype = ci
+    L.tcw_upload_wait.argtypes = [vp]
     L.tcw_search.restype = ci
     L.tcw_search.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
     L.tcw_search_host.restype = ci
@@ -171,7 +175,7 @@ class Handle:
     """tcw_create / tcw_search / tcw_destroy with the same argument meaning as include/tcw.h."""
 
     def __init__(self, spectrogram, fmt, n_bins: int, f_min: float, T_sft: float, timestamps, velocities,
-                 stream=None):
+                 stream=None, async_upload: bool = False):
         """`spectrogram`: a CUDA torch tensor, or a host numpy array / CPU torch tensor, 2-D,
         SFT-major, dtype float32 (fmt "f32"), uint8 ("u8") or int32/uint32 words ("bits")."""
         import torch
@@ -190,7 +194,9 @@ class Handle:
         if ts.shape != (n_sft,) or vel.shape != (n_sft, 3):
             raise ValueError("timestamps must be [n_sft] and velocities [n_sft][3]")
         self.n_sft, self.n_bins = int(n_sft), int(n_bins)
-        _check(L.tcw_create(ctypes.byref(self._h), ptr, self.fmt, pitch, self.n_sft, self.n_bins,
+        self._keep = spec if async_upload else None     # tcw_create_async reads the host rows after returning
+        create = L.tcw_create_async if async_upload else L.tcw_create
+        _check(create(ctypes.byref(self._h), ptr, self.fmt, pitch, self.n_sft, self.n_bins,
                             float(f_min), float(T_sft), _dp(ts), _dp(vel), _stream_ptr(stream)))
 
     @classmethod
@@ -374,6 +380,10 @@ class Handle:
         d = np.empty((len(grid.sky), self.n_sft), dtype=np.float64)
         _check(L.tcw_tables(self._h, _dp(g), _dp(d), _stream_ptr(stream)))
         return g, d
+
+    def upload_wait(self):
+        """tcw_upload_wait: block until an asynchronous upload (async_upload=True) has arrived."""
+        _check(load_library().tcw_upload_wait(self._h))
 
     def set_option(self, key: int, value: int):
         _check(load_library().tcw_set_option(self._h, int(key), int(value)))

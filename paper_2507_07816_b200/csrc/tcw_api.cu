@@ -185,6 +185,12 @@ struct tcw_handle {
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
+    // asynchronous upload (tcw_create_async): pieces of rows copied on up_stream, one event per piece
+    cudaStream_t up_stream = nullptr;
+    std::vector<cudaEvent_t> up_ev;
+    long up_rows = 0;            // rows per piece
+    bool up_pending = false;     // the first search still has to wait for the pieces
+    void *up_staging = nullptr;  // tightly packed device copy the pieces land in before the re-lay
     long info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 0};
     // last tables
     int tab_tau = 0, tab_brk = 0, tab_sky = 0;
@@ -441,9 +447,9 @@ extern "C" {
 
 const char *tcw_last_error(void) { return g_err; }
 
-int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes, int n_sft,
-               int n_bins, double f_min, double T_sft, const double *timestamps, const double *velocities,
-               void *stream)
+static int create_impl(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes, int n_sft,
+                       int n_bins, double f_min, double T_sft, const double *timestamps, const double *velocities,
+                       void *stream, bool async_upload)
 {
     if (!out) return fail(TCW_EINVAL, "out is NULL");
     *out = nullptr;
@@ -535,7 +541,31 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
         const bool on_device = cudaPointerGetAttributes(&attr, spectrogram) == cudaSuccess &&
                                (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
         cudaGetLastError();
-        if (!on_device && (size_t)row_pitch_bytes == dev_row) {
+        if (async_upload && !on_device && (size_t)row_pitch_bytes == dev_row) {
+            // tcw_create_async: the rows travel in pieces of about 16 MB on a copy stream of the handle's
+            // own, each piece followed by its re-lay and an event; the first search waits per SFT chunk.
+            CREATE_TRY(dev_alloc(&h->up_staging, dev_row * n_sft, st));
+            CREATE_TRY(cudaStreamCreateWithFlags(&h->up_stream, cudaStreamNonBlocking));
+            cudaEvent_t ready;
+            CREATE_TRY(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+            cudaEventRecord(ready, st);                       // allocations and the zero fill precede the pieces
+            cudaStreamWaitEvent(h->up_stream, ready, 0);
+            cudaEventDestroy(ready);
+            h->up_rows = std::max<long>(64, (long)((16 << 20) / dev_row));
+            for (long j0 = 0; j0 < n_sft; j0 += h->up_rows) {
+                const size_t nr = (size_t)std::min<long>(h->up_rows, n_sft - j0);
+                unsigned char *stg = (unsigned char *)h->up_staging + (size_t)j0 * dev_row;
+                CREATE_TRY(cudaMemcpyAsync(stg, (const unsigned char *)spectrogram + (size_t)j0 * dev_row, nr * dev_row,
+                                           cudaMemcpyHostToDevice, h->up_stream));
+                CREATE_TRY(cudaMemcpy2DAsync(h->d_spec + h->pad_bytes + (size_t)j0 * h->pitch, (size_t)h->pitch, stg, dev_row,
+                                             dev_row, nr, cudaMemcpyDeviceToDevice, h->up_stream));
+                cudaEvent_t e;
+                CREATE_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                h->up_ev.push_back(e);
+                CREATE_TRY(cudaEventRecord(e, h->up_stream));
+            }
+            h->up_pending = true;
+        } else if (!on_device && (size_t)row_pitch_bytes == dev_row) {
             CREATE_TRY(dev_alloc(&d_words, dev_row * n_sft, st));
             CREATE_TRY(cudaMemcpyAsync(d_words, spectrogram, dev_row * n_sft, cudaMemcpyHostToDevice, st));
             CREATE_TRY(cudaMemcpy2DAsync(h->d_spec + h->pad_bytes, (size_t)h->pitch, d_words, dev_row, dev_row,
@@ -555,13 +585,60 @@ int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_p
     return TCW_OK;
 }
 
+int tcw_create(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes, int n_sft,
+               int n_bins, double f_min, double T_sft, const double *timestamps, const double *velocities,
+               void *stream)
+{
+    return create_impl(out, spectrogram, format, row_pitch_bytes, n_sft, n_bins, f_min, T_sft, timestamps, velocities,
+                       stream, false);
+}
+
+int tcw_create_async(tcw_handle **out, const void *spectrogram, int format, long row_pitch_bytes, int n_sft,
+                     int n_bins, double f_min, double T_sft, const double *timestamps, const double *velocities,
+                     void *stream)
+{
+    return create_impl(out, spectrogram, format, row_pitch_bytes, n_sft, n_bins, f_min, T_sft, timestamps, velocities,
+                       stream, true);
+}
+
+// Make `st` wait for the uploaded rows [0, j_end) of a handle created by tcw_create_async.
+static void upload_wait_rows(tcw_handle *h, long j_end, cudaStream_t st)
+{
+    if (!h->up_pending || h->up_ev.empty()) return;
+    long k = (std::max<long>(j_end, 1) - 1) / h->up_rows;
+    k = std::min<long>(k, (long)h->up_ev.size() - 1);
+    cudaStreamWaitEvent(st, h->up_ev[(size_t)k], 0);
+}
+
+// Every piece has been waited for on `st`: later calls need no waits; the staging copy goes back to the pool.
+static void upload_done(tcw_handle *h, cudaStream_t st)
+{
+    if (!h->up_pending) return;
+    h->up_pending = false;
+    dev_free(h->up_staging, st);
+    h->up_staging = nullptr;
+}
+
+int tcw_upload_wait(tcw_handle *h)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    if (h->up_stream) CUDA_TRY(cudaStreamSynchronize(h->up_stream));
+    return TCW_OK;
+}
+
 int tcw_destroy(tcw_handle *h)
 {
     if (!h) return TCW_OK;
     cudaSetDevice(h->device);
     // nothing enqueued by this handle may still be running when its memory goes back to the pool
     cudaStreamSynchronize(h->last_stream);
+    if (h->up_stream) {
+        cudaStreamSynchronize(h->up_stream);
+        for (auto &e : h->up_ev) cudaEventDestroy(e);
+        cudaStreamDestroy(h->up_stream);
+    }
     g_alloc_stream = h->last_stream;
+    dev_free(h->up_staging, h->last_stream);
     dev_free(h->d_spec, h->last_stream);
     dev_free(h->d_ts, h->last_stream);
     dev_free(h->d_vel, h->last_stream);
@@ -792,10 +869,25 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         q.n_blocks = n_blocks;
     }
     if (tm) CUDA_TRY(cudaEventRecord(ev[1], st));
-    if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
-    else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, wgt, p, n_ctas, smem, st);
-    else rc = launch_gather(h->fmt_dev, h->t_pow2, wgt, p, n_ctas, st);
+    int extra_launches = 0;
+    if (h->up_pending && kernel == 2 && p.n_chunks > 1) {
+        // the spectrogram is still arriving (tcw_create_async): one launch per SFT chunk, each behind
+        // the upload event of the chunk's last row, so the search overlaps the rest of the transfer
+        for (int c = 0; c < p.n_chunks && rc == TCW_OK; ++c) {
+            upload_wait_rows(h, std::min<long>(h->n_sft, (long)p.j_begin + (long)(c + 1) * p.chunk_rows), st);
+            tcw::SumParams pc = p;
+            pc.chunk0 = c;
+            rc = launch_staged(h->fmt_dev, r, h->t_pow2, wgt, pc, n_partial, smem, st);
+        }
+        extra_launches = p.n_chunks - 1;
+    } else {
+        upload_wait_rows(h, h->n_sft, st);
+        if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
+        else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, wgt, p, n_ctas, smem, st);
+        else rc = launch_gather(h->fmt_dev, h->t_pow2, wgt, p, n_ctas, st);
+    }
     if (rc != TCW_OK) return rc;
+    upload_done(h, st);
     if (p.n_chunks > 1) {
         if (wgt) tcw::chunk_reduce_kernel<float, true><<<(unsigned)n_partial, 256, 0, st>>>(p);
         else if (h->format == TCW_F32_POWER) tcw::chunk_reduce_kernel<float, false><<<(unsigned)n_partial, 256, 0, st>>>(p);
@@ -821,7 +913,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     h->info[3] = (long)smem;
     h->info[6] = stages;
     h->info[7] = 32 * sky_sc;
-    h->info[5] = (kernel == 3 ? 5 : 4) + (p.n_chunks > 1 ? 1 : 0);  // doppler table, spin-down table, (sky-block table,) sum, (chunk reduce,) best
+    h->info[5] = (kernel == 3 ? 5 : 4) + (p.n_chunks > 1 ? 1 : 0) + extra_launches;  // doppler table, spin-down table, (sky-block table,) sum, (chunk reduce,) best
     h->info[8] = p.n_chunks;
     h->info[9] = p.chunk_rows;
     return TCW_OK;
@@ -916,6 +1008,8 @@ int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *ou
     p.n_exact = h->d_counter;
     const long n_ctas = (n + tcw::BANK_THREADS - 1) / tcw::BANK_THREADS;
     if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "bank needs more than 2^31-1 CTAs; split the search");
+    upload_wait_rows(h, h->n_sft, st);
+    upload_done(h, st);
     if (h->fmt_dev == tcw::FMT_F32) {
         if (h->t_pow2) tcw::sum_bank_kernel<tcw::FMT_F32, true><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);
         else tcw::sum_bank_kernel<tcw::FMT_F32, false><<<(unsigned)n_ctas, tcw::BANK_THREADS, 0, st>>>(p);

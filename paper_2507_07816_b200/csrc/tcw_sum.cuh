@@ -64,6 +64,8 @@ struct SumParams {
     int stages, slot_bytes;     // staged kernel: ring depth per warp (slots of RB rows), bytes per staged row
     long n_groups;              // n_sky * n_tau * n_brk
     int chunk_rows, n_chunks;   // staged kernel: SFT rows per chunk, number of chunks (1 = whole span per CTA)
+    int chunk0;                 // first chunk of this launch (a search over a spectrogram that is still being
+                                // uploaded launches chunk by chunk; otherwise 0 and one launch covers every chunk)
     void *cpart;                // chunked: float32 / int32 [n_chunks][n_groups][n_f0] partial sums
     unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
@@ -309,7 +311,7 @@ sum_staged_kernel(const SumParams p)
     const int tile = p.n_tiles - 1 - (int)(bq % p.n_tiles);
     bq /= p.n_tiles;
     const long grp = bq % p.n_groups;
-    const int chunk = (int)(bq / p.n_groups);
+    const int chunk = p.chunk0 + (int)(bq / p.n_groups);
     const int i0 = tile * F;
     const int i_last = min(i0 + F, p.n_f0) - 1;
     const int j0 = p.j_begin + chunk * p.chunk_rows;

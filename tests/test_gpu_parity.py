@@ -368,3 +368,47 @@ def test_T0_after_the_last_sft_gives_empty_spans(tcw, cfg1, fmt):
         torch.cuda.synchronize()
         assert not psi.any().item() and not stat.any().item() and not best[:, 1].any().item()
         assert not bstat.any().item() and not inband.any().item()
+
+
+@pytest.mark.parametrize("fmt", ["f32", "u8", "bits"])
+def test_async_upload_gives_identical_results(tcw, fmt):
+    """tcw_create_async: the first search runs chunk by chunk behind the upload pieces; results are
+    bit-identical to a handle made by tcw_create, for the first search and for later ones, and for
+    the other entry points whose first call has to wait for the whole upload."""
+    import torch
+    rng = np.random.default_rng(31)
+    n_sft, n_bins = 1500, 6000            # 36 MB of float32: several 16 MB upload pieces
+    ts = 8.0 * np.arange(n_sft) + 4.0
+    rho = rng.standard_exponential((n_sft, n_bins)).astype(np.float32)
+    w = tcw_inputs.Workload("async", "f32", rho, n_sft, n_bins, 500.0, 8.0, ts, tcw_inputs.detector_velocity(ts), 0.0,
+                            500.0 + 0.125 * np.arange(3000), np.geomspace(3500.0, 35000.0, 3), np.array([3.0, 5.0]),
+                            tcw_inputs.sky_vector(1.0, 0.3)[None]).with_format(fmt)
+    grid = tcw.Grid.of(w)
+    arr = np.ascontiguousarray(w.spectrogram)
+    if arr.dtype == np.uint32:
+        arr = arr.view(np.int32)
+    pinned = torch.from_numpy(arr).pin_memory()
+    with tcw.Handle(pinned, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities) as h0:
+        h0.set_option(tcw.TCW_OPT_CHUNK_ROWS, 256)
+        ref_stat, ref_best = h0.search(grid)
+        ref_bank, _, _ = h0.search_bank(w.f0[:200], np.full(200, 9000.0), np.full(200, 4.0), w.sky[0])
+        torch.cuda.synchronize()
+    for first in ("search", "bank"):
+        with tcw.Handle(pinned, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, async_upload=True) as h:
+            h.set_option(tcw.TCW_OPT_CHUNK_ROWS, 256)
+            if first == "bank":
+                bank, _, _ = h.search_bank(w.f0[:200], np.full(200, 9000.0), np.full(200, 4.0), w.sky[0])
+                torch.cuda.synchronize()
+                assert torch.equal(bank, ref_bank)
+            stat, best = h.search(grid)
+            torch.cuda.synchronize()
+            info = h.info()
+            assert info["chunks"] == 6 and info["status"] == 0
+            assert torch.equal(stat, ref_stat) and torch.equal(best, ref_best)
+            stat2, best2 = h.search(grid)             # upload long finished: single launch again
+            torch.cuda.synchronize()
+            assert torch.equal(stat2, ref_stat) and torch.equal(best2, ref_best)
+            h.upload_wait()
+    # a handle destroyed while its upload may still be in flight
+    h = tcw.Handle(pinned, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, async_upload=True)
+    h.close()
