@@ -13,7 +13,7 @@
 //   1. fast:  x~ = (f0*T) * exp2(e * log2(1 + (t_j - T0)/tau)) * D  in plain binary64, with a
 //      table-driven log2 and exp2 (bank_pow below, about 20 FP64 operations).  Its relative distance
 //      from the oracle's x is below 2^-45 (error budget in DESIGN.md section 7; it needs
-//      |e| <= 4, base < 2^40 and |e*log2 base| <= 64, which are checked).
+//      |e| <= 4, base < 2^40 and |e*log2 base| <= 64, which are checked once per template).
 //   2. if x~ lies within x~ * 2^-40 of a half-integer (about 1.5e-8 of all lookups at 1 kHz), or
 //      the checks of step 1 fail, the bin is recomputed by the defining chain: base and exponent
 //      in single IEEE operations, the double-double power of tcw_tables.cuh rounded once, then
@@ -117,7 +117,10 @@ sum_bank_kernel(const BankParams p)
     const double inv_tau = 1.0 / tau;
     const double e = __ddiv_rn(1.0, __dsub_rn(1.0, brk));
     const double f0T = f0 * p.T;
-    const bool fast_ok = fabs(e) <= 4.0;
+    // preconditions of the fast evaluation, checked once per template: the base grows with t, so its
+    // largest value (last SFT) bounds both the base and |e*log2(base)| of every lookup
+    const double b_last = fma(__dsub_rn(__ldg(p.ts + p.n_sft - 1), p.T0), inv_tau, 1.0);
+    const bool fast_ok = fabs(e) <= 4.0 && b_last < 1.0e12 && fabs(e) * log2(fmax(b_last, 1.0)) <= 63.0;
     const double below = (double)p.k_min - 1.0;
     constexpr double INV_C = 1.0 / 299792458.0;
     constexpr double GUARD = 9.094947017729282e-13;   // 2^-40
@@ -153,7 +156,7 @@ sum_bank_kernel(const BankParams p)
             const double D = p.dshared ? c.y : fma(fma(c.w, nz, fma(c.z, ny, c.y * nx)), INV_C, 1.0);
             const double b = fma(c.x, inv_tau, 1.0);
             double E;
-            const double g = bank_pow(b < 1.0e12 ? b : 1.0, e, logt, expt, E);
+            const double g = bank_pow(fast_ok ? b : 1.0, e, logt, expt, E);
             const double fg = f0T * g;
             // the track only moves down (g decreases with t): once it is a whole bin below the band for
             // the largest Doppler factor, it stays there
@@ -162,7 +165,7 @@ sum_bank_kernel(const BankParams p)
             const double y = x + TCW_MAGIC;
             int lo = __double2loint(y);
             const double d = x - (y - TCW_MAGIC);
-            if (!(fabs(d) < 0.5 - x * GUARD) || !fast_ok || !(fabs(E) <= 64.0) || !(b < 1.0e12)) {
+            if (!(fabs(d) < 0.5 - x * GUARD) || !fast_ok) {
                 const int j = j0 + t;
                 double De = D;
                 if (!p.dshared) {
