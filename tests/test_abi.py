@@ -113,7 +113,38 @@ def test_null_handle_calls(lib):
     assert lib.tcw_get_info(None, None) == tcw.TCW_EINVAL
     assert lib.tcw_tables(None, None, None, None) == tcw.TCW_EINVAL
     assert lib.tcw_track_indices(None, None, 0, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_search_weighted(None, None, None, None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_search_bank(None, None, None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_topk(None, None, 0, 1, 1, None, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_select_above(None, None, 0, 1, 0.0, 0, None, None, None) == tcw.TCW_EINVAL
+    assert lib.tcw_get_counter(None, 0, None) == tcw.TCW_EINVAL
+    assert lib.tcw_upload_wait(None) == tcw.TCW_EINVAL
     assert isinstance(lib.tcw_last_error(), bytes)
+
+
+def test_prepare_rejects_bad_arguments_without_cuda(lib):
+    """tcw_prepare validates sizes before the first CUDA call (no handle is involved)."""
+    from paper_2507_07816_b200 import _CPrep
+    x = np.zeros(4096, dtype=np.float32)
+    n = ctypes.c_int(0)
+    good = dict(fs=64.0, T_sft=8.0, f_min=8.0, n_bins=64, median_bins=9, threshold=1.6)
+    def call(**kw):
+        a = dict(good); a.update(kw)
+        cp = _CPrep(a["fs"], a["T_sft"], a["f_min"], a["n_bins"], a["median_bins"], a["threshold"])
+        return lib.tcw_prepare(x.ctypes.data, x.size, ctypes.byref(cp), 0, 1, 4 * a["n_bins"], ctypes.byref(n), None)
+    for kw in (dict(fs=0.0), dict(fs=63.9), dict(n_bins=0), dict(median_bins=4), dict(f_min=0.05),
+               dict(f_min=31.0, n_bins=40), dict(f_min=0.0)):
+        assert call(**kw) == tcw.TCW_EINVAL, kw
+    assert lib.tcw_prepare(None, 0, None, 0, None, 0, None, None) == tcw.TCW_EINVAL
+
+
+def test_create_async_rejects_bad_arguments_without_cuda(lib):
+    spec, ts, vel = _create_args()
+    h = ctypes.c_void_p()
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = lib.tcw_create_async(ctypes.byref(h), spec.ctypes.data, 7, 32, 4, 8, 500.0, 8.0, ts.ctypes.data_as(dp),
+                              vel.ctypes.data_as(dp), None)
+    assert rc == tcw.TCW_EINVAL and not h.value
 
 
 def test_no_cuda_device_fails_loudly(lib):
