@@ -1191,7 +1191,6 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     const bool on_device = cudaPointerGetAttributes(&attr, strain) == cudaSuccess &&
                            (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
     cudaGetLastError();   // a plain host pointer may leave an error state on older runtimes
-    bool have_plan = false;
     int rc = TCW_OK;
 #define PREP_TRY(call)                                                                              \
     do {                                                                                            \
@@ -1207,12 +1206,22 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     tcw::prep_window_table_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, d_win);
     PREP_TRY(cudaGetLastError());
     {
-        int dims[1] = {N};
-        if (cufftPlanMany(&plan, 1, dims, nullptr, 1, N, nullptr, 1, n_half, CUFFT_R2C, batch) != CUFFT_SUCCESS) {
-            rc = fail(TCW_ECUDA, "cufftPlanMany failed");
-            goto done;
+        // one cached plan per thread (device, N, batch): creating a plan costs more than transforming a day of data
+        struct PlanCache { cufftHandle plan; int dev, N, batch; bool ok; };
+        static thread_local PlanCache pc = {0, -1, 0, 0, false};
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (!pc.ok || pc.dev != dev || pc.N != N || pc.batch != batch) {
+            if (pc.ok) cufftDestroy(pc.plan);
+            pc.ok = false;
+            int dims[1] = {N};
+            if (cufftPlanMany(&pc.plan, 1, dims, nullptr, 1, N, nullptr, 1, n_half, CUFFT_R2C, batch) != CUFFT_SUCCESS) {
+                rc = fail(TCW_ECUDA, "cufftPlanMany failed");
+                goto done;
+            }
+            pc.dev = dev; pc.N = N; pc.batch = batch; pc.ok = true;
         }
-        have_plan = true;
+        plan = pc.plan;
         if (cufftSetStream(plan, st) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftSetStream failed"); goto done; }
     }
     PREP_TRY(cudaFuncSetAttribute(tcw::prep_normalise_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -1242,7 +1251,6 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     *n_sft = (int)n_seg;
 done:
 #undef PREP_TRY
-    if (have_plan) cufftDestroy(plan);
     dev_free(d_x, st);
     dev_free(d_win, st);
     dev_free(d_spec, st);
