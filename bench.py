@@ -538,7 +538,7 @@ def main():
     ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--format", default=None, choices=["f32", "u8", "bits"])
     ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged", "skyblock"])
-    ap.add_argument("--sky-block", type=int, default=0, choices=[0, 64, 128])
+    ap.add_argument("--sky-block", type=int, default=0, choices=[0, 64, 128, 256])
     ap.add_argument("--f0-per-lane", type=int, default=0)
     ap.add_argument("--chunk-rows", type=int, default=0, help="staged kernel: SFT rows per chunk (0 auto, -1 never)")
     ap.add_argument("--stages", type=int, default=0, help="staged kernel: ring depth limit (0 auto)")

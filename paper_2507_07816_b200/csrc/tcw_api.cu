@@ -23,6 +23,7 @@
 #include "tcw_sum.cuh"
 #include "tcw_tables.cuh"
 #include "tcw_skyblock.cuh"
+#include "tcw_skyblock2.cuh"
 #include "tcw_bank.cuh"
 #include "tcw_select.cuh"
 #include "tcw_prep.cuh"
@@ -691,7 +692,8 @@ int tcw_set_option(tcw_handle *h, int key, long value)
         h->opt_stages = (int)value;
         return TCW_OK;
     case TCW_OPT_SKY_BLOCK:
-        if (value != 0 && value != 64 && value != 128) return fail(TCW_EINVAL, "TCW_OPT_SKY_BLOCK must be 0, 64 or 128");
+        if (value != 0 && value != 64 && value != 128 && value != 256)
+            return fail(TCW_EINVAL, "TCW_OPT_SKY_BLOCK must be 0, 64, 128 or 256");
         h->opt_sky = (int)value;
         return TCW_OK;
     case TCW_OPT_CHUNK_ROWS:
@@ -729,11 +731,23 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     if (h->opt_kernel == 3 && h->fmt_dev != tcw::FMT_U8)
         return fail(TCW_EUNSUPPORTED, "the sky-block kernel serves the count formats only");
     if (!wgt && h->fmt_dev == tcw::FMT_U8 && (h->opt_kernel == 3 || (h->opt_kernel == 0 && grid->n_sky >= 16))) {
-        const int sc = h->opt_sky == 128 ? 4 : 2, rr = sc == 2 ? 16 : 8, S = 32 * sc;
         // two sky points differ by |D_s - D_s'| <= 2 vmax / c whatever the block holds
         const double spread = grid->f0[grid->n_f0 - 1] * h->T * 2.0 * (h->vmax / C_LIGHT) * (1.0 + 1e-5);
+        // two-level blocks of 256 sky points (tcw_skyblock2.cuh): bit-packed input only (0/1 values keep
+        // the packed int16 corrections exact), at most 32767 SFTs, and enough sky points to fill a block
+        const bool can2 = h->format == TCW_BIT_COUNT && h->n_sft <= 32767;
+        if (h->opt_sky == 256 && !can2)
+            return fail(TCW_EUNSUPPORTED, "256-point sky blocks need bit-packed input and at most 32767 SFTs");
+        if (can2 && (h->opt_sky == 256 || (h->opt_sky == 0 && grid->n_sky >= 128))) {
+            const long w2 = max_window_bins(grid, tcw::F2, p.dmaxT) + (long)std::ceil(spread) + 2;
+            const int sb2 = tcw::DTS2_BYTES + (int)((w2 + 32 + 15) & ~15L);
+            if (w2 <= tcw::PAD_BINS && tcw::sky2_smem_bytes(sb2) <= SMEM_MAX) {
+                kernel = 3; r = tcw::R2; sky_sc = 8; stages = tcw::D2; slot = sb2; smem = tcw::sky2_smem_bytes(sb2);
+            }
+        }
+        const int sc = h->opt_sky == 128 ? 4 : 2, rr = sc == 2 ? 16 : 8, S = 32 * sc;
         const long w_bins = max_window_bins(grid, 32 * rr, p.dmaxT) + (long)std::ceil(spread) + 2;
-        if (w_bins <= tcw::PAD_BINS) {
+        if (!kernel && w_bins <= tcw::PAD_BINS) {
             const int sb = 8 * S + (int)((w_bins + 32 + 15) & ~15L);
             for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 4; s >= 2; --s) {
                 const size_t b = tcw::sky_smem_bytes(s, sb, 32 * rr, S);
@@ -816,7 +830,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     if (!out_best && (rc = h->d_best.reserve((size_t)n_groups * 8)) != TCW_OK) return rc;
     if (kernel == 3) {
         const size_t rows = (size_t)n_blocks * h->n_sft;
-        if ((rc = h->d_dts.reserve(rows * 32 * sky_sc)) != TCW_OK) return rc;
+        if ((rc = h->d_dts.reserve(rows * (sky_sc == 8 ? (size_t)(tcw::DTS2_BYTES / 8) : (size_t)(32 * sky_sc)))) != TCW_OK) return rc;
         if ((rc = h->d_dmm.reserve(rows * 2)) != TCW_OK) return rc;
     }
     if (p.n_chunks > 1) {
@@ -861,7 +875,17 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     p.gtab = h->d_g.p;
     p.dtab = h->d_d.p;
     if (kernel == 3) {
-        if ((rc = launch_sky_table(sky_sc, h->t_pow2, h, h->a_sky, n_blocks, st)) != TCW_OK) return rc;
+        if (sky_sc == 8) {
+            const long warps = (long)n_blocks * h->n_sft;
+            const unsigned blocks = (unsigned)((warps * 32 + 255) / 256);
+            if (h->t_pow2)
+                tcw::skyblock2_table_kernel<true><<<blocks, 256, 0, st>>>(h->d_vel, h->n_sft, h->a_sky, h->d_slot.p, n_blocks, h->T,
+                                                                         h->d_dts.p, h->d_dmm.p);
+            else
+                tcw::skyblock2_table_kernel<false><<<blocks, 256, 0, st>>>(h->d_vel, h->n_sft, h->a_sky, h->d_slot.p, n_blocks, h->T,
+                                                                          h->d_dts.p, h->d_dmm.p);
+            CUDA_TRY(cudaGetLastError());
+        } else if ((rc = launch_sky_table(sky_sc, h->t_pow2, h, h->a_sky, n_blocks, st)) != TCW_OK) return rc;
         q.dts = h->d_dts.p;
         q.dmm = h->d_dmm.p;
         q.slot_sky = h->d_slot.p;
@@ -882,7 +906,16 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         extra_launches = p.n_chunks - 1;
     } else {
         upload_wait_rows(h, h->n_sft, st);
-        if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
+        if (kernel == 3 && sky_sc == 8) {
+            if (h->t_pow2) {
+                CUDA_TRY(cudaFuncSetAttribute(tcw::sum_skyblock2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                tcw::sum_skyblock2_kernel<true><<<(unsigned)n_ctas, tcw::SKY2_THREADS, smem, st>>>(p, q);
+            } else {
+                CUDA_TRY(cudaFuncSetAttribute(tcw::sum_skyblock2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                tcw::sum_skyblock2_kernel<false><<<(unsigned)n_ctas, tcw::SKY2_THREADS, smem, st>>>(p, q);
+            }
+            CUDA_TRY(cudaGetLastError());
+        } else if (kernel == 3) rc = launch_sky(sky_sc, h->t_pow2, p, q, n_ctas, smem, st);
         else if (kernel == 2) rc = launch_staged(h->fmt_dev, r, h->t_pow2, wgt, p, n_ctas, smem, st);
         else rc = launch_gather(h->fmt_dev, h->t_pow2, wgt, p, n_ctas, st);
     }

@@ -139,3 +139,51 @@ def test_cfg5_all_sky_subset_equals_per_sky_kernel(tcw):
     groups = np.array([0, 299, 598])
     ref = oracle.evaluate(w, sel=oracle.group_templates(w, groups))
     assert_stat_parity(w, got.reshape(-1, 4000)[groups].reshape(-1), ref.stat)
+
+
+def _sky_search(tcw, w, sky_block):
+    import torch
+    with tcw.Handle.from_workload(w) as h:
+        h.set_option(tcw.TCW_OPT_KERNEL, 3)
+        h.set_option(tcw.TCW_OPT_SKY_BLOCK, sky_block)
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["status"] == 0 and info["kernel"] == "skyblock" and info["sky_block"] == sky_block
+        return stat.cpu().numpy(), best.cpu().numpy()
+
+
+def test_two_level_blocks_of_256_equal_blocks_of_64_and_the_oracle(tcw, cfg1):
+    """The two-level kernel (256 sky points = 4 sub-blocks of 64, packed int16 corrections) on
+    bit-packed input: bit-identical to the 64-point kernel and to the oracle -- a 10-degree cap
+    (mostly level-0 agreement), the full sphere in arbitrary order (levels 1 and 2 busy), a ragged
+    block (300 sky points) and a ragged f0 tile."""
+    import oracle
+    for sky in (tcw_inputs.fibonacci_cap(300, 3.45, -0.41, 10.0),
+                tcw_inputs.fibonacci_sphere(512)[np.random.default_rng(3).permutation(512)]):
+        w = dataclasses.replace(cfg1.with_format("bits"), sky=sky, f0=520.0 + 0.125 * np.arange(300),
+                                tau=cfg1.tau[:2], brk=cfg1.brk[:2])
+        s256, b256 = _sky_search(tcw, w, 256)
+        s64, b64 = _sky_search(tcw, w, 64)
+        assert np.array_equal(s256, s64) and np.array_equal(b256, b64)
+        groups = np.array([0, 3, w.n_groups // 2, w.n_groups - 1])
+        ref = oracle.evaluate(w, sel=oracle.group_templates(w, groups))
+        got = s256.reshape(-1, len(w.f0))[groups].reshape(-1)
+        assert np.array_equal(got.astype(np.int64), ref.stat)
+
+
+def test_two_level_blocks_need_bit_packed_input(tcw, cfg1):
+    w = dataclasses.replace(cfg1.with_format("u8"), sky=tcw_inputs.fibonacci_cap(300, 3.45, -0.41, 10.0))
+    with tcw.Handle.from_workload(w) as h:
+        h.set_option(tcw.TCW_OPT_SKY_BLOCK, 256)
+        with pytest.raises(tcw.TcwError) as e:
+            h.search(tcw.Grid.of(w))
+        assert e.value.code == tcw.TCW_EUNSUPPORTED
+
+
+def test_cfg3_bits_whole_patch_two_level_equals_64(tcw):
+    """cfg3's whole sky patch (256 points = one block) on a slice of the (tau, n) axes, 4000 f0."""
+    w = tcw_inputs.make_workload("cfg3", fmt="bits").subgrid(tau=slice(0, 16, 5), brk=slice(0, 5, 2))
+    s256, b256 = _sky_search(tcw, w, 256)
+    s64, b64 = _sky_search(tcw, w, 64)
+    assert np.array_equal(s256, s64) and np.array_equal(b256, b64)
