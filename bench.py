@@ -50,9 +50,9 @@ NCU_TRAFFIC_BYTES = {
     "cfg4:f32": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
     "cfg3": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
     "cfg3:u8": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
-    "cfg3:bits": (145765888 + 305440256, "profiles/r1d_cfg3bits_sky_full.md"),
-    "cfg5": (803163136 + 1557699000, "profiles/r1d_cfg5_sky_full.md"),
-    "cfg5:bits": (803163136 + 1557699000, "profiles/r1d_cfg5_sky_full.md"),
+    "cfg3:bits": (163176448 + 305449216, "profiles/r1i_cfg3bits_sky2_full.md"),
+    "cfg5": (934601984 + 1564271000, "profiles/r1i_cfg5_sky2_full.md"),
+    "cfg5:bits": (934601984 + 1564271000, "profiles/r1i_cfg5_sky2_full.md"),
 }
 
 
@@ -376,7 +376,8 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic[0] if traffic else None,
                      "traffic_source": traffic[1] if traffic else None, "peak_source": peak_src,
-                     "kernel": f"sum_{info['kernel']}_kernel", "algorithmic_bytes_per_launch": b_comp,
+                     "kernel": ("sum_skyblock2_kernel" if info["kernel"] == "skyblock" and info["sky_block"] == 256
+                                else f"sum_{info['kernel']}_kernel"), "algorithmic_bytes_per_launch": b_comp,
                      "kernel_ms": sum_ms,
                      "bytes_per_inband_lookup": b_comp / inband if inband else None},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
