@@ -23,8 +23,8 @@
 namespace tcw {
 
 constexpr int S2 = 256, Q2 = 4, R2 = 8, F2 = 32 * R2;   // sky points per block, sub-blocks, templates per lane / tile
-constexpr int NW2 = 15, SKY2_THREADS = 32 * NW2, D2 = 2; // warps per CTA, ring depth per warp (shared memory: 132 KB of
-                                                         // corrections leave room for 12 two-deep rings of 2.4 KB rows)
+constexpr int NW2 = 16, SKY2_THREADS = 32 * NW2, D2 = 2; // warps per CTA, ring depth per warp (shared memory: 129 KB of
+                                                         // corrections leave room for 16 two-deep rings of 2.4 KB rows)
 constexpr int CW2 = S2 / 2 + 1;                          // corr row stride in 32-bit words (odd)
 constexpr int DTS2_BYTES = 8 * S2 + 64;                  // staged per row: 256 Doppler factors + 4 {min, max} pairs
 
