@@ -316,9 +316,9 @@ enum {
     TCW_OPT_F0_PER_LANE = 2,/* staged kernel: templates per lane, 4, 8 or 16 (tile = 32x that); 0 auto */
     TCW_OPT_STAGES = 3,     /* staged kernel: upper limit of the per-warp ring depth, 2..16; 0 auto  */
     TCW_OPT_SKY_BLOCK = 4,  /* sky-block kernel: sky points per block, 64, 128 or 256 (256 = the two-level
-                               kernel: bit-packed input with at most 32767 SFTs only, else
-                               TCW_EUNSUPPORTED at search); 0 auto (256 for bit-packed input and >= 128
-                               sky points, else 64)                                                  */
+                               kernel: needs n_sft * (largest count in the spectrogram) <= 32767, else
+                               TCW_EUNSUPPORTED at search); 0 auto (256 when that holds and the grid has
+                               >= 128 sky points, else 64)                                           */
     TCW_OPT_CHUNK_ROWS = 5  /* staged kernel: SFT rows per chunk (rounded up to a multiple of 64).  A
                                chunked search runs every (group, f0 tile) over one chunk of SFTs
                                before any over the next, so the rows in use stay in L2; per-chunk

@@ -160,6 +160,7 @@ struct tcw_handle {
     double f_min = 0, T = 0;
     bool t_pow2 = false;
     double vmax = 0;  // max |v_j|
+    int count_max = 1;  // count formats: largest element of the spectrogram (1 for bit-packed input)
     double vmid[3] = {0, 0, 0};  // velocity at the middle SFT: sort key of the sky-block kernel
     std::vector<double> ts;
     unsigned char *d_spec = nullptr;
@@ -576,6 +577,16 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
                                          dev_row, (size_t)n_sft, cudaMemcpyDefault, st));
         }
     }
+    if (format == TCW_U8_COUNT && !h->up_pending) {
+        // the largest count decides whether the two-level sky-block kernel may serve this data
+        // (d_status doubles as the result word; it is cleared again below)
+        tcw::max_u8_kernel<<<148 * 8, 256, 0, st>>>(h->d_spec + h->pad_bytes, h->pitch, n_sft, n_bins, h->d_status);
+        CREATE_TRY(cudaGetLastError());
+        CREATE_TRY(cudaMemcpyAsync(&h->count_max, h->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
+    } else if (format == TCW_U8_COUNT) {
+        h->count_max = 255;   // asynchronous upload: the data are not here yet; assume the worst
+    }
     CREATE_TRY(cudaMemcpyAsync(h->d_ts, timestamps, sizeof(double) * n_sft, cudaMemcpyHostToDevice, st));
     CREATE_TRY(cudaMemcpyAsync(h->d_vel, velocities, sizeof(double) * 3 * (size_t)n_sft, cudaMemcpyHostToDevice, st));
     CREATE_TRY(cudaEventRecord(h->ev_stage, st));
@@ -733,11 +744,11 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     if (!wgt && h->fmt_dev == tcw::FMT_U8 && (h->opt_kernel == 3 || (h->opt_kernel == 0 && grid->n_sky >= 16))) {
         // two sky points differ by |D_s - D_s'| <= 2 vmax / c whatever the block holds
         const double spread = grid->f0[grid->n_f0 - 1] * h->T * 2.0 * (h->vmax / C_LIGHT) * (1.0 + 1e-5);
-        // two-level blocks of 256 sky points (tcw_skyblock2.cuh): bit-packed input only (0/1 values keep
-        // the packed int16 corrections exact), at most 32767 SFTs, and enough sky points to fill a block
-        const bool can2 = h->format == TCW_BIT_COUNT && h->n_sft <= 32767;
+        // two-level blocks of 256 sky points (tcw_skyblock2.cuh): the packed int16 corrections are exact while
+        // n_sft * (largest count) < 2^15 (bit-packed input: counts are 0/1), and enough sky points to fill a block
+        const bool can2 = (long)h->n_sft * std::max(h->count_max, 1) <= 32767;
         if (h->opt_sky == 256 && !can2)
-            return fail(TCW_EUNSUPPORTED, "256-point sky blocks need bit-packed input and at most 32767 SFTs");
+            return fail(TCW_EUNSUPPORTED, "256-point sky blocks need n_sft * (largest count) <= 32767");
         if (can2 && (h->opt_sky == 256 || (h->opt_sky == 0 && grid->n_sky >= 128))) {
             const long w2 = max_window_bins(grid, tcw::F2, p.dmaxT) + (long)std::ceil(spread) + 2;
             const int sb2 = tcw::DTS2_BYTES + (int)((w2 + 32 + 15) & ~15L);

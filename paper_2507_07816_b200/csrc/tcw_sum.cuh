@@ -644,4 +644,18 @@ expand_bits_kernel(const uint32_t *__restrict__ words, long words_pitch, int n_s
     }
 }
 
+
+// Largest element of a uint8 spectrogram (rows at `pitch`): tells the host whether the packed
+// int16 corrections of the two-level sky-block kernel are exact for this data.
+__global__ void __launch_bounds__(256)
+max_u8_kernel(const unsigned char *__restrict__ src, long pitch, int n_sft, int n_bins, int *__restrict__ out)
+{
+    const long total = (long)n_sft * n_bins;
+    int m = 0;
+    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long)gridDim.x * blockDim.x)
+        m = max(m, (int)src[(q / n_bins) * pitch + (q % n_bins)]);
+    for (int o = 16; o; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
 }  // namespace tcw

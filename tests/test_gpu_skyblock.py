@@ -172,13 +172,27 @@ def test_two_level_blocks_of_256_equal_blocks_of_64_and_the_oracle(tcw, cfg1):
         assert np.array_equal(got.astype(np.int64), ref.stat)
 
 
-def test_two_level_blocks_need_bit_packed_input(tcw, cfg1):
-    w = dataclasses.replace(cfg1.with_format("u8"), sky=tcw_inputs.fibonacci_cap(300, 3.45, -0.41, 10.0))
-    with tcw.Handle.from_workload(w) as h:
+def test_two_level_blocks_need_small_counts(tcw, cfg1):
+    """The packed int16 corrections are exact while n_sft * (largest count) < 2^15: uint8 data with 0/1
+    values take the two-level kernel like bit-packed data; large counts are refused (and auto falls
+    back to 64-point blocks)."""
+    import torch
+    sky = tcw_inputs.fibonacci_cap(300, 3.45, -0.41, 10.0)
+    w = dataclasses.replace(cfg1.with_format("u8"), sky=sky)
+    s256, b256 = _sky_search(tcw, w, 256)
+    s64, b64 = _sky_search(tcw, w, 64)
+    assert np.array_equal(s256, s64) and np.array_equal(b256, b64)
+    big = dataclasses.replace(w, spectrogram=(w.spectrogram * 200).astype(np.uint8))      # 256 SFTs x 200 > 32767
+    with tcw.Handle.from_workload(big) as h:
         h.set_option(tcw.TCW_OPT_SKY_BLOCK, 256)
         with pytest.raises(tcw.TcwError) as e:
-            h.search(tcw.Grid.of(w))
+            h.search(tcw.Grid.of(big))
         assert e.value.code == tcw.TCW_EUNSUPPORTED
+        h.set_option(tcw.TCW_OPT_SKY_BLOCK, 0)
+        stat, _ = h.search(tcw.Grid.of(big))
+        torch.cuda.synchronize()
+        assert h.info()["sky_block"] == 64
+        assert np.array_equal(stat.cpu().numpy(), 200 * s64)
 
 
 def test_cfg3_bits_whole_patch_two_level_equals_64(tcw):
