@@ -53,7 +53,7 @@ struct PrepParams {
 __global__ void __launch_bounds__(256)
 prep_normalise_kernel(const PrepParams p)
 {
-    extern __shared__ __align__(16) unsigned char smem[];
+    extern __shared__ __align__(128) unsigned char smem[];
     float *P = (float *)smem;
     const int n_in = p.n_bins + 2 * p.h;
     unsigned char *nu = smem + (((size_t)n_in * 4 + 15) & ~(size_t)15);

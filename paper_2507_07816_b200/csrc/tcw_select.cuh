@@ -337,9 +337,11 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
                 const unsigned long long pos = base_gt + r2++;
                 if (THR) { if ((long)pos < capacity) out_idx[pos] = i + c; }
                 else { cand_bits[pos] = b[c]; out_idx[pos] = i + c; }
-            } else if (!THR && cls[c] == 1) {
-                const unsigned long long q = base_eq + r1++;
-                if (q < eq_budget) { cand_bits[n_greater + q] = b[c]; out_idx[n_greater + q] = i + c; }
+            } else if constexpr (!THR) {
+                if (cls[c] == 1) {
+                    const unsigned long long q = base_eq + r1++;
+                    if (q < eq_budget) { cand_bits[n_greater + q] = b[c]; out_idx[n_greater + q] = i + c; }
+                }
             }
         }
         base_gt += tot2;
