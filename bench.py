@@ -379,6 +379,8 @@ def run_ours(args):
                      "kernel": ("sum_skyblock2_kernel" if info["kernel"] == "skyblock" and info["sky_block"] == 256
                                 else f"sum_{info['kernel']}_kernel"), "algorithmic_bytes_per_launch": b_comp,
                      "kernel_ms": sum_ms,
+                     "binding_bound": ("warp-instruction issue / FP64 (rows are served from L2: DESIGN.md section 6); "
+                                       "the HBM model is the roofline BASELINE.json asks for"),
                      "bytes_per_inband_lookup": b_comp / inband if inband else None},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,

@@ -55,7 +55,7 @@ constexpr size_t TIMING_MAX = 4096;  // timed searches kept between two tcw_get_
 // staged kernel, SFT chunking: used when the spectrogram rows of the span exceed CHUNK_MIN_BYTES;
 // a chunk then holds about CHUNK_TARGET_BYTES of rows (inside the 126 MB L2) and at most
 // CHUNK_MAX_ROWS rows (measured on B200: cfg4 is fastest at 1024-1280 rows of 80 KB, cfg2 at 2048
-// rows of 16 KB; _work sweeps of round 1d)
+// rows of 16 KB; chunk-size sweeps of round 1d)
 constexpr double CHUNK_MIN_BYTES = 96e6, CHUNK_TARGET_BYTES = 80e6, CHUNK_SCRATCH_MAX = 16e9;
 constexpr long CHUNK_MAX_ROWS = 2048;
 
