@@ -56,6 +56,14 @@ NCU_TRAFFIC_BYTES = {
 }
 
 
+# smsp__issue_active.avg.pct_of_peak_sustained_active of the same kernels, from the same captures:
+# the configurations are bound by warp-instruction issue, not by HBM.
+NCU_ISSUE_ACTIVE_PCT = {
+    "cfg2": 72.7, "cfg2:f32": 72.7, "cfg4": 73.1, "cfg4:f32": 73.1,
+    "cfg3": 63.0, "cfg3:u8": 63.0, "cfg3:bits": 63.0, "cfg5": 62.1, "cfg5:bits": 62.1,
+}
+
+
 # ----------------------------------------------------------------------------- helpers
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -392,6 +400,8 @@ def run_ours(args):
                      "kernel": ("sum_skyblock2_kernel" if info["kernel"] == "skyblock" and info["sky_block"] == 256
                                 else f"sum_{info['kernel']}_kernel"), "algorithmic_bytes_per_launch": b_comp,
                      "kernel_ms": sum_ms,
+                     "issue_active_pct_ncu": NCU_ISSUE_ACTIVE_PCT.get(args.config if args.format is None
+                                                                      else f"{args.config}:{args.format}"),
                      "binding_bound": ("warp-instruction issue / FP64 (rows are served from L2: DESIGN.md section 6); "
                                        "the HBM model is the roofline BASELINE.json asks for"),
                      "bytes_per_inband_lookup": b_comp / inband if inband else None},
