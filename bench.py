@@ -48,8 +48,8 @@ NCU_TRAFFIC_BYTES = {
     "cfg2:f32": (164000256 + 10949120, "profiles/r1d_cfg2_sum_full.md"),
     "cfg4": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
     "cfg4:f32": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
-    "cfg3": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
-    "cfg3:u8": (148593408 + 306204672, "profiles/r1c_cfg3u8_skyblock_full.md"),
+    "cfg3": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md (same kernel and device data as the uint8 input)"),
+    "cfg3:u8": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md (same kernel and device data as the uint8 input)"),
     "cfg3:bits": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md"),
     "cfg5": (940257280 + 1564303000, "profiles/r1i_cfg5_sky2_full.md"),
     "cfg5:bits": (940257280 + 1564303000, "profiles/r1i_cfg5_sky2_full.md"),
