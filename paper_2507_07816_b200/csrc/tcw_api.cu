@@ -547,7 +547,12 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
             // tcw_create_async: the rows travel in pieces of about 16 MB on a copy stream of the handle's
             // own, each piece followed by its re-lay and an event; the first search waits per SFT chunk.
             CREATE_TRY(dev_alloc(&h->up_staging, dev_row * n_sft, st));
-            CREATE_TRY(cudaStreamCreateWithFlags(&h->up_stream, cudaStreamNonBlocking));
+            {
+                // highest priority: the re-lay copies must not queue behind the search's CTAs
+                int prio_lo = 0, prio_hi = 0;
+                cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+                CREATE_TRY(cudaStreamCreateWithPriority(&h->up_stream, cudaStreamNonBlocking, prio_hi));
+            }
             cudaEvent_t ready;
             CREATE_TRY(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
             cudaEventRecord(ready, st);                       // allocations and the zero fill precede the pieces
