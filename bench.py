@@ -275,6 +275,10 @@ def run_ours(args):
         h.set_option(tcw.TCW_OPT_CHUNK_ROWS, args.chunk_rows)
     if args.stages:
         h.set_option(tcw.TCW_OPT_STAGES, args.stages)
+    if args.exact_index:
+        h.set_option(tcw.TCW_OPT_EXACT_INDEX, 1)
+    if args.general_f0:
+        h.set_option(tcw.TCW_OPT_GENERAL_F0, 1)
     out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
     out_best = torch.empty((n_groups, 2), dtype=torch.int32, device=dev)
 
@@ -568,6 +572,8 @@ def main():
     ap.add_argument("--f0-per-lane", type=int, default=0)
     ap.add_argument("--chunk-rows", type=int, default=0, help="staged kernel: SFT rows per chunk (0 auto, -1 never)")
     ap.add_argument("--stages", type=int, default=0, help="staged kernel: ring depth limit (0 auto)")
+    ap.add_argument("--exact-index", action="store_true", help="staged kernel: defining chain for every bin (no fast index)")
+    ap.add_argument("--general-f0", action="store_true", help="staged kernel: do not use the equally-spaced-f0 instantiation")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -43,7 +43,10 @@ enum {
     TCW_EINVAL = -1,       /* bad argument (NULL, size, ordering, range) */
     TCW_ENOMEM = -2,       /* host or device allocation failed */
     TCW_ECUDA = -3,        /* a CUDA runtime call failed (message in tcw_last_error) */
-    TCW_EUNSUPPORTED = -4  /* valid request the library cannot serve */
+    TCW_EUNSUPPORTED = -4, /* valid request the library cannot serve */
+    TCW_EINTERNAL = -5     /* a kernel found a staged window larger than the bound the host planned and
+                              skipped rows: the results of that search are NOT valid (never expected;
+                              reported by tcw_search_host, tcw_check, tcw_get_timing, tcw_get_info) */
 };
 
 /* Spectrogram element formats (normalised power rho or number count nu). */
@@ -141,9 +144,38 @@ typedef struct {
  */
 int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_best, void *stream);
 
+/* tcw_search_groups -- tcw_search restricted to the groups [group_begin, group_end) of the grid's
+ * flattened group index (s*n_tau + a)*n_brk + b: the unit of the multi-GPU partition (SURVEY.md
+ * section 8(e): whole (tau, n, sky) groups per GPU, spectrogram replicated, no collective).
+ *  out_stat  DEVICE, [(group_end - group_begin)][n_f0], the range's slice of tcw_search's out_stat; may be NULL.
+ *  out_best  DEVICE, [(group_end - group_begin)] candidate records; may be NULL (not both).
+ * The range is served as at most seven sub-grid searches (whole sky points, whole tau rows, part of a
+ * tau row), enqueued on `stream`; every template is evaluated exactly as by tcw_search, so the
+ * outputs equal the corresponding slices of a whole-grid search bit for bit.  Asynchronous.
+ * TCW_EINVAL for an empty range or one outside 0..n_groups. */
+int tcw_search_groups(tcw_handle *h, const tcw_grid *grid, long group_begin, long group_end,
+                      void *out_stat, void *out_best, void *stream);
+
+/* tcw_split_groups -- the decomposition tcw_search_groups uses, as a host-only call (no CUDA): the
+ * range [group_begin, group_end) of the flattened group index as *n_rects <= 7 sub-grids in
+ * ascending group order, rects[i] = { sky_begin, sky_end, tau_begin, tau_end, brk_begin, brk_end }
+ * (half-open index ranges).  Each sub-grid's own [sky][tau][brk] order is a contiguous run of the
+ * flattened index.  An empty range gives *n_rects = 0.  TCW_EINVAL for non-positive sizes. */
+int tcw_split_groups(int n_tau, int n_brk, long group_begin, long group_end, int rects[7][6], int *n_rects);
+
+/* tcw_check -- synchronise the handle's last stream and report whether the last search on it was
+ * valid: TCW_OK, or TCW_EINTERNAL if a kernel set the device status word (see TCW_EINTERNAL).
+ * tcw_search, tcw_search_weighted, tcw_search_groups and tcw_search_bank are asynchronous and cannot
+ * report this themselves: a caller that does not use tcw_search_host should call tcw_check (or
+ * tcw_get_info) once the outputs are needed.  Every search clears the status word when it starts. */
+int tcw_check(tcw_handle *h);
+
 /* tcw_search_host -- the same search with HOST output buffers (either may be NULL, not both):
  * runs tcw_search into library scratch, copies the results to the host and synchronises the
- * stream before returning. */
+ * stream before returning.  An out_stat of 64 MiB or more is produced tau range by tau range and each
+ * range is copied on a second stream while the next is searched (pinned host buffers are needed for
+ * that overlap); the values are those of the one-piece search, bit for bit.  Returns TCW_EINTERNAL
+ * if a kernel set the device status word (see above). */
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host,
                     void *stream);
 
@@ -304,6 +336,19 @@ int tcw_track_indices(tcw_handle *h, const tcw_grid *grid, long n_sel, const lon
  * Either may be NULL.  Synchronises `stream`. */
 int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
 
+/* tcw_measure_peaks -- microbenchmarks of the limits that bind the track-sum kernels on the current
+ * device (SURVEY.md section 0 asks the builder to measure them): kernels that
+ * only issue independent instructions of one kind, timed with CUDA events on `stream` (best of three
+ * launches after a warm-up).  Whole-GPU rates per second:
+ *  out[0] FP64 DFMA warp instructions/s   out[1] FP64 DMUL   out[2] FP64 DADD
+ *  out[3] FP32 FFMA warp instructions/s (= the schedulers' issue limit, one per scheduler per cycle)
+ *  out[4] LDS.32 warp instructions/s for the staged kernel's gather pattern (conflict-free, stride < 1 word)
+ *  out[5] lookups/s of the bare lookup chain of sum_staged_kernel (DFMA, address, LDS.32, FADD, half a
+ *         VIMNMX3 per lookup; no staging, metadata or band edges): the speed of light of the instruction mix
+ *  out[6] number of SMs   out[7] nominal maximum SM clock in Hz
+ * n_out must be >= 8.  Synchronous; takes about 0.1 s. */
+int tcw_measure_peaks(double *out, int n_out, void *stream);
+
 /* Options.  tcw_set_option returns TCW_EINVAL for an unknown key or value. */
 enum {
     TCW_OPT_KERNEL = 0,     /* 0 auto (default), 1 force the global-memory gather kernel,
@@ -319,11 +364,20 @@ enum {
                                kernel: needs n_sft * (largest count in the spectrogram) <= 32767, else
                                TCW_EUNSUPPORTED at search); 0 auto (256 when that holds and the grid has
                                >= 128 sky points, else 64)                                           */
-    TCW_OPT_CHUNK_ROWS = 5  /* staged kernel: SFT rows per chunk (rounded up to a multiple of 64).  A
+    TCW_OPT_CHUNK_ROWS = 5, /* staged kernel: SFT rows per chunk (rounded up to a multiple of 64).  A
                                chunked search runs every (group, f0 tile) over one chunk of SFTs
                                before any over the next, so the rows in use stay in L2; per-chunk
                                partial sums are then added in ascending chunk order (fixed order).
                                0 auto (chunk only spectrograms larger than L2), -1 never chunk    */
+    TCW_OPT_EXACT_INDEX = 6,/* staged kernel: 1 = decide every bin by the defining chain of three binary64
+                               operations instead of the one-FMA fast index with its guard band (same
+                               bins either way; the tests compare the two); 0 default                  */
+    TCW_OPT_GENERAL_F0 = 7, /* staged kernel: 1 = treat the f0 axis as arbitrary even when it is equally spaced (the
+                               equally spaced instantiation derives the templates of a lane from one product
+                               and a stride; same bins either way); 0 default                              */
+    TCW_OPT_DEBUG_SHRINK_SLOT = 100 /* test hook: the kernels check their staged windows against the planned
+                               bound minus this many bytes, which forces the device status word and
+                               hence TCW_EINTERNAL; 0 default.  Not for production use.               */
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 

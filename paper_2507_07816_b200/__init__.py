@@ -16,19 +16,22 @@ import numpy as np
 from . import build as _build
 
 __all__ = [
-    "TcwError", "Handle", "Grid", "load_library", "library_path", "shard_groups",
+    "TcwError", "Handle", "Grid", "load_library", "library_path", "shard_groups", "split_groups", "measure_peaks",
     "TCW_F32_POWER", "TCW_U8_COUNT", "TCW_BIT_COUNT", "FORMATS",
 ]
 
-TCW_OK, TCW_EINVAL, TCW_ENOMEM, TCW_ECUDA, TCW_EUNSUPPORTED = 0, -1, -2, -3, -4
+TCW_OK, TCW_EINVAL, TCW_ENOMEM, TCW_ECUDA, TCW_EUNSUPPORTED, TCW_EINTERNAL = 0, -1, -2, -3, -4, -5
 TCW_F32_POWER, TCW_U8_COUNT, TCW_BIT_COUNT = 0, 1, 2
 TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE, TCW_OPT_STAGES, TCW_OPT_SKY_BLOCK = 0, 1, 2, 3, 4
 TCW_OPT_CHUNK_ROWS = 5
+TCW_OPT_EXACT_INDEX = 6
+TCW_OPT_GENERAL_F0 = 7
+TCW_OPT_DEBUG_SHRINK_SLOT = 100
 KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_create_async", "tcw_upload_wait", "tcw_search", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_create_async", "tcw_upload_wait", "tcw_search", "tcw_search_groups", "tcw_split_groups", "tcw_check", "tcw_measure_peaks", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -88,6 +91,14 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_upload_wait.argtypes = [vp]
     L.tcw_search.restype = ci
     L.tcw_search.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
+    L.tcw_search_groups.restype = ci
+    L.tcw_search_groups.argtypes = [vp, ctypes.POINTER(_CGrid), cl, cl, vp, vp, vp]
+    L.tcw_split_groups.restype = ci
+    L.tcw_split_groups.argtypes = [ci, ci, cl, cl, vp, ctypes.POINTER(ci)]
+    L.tcw_measure_peaks.restype = ci
+    L.tcw_measure_peaks.argtypes = [dp, ci, vp]
+    L.tcw_check.restype = ci
+    L.tcw_check.argtypes = [vp]
     L.tcw_search_host.restype = ci
     L.tcw_search_host.argtypes = [vp, ctypes.POINTER(_CGrid), vp, vp, vp]
     L.tcw_search_weighted.restype = ci
@@ -237,6 +248,28 @@ class Handle:
                             out_stat.data_ptr() if out_stat is not None else None,
                             out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
         return out_stat, out_best
+
+    def search_groups(self, grid: Grid, group_begin: int, group_end: int, out_stat=None, out_best=None,
+                      want_stat: bool = True, want_best: bool = True, stream=None):
+        """tcw_search_groups: the groups [group_begin, group_end) of the grid's flattened
+        (sky, tau, n) index.  Returns (stat [n][n_f0], best [n][2]) for those groups.  Asynchronous."""
+        import torch
+        L = load_library()
+        dev = torch.device("cuda", torch.cuda.current_device())
+        n = int(group_end) - int(group_begin)
+        if out_stat is None and want_stat:
+            out_stat = torch.empty((max(n, 0), len(grid.f0)), dtype=self.stat_dtype, device=dev)
+        if out_best is None and want_best:
+            out_best = torch.empty((max(n, 0), 2), dtype=torch.int32, device=dev)
+        cg = grid._c()
+        _check(L.tcw_search_groups(self._h, ctypes.byref(cg), int(group_begin), int(group_end),
+                                   out_stat.data_ptr() if out_stat is not None else None,
+                                   out_best.data_ptr() if out_best is not None else None, _stream_ptr(stream)))
+        return out_stat, out_best
+
+    def check(self):
+        """tcw_check: synchronise and raise TcwError(TCW_EINTERNAL) if the last search was invalid."""
+        _check(load_library().tcw_check(self._h))
 
     def search_weighted(self, grid: Grid, weights, mean1: float, var1: float, out_psi=None, out_stat=None,
                         out_best=None, want_psi: bool = True, want_stat: bool = True, want_best: bool = True,
@@ -396,9 +429,13 @@ class Handle:
         _check(load_library().tcw_get_timing(self._h, ms, ctypes.byref(n)))
         return tuple(float(x) for x in ms), int(n.value)
 
-    def info(self) -> dict:
+    def info(self, check: bool = True) -> dict:
+        """tcw_get_info.  Raises TcwError(TCW_EINTERNAL) if the device status word is set, unless
+        check=False (the dict's "status" then carries the word)."""
         v = (ctypes.c_long * 10)()
-        _check(load_library().tcw_get_info(self._h, v))
+        rc = load_library().tcw_get_info(self._h, v)
+        if rc != TCW_OK and (check or rc != TCW_EINTERNAL):
+            _check(rc)
         return dict(kernel={1: "gather", 2: "staged", 3: "skyblock", 4: "bank"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
                     smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]),
                     sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]))
@@ -451,12 +488,32 @@ def prepare(strain, fs: float, T_sft: float, f_min: float, n_bins: int, median_b
     return out[: got.value]
 
 
-def shard_groups(n_sky: int, rank: int, world_size: int) -> slice:
-    """Multi-GPU partition: whole sky points -- hence whole (sky, tau, n)
-    groups, so each per-group argmax stays on one rank -- split into contiguous, nearly equal
-    ranges.  No collective is needed on the data path; the spectrogram is replicated."""
+def measure_peaks(stream=None) -> dict:
+    """tcw_measure_peaks: measured whole-GPU rates of the limits that bind the kernels (per second)."""
+    out = (ctypes.c_double * 8)()
+    _check(load_library().tcw_measure_peaks(out, 8, _stream_ptr(stream)))
+    keys = ("fp64_dfma_winst_per_s", "fp64_dmul_winst_per_s", "fp64_dadd_winst_per_s", "issue_winst_per_s",
+            "lds32_winst_per_s", "chain_lookups_per_s", "n_sm", "sm_clock_max_hz")
+    return dict(zip(keys, (float(x) for x in out)))
+
+
+def split_groups(n_tau: int, n_brk: int, group_begin: int, group_end: int) -> list[tuple[slice, slice, slice]]:
+    """tcw_split_groups: the sub-grids (sky, tau, brk index slices) that tile a contiguous range
+    of the flattened group index, in ascending order (host-only; what tcw_search_groups runs)."""
+    rects = ((ctypes.c_int * 6) * 7)()
+    n = ctypes.c_int(0)
+    _check(load_library().tcw_split_groups(int(n_tau), int(n_brk), int(group_begin), int(group_end), rects, ctypes.byref(n)))
+    return [(slice(r[0], r[1]), slice(r[2], r[3]), slice(r[4], r[5])) for r in list(rects)[: n.value]]
+
+
+def shard_groups(n_groups: int, rank: int, world_size: int) -> tuple[int, int]:
+    """Multi-GPU partition: the flattened (sky, tau, n)
+    group index 0..n_groups-1 is cut into world_size contiguous, nearly equal ranges and rank r
+    searches [begin, end) with Handle.search_groups.  Whole groups per rank, so each per-group
+    argmax stays on one rank; the spectrogram is replicated; no collective on the data path.
+    A rank may get an empty range (begin == end) when world_size > n_groups."""
     if not (0 <= rank < world_size):
         raise ValueError("rank out of range")
-    base, rem = divmod(n_sky, world_size)
+    base, rem = divmod(int(n_groups), world_size)
     lo = rank * base + min(rank, rem)
-    return slice(lo, lo + base + (1 if rank < rem else 0))
+    return lo, lo + base + (1 if rank < rem else 0)

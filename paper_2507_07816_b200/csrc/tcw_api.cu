@@ -27,6 +27,7 @@
 #include "tcw_bank.cuh"
 #include "tcw_select.cuh"
 #include "tcw_prep.cuh"
+#include "tcw_peaks.cuh"
 
 namespace {
 
@@ -161,6 +162,7 @@ struct tcw_handle {
     bool t_pow2 = false;
     double vmax = 0;  // max |v_j|
     int count_max = 1;  // count formats: largest element of the spectrogram (1 for bit-packed input)
+    bool count_known = true;  // false while an asynchronous uint8 upload has not been scanned yet
     double vmid[3] = {0, 0, 0};  // velocity at the middle SFT: sort key of the sky-block kernel
     std::vector<double> ts;
     unsigned char *d_spec = nullptr;
@@ -172,7 +174,8 @@ struct tcw_handle {
     DevBuf<unsigned char> d_selws;           // selection scratch (histogram, state, block counts, candidates)
     DevBuf<double> d_bank;                   // bank searches: f0, tau, brk [n] and sky [n][3] or [3]
     unsigned long long *d_counter = nullptr; // bank searches: lookups decided by the defining chain
-    DevBuf<float> d_w, d_cw;                 // weighted searches: weights [n_sky][n_sft]; per-chunk sums of w and w^2
+    DevBuf<float> d_w;                       // weighted searches: weights [n_sky][n_sft]
+    DevBuf<double> d_cw;                     // weighted searches: per-chunk sums of w and w^2 (float64)
     DevBuf<long> d_sel;
     DevBuf<double> d_dts, d_dmm;  // sky-block kernel: per-block Doppler rows and their {min, max}
     DevBuf<int> d_slot;           // sky index of each block slot
@@ -182,8 +185,13 @@ struct tcw_handle {
     size_t h_stage_cap = 0;     // bytes
     cudaEvent_t ev_stage = nullptr;
     // options
-    int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0, opt_sky = 0;
+    int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0, opt_sky = 0, opt_exact = 0;
     long opt_chunk = 0;  // SFT rows per chunk of the staged kernel: 0 auto, -1 never chunk
+    cudaStream_t dl_stream = nullptr;        // tcw_search_host: read-back stream and one event per part
+    std::vector<cudaEvent_t> dl_ev;
+    int opt_nonuniform = 0;   // 1: never take the equally-spaced-f0 instantiation of the staged kernel
+    bool keep_status = false; // a multi-part search (tcw_search_groups, tcw_search_host) clears the status word once
+    int dbg_slot_shrink = 0;  // test hook: bytes taken off the kernels' own window bound
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
@@ -201,6 +209,19 @@ struct tcw_handle {
 };
 
 namespace {
+
+// The kernels set the device status word when a window bound computed on the host is violated
+// (rows are then skipped, so the sums would be wrong).  Call with the search's stream synchronised.
+int check_status(tcw_handle *h)
+{
+    int status = 0;
+    CUDA_TRY(cudaMemcpy(&status, h->d_status, sizeof(int), cudaMemcpyDeviceToHost));
+    h->info[4] = status;
+    if (status != 0)
+        return fail(TCW_EINTERNAL, "device status word %d: a staged window exceeded the bound planned on the host; "
+                                   "the results of the last search on this handle are not valid", status);
+    return TCW_OK;
+}
 
 // Start of an API call on `st`: scratch of this call is allocated on st; if the previous call on
 // this handle used another stream, wait for it (buffers are reused across calls).
@@ -232,8 +253,11 @@ int validate_grid(const tcw_handle *h, const tcw_grid *g)
         double nrm = std::sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
         if (!(std::fabs(nrm - 1.0) <= 1e-6)) return fail(TCW_EINVAL, "sky[%d] is not a unit vector", i);
     }
-    long n_groups = (long)g->n_sky * g->n_tau * g->n_brk;
-    if (n_groups * (long)g->n_f0 / g->n_f0 != n_groups || n_groups > (1L << 40))
+    long n_groups = 0, n_templates = 0;
+    if (__builtin_mul_overflow((long)g->n_sky, (long)g->n_tau, &n_groups) ||
+        __builtin_mul_overflow(n_groups, (long)g->n_brk, &n_groups) ||
+        __builtin_mul_overflow(n_groups, (long)g->n_f0, &n_templates) || n_groups > (1L << 40) ||
+        n_templates > (1L << 48))
         return fail(TCW_EINVAL, "grid too large");
     return TCW_OK;
 }
@@ -315,7 +339,7 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
     std::memset(&p, 0, sizeof p);
     p.spec = h->d_spec + h->pad_bytes;
     p.spec_pad = h->d_spec;
-    p.pad16 = (int)(h->pad_bytes >> 4);
+    p.pad_bytes = h->pad_bytes;
     p.pitch = h->pitch;
     p.n_sft = h->n_sft;
     p.n_bins = h->n_bins;
@@ -334,6 +358,36 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
     const double dmax = 1.0 + (h->vmax / C_LIGHT) * (1.0 + 1e-5) + 1e-15;
     p.dmaxT = dmax * h->T * (1.0 + 1e-12);
     p.status = h->d_status;
+    // fast bin index of the staged kernel: |fast x - oracle's x| <= 3*x*2^-52 + 2^-32 bins;
+    // thr is that bound with a margin, in units of 2^-32 bin, never below 64 units (1.5e-8 bin)
+    {
+        const double x_max = g->f0[g->n_f0 - 1] * p.dmaxT;
+        const double units = std::ceil((4.0 * x_max * 0x1p-52 + 0x1p-31) * 0x1p32);
+        double thr_units = std::max(64.0, units);
+        // equally spaced f0 (the cubic lattice of PAPER.md:63): f0[i] = f0[0] + i*delta up to a deviation worth
+        // less than 2^-34 bin.  The kernel then needs no per-template f0 registers.
+        p.d32 = 0.0;
+        if (g->n_f0 >= 2 && !h->opt_nonuniform) {
+            const long double delta = ((long double)g->f0[g->n_f0 - 1] - (long double)g->f0[0]) / (long double)(g->n_f0 - 1);
+            long double dev = 0;
+            for (int i = 0; i < g->n_f0; ++i)
+                dev = std::max(dev, fabsl((long double)g->f0[i] - ((long double)g->f0[0] + (long double)i * delta)));
+            const double d = (double)delta;
+            // delta must be exact in binary64 and lane*delta, 32*delta exact as well (8 spare mantissa bits)
+            const bool exact = (long double)d == delta && std::fabs(std::remainder(std::ldexp(d, 44 - std::ilogb(d)), 1.0)) == 0.0;
+            if (exact && (double)dev * p.dmaxT <= 0x1p-34) {
+                p.d32 = 32.0 * d;
+                thr_units += 2.0;
+            }
+        }
+        if (h->opt_exact || thr_units > 1048576.0) {
+            p.thr2 = 0xffffffffu;
+            p.fix_add = 0.5 + (double)tcw::FIX_OFF;
+        } else {
+            p.thr2 = (uint32_t)(2.0 * thr_units);
+            p.fix_add = 0.5 + thr_units * 0x1p-32 + (double)tcw::FIX_OFF;
+        }
+    }
     return p;
 }
 
@@ -358,40 +412,44 @@ int slot_bytes_for(int fmt_dev, long w_bins)
     return b > (1L << 30) ? (1 << 30) : (int)b;
 }
 
-template <int FMT, int R, bool P2, bool WGT>
+template <int FMT, int R, bool P2, bool WGT, bool UNI>
 int launch_staged_t(const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    auto kern = tcw::sum_staged_kernel<FMT, R, P2, WGT>;
+    auto kern = tcw::sum_staged_kernel<FMT, R, P2, WGT, UNI>;
     CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)n_ctas, tcw::STAGED_THREADS, smem, st>>>(p);
     CUDA_TRY(cudaGetLastError());
     return TCW_OK;
 }
 
-template <int FMT, bool P2, bool WGT>
+template <int FMT, bool P2, bool WGT, bool UNI>
 int launch_staged_r(int r, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
     switch (r) {
-    case 16: return launch_staged_t<FMT, 16, P2, WGT>(p, n_ctas, smem, st);
-    case 8: return launch_staged_t<FMT, 8, P2, WGT>(p, n_ctas, smem, st);
-    default: return launch_staged_t<FMT, 4, P2, WGT>(p, n_ctas, smem, st);
+    case 16: return launch_staged_t<FMT, 16, P2, WGT, UNI>(p, n_ctas, smem, st);
+    case 8: return launch_staged_t<FMT, 8, P2, WGT, UNI>(p, n_ctas, smem, st);
+    default: return launch_staged_t<FMT, 4, P2, WGT, UNI>(p, n_ctas, smem, st);
     }
 }
 
-template <bool WGT>
+template <bool WGT, bool UNI>
 int launch_staged_w(int fmt, int r, bool p2, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
     if (fmt == tcw::FMT_F32)
-        return p2 ? launch_staged_r<tcw::FMT_F32, true, WGT>(r, p, n_ctas, smem, st)
-                  : launch_staged_r<tcw::FMT_F32, false, WGT>(r, p, n_ctas, smem, st);
-    return p2 ? launch_staged_r<tcw::FMT_U8, true, WGT>(r, p, n_ctas, smem, st)
-              : launch_staged_r<tcw::FMT_U8, false, WGT>(r, p, n_ctas, smem, st);
+        return p2 ? launch_staged_r<tcw::FMT_F32, true, WGT, UNI>(r, p, n_ctas, smem, st)
+                  : launch_staged_r<tcw::FMT_F32, false, WGT, UNI>(r, p, n_ctas, smem, st);
+    return p2 ? launch_staged_r<tcw::FMT_U8, true, WGT, UNI>(r, p, n_ctas, smem, st)
+              : launch_staged_r<tcw::FMT_U8, false, WGT, UNI>(r, p, n_ctas, smem, st);
 }
 
+// p.d32 != 0 selects the instantiation for an equally spaced f0 axis
 int launch_staged(int fmt, int r, bool p2, bool wgt, const tcw::SumParams &p, long n_ctas, size_t smem, cudaStream_t st)
 {
-    return wgt ? launch_staged_w<true>(fmt, r, p2, p, n_ctas, smem, st)
-               : launch_staged_w<false>(fmt, r, p2, p, n_ctas, smem, st);
+    if (p.d32 != 0.0)
+        return wgt ? launch_staged_w<true, true>(fmt, r, p2, p, n_ctas, smem, st)
+                   : launch_staged_w<false, true>(fmt, r, p2, p, n_ctas, smem, st);
+    return wgt ? launch_staged_w<true, false>(fmt, r, p2, p, n_ctas, smem, st)
+               : launch_staged_w<false, false>(fmt, r, p2, p, n_ctas, smem, st);
 }
 
 template <int FMT, bool WGT> int launch_gather_t(bool p2, const tcw::SumParams &p, long n_ctas, cudaStream_t st)
@@ -590,7 +648,8 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
         CREATE_TRY(cudaMemcpyAsync(&h->count_max, h->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
         CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     } else if (format == TCW_U8_COUNT) {
-        h->count_max = 255;   // asynchronous upload: the data are not here yet; assume the worst
+        h->count_max = 255;   // asynchronous upload: the data are not here yet; the first search scans them
+        h->count_known = false;
     }
     CREATE_TRY(cudaMemcpyAsync(h->d_ts, timestamps, sizeof(double) * n_sft, cudaMemcpyHostToDevice, st));
     CREATE_TRY(cudaMemcpyAsync(h->d_vel, velocities, sizeof(double) * 3 * (size_t)n_sft, cudaMemcpyHostToDevice, st));
@@ -649,6 +708,11 @@ int tcw_destroy(tcw_handle *h)
     cudaSetDevice(h->device);
     // nothing enqueued by this handle may still be running when its memory goes back to the pool
     cudaStreamSynchronize(h->last_stream);
+    if (h->dl_stream) {
+        cudaStreamSynchronize(h->dl_stream);
+        for (auto &e : h->dl_ev) cudaEventDestroy(e);
+        cudaStreamDestroy(h->dl_stream);
+    }
     if (h->up_stream) {
         cudaStreamSynchronize(h->up_stream);
         for (auto &e : h->up_ev) cudaEventDestroy(e);
@@ -712,6 +776,18 @@ int tcw_set_option(tcw_handle *h, int key, long value)
             return fail(TCW_EINVAL, "TCW_OPT_SKY_BLOCK must be 0, 64, 128 or 256");
         h->opt_sky = (int)value;
         return TCW_OK;
+    case TCW_OPT_EXACT_INDEX:
+        if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_EXACT_INDEX must be 0 or 1");
+        h->opt_exact = (int)value;
+        return TCW_OK;
+    case TCW_OPT_GENERAL_F0:
+        if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_GENERAL_F0 must be 0 or 1");
+        h->opt_nonuniform = (int)value;
+        return TCW_OK;
+    case TCW_OPT_DEBUG_SHRINK_SLOT:
+        if (value < 0 || value > (1 << 20)) return fail(TCW_EINVAL, "TCW_OPT_DEBUG_SHRINK_SLOT must be 0..2^20");
+        h->dbg_slot_shrink = (int)value;
+        return TCW_OK;
     case TCW_OPT_CHUNK_ROWS:
         if (value < -1 || value > (1L << 30)) return fail(TCW_EINVAL, "TCW_OPT_CHUNK_ROWS must be -1, 0 or a row count");
         h->opt_chunk = value;
@@ -737,6 +813,21 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     cudaStream_t st = (cudaStream_t)stream;
     enter(h, st);
     const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
+    if (!h->count_known) {
+        // uint8 handle of tcw_create_async: the launch plan needs the largest count, so wait for the
+        // upload and scan the rows now (tcw_create does this before returning)
+        CUDA_TRY(cudaSetDevice(h->device));
+        if (h->up_stream) CUDA_TRY(cudaStreamSynchronize(h->up_stream));
+        int *d_max = nullptr;
+        CUDA_TRY(dev_alloc((void **)&d_max, sizeof(int), st));
+        CUDA_TRY(cudaMemsetAsync(d_max, 0, sizeof(int), st));
+        tcw::max_u8_kernel<<<148 * 8, 256, 0, st>>>(h->d_spec + h->pad_bytes, h->pitch, h->n_sft, h->n_bins, d_max);
+        CUDA_TRY(cudaGetLastError());
+        CUDA_TRY(cudaMemcpyAsync(&h->count_max, d_max, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        dev_free(d_max, st);
+        h->count_known = true;
+    }
 
     tcw::SumParams p = base_params(h, grid);
     tcw::SkyParams q;
@@ -782,7 +873,10 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         const int all[3] = {16, 8, 4};
         for (int c = 0; c < 3 && !kernel; ++c) {
             if (h->opt_r && all[c] != h->opt_r) continue;
-            const long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
+            long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
+            // equally spaced f0: the lanes past the end of a ragged last tile still form addresses (their sums
+            // are discarded), so every slot holds the window of a whole tile
+            if (p.d32 != 0.0) w_bins = std::max(w_bins, (long)std::floor((32 * all[c] - 1) * (p.d32 / 32.0) * p.dmaxT) + 3);
             if (w_bins > tcw::PAD_BINS) continue;
             const int sb = slot_bytes_for(h->fmt_dev, w_bins);
             // rings two slots deep (a slot is RB rows) hide the L2 latency; three CTAs of four warps per SM
@@ -803,6 +897,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     p.n_tiles = (grid->n_f0 + p.tile - 1) / p.tile;
     p.stages = stages;
     p.slot_bytes = slot;
+    p.slot_limit = slot - h->dbg_slot_shrink;   // = slot except under the test hook TCW_OPT_DEBUG_SHRINK_SLOT
     const long n_partial = n_groups * p.n_tiles;
     long n_ctas = n_partial;
     if (kernel == 2) {
@@ -816,7 +911,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         if (c_rows > 0) {
             c_rows = std::max<long>(64, (c_rows + 63) / 64 * 64);
             long nc = (rows + c_rows - 1) / c_rows;
-            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * (wgt ? 12.0 : 4.0);
+            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * (wgt ? 20.0 : 4.0);
             if (nc > 1 && nc <= 255 && scratch <= CHUNK_SCRATCH_MAX && nc * n_partial <= 2147483647L) {
                 p.chunk_rows = (int)c_rows;
                 p.n_chunks = (int)nc;
@@ -886,6 +981,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         ev = h->ev.data() + 4 * h->timing_n;
         CUDA_TRY(cudaEventRecord(ev[0], st));
     }
+    if (!h->keep_status) CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     if ((rc = prepare(h, grid, 0, nullptr, st, kernel == 3 ? &h->slot_host : nullptr)) != TCW_OK) return rc;
     p.f0 = h->a_f0;
     p.gtab = h->d_g.p;
@@ -1306,6 +1402,95 @@ done:
     return rc;
 }
 
+// A contiguous range [g0, g1) of the flattened group index (s*n_tau + a)*n_brk + b as at most seven
+// sub-grids, in ascending group order; the output of each (its own [s][a][b][f0] layout) is then a
+// contiguous slice of the full output: whole sky points, whole tau rows of one sky point, or part
+// of one tau row.
+struct GroupRect { int s0, s1, a0, a1, b0, b1; };
+static std::vector<GroupRect> split_groups(int n_tau, int n_brk, long g0, long g1)
+{
+    std::vector<GroupRect> out;
+    const long per_sky = (long)n_tau * n_brk;
+    long cur = g0;
+    while (cur < g1) {
+        const long s = cur / per_sky, rem = cur % per_sky;
+        if (rem == 0 && g1 - cur >= per_sky) {
+            const long ns = (g1 - cur) / per_sky;
+            out.push_back({(int)s, (int)(s + ns), 0, n_tau, 0, n_brk});
+            cur += ns * per_sky;
+            continue;
+        }
+        const long e = std::min(g1, (s + 1) * per_sky) - s * per_sky;   // end of the range inside sky point s
+        const int a = (int)(rem / n_brk), b = (int)(rem % n_brk);
+        if (b != 0 || e - rem < n_brk) {
+            const int b1 = (int)std::min<long>(n_brk, b + (e - rem));
+            out.push_back({(int)s, (int)s + 1, a, a + 1, b, b1});
+            cur += b1 - b;
+        } else {
+            const int na = (int)((e - rem) / n_brk);
+            out.push_back({(int)s, (int)s + 1, a, a + na, 0, n_brk});
+            cur += (long)na * n_brk;
+        }
+    }
+    return out;
+}
+
+static tcw_grid sub_grid(const tcw_grid *g, const GroupRect &r)
+{
+    tcw_grid s = *g;
+    s.n_sky = r.s1 - r.s0; s.sky = g->sky + 3 * (size_t)r.s0;
+    s.n_tau = r.a1 - r.a0; s.tau = g->tau + r.a0;
+    s.n_brk = r.b1 - r.b0; s.brk = g->brk + r.b0;
+    return s;
+}
+
+int tcw_split_groups(int n_tau, int n_brk, long group_begin, long group_end, int rects[7][6], int *n_rects)
+{
+    if (!rects || !n_rects) return fail(TCW_EINVAL, "NULL argument");
+    if (n_tau <= 0 || n_brk <= 0 || group_begin < 0 || group_begin > group_end)
+        return fail(TCW_EINVAL, "sizes must be positive and the range ordered");
+    const std::vector<GroupRect> v = split_groups(n_tau, n_brk, group_begin, group_end);
+    if (v.size() > 7) return fail(TCW_EINTERNAL, "group range split into %zu rectangles", v.size());
+    for (size_t i = 0; i < v.size(); ++i) {
+        const int r[6] = {v[i].s0, v[i].s1, v[i].a0, v[i].a1, v[i].b0, v[i].b1};
+        std::memcpy(rects[i], r, sizeof r);
+    }
+    *n_rects = (int)v.size();
+    return TCW_OK;
+}
+
+int tcw_search_groups(tcw_handle *h, const tcw_grid *grid, long group_begin, long group_end, void *out_stat,
+                      void *out_best, void *stream)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    int rc = validate_grid(h, grid);
+    if (rc != TCW_OK) return rc;
+    if (!out_stat && !out_best) return fail(TCW_EINVAL, "out_stat and out_best are both NULL");
+    const long n_groups = (long)grid->n_sky * grid->n_tau * grid->n_brk;
+    if (group_begin < 0 || group_end > n_groups || group_begin >= group_end)
+        return fail(TCW_EINVAL, "group range [%ld, %ld) is empty or outside 0..%ld", group_begin, group_end, n_groups);
+    cudaStream_t st = (cudaStream_t)stream;
+    enter(h, st);
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
+    h->keep_status = true;
+    long info_sum[3] = {0, 0, 0};   // CTAs, kernels launched, parts
+    for (const GroupRect &r : split_groups(grid->n_tau, grid->n_brk, group_begin, group_end)) {
+        const tcw_grid sub = sub_grid(grid, r);
+        const long first = ((long)r.s0 * grid->n_tau + r.a0) * grid->n_brk + r.b0 - group_begin;
+        rc = search_impl(h, &sub, nullptr, out_stat ? (char *)out_stat + (size_t)first * grid->n_f0 * 4 : nullptr, nullptr,
+                         out_best ? (char *)out_best + (size_t)first * 8 : nullptr, stream);
+        if (rc != TCW_OK) break;
+        info_sum[0] += h->info[2]; info_sum[1] += h->info[5]; info_sum[2]++;
+    }
+    h->keep_status = false;
+    if (rc == TCW_OK) { h->info[2] = info_sum[0]; h->info[5] = info_sum[1]; }
+    return rc;
+}
+
+// Outputs of at least this many bytes are read back part by part (tau sub-ranges) while the next part is searched.
+constexpr size_t HOST_OVERLAP_MIN_BYTES = 64u << 20, HOST_PART_BYTES = 40u << 20;
+
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host, void *stream)
 {
     if (!h) return fail(TCW_EINVAL, "handle is NULL");
@@ -1319,14 +1504,122 @@ int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, vo
     CUDA_TRY(cudaSetDevice(h->device));
     if (out_stat_host && (rc = h->d_stat.reserve(n_templates * 4)) != TCW_OK) return rc;
     if ((rc = h->d_best.reserve(n_groups * 8)) != TCW_OK) return rc;
-    rc = tcw_search(h, grid, out_stat_host ? (void *)h->d_stat.p : nullptr, h->d_best.p, stream);
-    if (rc != TCW_OK) return rc;
-    if (out_stat_host)
-        CUDA_TRY(cudaMemcpyAsync(out_stat_host, h->d_stat.p, n_templates * 4, cudaMemcpyDeviceToHost, st));
-    if (out_best_host)
-        CUDA_TRY(cudaMemcpyAsync(out_best_host, h->d_best.p, n_groups * 8, cudaMemcpyDeviceToHost, st));
+    int n_parts = 1;
+    if (out_stat_host && n_templates * 4 >= HOST_OVERLAP_MIN_BYTES)
+        n_parts = (int)std::min<size_t>({(size_t)grid->n_tau, (n_templates * 4 + HOST_PART_BYTES / 2) / HOST_PART_BYTES, (size_t)16});
+    if (n_parts <= 1) {
+        rc = tcw_search(h, grid, out_stat_host ? (void *)h->d_stat.p : nullptr, h->d_best.p, stream);
+        if (rc != TCW_OK) return rc;
+        if (out_stat_host)
+            CUDA_TRY(cudaMemcpyAsync(out_stat_host, h->d_stat.p, n_templates * 4, cudaMemcpyDeviceToHost, st));
+        if (out_best_host)
+            CUDA_TRY(cudaMemcpyAsync(out_best_host, h->d_best.p, n_groups * 8, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        return check_status(h);
+    }
+    // Large outputs: the tau axis is cut into parts; part p is searched into its own contiguous piece of
+    // the scratch and copied to the host (one strided copy: a part is n_sky rows of the full layout) on a
+    // second stream while part p + 1 is searched.  Same kernels, same per-template arithmetic: results
+    // are bit-identical to the one-piece search.
+    if (!h->dl_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->dl_stream, cudaStreamNonBlocking));
+    while ((int)h->dl_ev.size() < n_parts) {
+        cudaEvent_t e;
+        CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        h->dl_ev.push_back(e);
+    }
+    CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
+    h->keep_status = true;
+    const size_t row_t = (size_t)grid->n_brk * grid->n_f0 * 4, row_b = (size_t)grid->n_brk * 8;   // bytes per (sky, tau)
+    size_t off_t = 0, off_b = 0;
+    long info_sum[2] = {0, 0};
+    for (int p = 0; p < n_parts && rc == TCW_OK; ++p) {
+        const int a0 = (int)((long)grid->n_tau * p / n_parts), a1 = (int)((long)grid->n_tau * (p + 1) / n_parts);
+        const tcw_grid sub = sub_grid(grid, {0, grid->n_sky, a0, a1, 0, grid->n_brk});
+        unsigned char *dst_t = h->d_stat.p + off_t, *dst_b = h->d_best.p + off_b;
+        rc = search_impl(h, &sub, nullptr, dst_t, nullptr, dst_b, stream);
+        if (rc != TCW_OK) break;
+        info_sum[0] += h->info[2]; info_sum[1] += h->info[5];
+        cudaError_t e = cudaEventRecord(h->dl_ev[(size_t)p], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(h->dl_stream, h->dl_ev[(size_t)p], 0);
+        const size_t w_t = (size_t)(a1 - a0) * row_t, w_b = (size_t)(a1 - a0) * row_b;
+        if (e == cudaSuccess)
+            e = cudaMemcpy2DAsync((char *)out_stat_host + (size_t)a0 * row_t, (size_t)grid->n_tau * row_t, dst_t, w_t, w_t,
+                                  (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
+        if (e == cudaSuccess && out_best_host)
+            e = cudaMemcpy2DAsync((char *)out_best_host + (size_t)a0 * row_b, (size_t)grid->n_tau * row_b, dst_b, w_b, w_b,
+                                  (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
+        if (e != cudaSuccess) rc = fail(TCW_ECUDA, "read-back of part %d: %s", p, cudaGetErrorString(e));
+        off_t += w_t * grid->n_sky;
+        off_b += w_b * grid->n_sky;
+    }
+    h->keep_status = false;
+    cudaStreamSynchronize(h->dl_stream);
     CUDA_TRY(cudaStreamSynchronize(st));
-    return TCW_OK;
+    if (rc != TCW_OK) return rc;
+    h->info[2] = info_sum[0];
+    h->info[5] = info_sum[1];
+    return check_status(h);
+}
+
+int tcw_measure_peaks(double *out, int n_out, void *stream)
+{
+    if (!out || n_out < 8) return fail(TCW_EINVAL, "out must hold 8 doubles");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    float *d_out = nullptr;
+    CUDA_TRY(cudaMalloc((void **)&d_out, 64));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    const int ctas = n_sm * 8, iters = 4096;
+    const double warps = (double)ctas * (tcw::PEAK_THREADS / 32);
+    int rc = TCW_OK;
+    // each measurement: one warm-up launch, then the best of three timed launches
+    auto timed = [&](auto launch, double work, double *rate) {
+        launch();
+        float best = 1e30f;
+        for (int rep = 0; rep < 3; ++rep) {
+            cudaEventRecord(e0, st);
+            launch();
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = fail(TCW_ECUDA, "peak kernel: %s", cudaGetErrorString(cudaGetLastError())); return; }
+            float ms = 0;
+            cudaEventElapsedTime(&ms, e0, e1);
+            best = std::min(best, ms);
+        }
+        *rate = work / (best * 1e-3);
+    };
+    const double fp64_inst = warps * iters * 4.0 * tcw::PEAK_ILP;
+    timed([&] { tcw::peak_fp64_kernel<0><<<ctas, tcw::PEAK_THREADS, 0, st>>>(iters, 1.0, (double *)d_out); }, fp64_inst, &out[0]);
+    timed([&] { tcw::peak_fp64_kernel<1><<<ctas, tcw::PEAK_THREADS, 0, st>>>(iters, 1.0, (double *)d_out); }, fp64_inst, &out[1]);
+    timed([&] { tcw::peak_fp64_kernel<2><<<ctas, tcw::PEAK_THREADS, 0, st>>>(iters, 1.0, (double *)d_out); }, fp64_inst, &out[2]);
+    timed([&] { tcw::peak_issue_kernel<<<ctas, tcw::PEAK_THREADS, 0, st>>>(4 * iters, 1.0f, d_out); }, 4.0 * fp64_inst, &out[3]);
+    timed([&] { tcw::peak_lds_kernel<<<ctas, tcw::PEAK_THREADS, 0, st>>>(iters, d_out); }, warps * iters * 16.0, &out[4]);
+    {
+        const int rows = 8192, c_ctas = n_sm * 3 * 4;
+        // y = dlane*c + r*4c + q stays inside [1.5*2^20 + 8, 1.5*2^20 + 640)
+        timed([&] { tcw::peak_chain_kernel<<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, d_out); },
+              (double)c_ctas * 128.0 * rows * 16.0, &out[5]);
+    }
+    out[6] = (double)n_sm;
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+    out[7] = (double)khz * 1e3;     // the device's nominal maximum SM clock (Hz)
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_out);
+    if (rc == TCW_OK) CUDA_TRY(cudaGetLastError());
+    return rc;
+}
+
+int tcw_check(tcw_handle *h)
+{
+    if (!h) return fail(TCW_EINVAL, "handle is NULL");
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaStreamSynchronize(h->last_stream));
+    return check_status(h);
 }
 
 int tcw_track_indices(tcw_handle *h, const tcw_grid *grid, long n_sel, const long *sel, int *out_k, void *stream)
@@ -1385,7 +1678,7 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches)
     for (int c = 0; c < 4; ++c) ms[c] = (float)(acc[c] / (double)h->timing_n);
     if (n_searches) *n_searches = (int)h->timing_n;
     h->timing_n = 0;
-    return TCW_OK;
+    return check_status(h);   // the last timed search has completed: times of an invalid search are an error
 }
 
 int tcw_get_info(tcw_handle *h, long info[10])
@@ -1394,11 +1687,9 @@ int tcw_get_info(tcw_handle *h, long info[10])
     if (!h->info[0]) return fail(TCW_EINVAL, "no search has been run on this handle");
     CUDA_TRY(cudaSetDevice(h->device));
     CUDA_TRY(cudaStreamSynchronize(h->last_stream));
-    int status = 0;
-    CUDA_TRY(cudaMemcpy(&status, h->d_status, sizeof(int), cudaMemcpyDeviceToHost));
-    h->info[4] = status;
-    std::memcpy(info, h->info, sizeof h->info);
-    return TCW_OK;
+    const int rc = check_status(h);
+    std::memcpy(info, h->info, sizeof h->info);   // filled either way: info[4] holds the status word
+    return rc;
 }
 
 }  // extern "C"

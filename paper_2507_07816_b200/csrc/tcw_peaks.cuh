@@ -1,0 +1,149 @@
+// tcw_peaks.cuh -- microbenchmarks of the limits that bind the track-sum kernels on this GPU (sm_100a).
+//
+// The gather-accumulate kernels are bound by warp-instruction issue, the FP64 pipe and shared-memory
+// gathers, not by HBM; MEASURED_PEAKS.json has no entry for any of those
+// ("the builder must micro-benchmark those").  tcw_measure_peaks times, with
+// CUDA events, kernels that do nothing but
+//   * independent FP64 instructions (DFMA, DMUL, DADD) -- the FP64 pipe's warp-instruction rate,
+//   * independent FP32 FFMA                            -- the schedulers' warp-instruction issue rate,
+//   * independent LDS.32 gathers of the access pattern the staged kernel has (lanes on consecutive
+//     templates read words at a stride below one) -- the shared-memory gather rate,
+//   * the bare lookup chain of the staged kernel (one DFMA, one address LEA, one LDS.32, one FADD,
+//     half a VIMNMX3 per lookup, 16 lookups per straight-line block) -- the speed of light of the
+//     design's instruction mix, in lookups per second.
+// Rates are whole-GPU, per second.  The numbers are only as good as the clocks of the moment; bench.py
+// measures them in the same process as the timed search and prints the SM clock beside them.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tcw {
+
+constexpr int PEAK_THREADS = 256;
+constexpr int PEAK_ILP = 8;
+
+// kind 0: DFMA, 1: DMUL, 2: DADD.  PEAK_ILP independent chains per thread, `iters` rounds.
+template <int KIND>
+__global__ void __launch_bounds__(PEAK_THREADS)
+peak_fp64_kernel(int iters, double seed, double *out)
+{
+    double a[PEAK_ILP];
+#pragma unroll
+    for (int i = 0; i < PEAK_ILP; ++i) a[i] = seed + (double)(threadIdx.x + i);
+    const double m = 1.0 + seed * 1e-9, c = seed * 1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int i = 0; i < PEAK_ILP; ++i) {
+                if (KIND == 0) a[i] = __fma_rn(a[i], m, c);
+                else if (KIND == 1) a[i] = __dmul_rn(a[i], m);
+                else a[i] = __dadd_rn(a[i], c);
+            }
+        }
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < PEAK_ILP; ++i) s += a[i];
+    if (s == 12345.678) out[0] = s;          // never true: keeps the chains alive
+}
+
+// Independent FP32 FFMA chains: one warp instruction per scheduler per cycle is the issue limit.
+__global__ void __launch_bounds__(PEAK_THREADS)
+peak_issue_kernel(int iters, float seed, float *out)
+{
+    float a[PEAK_ILP];
+#pragma unroll
+    for (int i = 0; i < PEAK_ILP; ++i) a[i] = seed + (float)(threadIdx.x + i);
+    const float m = 1.0f + seed * 1e-6f, c = seed * 1e-3f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int i = 0; i < PEAK_ILP; ++i) a[i] = __fmaf_rn(a[i], m, c);
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < PEAK_ILP; ++i) s += a[i];
+    if (s == 12345.678f) out[0] = s;
+}
+
+// LDS.32 gathers with the staged kernel's pattern: lane l, lookup r reads word (l*s + r*32*s) of a
+// 2 KB window, s = 0.93 (a spin-down factor times a Doppler factor); 16 independent loads per round.
+__global__ void __launch_bounds__(PEAK_THREADS)
+peak_lds_kernel(int iters, float *out)
+{
+    __shared__ float win[8 * 640];
+    for (int i = threadIdx.x; i < 8 * 640; i += PEAK_THREADS) win[i] = (float)i * 1e-6f;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t idx[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) idx[r] = (uint32_t)(warp * 640) + (uint32_t)((lane + 32 * r) * 0.93f);
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(win);
+    float acc[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) acc[r] = 0.0f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            float v;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + 4u * idx[r]));
+            acc[r] += v;
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) s += acc[r];
+    if (s == 12345.678f) out[0] = s;
+}
+
+// The bare lookup chain of sum_staged_kernel: per row 16 x { DFMA, address, LDS.32, FADD } plus the
+// minimum of the fraction words; nothing else (no staging, no metadata, no band edges).
+__global__ void __launch_bounds__(128, 3)
+peak_chain_kernel(int rows, double c0, double q0, float *out)
+{
+    __shared__ float win[4 * 640];
+    for (int i = threadIdx.x; i < 4 * 640; i += 128) win[i] = (float)i * 1e-6f;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(win) + (uint32_t)(warp * 640 * 4) - 4u * 0x41380000u;
+    const double dlane = 0.125 * lane;
+    float acc[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) acc[r] = 0.0f;
+    uint32_t mn_all = 0xffffffffu;
+    double c = c0, q = q0;
+    for (int j = 0; j < rows; ++j) {
+        // c drifts a little from row to row like g*D does; q keeps y in [2^20 + 2^19, +600)
+        c = __dadd_rn(c, -1e-9);
+        const double y0 = __fma_rn(dlane, c, q);
+        const double step = __dmul_rn(4.0, c);
+        uint32_t hi[16], lo[16];
+        hi[0] = (uint32_t)__double2hiint(y0);
+        lo[0] = (uint32_t)__double2loint(y0);
+#pragma unroll
+        for (int r = 1; r < 16; ++r) {
+            const double y = __fma_rn(step, (double)r, y0);
+            hi[r] = (uint32_t)__double2hiint(y);
+            lo[r] = (uint32_t)__double2loint(y);
+        }
+        uint32_t m = min(lo[0], min(lo[1], lo[2]));
+#pragma unroll
+        for (int r = 3; r + 1 < 16; r += 2) m = min(m, min(lo[r], lo[r + 1]));
+        mn_all = min(mn_all, min(m, lo[15]));
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            float v;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + (hi[r] << 2)));
+            acc[r] += v;
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) s += acc[r];
+    if (s == 12345.678f || mn_all == 1u) out[0] = s;
+}
+
+}  // namespace tcw

@@ -209,7 +209,7 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = kf & ~15;                      // rounds towards -inf: may reach into the left padding
                 const int e_byte = (kl + 1 + 15) & ~15;
-                if (e_byte - a_byte + 8 * S > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                if (e_byte - a_byte + 8 * S > p.slot_limit || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
                     atomicOr(p.status, 1);  // host-side window bound violated: never expected
                 } else {
                     b_bytes = e_byte - a_byte;

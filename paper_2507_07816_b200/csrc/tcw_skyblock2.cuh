@@ -155,7 +155,7 @@ sum_skyblock2_kernel(const SumParams p, const SkyParams q)
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = kf & ~15;
                 const int e_byte = (kl + 1 + 15) & ~15;
-                if (e_byte - a_byte + DTS2_BYTES > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                if (e_byte - a_byte + DTS2_BYTES > p.slot_limit || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
                     atomicOr(p.status, 1);
                 } else {
                     b_bytes = e_byte - a_byte;

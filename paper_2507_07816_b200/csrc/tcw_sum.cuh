@@ -48,7 +48,7 @@ __device__ __forceinline__ int bin_lo(double f0, double g, double Dp, double T)
 struct SumParams {
     const unsigned char *spec;  // bin 0 of row 0 of the library's copy (PAD_BINS zero bins before it)
     const unsigned char *spec_pad;  // first byte of row 0 of that copy, left padding included (16-byte aligned)
-    int pad16;                  // bytes of the left padding / 16
+    long pad_bytes;             // bytes of the left padding (a multiple of 16)
     long pitch;                 // row pitch in bytes (multiple of 16), padding included
     int n_sft, n_bins, k_min;
     double T;
@@ -62,6 +62,7 @@ struct SumParams {
     void *partial;              // {stat, f0_index} [n_groups][n_tiles]
     int n_tiles, tile;          // tiles per group, templates per tile
     int stages, slot_bytes;     // staged kernel: ring depth per warp (slots of RB rows), bytes per staged row
+    int slot_limit;             // bytes a staged row may take (= slot_bytes; a test hook lowers it to force the status word)
     long n_groups;              // n_sky * n_tau * n_brk
     int chunk_rows, n_chunks;   // staged kernel: SFT rows per chunk, number of chunks (1 = whole span per CTA)
     int chunk0;                 // first chunk of this launch (a search over a spectrogram that is still being
@@ -69,11 +70,16 @@ struct SumParams {
     void *cpart;                // chunked: float32 / int32 [n_chunks][n_groups][n_f0] partial sums
     unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
+    // staged kernel, fast bin index (one fused multiply-add per lookup, see RowMeta below)
+    double fix_add;             // 0.5 + thr + FIX_OFF, thr = thr2 / 2^33 bins
+    double d32;                 // equally spaced f0 axis: 32 * spacing (Hz), else 0
+    uint32_t thr2;              // a row whose smallest fraction word is <= thr2 is decided by the defining chain;
+                                // 0xffffffff = always (fast index switched off)
     // weighted search (tcw_search_weighted; eq. (4)): s = sum w_j * spectrogram[j][k_j]
     const float *wtab;          // [n_sky][n_sft] weights, or NULL (all ones)
     double mean1, var1;         // per-bin noise mean and variance of the spectrogram elements
     float *out_psi;             // critical ratio [n_groups][n_f0]
-    float *cw1, *cw2;           // chunked: per-chunk sums of w and w^2 over the in-band SFTs, laid out like cpart
+    double *cw1, *cw2;          // chunked: per-chunk sums of w and w^2 over the in-band SFTs, laid out like cpart
 };
 
 template <int FMT> struct Acc { typedef int type; };
@@ -221,36 +227,58 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 constexpr int NW = TCW_NW;      // warps per CTA; warp w owns the rows j = j0 + w + NW*n of the CTA's SFT chunk
 constexpr int STAGED_THREADS = 32 * NW;
 constexpr int RB = TCW_RB;      // SFT rows per ring slot (one mbarrier phase, one wait, one refill per RB rows)
-constexpr int META_ROWS = 64;   // per-warp ring of row metadata: two batches of 32 rows
-static_assert(RB == 1 || RB == 2 || RB == 4, "RB must divide the 32-row metadata batch");
+static_assert(RB == 1 || RB == 2 || RB == 4 || RB == 8, "RB must divide the 32-row metadata batch");
 
-// What a warp needs to stage a row and to turn rint(x) into a shared-memory address of it.
-struct __align__(8) RowMeta {
-    double g, Dp;    // spin-down factor and Doppler factor (times T_sft when it is a power of two)
-    uint32_t off16;  // first staged byte of the row's window, in 16-byte units from SumParams::spec
-    int ab;          // low half: that byte relative to bin 0 of the row, in 16-byte units (signed);
-                     // high half: 16-byte units staged (> 0), 0 row with no in-band bin, -1 no further rows
+// ---- fast bin index of the staged kernel ("one FMA per lookup") -----------
+// The defining chain k = rint(RN(RN(f0*g)*D*T)) costs three FP64 instructions per lookup.  The
+// staged kernel evaluates, per lookup, ONE fused multiply-add
+//     y = fma(f0 - f_first, c, Q),   c = RN(g*D*T),   Q = RN(f_first*c) - rint(x_first) + 0.5 + thr + FIX_OFF + 1.5*2^20
+// whose result lies in [2^20, 2^21), where a double's unit in the last place is 2^-32: the high
+// word of y is FIX_HC + FIX_OFF + (k - k_first) -- the shared-memory index of the bin up to a
+// per-row constant -- and the low word is frac(x~ + 0.5 + thr) * 2^32, x~ the fast value of x.
+// |x~ - x| <= 3*x*2^-52 + 2^-32 =: B (error budget in DESIGN.md), thr >= B, so floor(x~ + 0.5 + thr)
+// equals rint(x) unless the low word is <= 2*thr*2^32.  Lanes track the minimum low word of a row;
+// where it is that small (about once in 1e7 lookups) the row's bins are recomputed by the defining
+// chain (bin_lo).  Either way the bin is the oracle's: tests compare both paths bit for bit.
+constexpr int FIX_OFF = 8;                   // keeps the fixed-point offset positive (x~ - k_first >= -0.5 - B)
+constexpr uint32_t FIX_HC = 0x41380000u;     // high word of 1.5 * 2^20
+#define TCW_FIX_BASE 1572864.0               /* 1.5 * 2^20 */
+
+// What a warp needs to stage a row and to turn the fast index into a shared-memory address of it.
+struct __align__(16) RowMeta {
+    double c, Q;      // the fused multiply-add operands above
+    uint32_t U;       // shared-memory byte address of the row's bin with high word 0:  address = U + BPB*HI (mod 2^32)
+    int by16;         // bytes staged (> 0, a multiple of 16), 0 row with no in-band bin, -1 no further rows
+    uint32_t src_lo, src_hi;   // first staged byte of the row's window, relative to SumParams::spec_pad
 };
-// weighted search: the row's weight, and whether every template of the tile is in band in this row
-// (then the weight sums W1, W2 advance by the same amount for the whole tile: one warp-uniform add)
-struct __align__(8) RowMetaW {
-    double g, Dp;
-    uint32_t off16;
-    int ab;
+// weighted search: the row's weight, whether every template of the tile is in band in this row
+// (then the weight sums W1, W2 advance by the same amount for the whole tile: one warp-uniform
+// add), and the constant that turns the fast index into a band-relative bin for the edge rows
+struct __align__(16) RowMetaW {
+    double c, Q;
+    uint32_t U;
+    int by16;
+    uint32_t src_lo, src_hi;
     float w;
     int full;
+    uint32_t ktest;   // bin - k_min = HI + ktest
+    int pad;
 };
 template <bool WGT> struct MetaT { typedef RowMeta type; };
 template <> struct MetaT<true> { typedef RowMetaW type; };
-static_assert(sizeof(RowMeta) == 24 && sizeof(RowMetaW) == 32, "RowMeta layout");
+static_assert(sizeof(RowMeta) == 32 && sizeof(RowMetaW) == 48, "RowMeta layout");
 
-// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*META_ROWS] [slot NW*D*RB*slot_bytes].  The slot
+// rows of the per-warp metadata ring: one batch of 32 rows plus the rows still in flight
+__host__ __device__ inline int staged_meta_rows(int stages) { return 32 + RB * stages; }
+
+// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*meta_rows] [slot NW*D*RB*slot_bytes].  The slot
 // region is reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has
 // completed; the mbarrier words are never reused as data (they are updated through the async proxy,
 // and a generic store to the same bytes is not ordered against that without a proxy fence).
+__host__ __device__ inline size_t staged_bar_bytes(int stages) { return ((size_t)NW * stages * 8 + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t staged_header_bytes(int stages, bool wgt)
 {
-    return ((size_t)NW * stages * 8 + (size_t)NW * META_ROWS * (wgt ? sizeof(RowMetaW) : sizeof(RowMeta)) + 127) & ~(size_t)127;
+    return (staged_bar_bytes(stages) + (size_t)NW * staged_meta_rows(stages) * (wgt ? sizeof(RowMetaW) : sizeof(RowMeta)) + 127) & ~(size_t)127;
 }
 __host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile, bool wgt)
 {
@@ -269,40 +297,46 @@ __device__ __forceinline__ void lds_v2(uint32_t a, uint32_t &x, uint32_t &y)
 {
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x), "=r"(y) : "r"(a));
 }
+__device__ __forceinline__ void lds_v4(uint32_t a, uint32_t &x, uint32_t &y, uint32_t &z, uint32_t &w)
+{
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(a));
+}
+__device__ __forceinline__ void lds_v2f64(uint32_t a, double &x, double &y)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(a));
+}
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a)
 {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ double lds_f64s(uint32_t a)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
-    return v;
-}
 
-template <int FMT, int R, bool TPOW2, bool WGT>
+template <int FMT, int R, bool TPOW2, bool WGT, bool UNI>
 __global__ void __launch_bounds__(STAGED_THREADS, 12 / NW)
 sum_staged_kernel(const SumParams p)
 {
+    constexpr bool PAIR = RB % 2 == 0;             // live slots are consumed two rows at a time
     typedef typename AccW<FMT, WGT>::type V;
-    typedef typename MetaT<WGT>::type RowMeta;     // shadows tcw::RowMeta
-    constexpr int META_BYTES = (int)sizeof(RowMeta);
+    typedef typename MetaT<WGT>::type Meta;
+    constexpr int MB = (int)sizeof(Meta);
     constexpr int F = 32 * R;                      // templates per tile
     constexpr int BPB = FMT == FMT_F32 ? 4 : 1;    // bytes per bin
-    constexpr uint32_t FULL = 0xffffffffu;
+    constexpr int SH = FMT == FMT_F32 ? 2 : 0;
     extern __shared__ __align__(128) unsigned char smem[];
     const int D = p.stages;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int MR = staged_meta_rows(D);
+    // the warp index through a warp reduction: the compiler then knows it is warp-uniform and keeps the
+    // ring pointers derived from it in uniform registers (the copy operands need them there)
+    const int warp = (int)__reduce_or_sync(0xffffffffu, threadIdx.x >> 5), lane = threadIdx.x & 31;
     uint64_t *bars = (uint64_t *)smem + warp * D;
-    RowMeta *meta = (RowMeta *)(smem + (size_t)NW * D * 8) + warp * META_ROWS;
+    Meta *meta = (Meta *)(smem + staged_bar_bytes(D)) + warp * MR;
     unsigned char *slots = smem + staged_header_bytes(D, WGT);
     const uint32_t slot_stride = (uint32_t)(RB * p.slot_bytes);
     const uint32_t slots_s = smem_u32(slots) + (uint32_t)(warp * D) * slot_stride;
     const uint32_t slots_e = slots_s + (uint32_t)D * slot_stride;
     const uint32_t bars_s = smem_u32(bars);
-    const uint32_t meta_s = smem_u32(meta), meta_e = meta_s + META_ROWS * META_BYTES;
+    const uint32_t meta_s = smem_u32(meta), meta_e = meta_s + (uint32_t)(MR * MB);
 
     // block -> (SFT chunk, group, f0 tile).  Chunks are the slowest index: the CTAs in flight work
     // on the same few hundred SFT rows, which therefore stay in L2 while every group reads them.
@@ -337,7 +371,8 @@ sum_staged_kernel(const SumParams p)
     __syncwarp();
 
     V acc[R];
-    double f0r[R];
+    double df[UNI ? 1 : R];      // f0 of the lane's templates minus the tile's first f0 (equally spaced f0: lane*delta instead)
+    const double dlane = __dmul_rn((double)lane, p.d32 * 0.03125);
     // weighted: sums of w and w^2 over the in-band SFTs.  Rows in which the whole tile is in band
     // advance a warp-uniform float64 pair; only rows that straddle a band edge are counted per lane.
     float w1p[WGT ? R : 1], w2p[WGT ? R : 1];
@@ -345,12 +380,11 @@ sum_staged_kernel(const SumParams p)
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         acc[r] = 0;
-        f0r[r] = p.f0[min(i0 + r * 32 + lane, i_last)];
+        if constexpr (!UNI) df[r] = __dsub_rn(p.f0[min(i0 + r * 32 + lane, i_last)], f_first);
         if (WGT) w1p[r] = w2p[r] = 0.0f;
     }
     const int jw = j0 + warp;
     const int n_rows = jw < j1 ? (j1 - jw + NW - 1) / NW : 0;
-    const uint32_t pitch16 = (uint32_t)(p.pitch >> 4);
 
     // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp),
     // and written to the warp's metadata ring; (g, D) of the next batch are loaded ahead of use.
@@ -361,138 +395,230 @@ sum_staged_kernel(const SumParams p)
         if (WGT && wr) wn = __ldg(wr + jw + NW * lane);
     }
 
+    int m_pos = lane;                            // (32*m + lane) mod MR: the row's place in the metadata ring
+    int m_slot = (lane / RB) % D;                // ((32*m + lane) / RB) mod D: the ring slot the row is staged in
+    const int slot_step = (32 / RB) % D;
     auto compute_batch = [&](int m) {
         const int n = 32 * m + lane;
-        RowMeta mt;
-        mt.g = gn;
-        mt.Dp = TPOW2 ? __dmul_rn(dn, p.T) : dn;
-        mt.off16 = 0;
-        mt.ab = -65536;
-        if constexpr (WGT) { mt.w = wn; mt.full = 0; }
+        const double gj = gn, dj = dn;
+        const double Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
+        Meta mt;
+        mt.c = TPOW2 ? __dmul_rn(gj, Dp) : __dmul_rn(__dmul_rn(gj, dj), p.T);
+        mt.Q = 0;
+        mt.U = 0;
+        mt.by16 = -1;
+        mt.src_lo = mt.src_hi = 0;
+        if constexpr (WGT) { mt.w = wn; mt.full = 0; mt.ktest = 0; mt.pad = 0; }
         if (n + 32 < n_rows) {
             gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32));
             if (WGT && wr) wn = __ldg(wr + jw + NW * (n + 32));
         }
         // once the highest template of the tile is below the band for the largest possible Doppler
         // factor, no later SFT can contribute
-        if (n < n_rows && !(f_last * mt.g * p.dmaxT < below)) {
-            const int kf = bin_lo<TPOW2>(f_first, mt.g, mt.Dp, p.T) - p.k_min;
-            const int kl = bin_lo<TPOW2>(f_last, mt.g, mt.Dp, p.T) - p.k_min;
-            mt.ab = 0;
+        if (n < n_rows && !(f_last * gj * p.dmaxT < below)) {
+            const int lo_f = bin_lo<TPOW2>(f_first, gj, Dp, p.T);
+            const int kf = lo_f - p.k_min;
+            const int kl = bin_lo<TPOW2>(f_last, gj, Dp, p.T) - p.k_min;
+            mt.by16 = 0;
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = (BPB * kf) & ~15;                 // rounds towards -inf: may reach into the left padding
                 const int e_byte = (BPB * (kl + 1) + 15) & ~15;
-                if (e_byte - a_byte > p.slot_bytes || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
-                    atomicOr(p.status, 1);  // host-side window bound violated: never expected
+                if (e_byte - a_byte > p.slot_limit || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                    atomicOr(p.status, 1);  // host-side window bound violated: the search reports TCW_EINTERNAL
                 } else {
-                    mt.off16 = (uint32_t)(jw + NW * n) * pitch16 + (uint32_t)(p.pad16 + (a_byte >> 4));
-                    mt.ab = (((e_byte - a_byte) >> 4) << 16) | ((a_byte >> 4) & 0xffff);
-                    if constexpr (WGT) mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
+                    const long src = (long)(jw + NW * n) * p.pitch + p.pad_bytes + a_byte;
+                    mt.src_lo = (uint32_t)src;
+                    mt.src_hi = (uint32_t)(src >> 32);
+                    mt.by16 = e_byte - a_byte;
+                    const uint32_t S = slots_s + (uint32_t)m_slot * slot_stride + (uint32_t)(lane % RB) * (uint32_t)p.slot_bytes;
+                    // byte address of band-relative bin b: S + BPB*b - a_byte; the fast index is HI = FIX_HC + FIX_OFF + (b - kf)
+                    mt.U = S + (uint32_t)(BPB * kf - a_byte) - (uint32_t)BPB * (FIX_HC + (uint32_t)FIX_OFF);
+                    mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add), TCW_FIX_BASE);
+                    if constexpr (WGT) {
+                        mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
+                        mt.ktest = (uint32_t)kf - (FIX_HC + (uint32_t)FIX_OFF);
+                    }
                 }
             }
         }
-        meta[n & (META_ROWS - 1)] = mt;
+        meta[m_pos] = mt;
+        m_pos += 32;
+        if (m_pos >= MR) m_pos -= MR;
+        m_slot += slot_step;
+        if (m_slot >= D) m_slot -= D;
         __syncwarp();
     };
 
     int ni = 0;                                  // next slot (RB rows) to stage
-    uint32_t bar_i = bars_s, slot_i = slots_s, meta_i = meta_s + 16u;
-    // Stage the rows RB*ni .. RB*ni + RB-1.  Every lane reads the rows' metadata and a warp-wide OR
-    // makes the copy operands warp-uniform (uniform registers); one elected lane then issues one TMA
-    // bulk copy per staged row, all counted on the slot's mbarrier.
+    uint32_t bar_i = bars_s, slot_i = slots_s, meta_i = meta_s;
+    // Stage the rows RB*ni .. RB*ni + RB-1: one elected lane reads the rows' copy descriptors and
+    // issues one TMA bulk copy per staged row, all counted on the slot's mbarrier.
     auto stage_next = [&]() {
         if ((ni & (32 / RB - 1)) == 0) compute_batch(ni / (32 / RB));
-        uint32_t off[RB];
-        int by[RB], tot = 0;
-#pragma unroll
-        for (int q = 0; q < RB; ++q) {
-            uint32_t o, ab;
-            lds_v2(meta_i + (uint32_t)(q * META_BYTES), o, ab);
-            off[q] = __reduce_or_sync(FULL, o);
-            by[q] = (int)__reduce_or_sync(FULL, ab) >> 16;
-            tot += max(by[q], 0);
-        }
         if (elect_one()) {
+            uint32_t u[RB], lo[RB], hi[RB];
+            int by[RB], tot = 0;
+#pragma unroll
+            for (int q = 0; q < RB; ++q) {
+                uint32_t b;
+                lds_v4(meta_i + (uint32_t)(q * MB) + 16u, u[q], b, lo[q], hi[q]);
+                by[q] = (int)b;
+                tot += max(by[q], 0);
+            }
             if (tot > 0) {
-                mbar_arrive_expect_tx(bar_i, (uint32_t)tot << 4);
+                mbar_arrive_expect_tx(bar_i, (uint32_t)tot);
 #pragma unroll
                 for (int q = 0; q < RB; ++q)
                     if (by[q] > 0)
-                        bulk_g2s(slot_i + (uint32_t)(q * p.slot_bytes), p.spec_pad + ((size_t)off[q] << 4),
-                                 (uint32_t)by[q] << 4, bar_i);
+                        bulk_g2s(slot_i + (uint32_t)(q * p.slot_bytes), p.spec_pad + (((size_t)hi[q] << 32) | lo[q]),
+                                 (uint32_t)by[q], bar_i);
             } else if (by[0] >= 0) {
                 mbar_arrive(bar_i);   // every use of a slot completes one phase of its barrier
             }
         }
         ++ni;
-        bar_i += 8u; slot_i += slot_stride; meta_i += RB * META_BYTES;
+        bar_i += 8u; slot_i += slot_stride; meta_i += RB * MB;
         if (slot_i == slots_e) { slot_i = slots_s; bar_i = bars_s; }
-        if (meta_i == meta_e + 16u) meta_i = meta_s + 16u;
+        if (meta_i == meta_e) meta_i = meta_s;
     };
 
     for (int q = 0; q < D - 1; ++q) stage_next();
 
+    // ---- consumer pieces (all inlined; the arrays live in registers)
+    // fast indices of the lane's R templates in the row whose metadata sits at mq: hi[r] = FIX_HC + FIX_OFF +
+    // (bin - first bin of the tile); returns the smallest fraction word (see the comment at FIX_OFF)
+    auto fast_row = [&](uint32_t mq, uint32_t (&hi)[R]) -> uint32_t {
+        double c, Q;
+        lds_v2f64(mq, c, Q);
+        uint32_t lo[R];
+        if constexpr (UNI) {
+            // equally spaced f0: template 32*r + lane sits at y0 + r*step, step = 32*delta*c
+            const double y0 = __fma_rn(dlane, c, Q);
+            const double step = __dmul_rn(p.d32, c);
+            hi[0] = (uint32_t)__double2hiint(y0);
+            lo[0] = (uint32_t)__double2loint(y0);
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                const double y = __fma_rn(step, (double)r, y0);
+                hi[r] = (uint32_t)__double2hiint(y);
+                lo[r] = (uint32_t)__double2loint(y);
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double y = __fma_rn(df[r], c, Q);
+                hi[r] = (uint32_t)__double2hiint(y);
+                lo[r] = (uint32_t)__double2loint(y);
+            }
+        }
+        auto min3 = [](uint32_t x, uint32_t y, uint32_t z) { return min(x, min(y, z)); };
+        if constexpr (R == 4) return min(min3(lo[0], lo[1], lo[2]), lo[3]);
+        else if constexpr (R == 8) return min3(min3(lo[0], lo[1], lo[2]), min3(lo[3], lo[4], lo[5]), min(lo[6], lo[7]));
+        else {
+            static_assert(R == 4 || R == 8 || R == 16, "templates per lane");
+            const uint32_t a0 = min3(lo[0], lo[1], lo[2]), a1 = min3(lo[3], lo[4], lo[5]), a2 = min3(lo[6], lo[7], lo[8]);
+            const uint32_t a3 = min3(lo[9], lo[10], lo[11]), a4 = min3(lo[12], lo[13], lo[14]);
+            return min(min3(a0, a1, a2), min3(a3, a4, lo[15]));
+        }
+    };
+    // the same indices by the defining chain (bin_lo): taken where a lookup of this lane lies within thr of a
+    // rounding boundary, or always when the fast index is switched off
+    auto exact_row = [&](int n, uint32_t (&hi)[R]) {
+        const int j = jw + NW * n;
+        const double gj = __ldg(g + j), dj = __ldg(d + j);
+        const double Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
+        const uint32_t base = FIX_HC + (uint32_t)FIX_OFF - (uint32_t)bin_lo<TPOW2>(f_first, gj, Dp, p.T);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            hi[r] = base + (uint32_t)bin_lo<TPOW2>(__ldg(p.f0 + min(i0 + r * 32 + lane, i_last)), gj, Dp, p.T);
+    };
+    // gather the row's elements from its staged window and accumulate
+    auto add_row = [&](uint32_t mq, const uint32_t (&hi)[R]) {
+        const uint32_t U = lds_u32(mq + 16u);
+        if constexpr (WGT) {
+            const float wj = lds_f32(mq + 32u);
+            if (lds_u32(mq + 36u)) {          // warp-uniform: the whole tile is in band
+                const double wd = (double)wj;
+                W1u = __dadd_rn(W1u, wd);
+                W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const uint32_t a = U + (hi[r] << SH);
+                    const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
+                    acc[r] = __fmaf_rn(wj, v, acc[r]);
+                }
+            } else {
+                const float wj2 = __fmul_rn(wj, wj);
+                const uint32_t ktest = lds_u32(mq + 40u);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const uint32_t a = U + (hi[r] << SH);
+                    const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
+                    acc[r] = __fmaf_rn(wj, v, acc[r]);
+                    if (hi[r] + ktest < (uint32_t)p.n_bins) {
+                        w1p[r] = __fadd_rn(w1p[r], wj);
+                        w2p[r] = __fadd_rn(w2p[r], wj2);
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const uint32_t a = U + (hi[r] << SH);
+                if (FMT == FMT_F32) acc[r] += lds_f32(a);
+                else acc[r] += (V)lds_u8(a);
+            }
+        }
+    };
+
     uint32_t ph = 0;      // parity of the phase the slots complete in this pass over the ring
-    uint32_t bar_c = bars_s, slot_c = slots_s - (uint32_t)(BPB * p.k_min), meta_c = meta_s;
-    const uint32_t slots_ce = slots_e - (uint32_t)(BPB * p.k_min);
+    uint32_t bar_c = bars_s, meta_c = meta_s;
+    int sc = 0, nc = 0;   // slot of the ring and slot count of the consumer
     for (;;) {
         stage_next();     // refills the slot consumed in the previous iteration
-        int ab[RB];
-        bool any = false;
+        int by[RB];
+        bool any = false, all = true;
 #pragma unroll
         for (int q = 0; q < RB; ++q) {
-            ab[q] = (int)lds_u32(meta_c + (uint32_t)(q * META_BYTES) + 20u);
-            any |= ab[q] >= 65536;
+            by[q] = (int)lds_u32(meta_c + (uint32_t)(q * MB) + 20u);
+            any |= by[q] > 0;
+            all &= by[q] > 0;
         }
-        if (ab[0] < 0) break;
+        if (by[0] < 0) break;
         if (any) {
             mbar_wait(bar_c, ph);
+            if (PAIR && all) {
+                // the usual case, every row of the slot is live: two rows per straight-line block, so the
+                // index arithmetic of one row overlaps the shared-memory gathers of the other
 #pragma unroll
-            for (int q = 0; q < RB; ++q) {
-                if (ab[q] >= 65536) {
-                    const uint32_t mq = meta_c + (uint32_t)(q * META_BYTES);
-                    const double gj = lds_f64s(mq), Dp = lds_f64s(mq + 8u);
-                    // shared address of bin (0 - k_min) of the staged window
-                    const uint32_t rb = slot_c + (uint32_t)(q * p.slot_bytes) - (uint32_t)((int)((uint32_t)ab[q] << 16) >> 12);
-                    if constexpr (WGT) {
-                        const float wj = lds_f32(mq + 24u);
-                        if (lds_u32(mq + 28u)) {          // warp-uniform: the whole tile is in band
-                            const double wd = (double)wj;
-                            W1u = __dadd_rn(W1u, wd);
-                            W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
+                for (int q = 0; q < RB; q += 2) {
+                    const uint32_t mq0 = meta_c + (uint32_t)(q * MB), mq1 = mq0 + (uint32_t)MB;
+                    uint32_t hi0[R], hi1[R];
+                    const uint32_t mn0 = fast_row(mq0, hi0);
+                    const uint32_t mn1 = fast_row(mq1, hi1);
+                    if (min(mn0, mn1) <= p.thr2) {
+                        exact_row(RB * nc + q, hi0);
+                        exact_row(RB * nc + q + 1, hi1);
+                    }
+                    add_row(mq0, hi0);
+                    add_row(mq1, hi1);
+                }
+            } else {
 #pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
-                                const float v = FMT == FMT_F32 ? lds_f32(rb + 4u * lo) : (float)lds_u8(rb + lo);
-                                acc[r] = __fmaf_rn(wj, v, acc[r]);
-                            }
-                        } else {
-                            const float wj2 = __fmul_rn(wj, wj);
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
-                                const float v = FMT == FMT_F32 ? lds_f32(rb + 4u * lo) : (float)lds_u8(rb + lo);
-                                acc[r] = __fmaf_rn(wj, v, acc[r]);
-                                if (lo - (uint32_t)p.k_min < (uint32_t)p.n_bins) {
-                                    w1p[r] = __fadd_rn(w1p[r], wj);
-                                    w2p[r] = __fadd_rn(w2p[r], wj2);
-                                }
-                            }
-                        }
-                    } else {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const uint32_t lo = (uint32_t)bin_lo<TPOW2>(f0r[r], gj, Dp, p.T);
-                            if (FMT == FMT_F32) acc[r] += lds_f32(rb + 4u * lo);
-                            else acc[r] += (V)lds_u8(rb + lo);
-                        }
+                for (int q = 0; q < RB; ++q) {
+                    if (by[q] > 0) {
+                        const uint32_t mq = meta_c + (uint32_t)(q * MB);
+                        uint32_t hi[R];
+                        if (fast_row(mq, hi) <= p.thr2) exact_row(RB * nc + q, hi);
+                        add_row(mq, hi);
                     }
                 }
             }
         }
         __syncwarp();     // every lane has read the slot before the next iteration refills it
-        bar_c += 8u; slot_c += slot_stride; meta_c += RB * META_BYTES;
-        if (slot_c == slots_ce) { slot_c = slots_s - (uint32_t)(BPB * p.k_min); bar_c = bars_s; ph ^= 1u; }
+        ++nc;
+        bar_c += 8u; meta_c += RB * MB;
+        if (++sc == D) { sc = 0; bar_c = bars_s; ph ^= 1u; }
         if (meta_c == meta_e) meta_c = meta_s;
     }
 
@@ -533,8 +659,8 @@ sum_staged_kernel(const SumParams p)
                     W2 += wu[2 * w + 1] + (double)rw[(NW + w) * F + t];
                 }
                 if (p.n_chunks > 1) {
-                    p.cw1[cbase + i] = (float)W1;
-                    p.cw2[cbase + i] = (float)W2;
+                    p.cw1[cbase + i] = W1;
+                    p.cw2[cbase + i] = W2;
                 } else {
                     s = critical_ratio(s, W1, W2, p.mean1, p.var1);
                     if (p.out_psi) p.out_psi[grp * p.n_f0 + i] = s;
@@ -576,8 +702,8 @@ chunk_reduce_kernel(const SumParams p)
                 double W1 = 0, W2 = 0;
                 for (int c = 0; c < p.n_chunks; ++c)
                     if (live[c]) {
-                        W1 += (double)p.cw1[c * stride + grp * p.n_f0 + i];
-                        W2 += (double)p.cw2[c * stride + grp * p.n_f0 + i];
+                        W1 += p.cw1[c * stride + grp * p.n_f0 + i];
+                        W2 += p.cw2[c * stride + grp * p.n_f0 + i];
                     }
                 s = critical_ratio(s, W1, W2, p.mean1, p.var1);
                 if (p.out_psi) p.out_psi[grp * p.n_f0 + i] = s;

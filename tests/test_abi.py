@@ -41,6 +41,22 @@ def test_header_constants_match_binding():
         assert int(m.group(1)) == getattr(tcw, name), name
 
 
+def _sass_of(function: str) -> str:
+    """SASS of one kernel of the built library (cuobjdump prints every function; split by name)."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump) and not shutil.which("cuobjdump"):
+        pytest.skip("cuobjdump not available")
+    if not hasattr(_sass_of, "text"):
+        _sass_of.text = subprocess.run([cuobjdump, "-sass", tcw.library_path()], capture_output=True, text=True).stdout
+    parts = re.split(r"\n\s*Function : ", _sass_of.text)
+    for part in parts[1:]:
+        if part.split("\n", 1)[0].strip() == function:
+            return part
+    raise AssertionError(f"{function} not found in {tcw.library_path()}")
+
+
 def test_library_is_sm100a_and_has_tma_bulk_copies():
     """The .so carries sm_100a SASS and the staged kernel's TMA bulk copies (UBLKCP)."""
     import shutil
@@ -51,14 +67,26 @@ def test_library_is_sm100a_and_has_tma_bulk_copies():
     elf = subprocess.run([cuobjdump, "-lelf", tcw.library_path()], capture_output=True, text=True).stdout
     assert "sm_100a" in elf
     for wgt in ("0", "1"):               # plain and weighted instantiations
-        sass = subprocess.run([cuobjdump, "-sass", "-fun", f"_ZN3tcw17sum_staged_kernelILi0ELi8ELb1ELb{wgt}EEEvNS_9SumParamsE",
-                               tcw.library_path()], capture_output=True, text=True).stdout
+        sass = _sass_of(f"_ZN3tcw17sum_staged_kernelILi0ELi8ELb1ELb{wgt}ELb0EEEvNS_9SumParamsE")
         assert "UBLKCP" in sass and "SYNCS" in sass
-        # the index chain is never contracted; the weighted kernel's epilogue holds the IEEE division
-        # and square root of eq. (4), whose correctly rounded library sequences are built from DFMA
-        assert ("DFMA" in sass) == (wgt == "1")
+        # the fast index is ONE fused multiply-add per lookup (8 templates per lane x 4 rows per ring slot)
+        # and the defining chain (DMUL, DMUL, DADD) stays in the kernel as the guard band's fallback
+        assert sass.count("DFMA") >= 32
         assert "DMUL" in sass and "DADD" in sass
         assert ("FFMA" in sass) == (wgt == "1")   # only the weighted sum fuses weight * element + acc
+
+
+def test_defining_chain_is_never_contracted():
+    """The kernels that DEFINE the bins for the rest of the library -- the gather kernel and the
+    index export, both straight bin_lo chains -- contain no fused multiply-add: every step of
+    ((f0*g)*D)*T is one IEEE operation (build flag -fmad=false plus __dmul_rn / __dadd_rn)."""
+    for fn in ("_ZN3tcw17sum_gather_kernelILi0ELb1ELb0EEEvNS_9SumParamsE",
+               "_ZN3tcw17sum_gather_kernelILi1ELb0ELb0EEEvNS_9SumParamsE",
+               "_ZN3tcw18track_index_kernelILb1EEEvNS_9SumParamsEPKlliPi",
+               "_ZN3tcw18track_index_kernelILb0EEEvNS_9SumParamsEPKlliPi"):
+        sass = _sass_of(fn)
+        assert "DFMA" not in sass and "FFMA" not in sass, fn
+        assert "DMUL" in sass and "DADD" in sass, fn
 
 
 def _create_args(n_sft=4, n_bins=8):
@@ -165,9 +193,27 @@ def test_grid_marshalling_and_sharding():
     assert (c.n_f0, c.n_tau, c.n_brk, c.n_sky, c.T0) == (2, 1, 3, 2, 12.0)
     assert c.brk[2] == 7.0 and c.sky[4] == 1.0
     assert g.n_groups == 6 and g.n_templates == 12
-    for n_sky, world in [(256, 8), (7, 3), (2, 4), (4096, 5)]:
-        parts = [tcw.shard_groups(n_sky, r, world) for r in range(world)]
-        covered = np.concatenate([np.arange(n_sky)[p] for p in parts])
-        assert np.array_equal(covered, np.arange(n_sky))
-        sizes = [p.stop - p.start for p in parts]
+    for n_groups, world in [(160, 8), (7, 3), (2, 4), (98304, 5), (576, 7)]:
+        parts = [tcw.shard_groups(n_groups, r, world) for r in range(world)]
+        assert parts[0][0] == 0 and parts[-1][1] == n_groups
+        assert all(a[1] == b[0] for a, b in zip(parts, parts[1:]))
+        sizes = [hi - lo for lo, hi in parts]
         assert max(sizes) - min(sizes) <= 1
+
+
+def test_split_groups_tiles_every_range_in_order():
+    """tcw_split_groups (host-only): any contiguous range of the flattened (sky, tau, n) index is
+    tiled, in ascending order and without overlap, by at most seven sub-grids whose own order is a
+    contiguous run of the flattened index."""
+    rng = np.random.default_rng(5)
+    for n_sky, n_tau, n_brk in [(1, 32, 5), (1, 64, 9), (5, 4, 3), (3, 1, 7), (4, 6, 1), (256, 16, 5)]:
+        n_groups = n_sky * n_tau * n_brk
+        flat = np.arange(n_groups).reshape(n_sky, n_tau, n_brk)
+        ranges = [(0, n_groups), (0, 1), (n_groups - 1, n_groups), (3, 3)]
+        ranges += [tuple(sorted(rng.integers(0, n_groups + 1, size=2))) for _ in range(60)]
+        for g0, g1 in ranges:
+            rects = tcw.split_groups(n_tau, n_brk, int(g0), int(g1))
+            assert len(rects) <= 7
+            got = [flat[s, a, b].reshape(-1) for s, a, b in rects]
+            got = np.concatenate(got) if got else np.empty(0, dtype=int)
+            assert np.array_equal(got, np.arange(g0, g1)), (n_sky, n_tau, n_brk, g0, g1)
