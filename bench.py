@@ -1,21 +1,29 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the tCW track-sum hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|cfg1..cfg5] [--impl ours|reference]
 
 One "step" = one pass of the whole hot path (Doppler table, spin-down table, gather-accumulate,
-candidate reduction: SURVEY.md section 8(a) rows a1-a6) over the whole template grid of the
-workload.  The default workload is cfg2 = BASELINE.json:configs[1] (one day of 8-s SFTs,
-500-1000 Hz, float32 normalised power, 4000 f0 x 32 tau x 5 n x 1 sky = 640 000 templates).
+candidate reduction: SURVEY.md section 8(a) rows a1-a6) over the whole template grid of a
+workload.  With no --config (= "all") the headline workload is cfg4 = BASELINE.json:configs[3],
+the largest single-GPU configuration (three days of 8-s SFTs with gaps, 500-3000 Hz, float32
+normalised power, 1.67 GB; 20000 f0 x 64 tau x 9 n x 1 sky = 11.52 M templates), and the same
+measurements for cfg2, cfg3 (uint8 and bit-packed) and cfg5 are carried in `per_config`.
 
 Printed: ONE JSON line.  `value` = nominal template-SFT lookups/s (n_templates * n_sft per
-step, all ranks) with inputs resident in HBM; `e2e` = the same through tcw_create(HOST
+step, all ranks) with inputs resident in HBM; `e2e` = the same through tcw_create_async(HOST
 spectrogram) + tcw_search_host(HOST outputs) + tcw_destroy, copies inside the timed region;
 `roofline` = compulsory bytes B_comp of DESIGN.md section 6 over the gather-accumulate kernel's
-device time; `cpu_baseline` = oracle/ timed on this box's host cores on a bounded sample.
+device time against the measured HBM peak (the model BASELINE.json asks for); `roofline_binding`
+= the bound that actually binds -- warp-instruction issue -- with the kernel's instruction count
+(profiles/ncu_summary.json: ncu captures of the shipped build) over its device time against the
+issue rate tcw_measure_peaks measures in this process; `cpu_baseline` = oracle/ timed on this
+box's host cores on a bounded sample (the oracle is the unoptimised literal definition: a
+reported baseline, not a target).
 
-N > 1 (torchrun): weak scaling.  Rank r searches the same grid at its own sky point, the
-spectrogram is replicated, and there is no data-path collective.
+N > 1 (torchrun): strong scaling.  The flattened (sky, tau, n) group index of the headline grid
+is cut into N contiguous ranges (shard_groups), rank r searches its range with tcw_search_groups,
+the spectrogram is replicated, and there is no data-path collective.
 
 `--impl reference` times the oracle (oracle/, the paper's definition on the host cores); for
 this paper there is no reference code to install.
@@ -40,28 +48,21 @@ if ROOT not in sys.path:
 METRIC = "template-SFT lookups/s"
 UNIT = "lookups/s"
 C_LIGHT = 299792458.0
-
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the gather-accumulate kernel,
-# from the committed `ncu --set full` capture named beside each entry (None = not captured).
-NCU_TRAFFIC_BYTES = {
-    "cfg2": (164000256 + 10949120, "profiles/r1d_cfg2_sum_full.md"),
-    "cfg2:f32": (164000256 + 10949120, "profiles/r1d_cfg2_sum_full.md"),
-    "cfg4": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
-    "cfg4:f32": (13235930000 + 743397120, "profiles/r1d_cfg4_sum_full.md"),
-    "cfg3": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md (same kernel and device data as the uint8 input)"),
-    "cfg3:u8": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md (same kernel and device data as the uint8 input)"),
-    "cfg3:bits": (165622016 + 305288960, "profiles/r1i_cfg3bits_sky2_full.md"),
-    "cfg5": (940257280 + 1564303000, "profiles/r1i_cfg5_sky2_full.md"),
-    "cfg5:bits": (940257280 + 1564303000, "profiles/r1i_cfg5_sky2_full.md"),
-}
+HEADLINE = "cfg4"
+PER_CONFIG = (("cfg2", "f32"), ("cfg3", "u8"), ("cfg3", "bits"), ("cfg5", "bits"))
+L2_BYTES = 126e6
 
 
-# smsp__issue_active.avg.pct_of_peak_sustained_active of the same kernels, from the same captures:
-# the configurations are bound by warp-instruction issue, not by HBM.
-NCU_ISSUE_ACTIVE_PCT = {
-    "cfg2": 72.7, "cfg2:f32": 72.7, "cfg4": 73.1, "cfg4:f32": 73.1,
-    "cfg3": 63.0, "cfg3:u8": 63.0, "cfg3:bits": 63.0, "cfg5": 62.1, "cfg5:bits": 62.1,
-}
+def load_ncu_summary():
+    """profiles/ncu_summary.json: per workload, what `ncu --set full` measured on ONE launch of the
+    gather-accumulate kernel of the shipped build (DRAM traffic, warp instructions, issue-active), the
+    commit it was captured at and the profile file with the full command.  Written by
+    `python -m paper_2507_07816_b200.profiling summary ...`; bench.py only reads it."""
+    path = os.path.join(ROOT, "profiles", "ncu_summary.json")
+    if not os.path.exists(path):
+        return {}
+    with open(path) as f:
+        return json.load(f)
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -176,13 +177,20 @@ def time_oracle(w, budget_s: float, max_groups: int | None = None):
 
 
 def workload_config(w, extra=None):
+    """The keys that name the workload; identical in both arms (ours and --impl reference)."""
     cfg = {"workload": f"{w.name} (BASELINE.json:configs[{int(w.name[3:]) - 1}])", "format": w.fmt,
            "n_sft": int(w.n_sft), "n_bins": int(w.n_bins), "n_f0": len(w.f0), "n_tau": len(w.tau),
            "n_brk": len(w.brk), "n_sky": len(w.sky), "n_templates": int(w.n_templates),
-           "spectrogram_bytes": int(w.spectrogram.nbytes)}
+           "spectrogram_bytes": int(w.spectrogram.nbytes),
+           "l2_policy": ("input larger than L2 (no flush)" if w.spectrogram.nbytes > L2_BYTES else
+                         "input smaller than L2: a 256 MB buffer is written between timed steps (L2 flush)")}
     if extra:
         cfg.update(extra)
     return cfg
+
+
+def headline_name(args) -> tuple[str, str | None]:
+    return (HEADLINE, None) if args.config == "all" else (args.config, args.format)
 
 
 # ----------------------------------------------------------------------------- reference arm
@@ -191,7 +199,8 @@ def run_reference(args):
     if rank != 0:
         return 0
     import tcw_inputs
-    w = tcw_inputs.make_workload(args.config)
+    name, fmt = headline_name(args)
+    w = tcw_inputs.make_workload(name, fmt=fmt)
     per_step = max(1.0, min(20.0, 60.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
         time_oracle(w, per_step, max_groups=1)
@@ -205,8 +214,9 @@ def run_reference(args):
     value = tot_lookups / tot_s
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(w, {"note": "each step is a bounded sample of the workload on the host cores"}),
+            "higher_is_better": True, "scaling": "strong" if args.gpus > 1 else "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(w),
+            "note": "each step is a bounded sample of the workload evaluated by the oracle on the host cores",
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": samples[-1]},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -215,6 +225,232 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------- our arm
+def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=None, weighted=False, one_thread=False):
+    """Everything bench.py reports for ONE workload on this rank's GPU: device-resident throughput,
+    stage times, both rooflines, end to end from host buffers, and the oracle on the host cores."""
+    import torch
+    tcw, tcw_inputs, dist = ctx["tcw"], ctx["tcw_inputs"], ctx["dist"]
+    rank, world, dev = ctx["rank"], ctx["world"], ctx["dev"]
+    opts = opts or {}
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = tcw_inputs.make_workload(name, fmt=fmt)
+    key = f"{w.name}:{w.fmt}"
+    grid = tcw.Grid.of(w)
+    n_sft, n_f0 = w.n_sft, len(w.f0)
+    g_lo, g_hi = tcw.shard_groups(grid.n_groups, rank, world) if world > 1 else (0, grid.n_groups)
+    my_groups = g_hi - g_lo
+    nominal = float(grid.n_templates) * n_sft                       # whole job, all ranks
+    stream = torch.cuda.current_stream()
+
+    h = tcw.Handle.from_workload(w, device=dev)
+    # tcw_create alone (layout copy of a device-resident spectrogram into the padded pitch; untimed in
+    # `value`, reported separately as SURVEY.md section 8(d) asks)
+    spec_dev = torch.from_numpy(np.ascontiguousarray(w.spectrogram).view(np.int32) if w.spectrogram.dtype == np.uint32
+                                else np.ascontiguousarray(w.spectrogram)).to(dev)
+    tcw.Handle(spec_dev, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities).close()   # warm-up: the pool grows once
+    torch.cuda.synchronize()
+    t_c0 = time.perf_counter()
+    for _ in range(3):
+        tcw.Handle(spec_dev, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities).close()
+    torch.cuda.synchronize()
+    create_ms = 1e3 * (time.perf_counter() - t_c0) / 3
+    del spec_dev
+    for k, v in opts.items():
+        h.set_option(k, v)
+    out_stat = torch.empty((max(my_groups, 1), n_f0), dtype=h.stat_dtype, device=dev)
+    out_best = torch.empty((max(my_groups, 1), 2), dtype=torch.int32, device=dev)
+
+    if weighted:
+        # NEXT-1: the weighted statistic + critical ratio (tcw_search_weighted) on the same workload,
+        # device-resident weights; the step then produces Psi, s and the per-group best Psi
+        mean1, var1 = (1.0, 1.0) if w.fmt == "f32" else (math.exp(-1.6), math.exp(-1.6) * (1 - math.exp(-1.6)))
+        wts = torch.from_numpy(tcw_inputs.synthetic_weights(w.sky, w.timestamps, w.seed)).to(dev)
+        shape4 = (len(w.sky), len(w.tau), len(w.brk), n_f0)
+        out_psi = torch.empty(shape4, dtype=torch.float32, device=dev)
+        out_stat = torch.empty(shape4, dtype=torch.float32, device=dev)
+
+    def step():
+        if my_groups == 0:
+            return
+        if weighted:
+            h.search_weighted(grid, wts, mean1, var1, out_psi, out_stat, out_best)
+        elif world > 1:
+            h.search_groups(grid, g_lo, g_hi, out_stat, out_best)
+        else:
+            h.search(grid, out_stat, out_best)
+
+    # L2 policy (timing rules): inputs larger than L2 need no flush; smaller ones get a 256 MB write between steps
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if w.spectrogram.nbytes <= L2_BYTES else None
+    sampler = ClockSampler(ctx["local"])
+    for _ in range(warmup):
+        step()
+    h.set_option(tcw.TCW_OPT_TIMING, 1)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier()
+    if rank == 0:
+        sampler.start()
+    t_host0 = time.perf_counter()
+    for e0, e1 in evs:
+        if flush is not None:
+            flush.fill_(1)
+        e0.record(stream)
+        step()
+        e1.record(stream)
+    barrier()
+    t_host = time.perf_counter() - t_host0
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = float(sum(e0.elapsed_time(e1) for e0, e1 in evs))
+    stage_ms, n_timed = h.timing() if my_groups else ((0.0, 0.0, 0.0, 0.0), 0)
+    h.set_option(tcw.TCW_OPT_TIMING, 0)
+    info = h.info() if my_groups else {}
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / steps
+    value = nominal / (ms_step * 1e-3)
+
+    # in-band lookups: the same search over an all-ones uint8 spectrogram counts them exactly
+    inband = 0.0
+    if rank == 0:
+        ones = torch.ones((n_sft, w.n_bins), dtype=torch.uint8, device=dev)
+        with tcw.Handle(ones, "u8", w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities) as h1:
+            cnt, _ = h1.search(grid, want_best=False)
+            torch.cuda.synchronize()
+            inband = float(cnt.sum(dtype=torch.int64).item())
+        del ones, cnt
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    spec_np = np.ascontiguousarray(w.spectrogram)
+    if spec_np.dtype == np.uint32:
+        spec_np = spec_np.view(np.int32)
+    spec_pin = torch.from_numpy(spec_np).pin_memory()
+    e2e_steps = max(1, min(steps, e2e_steps))
+    if world == 1:
+        stat_pin = torch.empty((len(w.sky), len(w.tau), len(w.brk), n_f0), dtype=h.stat_dtype).pin_memory()
+        best_pin = torch.empty((grid.n_groups, 2), dtype=torch.int32).pin_memory()
+
+        def e2e_step():
+            # tcw_create_async: the pinned spectrogram travels in pieces while the search already runs;
+            # tcw_search_host: outputs of 64 MiB or more come back part by part under the next part's search
+            with tcw.Handle(spec_pin, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, async_upload=True) as hh:
+                for k, v in opts.items():
+                    hh.set_option(k, v)
+                hh.search_host(grid, stat_pin.numpy(), best_pin.numpy())
+        e2e_path = "tcw_create_async(pinned HOST spectrogram) + tcw_search_host(pinned HOST out_stat, out_best) + tcw_destroy"
+    else:
+        stat_pin = torch.empty((max(my_groups, 1), n_f0), dtype=h.stat_dtype).pin_memory()
+        best_pin = torch.empty((max(my_groups, 1), 2), dtype=torch.int32).pin_memory()
+
+        def e2e_step():
+            with tcw.Handle(spec_pin, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, async_upload=True) as hh:
+                if my_groups:
+                    hh.search_groups(grid, g_lo, g_hi, out_stat, out_best)
+                    stat_pin.copy_(out_stat, non_blocking=True)
+                    best_pin.copy_(out_best, non_blocking=True)
+                    hh.check()
+        e2e_path = ("per rank: tcw_create_async(pinned HOST spectrogram) + tcw_search_groups(own group range) + "
+                    "device-to-host copy of its out_stat / out_best slices + tcw_check + tcw_destroy")
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()                      # tcw_search_host / tcw_check synchronise before returning
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = int(world * (spec_np.nbytes + w.timestamps.nbytes + w.velocities.nbytes)
+              + 8 * (len(w.f0) + len(w.tau) + len(w.brk) + 3 * len(w.sky)))
+    d2h = int(4 * grid.n_templates + 8 * grid.n_groups)
+    e2e_value = nominal * e2e_steps / e2e_s
+    h.close()
+    del spec_pin, stat_pin, best_pin, out_stat, out_best, flush
+    torch.cuda.empty_cache()
+    if rank != 0:
+        return None
+
+    peak, peak_src = load_peaks()
+    b_comp = compulsory_bytes(w)
+    sum_ms = stage_ms[1]
+    achieved = b_comp / (sum_ms * 1e-3) / 1e9 if sum_ms > 0 else 0.0
+    ncu = ctx["ncu"].get("captures", {}).get(key)
+    kernel_name = ("sum_skyblock2_kernel" if info.get("kernel") == "skyblock" and info.get("sky_block") == 256
+                   else f"sum_{info.get('kernel')}_kernel")
+    block = {
+        "config": workload_config(w),
+        "value": value, "unit": UNIT, "ms_per_step": ms_step,
+        "templates_per_s": grid.n_templates / (ms_step * 1e-3),
+        "inband_lookups_per_s": inband / (ms_step * 1e-3),
+        "inband_fraction": inband / nominal,
+        "create_ms": create_ms,
+        "launch": {"kernel": info.get("kernel"), "tile_f0": info.get("tile"), "ctas": info.get("ctas"),
+                   "smem_bytes": info.get("smem_bytes"), "sky_block": info.get("sky_block"),
+                   "sft_chunks": info.get("chunks"), "chunk_rows": info.get("chunk_rows"), "ring_stages": info.get("stages"),
+                   "kernels_per_step": info.get("launches"),
+                   **({"statistic": "weighted s + critical ratio Psi (tcw_search_weighted), device-resident weights; "
+                                    "the e2e leg times the unweighted tcw_search_host"} if weighted else {})},
+        "stage_ms": {"tables": stage_ms[0], "sum": stage_ms[1], "best": stage_ms[2], "search": stage_ms[3],
+                     "searches_averaged": n_timed, "host_wall_ms_per_step": 1e3 * t_host / steps},
+        "kernel_ms": sum_ms,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": (ncu["dram_bytes_read"] + ncu["dram_bytes_write"]) if ncu else None,
+                     "traffic_source": ({"profile": ncu["profile"], "commit": ctx["ncu"].get("commit"), "kernel": ncu["kernel"]}
+                                        if ncu else None),
+                     "peak_source": peak_src, "kernel": kernel_name, "algorithmic_bytes_per_launch": b_comp, "kernel_ms": sum_ms,
+                     "bytes_per_inband_lookup": b_comp / inband if inband else None,
+                     "note": "compulsory-bytes model of BASELINE.json: every group is charged its own read of the rows, which "
+                             "L2 and the sky-block sharing serve; fractions above 1 mean the model is not what binds "
+                             "(see roofline_binding)"},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "path": e2e_path},
+        "gpu_launches": (info.get("launches") or 0) * steps,
+        "clocks": clocks,
+    }
+    pk = ctx["peaks"]
+    if ncu and pk and world == 1 and not opts and not weighted:
+        inst = float(ncu["inst_executed"])
+        ach = inst / (sum_ms * 1e-3)
+        block["roofline_binding"] = {
+            "bound": "issue", "achieved": ach, "peak": pk["issue_winst_per_s"], "unit": "warp instructions/s",
+            "frac": ach / pk["issue_winst_per_s"],
+            "inst_per_launch": inst, "inst_per_32_inband_lookups": 32.0 * inst / inband if inband else None,
+            "issue_active_pct_ncu": ncu.get("issue_active_pct"), "fp64_pipe_pct_ncu": ncu.get("fp64_pipe_pct"),
+            "inst_source": {"profile": ncu["profile"], "commit": ctx["ncu"].get("commit"), "kernel": ncu["kernel"],
+                            "kernel_ms_under_ncu": ncu.get("duration_ms")},
+            "peak_source": "tcw_measure_peaks in this process: independent FFMA streams, one warp instruction per scheduler per cycle",
+            "note": "warp instructions of one launch (ncu capture of the shipped build) over the live CUDA-event time of the "
+                    "kernel, against the measured issue rate; the instruction count per lookup is what a faster kernel lowers"}
+        if info.get("kernel") == "staged" and inband:
+            block["roofline_binding"]["lookup_chain"] = {
+                "achieved_inband_lookups_per_s": inband / (sum_ms * 1e-3), "peak_lookups_per_s": pk["chain_lookups_per_s"],
+                "frac": inband / (sum_ms * 1e-3) / pk["chain_lookups_per_s"],
+                "note": "the bare lookup chain of the staged kernel (DFMA, address, LDS.32, FADD, half a VIMNMX3 per lookup) "
+                        "measured alone by tcw_measure_peaks: staging, row metadata and band edges are what separates the two"}
+    if world == 1 and cpu_seconds > 0:
+        cb = time_oracle(w, cpu_seconds)
+        block["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        block["cpu_baseline"]["templates_per_s"] = cb["templates"] / cb["seconds"]
+        block["cpu_baseline"]["note"] = "the oracle as it stands: the literal float64 definition, not an optimised CPU code"
+        if one_thread:
+            # the same oracle on one thread (SURVEY.md section 8(d): all cores and one core), a smaller sample
+            import oracle
+            all_threads = oracle.num_threads()
+            oracle.set_num_threads(1)
+            c1 = time_oracle(w, min(4.0, cpu_seconds))
+            oracle.set_num_threads(all_threads)
+            block["cpu_baseline"]["one_thread"] = {"value": c1["value"], "unit": UNIT, "cores": 1, "sample": c1["sample"]}
+    return block
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -232,200 +468,64 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     tcw.load_library()
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    w = tcw_inputs.make_workload(args.config, fmt=args.format)
-    if world > 1:
-        # weak scaling: the same (f0, tau, n) grid at this rank's own sky points, spectrogram replicated
-        n_sky = len(w.sky)
-        if n_sky == 1:
-            cap = tcw_inputs.fibonacci_cap(world, 1.0, 0.3, 10.0)
-            w = w.subgrid()
-            w.sky = np.ascontiguousarray(cap[rank:rank + 1])
-        # (multi-sky configs keep their own sky list on every rank: per-GPU work is fixed)
-    grid = tcw.Grid.of(w)
-    n_sft, n_templates, n_groups = w.n_sft, grid.n_templates, grid.n_groups
-    nominal = float(n_templates) * n_sft
-    stream = torch.cuda.current_stream()
-
-    h = tcw.Handle.from_workload(w, device=dev)
-    # tcw_create alone (layout copy of a device-resident spectrogram into the padded pitch; untimed in
-    # `value`, reported separately as SURVEY.md section 8(d) asks)
-    spec_dev = torch.from_numpy(np.ascontiguousarray(w.spectrogram).view(np.int32) if w.spectrogram.dtype == np.uint32
-                                else np.ascontiguousarray(w.spectrogram)).to(dev)
-    tcw.Handle(spec_dev, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities).close()   # warm-up: the pool grows once
-    torch.cuda.synchronize()
-    t_c0 = time.perf_counter()
-    for _ in range(3):
-        tcw.Handle(spec_dev, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities).close()
-    torch.cuda.synchronize()
-    create_ms = 1e3 * (time.perf_counter() - t_c0) / 3
-    del spec_dev
-    if args.kernel:
-        h.set_option(tcw.TCW_OPT_KERNEL, tcw.KERNELS[args.kernel])
-    if args.sky_block:
-        h.set_option(tcw.TCW_OPT_SKY_BLOCK, args.sky_block)
-    if args.f0_per_lane:
-        h.set_option(tcw.TCW_OPT_F0_PER_LANE, args.f0_per_lane)
-    if args.chunk_rows:
-        h.set_option(tcw.TCW_OPT_CHUNK_ROWS, args.chunk_rows)
-    if args.stages:
-        h.set_option(tcw.TCW_OPT_STAGES, args.stages)
-    if args.exact_index:
-        h.set_option(tcw.TCW_OPT_EXACT_INDEX, 1)
-    if args.general_f0:
-        h.set_option(tcw.TCW_OPT_GENERAL_F0, 1)
-    out_stat = torch.empty((len(w.sky), len(w.tau), len(w.brk), len(w.f0)), dtype=h.stat_dtype, device=dev)
-    out_best = torch.empty((n_groups, 2), dtype=torch.int32, device=dev)
-
-    weighted = None
-    if args.weighted:
-        # NEXT-1: the weighted statistic + critical ratio (tcw_search_weighted) on the same workload,
-        # device-resident weights; the step then produces Psi, s and the per-group best Psi
-        mean1, var1 = (1.0, 1.0) if w.fmt == "f32" else (math.exp(-1.6), math.exp(-1.6) * (1 - math.exp(-1.6)))
-        wts = torch.from_numpy(tcw_inputs.synthetic_weights(w.sky, w.timestamps, w.seed)).to(dev)
-        out_psi = torch.empty(out_stat.shape, dtype=torch.float32, device=dev)
-        out_stat = torch.empty(out_stat.shape, dtype=torch.float32, device=dev)
-        weighted = dict(mean1=mean1, var1=var1)
-
-    def step():
-        if weighted:
-            h.search_weighted(grid, wts, mean1, var1, out_psi, out_stat, out_best)
-        else:
-            h.search(grid, out_stat, out_best)
-
-    sampler = ClockSampler(local)
-    for _ in range(args.warmup):
-        step()
-    h.set_option(tcw.TCW_OPT_TIMING, 1)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    ctx = dict(tcw=tcw, tcw_inputs=tcw_inputs, dist=dist, rank=rank, world=world, local=local, dev=dev,
+               ncu=load_ncu_summary(), peaks=None)
     if rank == 0:
-        sampler.start()
-    t_host0 = time.perf_counter()
-    ev0.record(stream)
-    for _ in range(args.steps):
-        step()
-    ev1.record(stream)
-    barrier()
-    t_host = time.perf_counter() - t_host0
-    clocks = sampler.stop() if rank == 0 else None
-    ms_total = ev0.elapsed_time(ev1)
-    stage_ms, n_timed = h.timing()
-    h.set_option(tcw.TCW_OPT_TIMING, 0)
-    info = h.info()
-    if info["status"] != 0:
-        raise SystemExit(f"bench.py: device status word {info['status']} (window bound violated)")
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / args.steps
-    value = world * nominal / (ms_step * 1e-3)
+        ctx["peaks"] = tcw.measure_peaks()          # issue / FP64 / LDS rates of this GPU, now
 
-    # in-band lookups: the same search over an all-ones uint8 spectrogram counts them exactly
-    ones = torch.ones((n_sft, w.n_bins), dtype=torch.uint8, device=dev)
-    with tcw.Handle(ones, "u8", w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities) as h1:
-        cnt, _ = h1.search(grid, want_best=False)
-        torch.cuda.synchronize()
-        inband = float(cnt.sum(dtype=torch.int64).item())
-    del ones, cnt
+    opts = {}
+    if args.kernel:
+        opts[tcw.TCW_OPT_KERNEL] = tcw.KERNELS[args.kernel]
+    if args.sky_block:
+        opts[tcw.TCW_OPT_SKY_BLOCK] = args.sky_block
+    if args.f0_per_lane:
+        opts[tcw.TCW_OPT_F0_PER_LANE] = args.f0_per_lane
+    if args.chunk_rows:
+        opts[tcw.TCW_OPT_CHUNK_ROWS] = args.chunk_rows
+    if args.stages:
+        opts[tcw.TCW_OPT_STAGES] = args.stages
+    if args.exact_index:
+        opts[tcw.TCW_OPT_EXACT_INDEX] = 1
+    if args.general_f0:
+        opts[tcw.TCW_OPT_GENERAL_F0] = 1
 
-    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
-    spec_np = np.ascontiguousarray(w.spectrogram)
-    if spec_np.dtype == np.uint32:
-        spec_np = spec_np.view(np.int32)
-    spec_pin = torch.from_numpy(spec_np).pin_memory()
-    stat_pin = torch.empty(out_stat.shape, dtype=h.stat_dtype).pin_memory()
-    best_pin = torch.empty((n_groups, 2), dtype=torch.int32).pin_memory()
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
-
-    def e2e_step():
-        # tcw_create_async: the pinned spectrogram travels in pieces while the search already runs
-        with tcw.Handle(spec_pin, w.fmt, w.n_bins, w.f_min, w.T_sft, w.timestamps, w.velocities, async_upload=True) as hh:
-            hh.search_host(grid, stat_pin.numpy(), best_pin.numpy())
-
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()                      # tcw_search_host synchronises the stream before returning
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    h2d = int(spec_np.nbytes + w.timestamps.nbytes + w.velocities.nbytes
-              + 8 * (len(w.f0) + len(w.tau) + len(w.brk) + 3 * len(w.sky)))
-    d2h = int(4 * n_templates + 8 * n_groups)
-    e2e_value = world * nominal * e2e_steps / e2e_s
-    h.close()
-
+    name, fmt = headline_name(args)
+    cpu_s = 0.0 if args.no_cpu_baseline else args.cpu_seconds
+    head = measure_config(ctx, name, fmt, args.steps, args.warmup, args.e2e_steps, cpu_s, opts, args.weighted, one_thread=True)
+    per = {}
+    if args.config == "all" and world == 1:
+        for cname, cfmt in PER_CONFIG:
+            # fewer steps for the side configurations keep the whole run inside a few minutes
+            blk = measure_config(ctx, cname, cfmt, min(args.steps, 20), max(3, min(args.warmup, 5)), min(args.e2e_steps, 5),
+                                 0.0 if args.no_cpu_baseline else min(3.0, args.cpu_seconds))
+            per[f"{cname}:{cfmt}"] = blk
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
-
-    peak, peak_src = load_peaks()
-    b_comp = compulsory_bytes(w)
-    sum_ms = stage_ms[1]
-    achieved = b_comp / (sum_ms * 1e-3) / 1e9
-    traffic = NCU_TRAFFIC_BYTES.get(args.config if args.format is None else f"{args.config}:{args.format}")
+    w_fmt = head["config"]["format"]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "strong" if world > 1 else "weak",
+        "vs_baseline": None,
         "dtype": {"f32": "f64 index + f32 accumulate", "u8": "f64 index + i32 accumulate",
-                  "bits": "f64 index + i32 accumulate"}[w.fmt],
+                  "bits": "f64 index + i32 accumulate"}[w_fmt],
         "data": "synthetic",
-        "config": workload_config(w, {
-            "parallelism": f"dp{world} (templates sharded by sky point, spectrogram replicated, no collective)",
-            "l2_policy": "inputs larger than L2 (no flush)" if w.spectrogram.nbytes > 126e6 else
-                         "input smaller than L2 (stays L2-resident between steps; no flush)",
-            "kernel": info["kernel"], "tile_f0": info["tile"], "ctas": info["ctas"], "smem_bytes": info["smem_bytes"],
-            "sky_block": info["sky_block"], "sft_chunks": info["chunks"], "chunk_rows": info["chunk_rows"],
-            "ring_stages": info["stages"],
-            **({"statistic": "weighted s + critical ratio Psi (tcw_search_weighted), device-resident weights; "
-                             "the e2e leg below times the unweighted tcw_search_host"} if weighted else {})}),
-        "templates_per_s": world * n_templates / (ms_step * 1e-3),
-        "inband_lookups_per_s": world * inband / (ms_step * 1e-3),
-        "inband_fraction": inband / nominal,
-        "create_ms": create_ms,
-        "stage_ms": {"tables": stage_ms[0], "sum": stage_ms[1], "best": stage_ms[2], "search": stage_ms[3],
-                     "searches_averaged": n_timed, "host_wall_ms_per_step": 1e3 * t_host / args.steps},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic[0] if traffic else None,
-                     "traffic_source": traffic[1] if traffic else None, "peak_source": peak_src,
-                     "kernel": ("sum_skyblock2_kernel" if info["kernel"] == "skyblock" and info["sky_block"] == 256
-                                else f"sum_{info['kernel']}_kernel"), "algorithmic_bytes_per_launch": b_comp,
-                     "kernel_ms": sum_ms,
-                     "issue_active_pct_ncu": NCU_ISSUE_ACTIVE_PCT.get(args.config if args.format is None
-                                                                      else f"{args.config}:{args.format}"),
-                     "binding_bound": ("warp-instruction issue / FP64 (rows are served from L2: DESIGN.md section 6); "
-                                       "the HBM model is the roofline BASELINE.json asks for"),
-                     "bytes_per_inband_lookup": b_comp / inband if inband else None},
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
-                "path": "tcw_create_async(pinned HOST spectrogram) + tcw_search_host(pinned HOST out_stat, out_best) + tcw_destroy"},
-        "gpu_launches": info["launches"] * args.steps,
-        "clocks": clocks,
+        "config": head["config"],
+        "parallelism": (f"dp{world}: contiguous ranges of the flattened (sky, tau, n) group index per rank "
+                        "(tcw_search_groups), spectrogram replicated, no collective" if world > 1 else "1 GPU"),
+        **{k: head[k] for k in ("templates_per_s", "inband_lookups_per_s", "inband_fraction", "create_ms", "launch",
+                                "stage_ms", "roofline", "e2e", "gpu_launches", "clocks") if k in head},
     }
-    if world == 1 and not args.no_cpu_baseline:
-        cb = time_oracle(w, args.cpu_seconds)
-        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
-        line["cpu_baseline"]["templates_per_s"] = cb["templates"] / cb["seconds"]
-        # the same oracle on one thread (all cores and one core), a smaller sample
-        import oracle
-        all_threads = oracle.num_threads()
-        oracle.set_num_threads(1)
-        c1 = time_oracle(w, min(4.0, args.cpu_seconds))
-        oracle.set_num_threads(all_threads)
-        line["cpu_baseline"]["one_thread"] = {"value": c1["value"], "unit": UNIT, "cores": 1, "sample": c1["sample"]}
+    for k in ("roofline_binding", "cpu_baseline"):
+        if k in head:
+            line[k] = head[k]
+    if ctx["peaks"]:
+        line["measured_peaks"] = ctx["peaks"]
+    if per:
+        line["per_config"] = per
+        line["gpu_launches"] += sum(b["gpu_launches"] for b in per.values())
+        line["gpu_launches_note"] = "kernels of the timed regions of the headline and of every per_config entry"
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -562,10 +662,11 @@ def run_prep(args):
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--config", default="all", choices=["all", "cfg1", "cfg2", "cfg3", "cfg4", "cfg5"],
+                    help="all (default): cfg4 as the headline plus per_config blocks for cfg2, cfg3 (u8, bits) and cfg5")
     ap.add_argument("--format", default=None, choices=["f32", "u8", "bits"])
     ap.add_argument("--kernel", default=None, choices=["auto", "gather", "staged", "skyblock"])
     ap.add_argument("--sky-block", type=int, default=0, choices=[0, 64, 128, 256])
@@ -574,8 +675,8 @@ def main():
     ap.add_argument("--stages", type=int, default=0, help="staged kernel: ring depth limit (0 auto)")
     ap.add_argument("--exact-index", action="store_true", help="staged kernel: defining chain for every bin (no fast index)")
     ap.add_argument("--general-f0", action="store_true", help="staged kernel: do not use the equally-spaced-f0 instantiation")
-    ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--e2e-steps", type=int, default=8)
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--bank", type=int, default=0, help="time tcw_search_bank on this many random templates (NEXT-2)")
     ap.add_argument("--select", type=int, default=0, help="time tcw_topk / tcw_select_above over this many float32 values (NEXT-4)")
@@ -585,6 +686,8 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                  # timing rule: at least 3 warm-up steps
+    if (args.bank or args.select or args.prep) and args.config == "all":
+        args.config = "cfg2"
     if args.prep and args.impl == "ours":
         return run_prep(args)
     if args.select and args.impl == "ours":

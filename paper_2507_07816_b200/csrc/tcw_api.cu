@@ -382,10 +382,10 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
         }
         if (h->opt_exact || thr_units > 1048576.0) {
             p.thr2 = 0xffffffffu;
-            p.fix_add = 0.5 + (double)tcw::FIX_OFF;
+            p.fix_add = 0.5;
         } else {
             p.thr2 = (uint32_t)(2.0 * thr_units);
-            p.fix_add = 0.5 + thr_units * 0x1p-32 + (double)tcw::FIX_OFF;
+            p.fix_add = 0.5 + thr_units * 0x1p-32;
         }
     }
     return p;

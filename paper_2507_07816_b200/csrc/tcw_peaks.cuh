@@ -70,28 +70,39 @@ peak_issue_kernel(int iters, float seed, float *out)
 }
 
 // LDS.32 gathers with the staged kernel's pattern: lane l, lookup r reads word (l*s + r*32*s) of a
-// 2 KB window, s = 0.93 (a spin-down factor times a Doppler factor); 16 independent loads per round.
+// 2 KB window, s = 0.93 (a spin-down factor times a Doppler factor); 16 independent loads per block,
+// four blocks per round at different immediate offsets (so that no two loads of a round coincide and
+// none can be merged), each load followed by the FADD that consumes it.
+template <int OFF>
+__device__ __forceinline__ float peak_lds_off(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    return v;
+}
 __global__ void __launch_bounds__(PEAK_THREADS)
 peak_lds_kernel(int iters, float *out)
 {
-    __shared__ float win[8 * 640];
-    for (int i = threadIdx.x; i < 8 * 640; i += PEAK_THREADS) win[i] = (float)i * 1e-6f;
+    __shared__ float win[8 * 640 + 64];
+    for (int i = threadIdx.x; i < 8 * 640 + 64; i += PEAK_THREADS) win[i] = (float)i * 1e-6f;
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t idx[16];
-#pragma unroll
-    for (int r = 0; r < 16; ++r) idx[r] = (uint32_t)(warp * 640) + (uint32_t)((lane + 32 * r) * 0.93f);
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(win);
+    uint32_t a[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) a[r] = base + 4u * ((uint32_t)(warp * 640) + (uint32_t)((lane + 32 * r) * 0.93f));
     float acc[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) acc[r] = 0.0f;
-    for (int it = 0; it < iters; ++it) {
+    for (int it = 0; it < iters; it += 4) {
 #pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            float v;
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + 4u * idx[r]));
-            acc[r] += v;
-        }
+        for (int r = 0; r < 16; ++r) acc[r] += peak_lds_off<0>(a[r]);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) acc[r] += peak_lds_off<64>(a[r]);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) acc[r] += peak_lds_off<128>(a[r]);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) acc[r] += peak_lds_off<192>(a[r]);
     }
     float s = 0;
 #pragma unroll

@@ -71,7 +71,7 @@ struct SumParams {
     unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
     // staged kernel, fast bin index (one fused multiply-add per lookup, see RowMeta below)
-    double fix_add;             // 0.5 + thr + FIX_OFF, thr = thr2 / 2^33 bins
+    double fix_add;             // 0.5 + thr, thr = thr2 / 2^33 bins
     double d32;                 // equally spaced f0 axis: 32 * spacing (Hz), else 0
     uint32_t thr2;              // a row whose smallest fraction word is <= thr2 is decided by the defining chain;
                                 // 0xffffffff = always (fast index switched off)
@@ -232,22 +232,23 @@ static_assert(RB == 1 || RB == 2 || RB == 4 || RB == 8, "RB must divide the 32-r
 // ---- fast bin index of the staged kernel ("one FMA per lookup") -----------
 // The defining chain k = rint(RN(RN(f0*g)*D*T)) costs three FP64 instructions per lookup.  The
 // staged kernel evaluates, per lookup, ONE fused multiply-add
-//     y = fma(f0 - f_first, c, Q),   c = RN(g*D*T),   Q = RN(f_first*c) - rint(x_first) + 0.5 + thr + FIX_OFF + 1.5*2^20
+//     y = fma(f0 - f_first, c, Q),   c = RN(g*D*T),   Q = RN(f_first*c) - rint(x_first) + 0.5 + thr + W + 1.5*2^20
 // whose result lies in [2^20, 2^21), where a double's unit in the last place is 2^-32: the high
-// word of y is FIX_HC + FIX_OFF + (k - k_first) -- the shared-memory index of the bin up to a
-// per-row constant -- and the low word is frac(x~ + 0.5 + thr) * 2^32, x~ the fast value of x.
+// word of y is FIX_HC + W + (k - k_first) -- with W the place of the tile's first bin in shared memory
+// (an integer), the index of the selected element itself -- and the low word is
+// frac(x~ + 0.5 + thr) * 2^32, x~ the fast value of x.
 // |x~ - x| <= 3*x*2^-52 + 2^-32 =: B (error budget in DESIGN.md), thr >= B, so floor(x~ + 0.5 + thr)
 // equals rint(x) unless the low word is <= 2*thr*2^32.  Lanes track the minimum low word of a row;
 // where it is that small (about once in 1e7 lookups) the row's bins are recomputed by the defining
 // chain (bin_lo).  Either way the bin is the oracle's: tests compare both paths bit for bit.
-constexpr int FIX_OFF = 8;                   // keeps the fixed-point offset positive (x~ - k_first >= -0.5 - B)
 constexpr uint32_t FIX_HC = 0x41380000u;     // high word of 1.5 * 2^20
 #define TCW_FIX_BASE 1572864.0               /* 1.5 * 2^20 */
 
 // What a warp needs to stage a row and to turn the fast index into a shared-memory address of it.
 struct __align__(16) RowMeta {
-    double c, Q;      // the fused multiply-add operands above
-    uint32_t U;       // shared-memory byte address of the row's bin with high word 0:  address = U + BPB*HI (mod 2^32)
+    double c, Q;      // the fused multiply-add operands above; Q also carries the row's place in shared memory:
+                      // byte address of the selected element = BPB * (high word of y - FIX_HC)
+    uint32_t flags;   // first row of a ring slot: bit q = row q of the slot is staged, bit 8 = no further rows
     int by16;         // bytes staged (> 0, a multiple of 16), 0 row with no in-band bin, -1 no further rows
     uint32_t src_lo, src_hi;   // first staged byte of the row's window, relative to SumParams::spec_pad
 };
@@ -256,7 +257,7 @@ struct __align__(16) RowMeta {
 // add), and the constant that turns the fast index into a band-relative bin for the edge rows
 struct __align__(16) RowMetaW {
     double c, Q;
-    uint32_t U;
+    uint32_t flags;
     int by16;
     uint32_t src_lo, src_hi;
     float w;
@@ -316,7 +317,8 @@ template <int FMT, int R, bool TPOW2, bool WGT, bool UNI>
 __global__ void __launch_bounds__(STAGED_THREADS, 12 / NW)
 sum_staged_kernel(const SumParams p)
 {
-    constexpr bool PAIR = RB % 2 == 0;             // live slots are consumed two rows at a time
+    constexpr bool PAIR = RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
+                                                   // per-lane weight sums leave no registers for that)
     typedef typename AccW<FMT, WGT>::type V;
     typedef typename MetaT<WGT>::type Meta;
     constexpr int MB = (int)sizeof(Meta);
@@ -405,7 +407,7 @@ sum_staged_kernel(const SumParams p)
         Meta mt;
         mt.c = TPOW2 ? __dmul_rn(gj, Dp) : __dmul_rn(__dmul_rn(gj, dj), p.T);
         mt.Q = 0;
-        mt.U = 0;
+        mt.flags = 0;
         mt.by16 = -1;
         mt.src_lo = mt.src_hi = 0;
         if constexpr (WGT) { mt.w = wn; mt.full = 0; mt.ktest = 0; mt.pad = 0; }
@@ -431,16 +433,20 @@ sum_staged_kernel(const SumParams p)
                     mt.src_hi = (uint32_t)(src >> 32);
                     mt.by16 = e_byte - a_byte;
                     const uint32_t S = slots_s + (uint32_t)m_slot * slot_stride + (uint32_t)(lane % RB) * (uint32_t)p.slot_bytes;
-                    // byte address of band-relative bin b: S + BPB*b - a_byte; the fast index is HI = FIX_HC + FIX_OFF + (b - kf)
-                    mt.U = S + (uint32_t)(BPB * kf - a_byte) - (uint32_t)BPB * (FIX_HC + (uint32_t)FIX_OFF);
-                    mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add), TCW_FIX_BASE);
+                    // byte address of band-relative bin b: S + BPB*b - a_byte (S and a_byte are multiples of 16), so the
+                    // tile's first bin kf sits at element W = (S - a_byte)/BPB + kf of shared memory (W < 2^16)
+                    const int W = (((int)S - a_byte) >> SH) + kf;     // exact: (S - a_byte) is a multiple of 16, kf - a_byte/BPB >= 0
+                    mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add + (double)W), TCW_FIX_BASE);
                     if constexpr (WGT) {
                         mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
-                        mt.ktest = (uint32_t)kf - (FIX_HC + (uint32_t)FIX_OFF);
+                        mt.ktest = (uint32_t)(kf - W) - FIX_HC;
                     }
                 }
             }
         }
+        // the first row of every ring slot carries the slot's summary for the consumer
+        const unsigned live = __ballot_sync(0xffffffffu, mt.by16 > 0);
+        mt.flags = ((live >> (lane & ~(RB - 1))) & ((1u << RB) - 1u)) | (mt.by16 < 0 ? 256u : 0u);
         meta[m_pos] = mt;
         m_pos += 32;
         if (m_pos >= MR) m_pos -= MR;
@@ -485,8 +491,8 @@ sum_staged_kernel(const SumParams p)
     for (int q = 0; q < D - 1; ++q) stage_next();
 
     // ---- consumer pieces (all inlined; the arrays live in registers)
-    // fast indices of the lane's R templates in the row whose metadata sits at mq: hi[r] = FIX_HC + FIX_OFF +
-    // (bin - first bin of the tile); returns the smallest fraction word (see the comment at FIX_OFF)
+    // fast indices of the lane's R templates in the row whose metadata sits at mq: hi[r] = FIX_HC + the element's
+    // place in shared memory; returns the smallest fraction word (see the comment at FIX_HC)
     auto fast_row = [&](uint32_t mq, uint32_t (&hi)[R]) -> uint32_t {
         double c, Q;
         lds_v2f64(mq, c, Q);
@@ -522,19 +528,23 @@ sum_staged_kernel(const SumParams p)
         }
     };
     // the same indices by the defining chain (bin_lo): taken where a lookup of this lane lies within thr of a
-    // rounding boundary, or always when the fast index is switched off
-    auto exact_row = [&](int n, uint32_t (&hi)[R]) {
+    // rounding boundary, or always when the fast index is switched off.  S = shared address of the row's slot.
+    auto exact_row = [&](int n, uint32_t S, uint32_t (&hi)[R]) {
         const int j = jw + NW * n;
         const double gj = __ldg(g + j), dj = __ldg(d + j);
         const double Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
-        const uint32_t base = FIX_HC + (uint32_t)FIX_OFF - (uint32_t)bin_lo<TPOW2>(f_first, gj, Dp, p.T);
+        const int lo_f = bin_lo<TPOW2>(f_first, gj, Dp, p.T);
+        const int kf = lo_f - p.k_min;
+        const int a_byte = (BPB * kf) & ~15;
+        const uint32_t base = FIX_HC + (uint32_t)((((int)S - a_byte) >> SH) + kf) - (uint32_t)lo_f;
 #pragma unroll
         for (int r = 0; r < R; ++r)
             hi[r] = base + (uint32_t)bin_lo<TPOW2>(__ldg(p.f0 + min(i0 + r * 32 + lane, i_last)), gj, Dp, p.T);
     };
-    // gather the row's elements from its staged window and accumulate
+    // gather the row's elements from its staged window and accumulate: the element with index word hi sits at
+    // shared byte address BPB*(hi - FIX_HC)
+    const uint32_t addr0 = 0u - ((uint32_t)BPB * FIX_HC);
     auto add_row = [&](uint32_t mq, const uint32_t (&hi)[R]) {
-        const uint32_t U = lds_u32(mq + 16u);
         if constexpr (WGT) {
             const float wj = lds_f32(mq + 32u);
             if (lds_u32(mq + 36u)) {          // warp-uniform: the whole tile is in band
@@ -543,7 +553,7 @@ sum_staged_kernel(const SumParams p)
                 W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const uint32_t a = U + (hi[r] << SH);
+                    const uint32_t a = addr0 + (hi[r] << SH);
                     const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
                     acc[r] = __fmaf_rn(wj, v, acc[r]);
                 }
@@ -552,7 +562,7 @@ sum_staged_kernel(const SumParams p)
                 const uint32_t ktest = lds_u32(mq + 40u);
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const uint32_t a = U + (hi[r] << SH);
+                    const uint32_t a = addr0 + (hi[r] << SH);
                     const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
                     acc[r] = __fmaf_rn(wj, v, acc[r]);
                     if (hi[r] + ktest < (uint32_t)p.n_bins) {
@@ -564,7 +574,7 @@ sum_staged_kernel(const SumParams p)
         } else {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                const uint32_t a = U + (hi[r] << SH);
+                const uint32_t a = addr0 + (hi[r] << SH);
                 if (FMT == FMT_F32) acc[r] += lds_f32(a);
                 else acc[r] += (V)lds_u8(a);
             }
@@ -572,53 +582,83 @@ sum_staged_kernel(const SumParams p)
     };
 
     uint32_t ph = 0;      // parity of the phase the slots complete in this pass over the ring
-    uint32_t bar_c = bars_s, meta_c = meta_s;
+    uint32_t bar_c = bars_s, meta_c = meta_s, slot_c = slots_s;
     int sc = 0, nc = 0;   // slot of the ring and slot count of the consumer
     for (;;) {
         stage_next();     // refills the slot consumed in the previous iteration
-        int by[RB];
-        bool any = false, all = true;
-#pragma unroll
-        for (int q = 0; q < RB; ++q) {
-            by[q] = (int)lds_u32(meta_c + (uint32_t)(q * MB) + 20u);
-            any |= by[q] > 0;
-            all &= by[q] > 0;
-        }
-        if (by[0] < 0) break;
-        if (any) {
+        const uint32_t flags = lds_u32(meta_c + 16u);     // bit q: row q of the slot is staged; bit 8: no further rows
+        if (flags & 256u) break;
+        if (flags) {
             mbar_wait(bar_c, ph);
-            if (PAIR && all) {
+            if (PAIR && flags == (1u << RB) - 1u) {
                 // the usual case, every row of the slot is live: two rows per straight-line block, so the
-                // index arithmetic of one row overlaps the shared-memory gathers of the other
+                // index arithmetic of one row overlaps the shared-memory gathers of the other.  The guard-band
+                // branch repeats the gathers instead of merging, which keeps the fast path free of register moves.
 #pragma unroll
                 for (int q = 0; q < RB; q += 2) {
                     const uint32_t mq0 = meta_c + (uint32_t)(q * MB), mq1 = mq0 + (uint32_t)MB;
                     uint32_t hi0[R], hi1[R];
                     const uint32_t mn0 = fast_row(mq0, hi0);
                     const uint32_t mn1 = fast_row(mq1, hi1);
-                    if (min(mn0, mn1) <= p.thr2) {
-                        exact_row(RB * nc + q, hi0);
-                        exact_row(RB * nc + q + 1, hi1);
+                    if constexpr (WGT || !UNI) {
+                        if (min(mn0, mn1) <= p.thr2) {
+                            uint32_t ex0[R], ex1[R];
+                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex0);
+                            exact_row(RB * nc + q + 1, slot_c + (uint32_t)((q + 1) * p.slot_bytes), ex1);
+                            add_row(mq0, ex0);
+                            add_row(mq1, ex1);
+                        } else {
+                            add_row(mq0, hi0);
+                            add_row(mq1, hi1);
+                        }
+                    } else {
+                        // the two rows' elements are gathered with the fast indices and summed BEFORE the guard
+                        // band is consulted (a fast index is at most one bin off, still inside the slot), so the
+                        // gathers do not wait for the minimum; only the accumulate does.  Fixed order:
+                        // acc += (row q + row q+1).
+                        V t[R];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const uint32_t a0 = addr0 + (hi0[r] << SH), a1 = addr0 + (hi1[r] << SH);
+                            if (FMT == FMT_F32) t[r] = lds_f32(a0) + lds_f32(a1);
+                            else t[r] = (V)(lds_u8(a0) + lds_u8(a1));
+                        }
+                        if (min(mn0, mn1) <= p.thr2) {
+                            uint32_t ex0[R], ex1[R];
+                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex0);
+                            exact_row(RB * nc + q + 1, slot_c + (uint32_t)((q + 1) * p.slot_bytes), ex1);
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const uint32_t a0 = addr0 + (ex0[r] << SH), a1 = addr0 + (ex1[r] << SH);
+                                if (FMT == FMT_F32) t[r] = lds_f32(a0) + lds_f32(a1);
+                                else t[r] = (V)(lds_u8(a0) + lds_u8(a1));
+                            }
+                        }
+#pragma unroll
+                        for (int r = 0; r < R; ++r) acc[r] += t[r];
                     }
-                    add_row(mq0, hi0);
-                    add_row(mq1, hi1);
                 }
             } else {
 #pragma unroll
                 for (int q = 0; q < RB; ++q) {
-                    if (by[q] > 0) {
+                    if (flags & (1u << q)) {
                         const uint32_t mq = meta_c + (uint32_t)(q * MB);
                         uint32_t hi[R];
-                        if (fast_row(mq, hi) <= p.thr2) exact_row(RB * nc + q, hi);
-                        add_row(mq, hi);
+                        if (fast_row(mq, hi) <= p.thr2) {
+                            uint32_t ex[R];
+                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex);
+                            add_row(mq, ex);
+                        } else {
+                            add_row(mq, hi);
+                        }
                     }
                 }
             }
         }
         __syncwarp();     // every lane has read the slot before the next iteration refills it
         ++nc;
-        bar_c += 8u; meta_c += RB * MB;
-        if (++sc == D) { sc = 0; bar_c = bars_s; ph ^= 1u; }
+        bar_c += 8u; meta_c += RB * MB; slot_c += slot_stride;
+        if (++sc == D) { sc = 0; bar_c = bars_s; slot_c = slots_s; ph ^= 1u; }
         if (meta_c == meta_e) meta_c = meta_s;
     }
 
