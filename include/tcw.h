@@ -172,10 +172,12 @@ int tcw_check(tcw_handle *h);
 
 /* tcw_search_host -- the same search with HOST output buffers (either may be NULL, not both):
  * runs tcw_search into library scratch, copies the results to the host and synchronises the
- * stream before returning.  An out_stat of 64 MiB or more is produced tau range by tau range and each
- * range is copied on a second stream while the next is searched (pinned host buffers are needed for
- * that overlap); the values are those of the one-piece search, bit for bit.  Returns TCW_EINTERNAL
- * if a kernel set the device status word (see above). */
+ * stream before returning.  For an out_stat of 64 MiB or more the search issues its CTAs tau range by
+ * tau range, every CTA counts itself done in a per-range device counter, and a second stream waits for
+ * each counter (cuStreamWaitValue32) and copies that range while the later ranges are still being
+ * searched (pinned host buffers are needed for the overlap).  It is one search, not several: the
+ * values are those of tcw_search, bit for bit.  Returns TCW_EINTERNAL if a kernel set the device
+ * status word (see above). */
 int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, void *out_best_host,
                     void *stream);
 
@@ -390,15 +392,16 @@ int tcw_set_option(tcw_handle *h, int key, long value);
  * waits for the last of them. */
 int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
 
-/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged, 4 bank,
- * 3 sky-block),
+/* tcw_get_info -- facts about the last tcw_search: info[0] kernel used (1 gather, 2 staged, 3 sky-block,
+ * 4 bank),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
  * info[5] kernels launched by the call, info[6] ring depth per warp (slots of two SFT rows in the staged kernel), info[7] sky points per
  * block (sky-block kernel, else 0), info[8] SFT chunks of the staged kernel (1 = not chunked),
- * info[9] SFT rows per chunk.
+ * info[9] SFT rows per chunk, info[10] tau ranges of the progressive read-back of the last search (tcw_search_host
+ * with a large out_stat; 0 = none), info[11] reserved (0).
  * Synchronises the search's stream. */
-int tcw_get_info(tcw_handle *h, long info[10]);
+int tcw_get_info(tcw_handle *h, long info[12]);
 
 #ifdef __cplusplus
 }

@@ -432,13 +432,13 @@ class Handle:
     def info(self, check: bool = True) -> dict:
         """tcw_get_info.  Raises TcwError(TCW_EINTERNAL) if the device status word is set, unless
         check=False (the dict's "status" then carries the word)."""
-        v = (ctypes.c_long * 10)()
+        v = (ctypes.c_long * 12)()
         rc = load_library().tcw_get_info(self._h, v)
         if rc != TCW_OK and (check or rc != TCW_EINTERNAL):
             _check(rc)
         return dict(kernel={1: "gather", 2: "staged", 3: "skyblock", 4: "bank"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
                     smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]),
-                    sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]))
+                    sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]), readback_parts=int(v[10]))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -7,6 +7,7 @@
 // tcw_tables.cuh and tcw_sum.cuh; there is no CPU fallback.
 #include "../../include/tcw.h"
 
+#include <cuda.h>           // driver API types only (cuStreamWaitValue32 is fetched at run time; no link dependency)
 #include <cuda_runtime.h>
 #include <cufft.h>
 
@@ -110,6 +111,46 @@ void dev_free(void *p, cudaStream_t st)
     else cudaFree(p);
 }
 
+// Progress counters of the progressive read-back (tcw_search_host): stream memory operations
+// (cuStreamWaitValue32) need a plain cudaMalloc allocation, not pool memory, and cudaMalloc / cudaFree per
+// handle would cost more than the read-back saves.  One block of PROGRESS_SLOTS x 16 counters per device,
+// allocated on first use and kept; handles borrow a slot.
+constexpr int PROGRESS_SLOTS = 256;
+struct ProgressPool {
+    std::mutex mu;
+    unsigned int *base[64] = {nullptr};
+    std::vector<int> free_slots[64];
+};
+ProgressPool &progress_pool()
+{
+    static ProgressPool pool;
+    return pool;
+}
+unsigned int *progress_acquire(int dev)
+{
+    if (dev < 0 || dev >= 64) return nullptr;
+    ProgressPool &pp = progress_pool();
+    std::lock_guard<std::mutex> lock(pp.mu);
+    if (!pp.base[dev]) {
+        if (cudaMalloc((void **)&pp.base[dev], (size_t)PROGRESS_SLOTS * 16 * sizeof(unsigned int)) != cudaSuccess) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        for (int i = PROGRESS_SLOTS - 1; i >= 0; --i) pp.free_slots[dev].push_back(i);
+    }
+    if (pp.free_slots[dev].empty()) return nullptr;
+    const int slot = pp.free_slots[dev].back();
+    pp.free_slots[dev].pop_back();
+    return pp.base[dev] + 16 * slot;
+}
+void progress_release(int dev, unsigned int *p)
+{
+    if (!p || dev < 0 || dev >= 64) return;
+    ProgressPool &pp = progress_pool();
+    std::lock_guard<std::mutex> lock(pp.mu);
+    pp.free_slots[dev].push_back((int)((p - pp.base[dev]) / 16));
+}
+
 // grow-only device buffer; allocates on the stream of the API call in progress
 template <typename T> struct DevBuf {
     T *p = nullptr;
@@ -187,8 +228,15 @@ struct tcw_handle {
     // options
     int opt_kernel = 0, opt_timing = 0, opt_r = 0, opt_stages = 0, opt_sky = 0, opt_exact = 0;
     long opt_chunk = 0;  // SFT rows per chunk of the staged kernel: 0 auto, -1 never chunk
-    cudaStream_t dl_stream = nullptr;        // tcw_search_host: read-back stream and one event per part
-    std::vector<cudaEvent_t> dl_ev;
+    cudaStream_t dl_stream = nullptr;        // tcw_search_host: read-back stream
+    cudaEvent_t dl_ready = nullptr;          // recorded once the progress counters of a search have been cleared
+    unsigned int *d_progress = nullptr;      // per-part completion counters of a progressive search (a borrowed slot
+                                             // of the library's cudaMalloc block: see progress_acquire)
+    int want_parts = 0;                      // set by tcw_search_host: cut the (tau, n) axis into this many parts
+    bool progress_active = false;            // the last search_impl ran with progress counters
+    int progress_np = 0;                     // ... over this many parts
+    unsigned int progress_target[16] = {0};  // CTAs per part
+    int progress_a0[17] = {0};               // tau index where each part starts
     int opt_nonuniform = 0;   // 1: never take the equally-spaced-f0 instantiation of the staged kernel
     bool keep_status = false; // a multi-part search (tcw_search_groups, tcw_search_host) clears the status word once
     int dbg_slot_shrink = 0;  // test hook: bytes taken off the kernels' own window bound
@@ -201,7 +249,7 @@ struct tcw_handle {
     long up_rows = 0;            // rows per piece
     bool up_pending = false;     // the first search still has to wait for the pieces
     void *up_staging = nullptr;  // tightly packed device copy the pieces land in before the re-lay
-    long info[10] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 0};
+    long info[12] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 0, 0, 0};
     // last tables
     int tab_tau = 0, tab_brk = 0, tab_sky = 0;
     // device axis pointers of the last prepared grid
@@ -710,7 +758,7 @@ int tcw_destroy(tcw_handle *h)
     cudaStreamSynchronize(h->last_stream);
     if (h->dl_stream) {
         cudaStreamSynchronize(h->dl_stream);
-        for (auto &e : h->dl_ev) cudaEventDestroy(e);
+        if (h->dl_ready) cudaEventDestroy(h->dl_ready);
         cudaStreamDestroy(h->dl_stream);
     }
     if (h->up_stream) {
@@ -737,6 +785,7 @@ int tcw_destroy(tcw_handle *h)
     h->d_selws.release();
     dev_free(h->d_counter, h->last_stream);
     h->d_cw.release();
+    progress_release(h->device, h->d_progress);
     h->d_sel.release();
     h->d_dts.release();
     h->d_dmm.release();
@@ -935,6 +984,26 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
             h->slot_host[t] = key[std::min(t, (size_t)grid->n_sky - 1)].second;
     }
     if (n_ctas > 2147483647L) return fail(TCW_EUNSUPPORTED, "grid needs more than 2^31-1 CTAs; split the search");
+    // progressive read-back (tcw_search_host): parts of the tau axis, CTAs issued part by part, one counter per part
+    h->progress_active = false;
+    if (h->want_parts > 1 && h->dl_ready && p.n_chunks == 1 && !wgt && !h->d_progress) h->d_progress = progress_acquire(h->device);
+    if (h->want_parts > 1 && h->dl_ready && p.n_chunks == 1 && !wgt && h->d_progress) {
+        const int np = std::min({h->want_parts, grid->n_tau, 16});
+        const long units = kernel == 3 ? n_blocks : grid->n_sky;
+        p.n_parts = np;
+        h->progress_np = np;
+        for (int r = 0; r <= np; ++r) {
+            h->progress_a0[r] = (int)((long)grid->n_tau * r / np);
+            p.part_ab0[r] = h->progress_a0[r] * grid->n_brk;
+        }
+        for (int r = 0; r < np; ++r)
+            h->progress_target[r] = (unsigned int)(units * (p.part_ab0[r + 1] - p.part_ab0[r]) * p.n_tiles);
+        CUDA_TRY(cudaSetDevice(h->device));
+        CUDA_TRY(cudaMemsetAsync(h->d_progress, 0, 16 * sizeof(unsigned int), st));
+        CUDA_TRY(cudaEventRecord(h->dl_ready, st));
+        p.progress = h->d_progress;
+        h->progress_active = true;
+    }
 
     CUDA_TRY(cudaSetDevice(h->device));
     if ((rc = h->d_partial.reserve((size_t)n_partial * 8)) != TCW_OK) return rc;
@@ -1061,6 +1130,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     h->info[5] = (kernel == 3 ? 5 : 4) + (p.n_chunks > 1 ? 1 : 0) + extra_launches;  // doppler table, spin-down table, (sky-block table,) sum, (chunk reduce,) best
     h->info[8] = p.n_chunks;
     h->info[9] = p.chunk_rows;
+    h->info[10] = h->progress_active ? h->progress_np : 0;
     return TCW_OK;
 }
 
@@ -1517,47 +1587,56 @@ int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, vo
         CUDA_TRY(cudaStreamSynchronize(st));
         return check_status(h);
     }
-    // Large outputs: the tau axis is cut into parts; part p is searched into its own contiguous piece of
-    // the scratch and copied to the host (one strided copy: a part is n_sky rows of the full layout) on a
-    // second stream while part p + 1 is searched.  Same kernels, same per-template arithmetic: results
-    // are bit-identical to the one-piece search.
+    // Large outputs: ONE search whose CTAs are issued tau range by tau range and count themselves done per
+    // range (SumParams::progress); the read-back stream waits for each counter (cuStreamWaitValue32) and
+    // copies that range -- n_sky rows of the [sky][tau][brk][f0] layout, one strided copy -- while the later
+    // ranges are still being searched.  No launch is split, so no wave is left half empty.
+    typedef CUresult (*wait_value_fn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+    static wait_value_fn wait_value = [] {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            fn = nullptr;
+        cudaGetLastError();
+        return (wait_value_fn)fn;
+    }();
     if (!h->dl_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->dl_stream, cudaStreamNonBlocking));
-    while ((int)h->dl_ev.size() < n_parts) {
-        cudaEvent_t e;
-        CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-        h->dl_ev.push_back(e);
-    }
-    CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
-    h->keep_status = true;
-    const size_t row_t = (size_t)grid->n_brk * grid->n_f0 * 4, row_b = (size_t)grid->n_brk * 8;   // bytes per (sky, tau)
-    size_t off_t = 0, off_b = 0;
-    long info_sum[2] = {0, 0};
-    for (int p = 0; p < n_parts && rc == TCW_OK; ++p) {
-        const int a0 = (int)((long)grid->n_tau * p / n_parts), a1 = (int)((long)grid->n_tau * (p + 1) / n_parts);
-        const tcw_grid sub = sub_grid(grid, {0, grid->n_sky, a0, a1, 0, grid->n_brk});
-        unsigned char *dst_t = h->d_stat.p + off_t, *dst_b = h->d_best.p + off_b;
-        rc = search_impl(h, &sub, nullptr, dst_t, nullptr, dst_b, stream);
-        if (rc != TCW_OK) break;
-        info_sum[0] += h->info[2]; info_sum[1] += h->info[5];
-        cudaError_t e = cudaEventRecord(h->dl_ev[(size_t)p], st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(h->dl_stream, h->dl_ev[(size_t)p], 0);
-        const size_t w_t = (size_t)(a1 - a0) * row_t, w_b = (size_t)(a1 - a0) * row_b;
-        if (e == cudaSuccess)
-            e = cudaMemcpy2DAsync((char *)out_stat_host + (size_t)a0 * row_t, (size_t)grid->n_tau * row_t, dst_t, w_t, w_t,
-                                  (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
-        if (e == cudaSuccess && out_best_host)
-            e = cudaMemcpy2DAsync((char *)out_best_host + (size_t)a0 * row_b, (size_t)grid->n_tau * row_b, dst_b, w_b, w_b,
-                                  (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
-        if (e != cudaSuccess) rc = fail(TCW_ECUDA, "read-back of part %d: %s", p, cudaGetErrorString(e));
-        off_t += w_t * grid->n_sky;
-        off_b += w_b * grid->n_sky;
-    }
-    h->keep_status = false;
-    cudaStreamSynchronize(h->dl_stream);
-    CUDA_TRY(cudaStreamSynchronize(st));
+    if (!h->dl_ready) CUDA_TRY(cudaEventCreateWithFlags(&h->dl_ready, cudaEventDisableTiming));
+    h->want_parts = wait_value ? n_parts : 0;
+    rc = tcw_search(h, grid, h->d_stat.p, h->d_best.p, stream);
+    h->want_parts = 0;
     if (rc != TCW_OK) return rc;
-    h->info[2] = info_sum[0];
-    h->info[5] = info_sum[1];
+    const size_t row_t = (size_t)grid->n_brk * grid->n_f0 * 4;   // bytes per (sky, tau)
+    const size_t pitch_t = (size_t)grid->n_tau * row_t;
+    if (h->progress_active) {
+        cudaError_t e = cudaStreamWaitEvent(h->dl_stream, h->dl_ready, 0);     // the counters have been cleared
+        for (int p = 0; p < h->progress_np && e == cudaSuccess; ++p) {
+            const int a0 = h->progress_a0[p], a1 = h->progress_a0[p + 1];     // np <= n_tau: never empty
+            const CUresult wr = wait_value((CUstream)h->dl_stream, (CUdeviceptr)(h->d_progress + p), h->progress_target[p],
+                                           CU_STREAM_WAIT_VALUE_GEQ);
+            if (wr != CUDA_SUCCESS) {
+                rc = fail(TCW_ECUDA, "cuStreamWaitValue32 failed for part %d (CUresult %d)", p, (int)wr);
+                break;
+            }
+            e = cudaMemcpy2DAsync((char *)out_stat_host + (size_t)a0 * row_t, pitch_t, h->d_stat.p + (size_t)a0 * row_t, pitch_t,
+                                  (size_t)(a1 - a0) * row_t, (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
+        }
+        if (e != cudaSuccess && rc == TCW_OK) rc = fail(TCW_ECUDA, "progressive read-back: %s", cudaGetErrorString(e));
+        if (rc != TCW_OK) {
+            // the waits may never be satisfied if something went wrong: let the search finish, then release them
+            cudaStreamSynchronize(st);
+            cudaMemsetAsync(h->d_progress, 0xff, 16 * sizeof(unsigned int), st);
+            cudaStreamSynchronize(st);
+            cudaStreamSynchronize(h->dl_stream);
+            return rc;
+        }
+    } else {
+        CUDA_TRY(cudaMemcpyAsync(out_stat_host, h->d_stat.p, n_templates * 4, cudaMemcpyDeviceToHost, st));
+    }
+    if (out_best_host)
+        CUDA_TRY(cudaMemcpyAsync(out_best_host, h->d_best.p, n_groups * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaStreamSynchronize(h->dl_stream));
     return check_status(h);
 }
 
@@ -1681,7 +1760,7 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches)
     return check_status(h);   // the last timed search has completed: times of an invalid search are an error
 }
 
-int tcw_get_info(tcw_handle *h, long info[10])
+int tcw_get_info(tcw_handle *h, long info[12])
 {
     if (!h || !info) return fail(TCW_EINVAL, "NULL argument");
     if (!h->info[0]) return fail(TCW_EINVAL, "no search has been run on this handle");

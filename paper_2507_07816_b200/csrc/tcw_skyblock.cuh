@@ -155,9 +155,9 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
     const uint32_t items_s = smem_u32(smem + sky_items_off(D)) + (uint32_t)(warp * 32 * 16);
 
     // heavy tiles (high f0 stays in band longest) are launched first
-    const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);
-    const int ab = (int)((blockIdx.x / p.n_tiles) % p.n_ab);
-    const int blk = (int)(blockIdx.x / ((long)p.n_tiles * p.n_ab));
+    int blk, ab, tile_raw, part;
+    block_map(p, blockIdx.x, q.n_blocks, blk, ab, tile_raw, part);
+    const int tile = p.n_tiles - 1 - tile_raw;
     const int i0 = tile * F;
     const int i_last = min(i0 + F, p.n_f0) - 1;
 
@@ -357,6 +357,7 @@ sum_skyblock_kernel(const SumParams p, const SkyParams q)
         }
         if (lane == 0) ((Best<int> *)p.partial)[grp * p.n_tiles + tile] = {best_v, best_i == INT32_MAX ? 0 : best_i};
     }
+    block_done(p, part);
 }
 
 }  // namespace tcw

@@ -103,9 +103,9 @@ sum_skyblock2_kernel(const SumParams p, const SkyParams q)
     const uint32_t corr_s = smem_u32(corr), sub_s = smem_u32(sub);
     const uint32_t f0_s = smem_u32(f0t);
 
-    const int tile = p.n_tiles - 1 - (int)(blockIdx.x % p.n_tiles);   // heavy tiles (high f0) first
-    const int ab = (int)((blockIdx.x / p.n_tiles) % p.n_ab);
-    const int blk = (int)(blockIdx.x / ((long)p.n_tiles * p.n_ab));
+    int blk, ab, tile_raw, part;
+    block_map(p, blockIdx.x, q.n_blocks, blk, ab, tile_raw, part);
+    const int tile = p.n_tiles - 1 - tile_raw;                        // heavy tiles (high f0) first
     const int i0 = tile * F2;
     const int i_last = min(i0 + F2, p.n_f0) - 1;
 
@@ -331,5 +331,6 @@ sum_skyblock2_kernel(const SumParams p, const SkyParams q)
         }
         if (lane == 0) ((Best<int> *)p.partial)[grp * p.n_tiles + tile] = {best_v, best_i == INT32_MAX ? 0 : best_i};
     }
+    block_done(p, part);
 }
 }  // namespace tcw

@@ -75,6 +75,13 @@ struct SumParams {
     double d32;                 // equally spaced f0 axis: 32 * spacing (Hz), else 0
     uint32_t thr2;              // a row whose smallest fraction word is <= thr2 is decided by the defining chain;
                                 // 0xffffffff = always (fast index switched off)
+    // progressive read-back (tcw_search_host with a large out_stat): the (tau, n) axis is cut into n_parts ranges
+    // [part_ab0[r], part_ab0[r+1]); CTAs are issued range by range, and each CTA adds one to progress[r] once its
+    // outputs are written, so a copy stream can wait for a range (cuStreamWaitValue32) and fetch it while later
+    // ranges are still being searched.  progress == NULL: plain block order, no counters.
+    unsigned int *progress;
+    int n_parts;
+    int part_ab0[17];
     // weighted search (tcw_search_weighted; eq. (4)): s = sum w_j * spectrogram[j][k_j]
     const float *wtab;          // [n_sky][n_sft] weights, or NULL (all ones)
     double mean1, var1;         // per-bin noise mean and variance of the spectrogram elements
@@ -128,6 +135,41 @@ __device__ __forceinline__ void block_best(V v, int i, Best<V> *red, Best<V> *ds
     }
 }
 
+// Block index -> (unit, (tau, n) index, raw tile index) where unit is a sky point or a sky block.
+// Plain order: unit slowest, tile fastest.  With progress counters: range of the (tau, n) axis slowest.
+__device__ __forceinline__ void block_map(const SumParams &p, long bq, int n_units, int &unit, int &ab, int &tile_raw, int &part)
+{
+    part = 0;
+    if (p.progress) {
+        for (;;) {
+            const long cnt = (long)n_units * (p.part_ab0[part + 1] - p.part_ab0[part]) * p.n_tiles;
+            if (bq < cnt || part == p.n_parts - 1) break;
+            bq -= cnt;
+            ++part;
+        }
+        const int nab = p.part_ab0[part + 1] - p.part_ab0[part];
+        tile_raw = (int)(bq % p.n_tiles);
+        bq /= p.n_tiles;
+        ab = p.part_ab0[part] + (int)(bq % nab);
+        unit = (int)(bq / nab);
+    } else {
+        tile_raw = (int)(bq % p.n_tiles);
+        bq /= p.n_tiles;
+        ab = (int)(bq % p.n_ab);
+        unit = (int)(bq / p.n_ab);
+    }
+}
+// Called by every thread of a CTA after its last output store: publishes the CTA's outputs and counts it.
+__device__ __forceinline__ void block_done(const SumParams &p, int part)
+{
+    if (!p.progress) return;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        atomicAdd(p.progress + part, 1u);
+    }
+}
+
 // --------------------------------------------------------------------------- gather kernel
 template <int FMT, bool TPOW2, bool WGT>
 __global__ void __launch_bounds__(128)
@@ -135,8 +177,9 @@ sum_gather_kernel(const SumParams p)
 {
     typedef typename AccW<FMT, WGT>::type V;
     __shared__ Best<V> red[4];
-    const int tile = blockIdx.x % p.n_tiles;
-    const long grp = blockIdx.x / p.n_tiles;
+    int sky_i, ab_i, tile, part;
+    block_map(p, blockIdx.x, (int)(p.n_groups / p.n_ab), sky_i, ab_i, tile, part);
+    const long grp = (long)sky_i * p.n_ab + ab_i;
     const int i = tile * p.tile + threadIdx.x;
     const bool valid = i < p.n_f0;
     const double f0 = p.f0[valid ? i : p.n_f0 - 1];
@@ -168,6 +211,7 @@ sum_gather_kernel(const SumParams p)
     } else if (valid && p.out_stat) ((V *)p.out_stat)[grp * p.n_f0 + i] = acc;
     block_best<V>(valid ? acc : lowest<V>(), valid ? i : INT32_MAX, red,
                   (Best<V> *)p.partial + grp * p.n_tiles + tile);
+    block_done(p, part);
 }
 
 // --------------------------------------------------------------------------- PTX wrappers
@@ -343,11 +387,12 @@ sum_staged_kernel(const SumParams p)
     // block -> (SFT chunk, group, f0 tile).  Chunks are the slowest index: the CTAs in flight work
     // on the same few hundred SFT rows, which therefore stay in L2 while every group reads them.
     // Within a group heavy tiles (high f0 stays in band longest) are launched first.
-    long bq = blockIdx.x;
-    const int tile = p.n_tiles - 1 - (int)(bq % p.n_tiles);
-    bq /= p.n_tiles;
-    const long grp = bq % p.n_groups;
-    const int chunk = p.chunk0 + (int)(bq / p.n_groups);
+    const long per_chunk = p.n_groups * p.n_tiles;
+    const int chunk = p.chunk0 + (int)(blockIdx.x / per_chunk);
+    int sky_i, ab_i, tile_raw, part;
+    block_map(p, blockIdx.x % per_chunk, (int)(p.n_groups / p.n_ab), sky_i, ab_i, tile_raw, part);
+    const int tile = p.n_tiles - 1 - tile_raw;
+    const long grp = (long)sky_i * p.n_ab + ab_i;
     const int i0 = tile * F;
     const int i_last = min(i0 + F, p.n_f0) - 1;
     const int j0 = p.j_begin + chunk * p.chunk_rows;
@@ -712,6 +757,7 @@ sum_staged_kernel(const SumParams p)
     if (p.n_chunks > 1) return;   // chunk_reduce_kernel adds the chunks and finds the tile's best
     __syncthreads();
     block_best<V>(best_v, best_i, (Best<V> *)slots, (Best<V> *)p.partial + grp * p.n_tiles + tile);
+    block_done(p, part);
 }
 
 // Chunked searches: out_stat[i] = sum over the live SFT chunks, in ascending chunk order, of the
