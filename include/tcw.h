@@ -348,7 +348,10 @@ int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
  *  out[5] lookups/s of the bare lookup chain of sum_staged_kernel (DFMA, address, LDS.32, FADD, half a
  *         VIMNMX3 per lookup; no staging, metadata or band edges): the speed of light of the instruction mix
  *  out[6] number of SMs   out[7] nominal maximum SM clock in Hz
- * n_out must be >= 8.  Synchronous; takes about 0.1 s. */
+ *  out[8] lookups/s of the count formats' chain with one byte per bin (the device layout: LDS.U8 + IADD)
+ *  out[9] the same chain gathering from bit-packed windows (LDS.U8 of byte k >> 3, shift by k & 7, mask):
+ *         the measurement behind keeping one byte per bin on the device
+ * n_out must be >= 10.  Synchronous; takes about 0.15 s. */
 int tcw_measure_peaks(double *out, int n_out, void *stream);
 
 /* Options.  tcw_set_option returns TCW_EINVAL for an unknown key or value. */

@@ -1393,7 +1393,9 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     if (format != TCW_F32_POWER && std::isnan(prep->threshold)) return fail(TCW_EINVAL, "threshold is NaN");
     if (out_pitch_bytes < (long)row_bytes(format, prep->n_bins) || (format != TCW_U8_COUNT && (out_pitch_bytes & 3)))
         return fail(TCW_EINVAL, "out_pitch_bytes is smaller than one row or not a multiple of 4");
-    const size_t smem = (((size_t)(prep->n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)prep->n_bins + 31) & ~(size_t)31);
+    int spc = tcw::PREP_SPC;                        // SFTs per CTA: two CTAs per SM when possible
+    while (spc > 1 && spc * tcw::prep_sft_smem(prep->n_bins, h) > SMEM_MAX / 2 - 1024) spc /= 2;
+    const size_t smem = spc * tcw::prep_sft_smem(prep->n_bins, h);
     if (smem > SMEM_MAX) return fail(TCW_EUNSUPPORTED, "band too wide for one CTA's shared memory (%zu bytes)", smem);
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -1446,7 +1448,13 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
             PREP_TRY(cudaMemsetAsync(d_x + (size_t)nb * N, 0, (size_t)(batch - nb) * N * sizeof(float), st));
         if (!on_device)
             PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyHostToDevice, st));
-        tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(on_device ? strain + j0 * N : d_x, d_win, nb, N, d_x);
+        {
+            const float *src = on_device ? strain + j0 * N : d_x;
+            if ((N & 3) == 0 && ((uintptr_t)src & 15) == 0)
+                tcw::prep_window4_kernel<<<dim3((unsigned)((N / 4 + 255) / 256), (unsigned)std::min(nb, 64)), 256, 0, st>>>(src, d_win, nb, N, d_x);
+            else
+                tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(src, d_win, nb, N, d_x);
+        }
         PREP_TRY(cudaGetLastError());
         if (cufftExecR2C(plan, d_x, (cufftComplex *)d_spec) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftExecR2C failed"); goto done; }
         tcw::PrepParams p;
@@ -1459,7 +1467,7 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         p.out_format = format;
         p.out = (unsigned char *)out_spectrogram + j0 * out_pitch_bytes;
         p.out_pitch = out_pitch_bytes;
-        tcw::prep_normalise_kernel<<<nb, tcw::PREP_THREADS, smem, st>>>(p);
+        tcw::prep_normalise_kernel<<<(nb + spc - 1) / spc, tcw::PREP_THREADS, smem, st>>>(p, nb, spc);
         PREP_TRY(cudaGetLastError());
     }
     PREP_TRY(cudaStreamSynchronize(st));
@@ -1642,7 +1650,7 @@ int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, vo
 
 int tcw_measure_peaks(double *out, int n_out, void *stream)
 {
-    if (!out || n_out < 8) return fail(TCW_EINVAL, "out must hold 8 doubles");
+    if (!out || n_out < 10) return fail(TCW_EINVAL, "out must hold 10 doubles");
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, n_sm = 0;
     CUDA_TRY(cudaGetDevice(&dev));
@@ -1681,6 +1689,12 @@ int tcw_measure_peaks(double *out, int n_out, void *stream)
         // y = dlane*c + r*4c + q stays inside [1.5*2^20 + 8, 1.5*2^20 + 640)
         timed([&] { tcw::peak_chain_kernel<<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, d_out); },
               (double)c_ctas * 128.0 * rows * 16.0, &out[5]);
+    }
+    {
+        const int rows = 8192, c_ctas = n_sm * 3 * 4;
+        const double work = (double)c_ctas * 128.0 * rows * 16.0;
+        timed([&] { tcw::peak_count_chain_kernel<false><<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, (int *)d_out); }, work, &out[8]);
+        timed([&] { tcw::peak_count_chain_kernel<true><<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, (int *)d_out); }, work, &out[9]);
     }
     out[6] = (double)n_sm;
     int khz = 0;

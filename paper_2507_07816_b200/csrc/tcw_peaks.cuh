@@ -157,4 +157,59 @@ peak_chain_kernel(int rows, double c0, double q0, float *out)
     if (s == 12345.678f || mn_all == 1u) out[0] = s;
 }
 
+// The count formats' lookup chain with one byte per bin (PACKED = false: the layout the kernels use; a
+// bit-packed input is expanded by tcw_create) against one BIT per bin (PACKED = true: byte = window[k >> 3],
+// value = (byte >> (k & 7)) & 1).  Same index arithmetic, 16 lookups per row; the two rates settle whether
+// gathering from packed words could pay on a kernel that is bound by instruction issue.
+template <bool PACKED>
+__global__ void __launch_bounds__(128, 3)
+peak_count_chain_kernel(int rows, double c0, double q0, int *out)
+{
+    __shared__ unsigned char win[4 * 1024];
+    for (int i = threadIdx.x; i < 4 * 1024; i += 128) win[i] = (unsigned char)((i * 2654435761u) >> 24 & (PACKED ? 255u : 1u));
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(win) + (uint32_t)(warp * 1024);
+    const double dlane = 0.125 * lane;
+    int acc[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) acc[r] = 0;
+    uint32_t mn_all = 0xffffffffu;
+    double c = c0;
+    for (int j = 0; j < rows; ++j) {
+        c = __dadd_rn(c, -1e-9);
+        const double y0 = __fma_rn(dlane, c, q0);
+        const double step = __dmul_rn(4.0, c);
+        uint32_t hi[16], lo[16];
+        hi[0] = (uint32_t)__double2hiint(y0);
+        lo[0] = (uint32_t)__double2loint(y0);
+#pragma unroll
+        for (int r = 1; r < 16; ++r) {
+            const double y = __fma_rn(step, (double)r, y0);
+            hi[r] = (uint32_t)__double2hiint(y);
+            lo[r] = (uint32_t)__double2loint(y);
+        }
+        uint32_t m = min(lo[0], min(lo[1], lo[2]));
+#pragma unroll
+        for (int r = 3; r + 1 < 16; r += 2) m = min(m, min(lo[r], lo[r + 1]));
+        mn_all = min(mn_all, min(m, lo[15]));
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const uint32_t k = hi[r] - 0x41380000u;          // bin inside the window, < 640
+            uint32_t v;
+            if (PACKED) {
+                asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(base + (k >> 3)));
+                v = (v >> (k & 7u)) & 1u;
+            } else {
+                asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(base + k));
+            }
+            acc[r] += (int)v;
+        }
+    }
+    int s = 0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) s += acc[r];
+    if (s == 123456789 || mn_all == 1u) out[0] = s;
+}
+
 }  // namespace tcw
