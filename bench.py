@@ -289,6 +289,12 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
     sampler = ClockSampler(ctx["local"])
     for _ in range(warmup):
         step()
+    # short steps: keep warming until the GPU has been busy for 50 ms (clocks and power state settle)
+    torch.cuda.synchronize()
+    t_w = time.perf_counter()
+    while time.perf_counter() - t_w < 0.05:
+        step()
+        torch.cuda.synchronize()
     h.set_option(tcw.TCW_OPT_TIMING, 1)
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier()
@@ -468,6 +474,13 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     tcw.load_library()
+    if args.shard:
+        # one rank's share of an N-GPU strong-scaling run, timed alone on this GPU (no process group): what
+        # rank R of `torchrun --nproc-per-node N bench.py --gpus N` executes, for boxes with a single GPU
+        r, n = (int(x) for x in args.shard.split("/"))
+        if world > 1 or not (0 <= r < n):
+            raise SystemExit("bench.py: --shard R/N needs a single process and 0 <= R < N")
+        return run_shard(args, tcw, tcw_inputs, dev, r, n)
     ctx = dict(tcw=tcw, tcw_inputs=tcw_inputs, dist=dist, rank=rank, world=world, local=local, dev=dev,
                ncu=load_ncu_summary(), peaks=None)
     if rank == 0:
@@ -529,6 +542,42 @@ def run_ours(args):
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_shard(args, tcw, tcw_inputs, dev, r, n):
+    import torch
+    name, fmt = headline_name(args)
+    w = tcw_inputs.make_workload(name, fmt=fmt)
+    grid = tcw.Grid.of(w)
+    lo, hi = tcw.shard_groups(grid.n_groups, r, n)
+    h = tcw.Handle.from_workload(w, device=dev)
+    out_stat = torch.empty((max(hi - lo, 1), len(w.f0)), dtype=h.stat_dtype, device=dev)
+    out_best = torch.empty((max(hi - lo, 1), 2), dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(args.warmup):
+        h.search_groups(grid, lo, hi, out_stat, out_best)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(args.steps):
+        h.search_groups(grid, lo, hi, out_stat, out_best)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    h.check()
+    ms = e0.elapsed_time(e1) / args.steps
+    info = h.info()
+    # the slice must equal the whole search's
+    full_stat, full_best = h.search(grid)
+    torch.cuda.synchronize()
+    same = bool(torch.equal(full_stat.reshape(-1, len(w.f0))[lo:hi], out_stat[: hi - lo]) and
+                torch.equal(full_best[lo:hi], out_best[: hi - lo]))
+    h.close()
+    print(json.dumps({"metric": METRIC + f" (rank {r} of {n}: its group range alone on one GPU)", "unit": UNIT,
+                      "config": workload_config(w), "group_range": [lo, hi], "n_groups": grid.n_groups,
+                      "ms_per_step": ms, "rank_lookups_per_s": (hi - lo) * len(w.f0) * w.n_sft / (ms * 1e-3),
+                      "kernels_per_step": info["launches"], "ctas": info["ctas"],
+                      "slice_equals_whole_search": same, "steps": args.steps, "warmup": args.warmup}), flush=True)
     return 0
 
 
@@ -675,6 +724,8 @@ def main():
     ap.add_argument("--stages", type=int, default=0, help="staged kernel: ring depth limit (0 auto)")
     ap.add_argument("--exact-index", action="store_true", help="staged kernel: defining chain for every bin (no fast index)")
     ap.add_argument("--general-f0", action="store_true", help="staged kernel: do not use the equally-spaced-f0 instantiation")
+    ap.add_argument("--shard", default=None, metavar="R/N",
+                    help="time rank R's group range of an N-GPU strong-scaling run alone on one GPU (and check it against the whole search)")
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -217,9 +217,9 @@ typedef struct {
  *            attaining it }; may be NULL (not all three NULL).
  *  stream    as for tcw_search (asynchronous).
  *
- * s accumulates in float32 (fused multiply-add of weight and element) in the fixed order of
- * tcw_search; W1 and W2 in float64, except over the SFTs in which a 32*R-template tile straddles
- * a band edge, where they are counted per template in float32.  Runs on the TMA-staged or the
+ * s accumulates in float32 (fused multiply-add of weight and element) in a fixed order; W1 and W2 in
+ * float64 (per-chunk partial sums of a chunked search included), except over the SFTs in which a
+ * 32*R-template tile straddles a band edge, where they are counted per template in float32.  Runs on the TMA-staged or the
  * gather kernel (one sky point at a time: weights differ between sky points, so the sky-block
  * kernel does not apply; forcing that kernel through tcw_set_option gives TCW_EUNSUPPORTED). */
 int tcw_search_weighted(tcw_handle *h, const tcw_grid *grid, const tcw_weighting *weighting,
@@ -253,7 +253,9 @@ typedef struct {
  *              moments: for unit weights Psi = (s - mean1*N)/sqrt(var1*N)); may be NULL.
  *  out_k       DEVICE, int32 [n][n_sft] bin indices (INT32_MIN where t_j < T0); inspection output
  *              for parity tests, may be NULL (and should be for large banks).
- * Power sums accumulate in float32 in ascending SFT order (deterministic); counts exactly.
+ * Power sums accumulate in float32 in a fixed order (ascending SFT order, except that the kernel keeps two
+ * gathers in flight and may add the last two in-band elements in swapped order): deterministic, run-to-run
+ * bit-identical; counts exactly.
  * Asynchronous like tcw_search. */
 int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *out_inband, int *out_k,
                     void *stream);
@@ -273,7 +275,9 @@ int tcw_get_counter(tcw_handle *h, int which, long long *value);
  * NaN is never selected; -0.0 equals +0.0.  Asynchronous on `stream`; `h` supplies the scratch. */
 
 /* tcw_topk -- the K largest values in descending order, equal values in ascending index order
- * (reading Q23).  K in 1..2048.  K = 1 on a noise-only search is Psi_noise max.
+ * (reading Q23).  K in 1..2048, n < 2^32.  K = 1 on a noise-only search is Psi_noise max.  Arrays of 2^22
+ * values or more are read twice (zoomed histogram, then ordered compaction of the candidates and an exact
+ * selection among them); smaller ones, and heavily tied ones, take five streaming passes.  Same results.
  *  out_val    DEVICE [K], same dtype as values;  out_idx  DEVICE [K] int64 indices into values;
  *  out_count  DEVICE int32 (may be NULL): entries written = min(K, selectable values). */
 int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *out_val,

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtcw.so")
 SOURCES = ["tcw_api.cu"]
-DEPENDS = ["tcw_api.cu", "tcw_sum.cuh", "tcw_tables.cuh", "tcw_skyblock.cuh", "tcw_skyblock2.cuh", "tcw_bank.cuh", "tcw_select.cuh", "tcw_prep.cuh", "tcw_median.cuh", "tcw_peaks.cuh", "tcw_exp_tables.inc", "tcw_pow_tables.inc", os.path.join("..", "..", "include", "tcw.h")]
+DEPENDS = ["tcw_api.cu", "tcw_sum.cuh", "tcw_tables.cuh", "tcw_skyblock.cuh", "tcw_skyblock2.cuh", "tcw_bank.cuh", "tcw_select.cuh", "tcw_prep.cuh", "tcw_peaks.cuh", "tcw_exp_tables.inc", "tcw_pow_tables.inc", os.path.join("..", "..", "include", "tcw.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17",
     "-gencode", "arch=compute_100a,code=sm_100a",

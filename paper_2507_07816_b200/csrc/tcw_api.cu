@@ -53,6 +53,7 @@ int fail(int code, const char *fmt, ...)
 
 constexpr double C_LIGHT = 299792458.0;
 constexpr size_t SMEM_MAX = 227 * 1024;
+constexpr long TOPK_TWO_READ_MIN = 1L << 22;   // tcw_topk: arrays of at least this many values take the two-read route
 constexpr size_t TIMING_MAX = 4096;  // timed searches kept between two tcw_get_timing calls
 // staged kernel, SFT chunking: used when the spectrogram rows of the span exceed CHUNK_MIN_BYTES;
 // a chunk then holds about CHUNK_TARGET_BYTES of rows (inside the 126 MB L2) and at most
@@ -213,6 +214,7 @@ struct tcw_handle {
     DevBuf<unsigned char> d_partial, d_stat, d_best;
     DevBuf<unsigned char> d_cpart, d_clive;  // chunked staged searches: per-chunk partial sums, live flags
     DevBuf<unsigned char> d_selws;           // selection scratch (histogram, state, block counts, candidates)
+    DevBuf<unsigned char> d_selzoom;         // top-K two-read route: per-CTA histograms, candidate keys and indices
     DevBuf<double> d_bank;                   // bank searches: f0, tau, brk [n] and sky [n][3] or [3]
     unsigned long long *d_counter = nullptr; // bank searches: lookups decided by the defining chain
     DevBuf<float> d_w;                       // weighted searches: weights [n_sky][n_sft]
@@ -362,6 +364,8 @@ int prepare(tcw_handle *h, const tcw_grid *g, long n_sel, const long *sel, cudaS
     h->a_brk = h->a_tau + g->n_tau;
     h->a_sky = h->a_brk + g->n_brk;
 
+    if ((long)g->n_sky * h->n_sft > (1L << 38) || (long)g->n_tau * h->n_sft > (1L << 37))
+        return fail(TCW_EUNSUPPORTED, "table of %ld x %d entries needs more than 2^31-1 CTAs; split the search", (long)g->n_sky, h->n_sft);
     {
         long total = (long)g->n_sky * h->n_sft;
         tcw::doppler_table_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(h->d_vel, h->n_sft, h->a_sky,
@@ -783,6 +787,7 @@ int tcw_destroy(tcw_handle *h)
     h->d_w.release();
     h->d_bank.release();
     h->d_selws.release();
+    h->d_selzoom.release();
     dev_free(h->d_counter, h->last_stream);
     h->d_cw.release();
     progress_release(h->device, h->d_progress);
@@ -1309,31 +1314,61 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
     if (dtype != 0 && dtype != 1) return fail(TCW_EINVAL, "dtype must be 0 (float32) or 1 (int32)");
     if (n <= 0) return fail(TCW_EINVAL, "n must be positive");
     if (K <= 0 || K > tcw::SEL_MAX_K) return fail(TCW_EINVAL, "K must be in 1..%d", tcw::SEL_MAX_K);
+    if (n >= (1L << 32)) return fail(TCW_EUNSUPPORTED, "n must be below 2^32 (the selection counters are 32-bit)");
     cudaStream_t st = (cudaStream_t)stream;
     enter(h, st);
     CUDA_TRY(cudaSetDevice(h->device));
     SelScratch sc;
     int rc = sel_scratch(h, &sc);
     if (rc != TCW_OK) return rc;
-    long seg;
-    int nb;
-    sel_grid(n, &seg, &nb);
     const unsigned int *v = (const unsigned int *)values;
-    const int vec = ((uintptr_t)values & 15) == 0;
     CUDA_TRY(cudaMemsetAsync(sc.hist, 0, 2048 * 4, st));
     CUDA_TRY(cudaMemsetAsync(sc.state, 0, sizeof(tcw::SelState), st));
-    tcw::sel_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
-    tcw::sel_pick_kernel<0><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
-    tcw::sel_pick_kernel<1><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_hist_kernel<2><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist);
-    tcw::sel_pick_kernel<2><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K);
-    tcw::sel_count_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq);
-    tcw::sel_scan_kernel<<<1, 256, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
-    tcw::sel_scatter_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq,
-                                                                    sc.off_gt, sc.off_eq, 0, sc.cand_bits, sc.cand_idx);
-    tcw::sel_sort_kernel<<<1, 1024, 0, st>>>(sc.cand_bits, sc.cand_idx, dtype, sc.state, (unsigned int *)out_val, out_idx,
-                                             out_count);
+    // the exact selection over `vals` (radix select of the K-th key, ordered compaction, sort); see sel_gate for `gate`
+    auto run_select = [&](const unsigned int *vals, long nn, int gate, const long long *idx_map) {
+        long seg;
+        int nb;
+        sel_grid(nn, &seg, &nb);
+        const int vec = ((uintptr_t)vals & 15) == 0;
+        tcw::sel_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(vals, nn, seg, dtype, vec, sc.state, sc.hist, gate);
+        tcw::sel_pick_kernel<0><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, gate);
+        tcw::sel_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(vals, nn, seg, dtype, vec, sc.state, sc.hist, gate);
+        tcw::sel_pick_kernel<1><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, gate);
+        tcw::sel_hist_kernel<2><<<nb, tcw::SEL_THREADS, 0, st>>>(vals, nn, seg, dtype, vec, sc.state, sc.hist, gate);
+        tcw::sel_pick_kernel<2><<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, gate);
+        tcw::sel_count_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(vals, nn, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq, gate);
+        tcw::sel_scan_kernel<<<1, 256, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state, gate);
+        tcw::sel_scatter_kernel<false><<<nb, tcw::SEL_THREADS, 0, st>>>(vals, nn, seg, dtype, vec, sc.state, 0.0, sc.blk_gt, sc.blk_eq,
+                                                                        sc.off_gt, sc.off_eq, 0, sc.cand_bits, sc.cand_idx, idx_map, gate);
+        tcw::sel_sort_kernel<<<1, 1024, 0, st>>>(sc.cand_bits, sc.cand_idx, dtype, sc.state, (unsigned int *)out_val, out_idx,
+                                                 out_count, gate);
+    };
+    if (n >= TOPK_TWO_READ_MIN) {
+        // two reads of the array: zoomed histogram (+ per-CTA histograms), then ordered compaction of the keys at or
+        // above the bin of the K-th largest into a candidate buffer; the exact selection then runs on the candidates
+        // (gate 2), or, if they did not fit (heavily tied data), on the full array (gate 1).  No host synchronisation.
+        long seg;
+        int nb;
+        sel_grid(n, &seg, &nb);
+        const int vec = ((uintptr_t)values & 15) == 0;
+        const size_t zbytes = (size_t)nb * 2048 * 4 + 2 * (size_t)tcw::SEL_MAX_BLOCKS * 4 + (size_t)tcw::SEL_MAX_CAND * 12 + 64;
+        if ((rc = h->d_selzoom.reserve(zbytes)) != TCW_OK) return rc;
+        long long *z_idx = (long long *)h->d_selzoom.p;
+        unsigned int *z_bits = (unsigned int *)(z_idx + tcw::SEL_MAX_CAND);
+        unsigned int *z_off = z_bits + tcw::SEL_MAX_CAND;
+        unsigned int *z_cnt = z_off + tcw::SEL_MAX_BLOCKS;
+        unsigned int *z_hist = z_cnt + tcw::SEL_MAX_BLOCKS;
+        tcw::sel_sample_kernel<<<1, 1024, 0, st>>>(v, n, dtype, sc.state);
+        tcw::sel_zoom_hist_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist, z_hist);
+        tcw::sel_zoom_pick_kernel<<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, dtype);
+        tcw::sel_zoom_count_kernel<<<(nb + 7) / 8, 256, 0, st>>>(z_hist, nb, sc.state, z_cnt);
+        tcw::sel_zoom_scan_kernel<<<1, 256, 0, st>>>(z_cnt, nb, z_off);
+        tcw::sel_zoom_compact_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, z_off, z_bits, z_idx);
+        run_select(z_bits, tcw::SEL_MAX_CAND, 2, z_idx);
+        run_select(v, n, 1, nullptr);
+    } else {
+        run_select(v, n, 0, nullptr);
+    }
     CUDA_TRY(cudaGetLastError());
     h->last_stream = st;
     return TCW_OK;
@@ -1347,6 +1382,7 @@ int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, doubl
     if (dtype != 0 && dtype != 1) return fail(TCW_EINVAL, "dtype must be 0 (float32) or 1 (int32)");
     if (n <= 0 || capacity < 0) return fail(TCW_EINVAL, "n must be positive and capacity >= 0");
     if (std::isnan(threshold)) return fail(TCW_EINVAL, "threshold is NaN");
+    if (n >= (1L << 32)) return fail(TCW_EUNSUPPORTED, "n must be below 2^32 (the per-block counters are 32-bit)");
     cudaStream_t st = (cudaStream_t)stream;
     enter(h, st);
     CUDA_TRY(cudaSetDevice(h->device));
@@ -1393,9 +1429,7 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     if (format != TCW_F32_POWER && std::isnan(prep->threshold)) return fail(TCW_EINVAL, "threshold is NaN");
     if (out_pitch_bytes < (long)row_bytes(format, prep->n_bins) || (format != TCW_U8_COUNT && (out_pitch_bytes & 3)))
         return fail(TCW_EINVAL, "out_pitch_bytes is smaller than one row or not a multiple of 4");
-    int spc = tcw::PREP_SPC;                        // SFTs per CTA: two CTAs per SM when possible
-    while (spc > 1 && spc * tcw::prep_sft_smem(prep->n_bins, h) > SMEM_MAX / 2 - 1024) spc /= 2;
-    const size_t smem = spc * tcw::prep_sft_smem(prep->n_bins, h);
+    const size_t smem = (((size_t)(prep->n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)prep->n_bins + 31) & ~(size_t)31);
     if (smem > SMEM_MAX) return fail(TCW_EUNSUPPORTED, "band too wide for one CTA's shared memory (%zu bytes)", smem);
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -1467,7 +1501,7 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         p.out_format = format;
         p.out = (unsigned char *)out_spectrogram + j0 * out_pitch_bytes;
         p.out_pitch = out_pitch_bytes;
-        tcw::prep_normalise_kernel<<<(nb + spc - 1) / spc, tcw::PREP_THREADS, smem, st>>>(p, nb, spc);
+        tcw::prep_normalise_kernel<<<nb, tcw::PREP_THREADS, smem, st>>>(p);
         PREP_TRY(cudaGetLastError());
     }
     PREP_TRY(cudaStreamSynchronize(st));

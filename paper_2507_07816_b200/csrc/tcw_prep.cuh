@@ -9,16 +9,18 @@
 // The DFT itself is a plain batched real-to-complex transform and is left to cuFFT (a library
 // primitive, like a GEMM left to cuBLAS).  Everything around it is here:
 //   * prep_window_kernel: window multiply into the batch buffer cuFFT reads (float32);
-//   * prep_normalise_kernel: four SFTs per CTA, 64 threads each: |X|^2 of the band and its two
-//     half-windows into shared memory, then every thread walks a run of consecutive bins with an
-//     exact sliding median that costs amortised O(1) per bin (tcw_median.cuh), and writes rho
-//     (float32), nu (uint8) or nu bit-packed (uint32 words, LSB first) straight into the spectrogram
-//     layout tcw_create reads.
+//   * prep_normalise_kernel: one CTA per SFT: |X|^2 of the band and its two half-windows into shared
+//     memory, then every thread walks a run of consecutive bins keeping the running median by
+//     counting (see the kernel), and writes rho (float32), nu (uint8) or nu bit-packed (uint32
+//     words, LSB first) straight into the spectrogram layout tcw_create reads.  (A per-thread sliding
+//     median with amortised O(1) updates -- counters plus the nearest elements on either side of the
+//     median in registers, window re-scan only when a list runs dry -- was built and measured in round 2:
+//     exact, but 3.9x SLOWER on B200 (616 against 160 us per 512 SFTs), because under SIMT a warp pays for
+//     the union of its lanes' branches and a re-scan that is rare per lane happens in most warps on most
+//     slides.  The counting form below, identical work in every lane, stays.)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
-
-#include "tcw_median.cuh"
 
 namespace tcw {
 
@@ -68,55 +70,57 @@ struct PrepParams {
     long out_pitch;         // bytes
 };
 
-// One CTA normalises spc SFTs (4 when their bands fit shared memory, else 2 or 1), 256/spc threads each.  Dynamic shared memory per SFT:
-// float P[n_bins + 2h] (16-byte rounded), then (count formats) unsigned char nu[n_bins rounded up to 32].
-constexpr int PREP_SPC = 4;                        // SFTs per CTA when they fit (else 2 or 1): 64 threads per SFT
-__host__ __device__ inline size_t prep_sft_smem(int n_bins, int h)
-{
-    return ((((size_t)(n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)n_bins + 31) & ~(size_t)31) + 127) & ~(size_t)127;
-}
-
-struct PrepView {                                   // a window of P in shared memory
-    const float *p;
-    __device__ __forceinline__ unsigned int bits(int q) const { return __float_as_uint(p[q]); }
-    __device__ __forceinline__ float value(int q) const { return p[q]; }
-    __device__ __forceinline__ float from_bits(unsigned int k) const { return __uint_as_float(k); }
-};
-
-__global__ void __launch_bounds__(PREP_THREADS)
-prep_normalise_kernel(const PrepParams p, int n_batch, int spc)
+// dynamic shared memory: float P[n_bins + 2h], then (count formats) unsigned char nu[n_bins rounded up to 32]
+__global__ void __launch_bounds__(256)
+prep_normalise_kernel(const PrepParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int PREP_TPS = PREP_THREADS / spc;       // threads per SFT
-    const int sub = threadIdx.x / PREP_TPS, t = threadIdx.x % PREP_TPS;
-    const int sft = blockIdx.x * spc + sub;
-    unsigned char *mine = smem + (size_t)sub * prep_sft_smem(p.n_bins, p.h);
-    float *P = (float *)mine;
+    float *P = (float *)smem;
     const int n_in = p.n_bins + 2 * p.h;
-    unsigned char *nu = mine + (((size_t)n_in * 4 + 15) & ~(size_t)15);
-    const bool live = sft < n_batch;
-    if (live) {
-        const float2 *row = p.spec + (long)sft * p.n_half + (p.k_min - p.h);
-        for (int q = t; q < n_in; q += PREP_TPS) {
-            const float2 c = row[q];
-            P[q] = c.x * c.x + c.y * c.y;
-        }
+    unsigned char *nu = smem + (((size_t)n_in * 4 + 15) & ~(size_t)15);
+    const float2 *row = p.spec + (long)blockIdx.x * p.n_half + (p.k_min - p.h);
+    for (int t = threadIdx.x; t < n_in; t += (int)blockDim.x) {
+        const float2 c = row[t];
+        P[t] = c.x * c.x + c.y * c.y;
     }
     __syncthreads();
 
-    // Every thread walks a run of consecutive bins with the exact sliding median of tcw_median.cuh:
-    // selection by bitwise search for its first window, then amortised O(1) per slide (two counters and
-    // the nearest elements on either side of the median in registers; a window re-scan only when one of
-    // those lists runs dry).  An odd run length puts the threads of a warp on different banks.
+    // Running median without per-thread sorted arrays (those live in local memory and serialise):
+    // the first bin of a thread's run selects the rank-h value of its window by a bitwise binary
+    // search on the float bits (P >= 0, so the bits order like the values); every further bin
+    // re-counts the slid window against the previous median m.  One element left and one entered,
+    // so #(x < m) <= h + 1 and #(x <= m) >= h: the new median is m, or the largest element below it,
+    // or the smallest element above it.  All reads are conflict-free shared-memory loads.
     const int W = 2 * p.h + 1, h = p.h;
-    const int run = ((p.n_bins + PREP_TPS - 1) / PREP_TPS) | 1;
-    const int k0 = min(t * run, p.n_bins), k1 = min(k0 + run, p.n_bins);
-    unsigned char *orow = p.out + (long)sft * p.out_pitch;
-    if (live && k0 < k1) {
-        MedianState st;
-        med_init(st, PrepView{P + k0}, W, h);
+    // an odd run length: lanes then start 'run' words apart, which visits all 32 banks (no conflicts)
+    const int run = ((p.n_bins + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
+    const int k0 = min((int)threadIdx.x * run, p.n_bins), k1 = min(k0 + run, p.n_bins);
+    unsigned char *orow = p.out + (long)blockIdx.x * p.out_pitch;
+    if (k0 < k1) {
+        const unsigned int *Pu = (const unsigned int *)P;
+        unsigned int key = 0;
+        for (int bit = 30; bit >= 0; --bit) {
+            const unsigned int cand = key | (1u << bit);
+            int c = 0;
+            for (int q = 0; q < W; ++q) c += Pu[k0 + q] < cand;
+            if (c <= h) key = cand;
+        }
+        float m = __uint_as_float(key);
         for (int k = k0; k < k1; ++k) {
-            const float m = k == k0 ? st.m : med_slide(st, PrepView{P + k}, W, h, P[k - 1], P[k + W - 1]);
+            if (k > k0) {
+                int c_less = 0, c_leq = 0;
+                float pred = -__int_as_float(0x7f800000), succ = __int_as_float(0x7f800000);
+                for (int q = 0; q < W; ++q) {
+                    const float x = P[k + q];
+                    const bool lt = x < m, gt = x > m;
+                    c_less += lt;
+                    c_leq += !gt;
+                    pred = fmaxf(pred, lt ? x : pred);
+                    succ = fminf(succ, gt ? x : succ);
+                }
+                if (c_less > h) m = pred;
+                else if (c_leq <= h) m = succ;
+            }
             const float rho = P[k + h] * 0.69314718055994531f / m;
             if (p.out_format == 0) ((float *)orow)[k] = rho;
             else nu[k] = rho > p.threshold ? 1 : 0;
@@ -124,12 +128,11 @@ prep_normalise_kernel(const PrepParams p, int n_batch, int spc)
     }
     if (p.out_format == 0) return;
     __syncthreads();
-    if (!live) return;
     if (p.out_format == 1) {
-        for (int k = t; k < p.n_bins; k += PREP_TPS) orow[k] = nu[k];
+        for (int k = threadIdx.x; k < p.n_bins; k += (int)blockDim.x) orow[k] = nu[k];
     } else {
         const int n_words = (p.n_bins + 31) / 32;
-        for (int wd = t; wd < n_words; wd += PREP_TPS) {
+        for (int wd = threadIdx.x; wd < n_words; wd += (int)blockDim.x) {
             uint32_t bits = 0;
             for (int b = 0; b < 32; ++b) {
                 const int k = 32 * wd + b;

@@ -14,6 +14,12 @@
 //   compaction (per-block counts -> one-block scan -> ordered scatter) of the keys above it plus
 //   the lowest-index keys equal to it, then a bitonic sort of the K candidates in one CTA.
 //   NaN is never selected; -0.0 equals +0.0.
+// Large arrays take a two-read route first (tcw_topk): a monotone 2048-bin map of the keys, zoomed on
+// the upper tail by a small sample, is histogrammed in ONE pass that also stores every CTA's own
+// histogram; the bin holding the K-th largest key is picked; a second pass compacts, in index order,
+// the keys at or above that bin (a few thousand for typical statistics) together with their indices;
+// the exact selection above then runs on the compacted candidates.  If the candidates would exceed
+// SEL_MAX_CAND (heavily tied data) the full-array route is taken instead.  Same results either way.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -23,6 +29,8 @@ namespace tcw {
 constexpr int SEL_THREADS = 256;
 constexpr int SEL_MAX_BLOCKS = 2048;   // the block-count scan runs in one CTA
 constexpr int SEL_MAX_K = 2048;        // candidates sorted in one CTA's shared memory
+constexpr int SEL_MAX_CAND = 1 << 20;  // two-read route: candidate buffer (key bits + index per entry)
+constexpr int SEL_SAMPLE = 2048;       // keys sampled to place the zoom window
 
 struct SelState {
     unsigned int prefix;        // high bits of the K-th largest key found so far
@@ -30,7 +38,21 @@ struct SelState {
     unsigned int k_eff;         // min(K, number of selectable values)
     unsigned int n_greater;     // keys strictly above the K-th largest (after the last pass)
     unsigned long long count;   // threshold selection: number of values above the threshold
+    // two-read route: monotone bin map  bin(key) = 0 if key >> z_top < z_prefix, 2047 if >, else
+    // clamp(((key >> z_shift) & 2047), 0, 2047); z_bin = the bin of the K-th largest key; n_cand = keys
+    // in bins >= z_bin; cand_ok = 1 when they fit the candidate buffer
+    unsigned int z_shift, z_top, z_prefix, z_bin, n_cand, cand_ok;
+    unsigned int z_val_lo;      // raw value (float bits / int) of the lowest key in a bin >= 1: smaller values skip the key arithmetic
+    unsigned int z_val_bin;     // raw value of the lowest key in a bin >= z_bin: only values at or above it can be candidates
 };
+
+// the monotone bin of a key under the zoom window (non-decreasing in key)
+__device__ __forceinline__ unsigned int sel_zoom_bin(unsigned int key, unsigned int z_shift, unsigned int z_top, unsigned int z_prefix)
+{
+    const unsigned int hi = z_top >= 32u ? 0u : key >> z_top;
+    if (hi != z_prefix) return hi < z_prefix ? 0u : 2047u;
+    return (key >> z_shift) & 2047u;
+}
 
 // order-preserving key of a float32 (NaN -> 0 = "not selectable"), or of an int32
 __device__ __forceinline__ unsigned int sel_key(unsigned int bits, int is_int)
@@ -44,6 +66,31 @@ __device__ __forceinline__ unsigned int sel_key(unsigned int bits, int is_int)
 __device__ __forceinline__ bool sel_valid(unsigned int bits, int is_int)
 {
     return is_int || (bits & 0x7fffffffu) <= 0x7f800000u;
+}
+
+// Kernels of the exact selection are enqueued for both routes; `gate` says which launch is live:
+// 0 always; 1 only if the two-read route found too many candidates (full array); 2 only if it did not
+// (then the array is the candidate buffer and its length is state->n_cand).
+__device__ __forceinline__ bool sel_gate(const SelState *__restrict__ state, int gate, long &n)
+{
+    if (gate == 0) return true;
+    const unsigned int ok = state->cand_ok;
+    if (gate == 1) return ok == 0u;
+    if (ok == 0u) return false;
+    n = (long)state->n_cand < n ? (long)state->n_cand : n;
+    return true;
+}
+
+// inverse of sel_key (for keys of selectable values)
+__device__ __forceinline__ unsigned int sel_unkey(unsigned int key, int is_int)
+{
+    if (is_int) return key ^ 0x80000000u;
+    return (key & 0x80000000u) ? (key & 0x7fffffffu) : ~key;
+}
+// raw value `b` is certainly below raw value `lim` (false for NaN: those take the exact path)
+__device__ __forceinline__ bool sel_raw_below(unsigned int b, unsigned int lim, int is_int)
+{
+    return is_int ? (int)b < (int)lim : __uint_as_float(b) < __uint_as_float(lim);
 }
 
 struct SelSeg { long begin, end; };
@@ -78,10 +125,11 @@ __device__ __forceinline__ void sel_load4(const unsigned int *__restrict__ vals,
 template <int PASS>
 __global__ void __launch_bounds__(SEL_THREADS)
 sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
-                const SelState *__restrict__ state, unsigned int *__restrict__ hist)
+                const SelState *__restrict__ state, unsigned int *__restrict__ hist, int gate = 0)
 {
     constexpr int COPIES = PASS == 0 ? 4 : 1;
     __shared__ unsigned int h[COPIES * 2048];
+    if (!sel_gate(state, gate, n)) return;
     for (int t = threadIdx.x; t < COPIES * 2048; t += SEL_THREADS) h[t] = 0;
     __syncthreads();
     const unsigned int prefix = PASS ? state->prefix : 0u;
@@ -143,10 +191,11 @@ sel_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_
 // (thread t sums the 8 bins [8t, 8t + 8); thread 0 walks the 256 partial sums, then the 8 bins)
 template <int PASS>
 __global__ void __launch_bounds__(256)
-sel_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, unsigned int K)
+sel_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, unsigned int K, int gate = 0)
 {
     constexpr int bins = PASS == 2 ? 1024 : 2048;
     __shared__ unsigned int part[256];
+    { long dummy = 0; if (!sel_gate(state, gate, dummy)) return; }
     unsigned int mine = 0;
     for (int b = 0; b < 8; ++b) { const int q = 8 * threadIdx.x + b; mine += q < bins ? hist[q] : 0u; }
     part[threadIdx.x] = mine;
@@ -182,6 +231,207 @@ sel_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, u
     for (int b = threadIdx.x; b < bins; b += 256) hist[b] = 0;   // ready for the next pass
 }
 
+__device__ __forceinline__ unsigned int sel_block_scan(unsigned int cnt, unsigned int *warp_tot, unsigned int &total);
+
+// ---- two-read route -------------------------------------------------------------------------
+// One CTA: SEL_SAMPLE keys at a fixed stride, sorted descending; the zoom window is placed on the highest
+// bit in which the sample's largest key and its 16th largest differ (a window of 11 bits from there down),
+// so that the bins resolve the upper tail.  Any window gives exact results; this one gives few candidates.
+__global__ void __launch_bounds__(1024)
+sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, SelState *__restrict__ state)
+{
+    __shared__ unsigned int key[SEL_SAMPLE];
+    const long stride = n / SEL_SAMPLE > 0 ? n / SEL_SAMPLE : 1;
+    for (int t = threadIdx.x; t < SEL_SAMPLE; t += 1024) {
+        const long i = (long)t * stride;
+        const unsigned int b = i < n ? __ldg(vals + i) : 0u;
+        key[t] = (i < n && sel_valid(b, is_int)) ? sel_key(b, is_int) : 0u;
+    }
+    __syncthreads();
+    for (int size = 2; size <= SEL_SAMPLE; size <<= 1)
+        for (int st = size >> 1; st > 0; st >>= 1) {
+            for (int t = threadIdx.x; t < SEL_SAMPLE / 2; t += 1024) {
+                const int lo = 2 * t - (t & (st - 1)), hi = lo + st;
+                const bool desc = (lo & size) == 0;
+                if ((key[lo] > key[hi]) != desc) { const unsigned int k = key[lo]; key[lo] = key[hi]; key[hi] = k; }
+            }
+            __syncthreads();
+        }
+    if (threadIdx.x == 0) {
+        const unsigned int diff = key[0] ^ key[15];
+        const int top_bit = diff ? 31 - __clz(diff) : 10;            // highest differing bit
+        const int shift = top_bit >= 10 ? top_bit - 10 : 0;
+        state->z_shift = (unsigned int)shift;
+        state->z_top = (unsigned int)(shift + 11);
+        state->z_prefix = shift + 11 >= 32 ? 0u : key[0] >> (shift + 11);
+        const unsigned int base = shift + 11 >= 32 ? 0u : (key[0] >> (shift + 11)) << (shift + 11);
+        state->z_val_lo = sel_unkey(base | (1u << shift), is_int);
+        state->z_val_bin = state->z_val_lo;
+        state->z_bin = 0;
+        state->n_cand = 0;
+        state->cand_ok = 0;
+    }
+}
+
+// Pass A: histogram of the zoom bins over all keys; every CTA also stores its own histogram (2048 words)
+// so that the candidates of pass B can be placed in index order without another read of the array.
+__global__ void __launch_bounds__(SEL_THREADS)
+sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
+                     const SelState *__restrict__ state, unsigned int *__restrict__ hist, unsigned int *__restrict__ blk_hist)
+{
+    __shared__ unsigned int h[2048];
+    for (int t = threadIdx.x; t < 2048; t += SEL_THREADS) h[t] = 0;
+    __syncthreads();
+    const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, vlo = state->z_val_lo;
+    const SelSeg sg = sel_segment(n, seg);
+    unsigned int *hc = h;      // one copy: the keys that reach the atomics are the few in and above the window
+    // almost every key lies below the zoom window (bin 0): those are counted in a register, not by
+    // thousands of atomics on one shared-memory word
+    unsigned int below = 0;
+    for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
+        unsigned int b0[4], b1[4];
+        int n0, n1;
+        sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, n0);
+        sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, n1);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            // one compare settles the values below the window; only the tail pays for the key arithmetic
+            if (c < n0) {
+                if (sel_raw_below(b0[c], vlo, is_int)) ++below;
+                else if (sel_valid(b0[c], is_int)) {
+                    const unsigned int d = sel_zoom_bin(sel_key(b0[c], is_int), zs, zt, zp);
+                    if (d) atomicAdd(&hc[d], 1u); else ++below;
+                }
+            }
+            if (c < n1) {
+                if (sel_raw_below(b1[c], vlo, is_int)) ++below;
+                else if (sel_valid(b1[c], is_int)) {
+                    const unsigned int d = sel_zoom_bin(sel_key(b1[c], is_int), zs, zt, zp);
+                    if (d) atomicAdd(&hc[d], 1u); else ++below;
+                }
+            }
+        }
+    }
+    for (int o = 16; o; o >>= 1) below += __shfl_xor_sync(0xffffffffu, below, o);
+    if ((threadIdx.x & 31) == 0 && below) atomicAdd(&h[0], below);
+    __syncthreads();
+    for (int t = threadIdx.x; t < 2048; t += SEL_THREADS) {
+        const unsigned int c = h[t];
+        blk_hist[(long)blockIdx.x * 2048 + t] = c;
+        if (c) atomicAdd(&hist[t], c);
+    }
+}
+
+// One CTA: the bin of the K-th largest key, the number of candidates (keys in bins >= it), whether they fit
+__global__ void __launch_bounds__(256)
+sel_zoom_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, unsigned int K, int is_int)
+{
+    __shared__ unsigned int part[256];
+    unsigned int mine = 0;
+    for (int b = 0; b < 8; ++b) mine += hist[8 * threadIdx.x + b];
+    part[threadIdx.x] = mine;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long total = 0;
+        for (int t = 0; t < 256; ++t) total += part[t];
+        const unsigned long long k = total < K ? total : K;
+        unsigned long long above = 0;
+        int d = 0;
+        if (k > 0) {
+            int t = 255;
+            for (; t > 0; --t) {
+                if (above + part[t] >= k) break;
+                above += part[t];
+            }
+            for (d = 8 * t + 7; d > 8 * t; --d) {
+                if (above + hist[d] >= k) break;
+                above += hist[d];
+            }
+        }
+        const unsigned long long n_cand = above + hist[d];
+        state->z_bin = (unsigned int)d;
+        {
+            // the lowest key of bin d (d >= 1) as a raw value: pass B tests values against it before any key arithmetic
+            const unsigned int zt = state->z_top, zs = state->z_shift;
+            const unsigned int base = zt >= 32u ? 0u : state->z_prefix << zt;
+            state->z_val_bin = sel_unkey(base | ((unsigned int)(d > 0 ? d : 1) << zs), is_int);
+        }
+        state->n_cand = n_cand > 0xffffffffull ? 0xffffffffu : (unsigned int)n_cand;
+        state->cand_ok = (k > 0 && n_cand <= (unsigned long long)SEL_MAX_CAND) ? 1u : 0u;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < 2048; b += 256) hist[b] = 0;
+}
+
+// per-CTA candidate counts from the stored histograms: one warp per CTA of pass A
+__global__ void __launch_bounds__(256)
+sel_zoom_count_kernel(const unsigned int *__restrict__ blk_hist, int n_blocks, const SelState *__restrict__ state,
+                      unsigned int *__restrict__ blk_cnt)
+{
+    const unsigned int d0 = state->z_bin;
+    const int b = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (b >= n_blocks) return;
+    unsigned int c = 0;
+    for (unsigned int d = d0 + lane; d < 2048u; d += 32) c += blk_hist[(long)b * 2048 + d];
+    for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (lane == 0) blk_cnt[b] = c;
+}
+// their exclusive scan (one CTA, <= 2048 entries: thread t owns 8)
+__global__ void __launch_bounds__(256)
+sel_zoom_scan_kernel(const unsigned int *__restrict__ blk_cnt, int n_blocks, unsigned int *__restrict__ blk_off)
+{
+    __shared__ unsigned int pa[256];
+    unsigned int a = 0;
+    for (int c = 0; c < 8; ++c) { const int q = 8 * threadIdx.x + c; a += q < n_blocks ? blk_cnt[q] : 0u; }
+    pa[threadIdx.x] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int s = 0;
+        for (int t = 0; t < 256; ++t) { const unsigned int v = pa[t]; pa[t] = s; s += v; }
+    }
+    __syncthreads();
+    a = pa[threadIdx.x];
+    for (int c = 0; c < 8; ++c) {
+        const int q = 8 * threadIdx.x + c;
+        if (q < n_blocks) { blk_off[q] = a; a += blk_cnt[q]; }
+    }
+}
+
+// Pass B: the keys in bins >= z_bin with their indices, in index order, into the candidate buffer
+__global__ void __launch_bounds__(SEL_THREADS)
+sel_zoom_compact_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
+                        const SelState *__restrict__ state, const unsigned int *__restrict__ blk_off,
+                        unsigned int *__restrict__ cand_bits, long long *__restrict__ cand_idx)
+{
+    __shared__ unsigned int wt[SEL_THREADS / 32];
+    if (!state->cand_ok) return;
+    const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, d0 = state->z_bin, vbin = state->z_val_bin;
+    unsigned int base = blk_off[blockIdx.x];
+    const SelSeg sg = sel_segment(n, seg);
+    for (long t0 = sg.begin; t0 < sg.end; t0 += SEL_TILE) {
+        const long i = t0 + 4 * threadIdx.x;
+        unsigned int b[4];
+        int nv;
+        bool take[4];
+        sel_load4(vals, i, sg.end, vec != 0, b, nv);
+        unsigned int c = 0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            // values below the lowest value of bin d0 cannot be candidates (d0 = 0: every selectable value is one)
+            take[q] = q < nv && (d0 == 0u || !sel_raw_below(b[q], vbin, is_int)) && sel_valid(b[q], is_int) &&
+                      sel_zoom_bin(sel_key(b[q], is_int), zs, zt, zp) >= d0;
+            c += take[q];
+        }
+        if (!__syncthreads_or((int)c)) continue;
+        unsigned int tot;
+        unsigned int r = sel_block_scan(c, wt, tot);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (take[q]) { cand_bits[base + r] = b[q]; cand_idx[base + r] = i + q; ++r; }
+        base += tot;
+    }
+}
+
 // ---- ordered compaction -------------------------------------------------------------------
 // predicate classes of one element: 2 = taken unconditionally, 1 = equal to the K-th key (taken
 // while the equal budget lasts, in index order), 0 = not taken
@@ -206,9 +456,10 @@ template <bool THR>
 __global__ void __launch_bounds__(SEL_THREADS)
 sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
                  const SelState *__restrict__ state, double thr,
-                 unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq)
+                 unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq, int gate = 0)
 {
     __shared__ unsigned int s_gt, s_eq;
+    if (!THR && !sel_gate(state, gate, n)) return;
     if (threadIdx.x == 0) s_gt = s_eq = 0;
     __syncthreads();
     const unsigned int kth = THR ? 0u : state->prefix;
@@ -240,9 +491,10 @@ sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is
 __global__ void __launch_bounds__(256)
 sel_scan_kernel(unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq, int n_blocks,
                 unsigned long long *__restrict__ off_gt, unsigned long long *__restrict__ off_eq,
-                SelState *__restrict__ state)
+                SelState *__restrict__ state, int gate = 0)
 {
     __shared__ unsigned long long pa[256], pb[256];
+    { long dummy = 0; if (!sel_gate(state, gate, dummy)) return; }
     unsigned long long a = 0, b = 0;
     for (int c = 0; c < 8; ++c) {
         const int q = 8 * threadIdx.x + c;
@@ -302,9 +554,11 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
                    const SelState *__restrict__ state, double thr,
                    const unsigned int *__restrict__ blk_gt, const unsigned int *__restrict__ blk_eq,
                    const unsigned long long *__restrict__ off_gt, const unsigned long long *__restrict__ off_eq,
-                   long capacity, unsigned int *__restrict__ cand_bits, long long *__restrict__ out_idx)
+                   long capacity, unsigned int *__restrict__ cand_bits, long long *__restrict__ out_idx,
+                   const long long *__restrict__ idx_map = nullptr, int gate = 0)
 {
     __shared__ unsigned int wt[SEL_THREADS / 32];
+    if (!THR && !sel_gate(state, gate, n)) return;
     const unsigned int kth = THR ? 0u : state->prefix;
     const unsigned long long n_greater = THR ? 0ull : state->n_greater;
     const unsigned long long eq_budget = THR ? 0ull : state->k_rem;
@@ -336,11 +590,11 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
             if (cls[c] == 2) {
                 const unsigned long long pos = base_gt + r2++;
                 if (THR) { if ((long)pos < capacity) out_idx[pos] = i + c; }
-                else { cand_bits[pos] = b[c]; out_idx[pos] = i + c; }
+                else { cand_bits[pos] = b[c]; out_idx[pos] = idx_map ? idx_map[i + c] : i + c; }
             } else if constexpr (!THR) {
                 if (cls[c] == 1) {
                     const unsigned long long q = base_eq + r1++;
-                    if (q < eq_budget) { cand_bits[n_greater + q] = b[c]; out_idx[n_greater + q] = i + c; }
+                    if (q < eq_budget) { cand_bits[n_greater + q] = b[c]; out_idx[n_greater + q] = idx_map ? idx_map[i + c] : i + c; }
                 }
             }
         }
@@ -353,10 +607,11 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
 __global__ void __launch_bounds__(1024)
 sel_sort_kernel(const unsigned int *__restrict__ cand_bits, const long long *__restrict__ cand_idx, int is_int,
                 const SelState *__restrict__ state, unsigned int *__restrict__ out_val,
-                long long *__restrict__ out_idx, int *__restrict__ out_count)
+                long long *__restrict__ out_idx, int *__restrict__ out_count, int gate = 0)
 {
     __shared__ unsigned int key[SEL_MAX_K], raw[SEL_MAX_K];
     __shared__ long long idx[SEL_MAX_K];
+    { long dummy = 0; if (!sel_gate(state, gate, dummy)) return; }
     const int k = (int)state->k_eff;
     for (int t = threadIdx.x; t < SEL_MAX_K; t += 1024) {
         if (t < k) { raw[t] = cand_bits[t]; key[t] = sel_key(raw[t], is_int); idx[t] = cand_idx[t]; }

@@ -42,6 +42,31 @@ def test_topk_float_random_and_tied(handle, n, K):
     _check_topk(handle, rng.integers(-3, 4, size=n).astype(np.float32), K)      # heavy ties: lowest index first
 
 
+@pytest.mark.parametrize("K", [1, 1000, 2048])
+def test_topk_two_read_route_large_arrays(handle, K):
+    """Arrays of 2^22 values or more take the two-read route (zoomed histogram, ordered compaction of the
+    candidates, exact selection on them) or, when the candidates do not fit, the full-array route; every
+    case must equal oracle/select.py exactly: values, indices, ties by lowest index."""
+    n = 5_000_011
+    rng = np.random.default_rng(K)
+    a = rng.standard_normal(n).astype(np.float32)                       # the shape of a Psi array
+    _check_topk(handle, a, K)
+    a[[11, 4_999_999, 2_500_000]] = [np.nan, np.inf, -np.inf]
+    a[123_456] = a[4_000_000] = a.max()                                  # a tie at the very top
+    _check_topk(handle, a, K)
+    _check_topk(handle, (10800.0 + 104.0 * rng.standard_normal(n)).astype(np.float32), K)   # power sums: all positive
+    p = (10800.0 + 104.0 * rng.standard_normal(n)).astype(np.float32)
+    p[rng.integers(0, n, size=n // 3)] = 0.0                             # many out-of-band templates with stat 0
+    _check_topk(handle, p, K)
+    _check_topk(handle, rng.integers(-3, 4, size=n).astype(np.float32), K)      # 7 distinct values: ties everywhere
+    _check_topk(handle, np.full(n, 2.5, dtype=np.float32), K)                   # one value: candidates cannot fit
+    c = rng.binomial(10800, 0.2019, size=n).astype(np.int32)                   # number counts (cfg5's out_stat)
+    _check_topk(handle, c, K)
+    c[[5, n - 1]] = [np.iinfo(np.int32).max, np.iinfo(np.int32).min]
+    _check_topk(handle, c, K)
+    _check_topk(handle, np.arange(n, dtype=np.int32)[::-1].copy(), K)           # all distinct, descending
+
+
 def test_topk_special_values(handle):
     v = np.array([0.5, np.nan, -0.0, 0.0, np.inf, -np.inf, 0.5, -np.nan, 1e-45, -1e-45, 3.4e38], dtype=np.float32)
     _check_topk(handle, v, 11)

@@ -87,15 +87,23 @@ def test_cfg1_weighted_parity(tcw, cfg1, fmt, kernel):
 
 
 def test_unit_weights_match_the_plain_search_bit_for_bit(tcw, cfg1):
-    """weights = NULL: fma(1, v, acc) = acc + v, so s is bit-identical to tcw_search's statistic;
+    """weights = NULL: fma(1, v, acc) = acc + v, so s is bit-identical to the statistic of a plain search that
+    adds the rows in the same order -- one at a time, which is what tcw_search does in its general-f0
+    instantiation (TCW_OPT_GENERAL_F0); the equally-spaced-f0 instantiation adds rows in pairs
+    (acc += row_q + row_q+1) and agrees to float32 rounding.
     Psi = (s - N_inband)/sqrt(N_inband)."""
     import torch
     with tcw.Handle.from_workload(cfg1) as h:
         grid = tcw.Grid.of(cfg1)
+        paired, _ = h.search(grid)
+        paired = paired.clone()
+        h.set_option(tcw.TCW_OPT_GENERAL_F0, 1)
         plain, _ = h.search(grid)
+        h.set_option(tcw.TCW_OPT_GENERAL_F0, 0)
         psi, stat, _ = h.search_weighted(grid, None, 1.0, 1.0)
         torch.cuda.synchronize()
         assert torch.equal(plain, stat)
+        assert torch.allclose(paired, stat, rtol=2e-6, atol=2e-6)
     ref = oracle.evaluate(cfg1)
     n = ref.n_inband.astype(np.float64)
     want = (stat.cpu().numpy().reshape(-1).astype(np.float64) - n) / np.sqrt(n)
