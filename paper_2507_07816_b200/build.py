@@ -13,7 +13,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libtcw.so")
+# TCW_LIBRARY: build / load the library at another path (e.g. a variant built with TCW_NVCC_FLAGS="-DTCW_RB=2")
+LIB = os.environ.get("TCW_LIBRARY") or os.path.join(HERE, "libtcw.so")
 SOURCES = ["tcw_api.cu"]
 DEPENDS = ["tcw_api.cu", "tcw_sum.cuh", "tcw_tables.cuh", "tcw_skyblock.cuh", "tcw_skyblock2.cuh", "tcw_bank.cuh", "tcw_select.cuh", "tcw_prep.cuh", "tcw_peaks.cuh", "tcw_exp_tables.inc", "tcw_pow_tables.inc", os.path.join("..", "..", "include", "tcw.h")]
 NVCC_FLAGS = [
@@ -43,7 +44,7 @@ def needs_build() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("TCW_NVCC_FLAGS", "").split(), *(["-Xptxas", "-v"] if verbose else []),
                "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.run(cmd, check=True)
     return LIB

@@ -420,14 +420,14 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
         // less than 2^-34 bin.  The kernel then needs no per-template f0 registers.
         p.d32 = 0.0;
         if (g->n_f0 >= 2 && !h->opt_nonuniform) {
-            const long double delta = ((long double)g->f0[g->n_f0 - 1] - (long double)g->f0[0]) / (long double)(g->n_f0 - 1);
+            // delta as the kernel will use it (a binary64 number); the deviation of the axis from f0[0] + i*delta is
+            // measured in extended precision and, times the largest D*T, must stay below 2^-34 bin.  The kernel's own
+            // roundings of lane*delta and 32*delta*c are relative 2^-53 errors on less than a window: far below that.
+            const double d = (double)(((long double)g->f0[g->n_f0 - 1] - (long double)g->f0[0]) / (long double)(g->n_f0 - 1));
             long double dev = 0;
             for (int i = 0; i < g->n_f0; ++i)
-                dev = std::max(dev, fabsl((long double)g->f0[i] - ((long double)g->f0[0] + (long double)i * delta)));
-            const double d = (double)delta;
-            // delta must be exact in binary64 and lane*delta, 32*delta exact as well (8 spare mantissa bits)
-            const bool exact = (long double)d == delta && std::fabs(std::remainder(std::ldexp(d, 44 - std::ilogb(d)), 1.0)) == 0.0;
-            if (exact && (double)dev * p.dmaxT <= 0x1p-34) {
+                dev = std::max(dev, fabsl((long double)g->f0[i] - ((long double)g->f0[0] + (long double)i * (long double)d)));
+            if (d > 0 && (double)dev * p.dmaxT <= 0x1p-34) {
                 p.d32 = 32.0 * d;
                 thr_units += 2.0;
             }
@@ -933,9 +933,9 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
             if (p.d32 != 0.0) w_bins = std::max(w_bins, (long)std::floor((32 * all[c] - 1) * (p.d32 / 32.0) * p.dmaxT) + 3);
             if (w_bins > tcw::PAD_BINS) continue;
             const int sb = slot_bytes_for(h->fmt_dev, w_bins);
-            // rings two slots deep (a slot is RB rows) hide the L2 latency; three CTAs of four warps per SM
-            const int per_sm = 12 / tcw::NW;
-            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : 2; s >= 2; --s) {
+            // rings holding at least six rows per warp (a slot is RB rows) hide the L2 latency; TCW_MINB CTAs of four warps per SM
+            const int per_sm = TCW_MINB;
+            for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : (tcw::RB >= 4 ? 2 : 6 / tcw::RB); s >= 2; --s) {
                 const size_t b = tcw::staged_smem_bytes(s, sb, 32 * all[c], wgt);
                 if (b <= SMEM_MAX / per_sm - 1024 || (s == 2 && b <= SMEM_MAX)) {
                     kernel = 2; r = all[c]; stages = s; slot = sb; smem = b;
@@ -1359,11 +1359,13 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
         unsigned int *z_cnt = z_off + tcw::SEL_MAX_BLOCKS;
         unsigned int *z_hist = z_cnt + tcw::SEL_MAX_BLOCKS;
         tcw::sel_sample_kernel<<<1, 1024, 0, st>>>(v, n, dtype, sc.state);
-        tcw::sel_zoom_hist_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, sc.hist, z_hist);
+        if (dtype) tcw::sel_zoom_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist);
+        else tcw::sel_zoom_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist);
         tcw::sel_zoom_pick_kernel<<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, dtype);
         tcw::sel_zoom_count_kernel<<<(nb + 7) / 8, 256, 0, st>>>(z_hist, nb, sc.state, z_cnt);
         tcw::sel_zoom_scan_kernel<<<1, 256, 0, st>>>(z_cnt, nb, z_off);
-        tcw::sel_zoom_compact_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, z_off, z_bits, z_idx);
+        if (dtype) tcw::sel_zoom_compact_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_bits, z_idx);
+        else tcw::sel_zoom_compact_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_bits, z_idx);
         run_select(z_bits, tcw::SEL_MAX_CAND, 2, z_idx);
         run_select(v, n, 1, nullptr);
     } else {

@@ -275,8 +275,12 @@ sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, Sel
 
 // Pass A: histogram of the zoom bins over all keys; every CTA also stores its own histogram (2048 words)
 // so that the candidates of pass B can be placed in index order without another read of the array.
+// Almost every key lies below the zoom window (bin 0): one compare per value settles those, branch-free,
+// and counts them in a register; only iterations that hold a value in or above the window take the key
+// arithmetic and the shared-memory atomics.
+template <int IS_INT>
 __global__ void __launch_bounds__(SEL_THREADS)
-sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
+sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int vec,
                      const SelState *__restrict__ state, unsigned int *__restrict__ hist, unsigned int *__restrict__ blk_hist)
 {
     __shared__ unsigned int h[2048];
@@ -284,30 +288,31 @@ sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, in
     __syncthreads();
     const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, vlo = state->z_val_lo;
     const SelSeg sg = sel_segment(n, seg);
-    unsigned int *hc = h;      // one copy: the keys that reach the atomics are the few in and above the window
-    // almost every key lies below the zoom window (bin 0): those are counted in a register, not by
-    // thousands of atomics on one shared-memory word
     unsigned int below = 0;
     for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
-        unsigned int b0[4], b1[4];
-        int n0, n1;
-        sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, n0);
-        sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, n1);
+        unsigned int b[8];
+        int nv[2];
+        {
+            unsigned int b0[4], b1[4];
+            sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, nv[0]);
+            sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, nv[1]);
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            // one compare settles the values below the window; only the tail pays for the key arithmetic
-            if (c < n0) {
-                if (sel_raw_below(b0[c], vlo, is_int)) ++below;
-                else if (sel_valid(b0[c], is_int)) {
-                    const unsigned int d = sel_zoom_bin(sel_key(b0[c], is_int), zs, zt, zp);
-                    if (d) atomicAdd(&hc[d], 1u); else ++below;
-                }
-            }
-            if (c < n1) {
-                if (sel_raw_below(b1[c], vlo, is_int)) ++below;
-                else if (sel_valid(b1[c], is_int)) {
-                    const unsigned int d = sel_zoom_bin(sel_key(b1[c], is_int), zs, zt, zp);
-                    if (d) atomicAdd(&hc[d], 1u); else ++below;
+            for (int c = 0; c < 4; ++c) { b[c] = b0[c]; b[4 + c] = b1[c]; }
+        }
+        unsigned int rest = 0;                                  // bit c: value c needs the exact path
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            const bool inr = (c & 3) < nv[c >> 2];
+            const bool lt = sel_raw_below(b[c], vlo, IS_INT);
+            below += (inr && lt) ? 1u : 0u;
+            rest |= (inr && !lt) ? (1u << c) : 0u;
+        }
+        if (rest) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                if ((rest >> c & 1u) && sel_valid(b[c], IS_INT)) {
+                    const unsigned int d = sel_zoom_bin(sel_key(b[c], IS_INT), zs, zt, zp);
+                    if (d) atomicAdd(&h[d], 1u); else ++below;
                 }
             }
         }
@@ -397,9 +402,12 @@ sel_zoom_scan_kernel(const unsigned int *__restrict__ blk_cnt, int n_blocks, uns
     }
 }
 
-// Pass B: the keys in bins >= z_bin with their indices, in index order, into the candidate buffer
+// Pass B: the keys in bins >= z_bin with their indices, in index order, into the candidate buffer.
+// One compare per value rules out everything below the lowest value of that bin; a tile pair without a
+// possible candidate costs two vector loads and one barrier.
+template <int IS_INT>
 __global__ void __launch_bounds__(SEL_THREADS)
-sel_zoom_compact_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
+sel_zoom_compact_kernel(const unsigned int *__restrict__ vals, long n, long seg, int vec,
                         const SelState *__restrict__ state, const unsigned int *__restrict__ blk_off,
                         unsigned int *__restrict__ cand_bits, long long *__restrict__ cand_idx)
 {
@@ -408,27 +416,40 @@ sel_zoom_compact_kernel(const unsigned int *__restrict__ vals, long n, long seg,
     const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, d0 = state->z_bin, vbin = state->z_val_bin;
     unsigned int base = blk_off[blockIdx.x];
     const SelSeg sg = sel_segment(n, seg);
-    for (long t0 = sg.begin; t0 < sg.end; t0 += SEL_TILE) {
-        const long i = t0 + 4 * threadIdx.x;
-        unsigned int b[4];
-        int nv;
-        bool take[4];
-        sel_load4(vals, i, sg.end, vec != 0, b, nv);
-        unsigned int c = 0;
+    for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
+        unsigned int b[8];
+        int nv[2];
+        {
+            unsigned int b0[4], b1[4];
+            sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, nv[0]);
+            sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, nv[1]);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            // values below the lowest value of bin d0 cannot be candidates (d0 = 0: every selectable value is one)
-            take[q] = q < nv && (d0 == 0u || !sel_raw_below(b[q], vbin, is_int)) && sel_valid(b[q], is_int) &&
-                      sel_zoom_bin(sel_key(b[q], is_int), zs, zt, zp) >= d0;
-            c += take[q];
+            for (int c = 0; c < 4; ++c) { b[c] = b0[c]; b[4 + c] = b1[c]; }
         }
-        if (!__syncthreads_or((int)c)) continue;
-        unsigned int tot;
-        unsigned int r = sel_block_scan(c, wt, tot);
+        unsigned int maybe = 0;
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (take[q]) { cand_bits[base + r] = b[q]; cand_idx[base + r] = i + q; ++r; }
-        base += tot;
+        for (int c = 0; c < 8; ++c)
+            maybe |= ((c & 3) < nv[c >> 2] && (d0 == 0u || !sel_raw_below(b[c], vbin, IS_INT))) ? (1u << c) : 0u;
+        if (!__syncthreads_or((int)maybe)) continue;
+        // some thread of the CTA may hold a candidate: exact test, then the two tiles in index order
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            bool take[4];
+            unsigned int cnt = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int c = 4 * half + q;
+                take[q] = (maybe >> c & 1u) && sel_valid(b[c], IS_INT) && sel_zoom_bin(sel_key(b[c], IS_INT), zs, zt, zp) >= d0;
+                cnt += take[q];
+            }
+            unsigned int tot;
+            unsigned int r = sel_block_scan(cnt, wt, tot);
+            const long i = t0 + (long)half * SEL_TILE + 4 * threadIdx.x;
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (take[q]) { cand_bits[base + r] = b[4 * half + q]; cand_idx[base + r] = i + q; ++r; }
+            base += tot;
+        }
     }
 }
 

@@ -358,10 +358,16 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t a)
 }
 
 template <int FMT, int R, bool TPOW2, bool WGT, bool UNI>
-__global__ void __launch_bounds__(STAGED_THREADS, 12 / NW)
+#ifndef TCW_MINB
+#define TCW_MINB (12 / TCW_NW)
+#endif
+__global__ void __launch_bounds__(STAGED_THREADS, TCW_MINB)
 sum_staged_kernel(const SumParams p)
 {
-    constexpr bool PAIR = RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
+#ifndef TCW_PAIR
+#define TCW_PAIR 1
+#endif
+    constexpr bool PAIR = TCW_PAIR && RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
                                                    // per-lane weight sums leave no registers for that)
     typedef typename AccW<FMT, WGT>::type V;
     typedef typename MetaT<WGT>::type Meta;

@@ -184,6 +184,30 @@ def test_search_groups_equals_slices_of_the_whole_search(tcw):
     assert_stat_parity(w, stat.reshape(-1), ref.stat)
 
 
+def test_search_groups_count_formats_across_sky_blocks(tcw):
+    """Group ranges of a 40-sky-point uint8 grid: the whole search runs on the sky-block kernel, a range is
+    served by whole-sky sub-grids (sky-block kernel) plus partial sky points (staged kernel); counts are exact
+    integers, so every slice must be identical whichever kernels produced it."""
+    import torch
+    rng = np.random.default_rng(17)
+    w = tcw_inputs.make_workload("cfg1").with_format("u8")
+    w.sky = tcw_inputs.fibonacci_cap(40, 1.0, 0.3, 10.0)
+    grid = tcw.Grid.of(w)
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(grid)
+        torch.cuda.synchronize()
+        assert h.info()["kernel"] == "skyblock"
+        stat = stat.reshape(-1, len(w.f0)).cpu().numpy()
+        best = best.cpu().numpy()
+        for g0, g1 in [(0, grid.n_groups), (5, 12 * 30 + 7), (12 * 3, 12 * 29)] + \
+                [tuple(sorted(rng.choice(grid.n_groups + 1, size=2, replace=False))) for _ in range(6)]:
+            s, b = h.search_groups(grid, int(g0), int(g1))
+            h.check()
+            assert np.array_equal(s.cpu().numpy(), stat[g0:g1]) and np.array_equal(b.cpu().numpy(), best[g0:g1]), (g0, g1)
+    ref = oracle.evaluate(w, sel=oracle.group_templates(w, np.array([0, 77, grid.n_groups - 1])))
+    assert np.array_equal(stat[[0, 77, grid.n_groups - 1]].reshape(-1).astype(np.int64), ref.stat)
+
+
 def test_search_host_overlapped_read_back_is_bit_identical(tcw):
     """An out_stat of more than 64 MiB goes to the host tau range by tau range while the later ranges are
     still being searched (tcw_search_host: per-range progress counters + cuStreamWaitValue32); the host
