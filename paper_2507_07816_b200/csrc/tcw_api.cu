@@ -1431,7 +1431,9 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     if (format != TCW_F32_POWER && std::isnan(prep->threshold)) return fail(TCW_EINVAL, "threshold is NaN");
     if (out_pitch_bytes < (long)row_bytes(format, prep->n_bins) || (format != TCW_U8_COUNT && (out_pitch_bytes & 3)))
         return fail(TCW_EINVAL, "out_pitch_bytes is smaller than one row or not a multiple of 4");
-    const size_t smem = (((size_t)(prep->n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)prep->n_bins + 31) & ~(size_t)31);
+    int spc = tcw::PREP_SPC;                        // SFTs per CTA: as many as leave room for two CTAs per SM
+    while (spc > 1 && spc * tcw::prep_sft_smem(prep->n_bins, h) > SMEM_MAX / 2 - 1024) spc /= 2;
+    const size_t smem = spc * tcw::prep_sft_smem(prep->n_bins, h);
     if (smem > SMEM_MAX) return fail(TCW_EUNSUPPORTED, "band too wide for one CTA's shared memory (%zu bytes)", smem);
 
     cudaStream_t st = (cudaStream_t)stream;
@@ -1503,7 +1505,7 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         p.out_format = format;
         p.out = (unsigned char *)out_spectrogram + j0 * out_pitch_bytes;
         p.out_pitch = out_pitch_bytes;
-        tcw::prep_normalise_kernel<<<nb, tcw::PREP_THREADS, smem, st>>>(p);
+        tcw::prep_normalise_kernel<<<(nb + spc - 1) / spc, tcw::PREP_THREADS, smem, st>>>(p, nb, spc);
         PREP_TRY(cudaGetLastError());
     }
     PREP_TRY(cudaStreamSynchronize(st));

@@ -9,7 +9,7 @@
 // The DFT itself is a plain batched real-to-complex transform and is left to cuFFT (a library
 // primitive, like a GEMM left to cuBLAS).  Everything around it is here:
 //   * prep_window_kernel: window multiply into the batch buffer cuFFT reads (float32);
-//   * prep_normalise_kernel: one CTA per SFT: |X|^2 of the band and its two half-windows into shared
+//   * prep_normalise_kernel: up to four SFTs per CTA: |X|^2 of the band and its two half-windows into shared
 //     memory, then every thread walks a run of consecutive bins keeping the running median by
 //     counting (see the kernel), and writes rho (float32), nu (uint8) or nu bit-packed (uint32
 //     words, LSB first) straight into the spectrogram layout tcw_create reads.  (A per-thread sliding
@@ -70,18 +70,34 @@ struct PrepParams {
     long out_pitch;         // bytes
 };
 
-// dynamic shared memory: float P[n_bins + 2h], then (count formats) unsigned char nu[n_bins rounded up to 32]
-__global__ void __launch_bounds__(256)
-prep_normalise_kernel(const PrepParams p)
+// One CTA normalises spc SFTs (4 when their bands fit two CTAs' worth of shared memory, else 2 or 1), 256/spc
+// threads each: the selection of a thread's first window costs as much as thirteen slides, so long runs (few
+// threads per SFT) pay, and several SFTs per CTA keep the SM full.  Dynamic shared memory per SFT:
+// float P[n_bins + 2h] (16-byte rounded), then (count formats) unsigned char nu[n_bins rounded up to 32].
+constexpr int PREP_SPC = 4;
+__host__ __device__ inline size_t prep_sft_smem(int n_bins, int h)
+{
+    return ((((size_t)(n_bins + 2 * h) * 4 + 15) & ~(size_t)15) + (((size_t)n_bins + 31) & ~(size_t)31) + 127) & ~(size_t)127;
+}
+
+__global__ void __launch_bounds__(PREP_THREADS)
+prep_normalise_kernel(const PrepParams p, int n_batch, int spc)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    float *P = (float *)smem;
+    const int tps = PREP_THREADS / spc;            // threads per SFT
+    const int sub = threadIdx.x / tps, t = threadIdx.x % tps;
+    const int sft = blockIdx.x * spc + sub;
+    unsigned char *mine = smem + (size_t)sub * prep_sft_smem(p.n_bins, p.h);
+    float *P = (float *)mine;
     const int n_in = p.n_bins + 2 * p.h;
-    unsigned char *nu = smem + (((size_t)n_in * 4 + 15) & ~(size_t)15);
-    const float2 *row = p.spec + (long)blockIdx.x * p.n_half + (p.k_min - p.h);
-    for (int t = threadIdx.x; t < n_in; t += (int)blockDim.x) {
-        const float2 c = row[t];
-        P[t] = c.x * c.x + c.y * c.y;
+    unsigned char *nu = mine + (((size_t)n_in * 4 + 15) & ~(size_t)15);
+    const bool live = sft < n_batch;
+    if (live) {
+        const float2 *row = p.spec + (long)sft * p.n_half + (p.k_min - p.h);
+        for (int q = t; q < n_in; q += tps) {
+            const float2 c = row[q];
+            P[q] = c.x * c.x + c.y * c.y;
+        }
     }
     __syncthreads();
 
@@ -93,10 +109,10 @@ prep_normalise_kernel(const PrepParams p)
     // or the smallest element above it.  All reads are conflict-free shared-memory loads.
     const int W = 2 * p.h + 1, h = p.h;
     // an odd run length: lanes then start 'run' words apart, which visits all 32 banks (no conflicts)
-    const int run = ((p.n_bins + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
-    const int k0 = min((int)threadIdx.x * run, p.n_bins), k1 = min(k0 + run, p.n_bins);
-    unsigned char *orow = p.out + (long)blockIdx.x * p.out_pitch;
-    if (k0 < k1) {
+    const int run = ((p.n_bins + tps - 1) / tps) | 1;
+    const int k0 = min(t * run, p.n_bins), k1 = min(k0 + run, p.n_bins);
+    unsigned char *orow = p.out + (long)sft * p.out_pitch;
+    if (live && k0 < k1) {
         const unsigned int *Pu = (const unsigned int *)P;
         unsigned int key = 0;
         for (int bit = 30; bit >= 0; --bit) {
@@ -105,22 +121,23 @@ prep_normalise_kernel(const PrepParams p)
             for (int q = 0; q < W; ++q) c += Pu[k0 + q] < cand;
             if (c <= h) key = cand;
         }
-        float m = __uint_as_float(key);
+        // the re-count works on the float bits: per window element two compares and four predicated integer instructions
+        unsigned int mu = key;
         for (int k = k0; k < k1; ++k) {
             if (k > k0) {
-                int c_less = 0, c_leq = 0;
-                float pred = -__int_as_float(0x7f800000), succ = __int_as_float(0x7f800000);
+                int c_less = 0, c_gt = 0;
+                unsigned int pred = 0u, succ = 0xffffffffu;
+                const unsigned int *wq = Pu + k;
+#pragma unroll 4
                 for (int q = 0; q < W; ++q) {
-                    const float x = P[k + q];
-                    const bool lt = x < m, gt = x > m;
-                    c_less += lt;
-                    c_leq += !gt;
-                    pred = fmaxf(pred, lt ? x : pred);
-                    succ = fminf(succ, gt ? x : succ);
+                    const unsigned int x = wq[q];
+                    if (x < mu) { ++c_less; pred = max(pred, x); }
+                    if (x > mu) { ++c_gt; succ = min(succ, x); }
                 }
-                if (c_less > h) m = pred;
-                else if (c_leq <= h) m = succ;
+                if (c_less > h) mu = pred;
+                else if (W - c_gt <= h) mu = succ;
             }
+            const float m = __uint_as_float(mu);
             const float rho = P[k + h] * 0.69314718055994531f / m;
             if (p.out_format == 0) ((float *)orow)[k] = rho;
             else nu[k] = rho > p.threshold ? 1 : 0;
@@ -128,11 +145,12 @@ prep_normalise_kernel(const PrepParams p)
     }
     if (p.out_format == 0) return;
     __syncthreads();
+    if (!live) return;
     if (p.out_format == 1) {
-        for (int k = threadIdx.x; k < p.n_bins; k += (int)blockDim.x) orow[k] = nu[k];
+        for (int k = t; k < p.n_bins; k += tps) orow[k] = nu[k];
     } else {
         const int n_words = (p.n_bins + 31) / 32;
-        for (int wd = threadIdx.x; wd < n_words; wd += (int)blockDim.x) {
+        for (int wd = t; wd < n_words; wd += tps) {
             uint32_t bits = 0;
             for (int b = 0; b < 32; ++b) {
                 const int k = 32 * wd + b;
