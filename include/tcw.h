@@ -403,7 +403,7 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
  * 4 bank),
  * info[1] templates per CTA tile, info[2] CTAs launched, info[3] dynamic shared memory bytes,
  * info[4] device status word (0 = ok; nonzero = an internal window-bound check failed),
- * info[5] kernels launched by the call, info[6] ring depth per warp (slots of two SFT rows in the staged kernel), info[7] sky points per
+ * info[5] kernels launched by the call, info[6] ring depth per warp (slots of four SFT rows in the staged kernel), info[7] sky points per
  * block (sky-block kernel, else 0), info[8] SFT chunks of the staged kernel (1 = not chunked),
  * info[9] SFT rows per chunk, info[10] tau ranges of the progressive read-back of the last search (tcw_search_host
  * with a large out_stat; 0 = none), info[11] reserved (0).

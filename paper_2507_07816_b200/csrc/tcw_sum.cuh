@@ -645,7 +645,11 @@ sum_staged_kernel(const SumParams p)
                 // the usual case, every row of the slot is live: two rows per straight-line block, so the
                 // index arithmetic of one row overlaps the shared-memory gathers of the other.  The guard-band
                 // branch repeats the gathers instead of merging, which keeps the fast path free of register moves.
+#ifdef TCW_PAIR_LOOP
+#pragma unroll 1
+#else
 #pragma unroll
+#endif
                 for (int q = 0; q < RB; q += 2) {
                     const uint32_t mq0 = meta_c + (uint32_t)(q * MB), mq1 = mq0 + (uint32_t)MB;
                     uint32_t hi0[R], hi1[R];
