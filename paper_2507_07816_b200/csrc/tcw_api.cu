@@ -638,8 +638,13 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
         // bit-packed input: stage the words on the device, then expand to one byte per bin
         const size_t wrow = row_bytes(format, n_bins);
         CREATE_TRY(dev_alloc(&d_words, wrow * n_sft, st));
-        CREATE_TRY(cudaMemcpy2DAsync(d_words, wrow, spectrogram, (size_t)row_pitch_bytes, wrow, (size_t)n_sft,
-                                     cudaMemcpyDefault, st));
+        // contiguous rows travel in one piece: a strided copy of 10 800 rows of 500 bytes from the host
+        // costs about 4 ms on B200 against 0.2 ms for the same 5.4 MB in one transfer
+        if ((size_t)row_pitch_bytes == wrow)
+            CREATE_TRY(cudaMemcpyAsync(d_words, spectrogram, wrow * n_sft, cudaMemcpyDefault, st));
+        else
+            CREATE_TRY(cudaMemcpy2DAsync(d_words, wrow, spectrogram, (size_t)row_pitch_bytes, wrow, (size_t)n_sft,
+                                         cudaMemcpyDefault, st));
         const long total = (long)n_sft * n_bins;
         const unsigned blocks = (unsigned)std::min<long>((total + 255) / 256, 148L * 16);
         tcw::expand_bits_kernel<<<blocks, 256, 0, st>>>((const uint32_t *)d_words, (long)(wrow / 4), n_sft, n_bins,

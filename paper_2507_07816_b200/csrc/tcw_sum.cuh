@@ -254,6 +254,16 @@ __device__ __forceinline__ float lds_f32(uint32_t a)
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
     return v;
 }
+// two float32 additions in one instruction (add.rn.f32x2, SASS FADD2): each half rounds exactly like a scalar
+// __fadd_rn, so results are bit-identical to the scalar form; the kernel is bound by instruction issue
+__device__ __forceinline__ void fadd2(float &o0, float &o1, float a0, float a1, float b0, float b1)
+{
+    unsigned long long a, b, r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(a0), "f"(a1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(b0), "f"(b1));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(o0), "=f"(o1) : "l"(r));
+}
 __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 {
     uint32_t v;
@@ -366,6 +376,9 @@ sum_staged_kernel(const SumParams p)
 {
 #ifndef TCW_PAIR
 #define TCW_PAIR 1
+#endif
+#ifndef TCW_FADD2
+#define TCW_FADD2 1
 #endif
     constexpr bool PAIR = TCW_PAIR && RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
                                                    // per-lane weight sums leave no registers for that)
@@ -672,11 +685,22 @@ sum_staged_kernel(const SumParams p)
                         // gathers do not wait for the minimum; only the accumulate does.  Fixed order:
                         // acc += (row q + row q+1).
                         V t[R];
+                        if constexpr (FMT == FMT_F32 && TCW_FADD2) {
+                            float v0[R], v1[R];
 #pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const uint32_t a0 = addr0 + (hi0[r] << SH), a1 = addr0 + (hi1[r] << SH);
-                            if (FMT == FMT_F32) t[r] = lds_f32(a0) + lds_f32(a1);
-                            else t[r] = (V)(lds_u8(a0) + lds_u8(a1));
+                            for (int r = 0; r < R; ++r) {
+                                v0[r] = lds_f32(addr0 + (hi0[r] << SH));
+                                v1[r] = lds_f32(addr0 + (hi1[r] << SH));
+                            }
+#pragma unroll
+                            for (int r = 0; r < R; r += 2) fadd2(t[r], t[r + 1], v0[r], v0[r + 1], v1[r], v1[r + 1]);
+                        } else {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const uint32_t a0 = addr0 + (hi0[r] << SH), a1 = addr0 + (hi1[r] << SH);
+                                if (FMT == FMT_F32) t[r] = lds_f32(a0) + lds_f32(a1);
+                                else t[r] = (V)(lds_u8(a0) + lds_u8(a1));
+                            }
                         }
                         if (min(mn0, mn1) <= p.thr2) {
                             uint32_t ex0[R], ex1[R];
@@ -689,8 +713,13 @@ sum_staged_kernel(const SumParams p)
                                 else t[r] = (V)(lds_u8(a0) + lds_u8(a1));
                             }
                         }
+                        if constexpr (FMT == FMT_F32 && TCW_FADD2) {
 #pragma unroll
-                        for (int r = 0; r < R; ++r) acc[r] += t[r];
+                            for (int r = 0; r < R; r += 2) fadd2(acc[r], acc[r + 1], acc[r], acc[r + 1], t[r], t[r + 1]);
+                        } else {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) acc[r] += t[r];
+                        }
                     }
                 }
             } else {
