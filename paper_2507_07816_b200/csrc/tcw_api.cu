@@ -192,6 +192,39 @@ bool is_pow2(double x)
     return x > 0 && std::isfinite(x) && std::frexp(x, &e) == 0.5;
 }
 
+// The library's copy of the spectrogram as a rank-3 tensor [n_sft][pitch/128][128 bytes] and, for n = 1 .. BOX_SEG_MAX,
+// the map whose box is {128 bytes, n segments, RB rows}: the RB consecutive SFT rows of one ring slot of the staged kernel,
+// n*128 bytes of each, in ONE TMA copy (cp.async.bulk.tensor.3d).  maps[0] is unused.  Out-of-range parts of a box read as
+// zero.  cuTensorMapEncodeTiled is fetched at run time (no link dependency on libcuda).
+constexpr int BOX_SEG_MAX = 31;
+bool encode_box_maps(const void *base, long pitch, int n_sft, std::vector<CUtensorMap> &maps)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = [] {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            fn = nullptr;
+        cudaGetLastError();
+        return (encode_fn)fn;
+    }();
+    if (!encode || pitch % 128 != 0 || ((uintptr_t)base & 127) != 0) return false;
+    maps.assign(BOX_SEG_MAX + 1, CUtensorMap());
+    const cuuint64_t dims[3] = {128, (cuuint64_t)(pitch / 128), (cuuint64_t)n_sft};
+    const cuuint64_t strides[2] = {128, (cuuint64_t)pitch};
+    const cuuint32_t es[3] = {1, 1, 1};
+    for (int n = 1; n <= BOX_SEG_MAX; ++n) {
+        const cuuint32_t box[3] = {128, (cuuint32_t)n, (cuuint32_t)tcw::RB};
+        if (encode(&maps[n], CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(base), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
+    }
+    return true;
+}
+
 }  // namespace
 
 struct tcw_handle {
@@ -208,6 +241,8 @@ struct tcw_handle {
     double vmid[3] = {0, 0, 0};  // velocity at the middle SFT: sort key of the sky-block kernel
     std::vector<double> ts;
     unsigned char *d_spec = nullptr;
+    unsigned char *d_tmaps = nullptr;  // staged kernel: CUtensorMap n at d_tmaps + 128*n, box {128 bytes, n segments, RB rows}
+    int max_seg = 0;                   // ... for n = 1 .. max_seg (0: no tensor maps, 1-D bulk copies only)
     double *d_ts = nullptr, *d_vel = nullptr;
     // grow-only scratch
     DevBuf<double> d_g, d_d, d_axes;
@@ -393,6 +428,8 @@ tcw::SumParams base_params(const tcw_handle *h, const tcw_grid *g)
     p.spec_pad = h->d_spec;
     p.pad_bytes = h->pad_bytes;
     p.pitch = h->pitch;
+    p.tmaps = h->d_tmaps;
+    p.max_seg = h->max_seg;
     p.n_sft = h->n_sft;
     p.n_bins = h->n_bins;
     p.k_min = h->k_min;
@@ -452,15 +489,18 @@ long max_window_bins(const tcw_grid *g, int tile, double dmaxT)
         int i1 = std::min(i0 + tile, g->n_f0) - 1;
         df = std::max(df, g->f0[i1] - g->f0[i0]);
     }
-    double w = std::floor(df * dmaxT) + 3.0;
+    // rint(x2) - rint(x1) <= floor(x2 - x1) + 1 for exact x; the relative 1e-9 covers the float64 error of the tracks
+    double w = std::floor(df * dmaxT * (1.0 + 1e-9) + 1e-6) + 2.0;
     return w > 1e9 ? (long)1e9 : (long)w;
 }
 
-// Bytes of one ring slot: the window's bins plus the 16-byte alignment slack at both ends.
-int slot_bytes_for(int fmt_dev, long w_bins)
+// Bytes of one staged row of a ring slot.  box = false: the window's bins plus the 16-byte alignment slack at both
+// ends (a 1-D bulk copy per row).  box = true: a whole number of 128-byte segments that holds the window wherever it
+// starts inside its first segment (one tensor-map copy per slot; the 1-D layout fits as well).
+int slot_bytes_for(int fmt_dev, long w_bins, bool box)
 {
-    long b = (fmt_dev == tcw::FMT_F32 ? 4 * w_bins : w_bins) + 32;
-    b = (b + 15) & ~15L;
+    const long wb = fmt_dev == tcw::FMT_F32 ? 4 * w_bins : w_bins;
+    long b = box ? (wb + 124 + 127) & ~127L : (wb + 32 + 15) & ~15L;
     return b > (1L << 30) ? (1 << 30) : (int)b;
 }
 
@@ -607,7 +647,8 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
     const size_t bpb = h->fmt_dev == tcw::FMT_F32 ? 4 : 1;
     const size_t dev_row = bpb * (size_t)n_bins;           // bytes of one row in the device format
     h->pad_bytes = (long)(bpb * tcw::PAD_BINS);            // multiple of 16
-    h->pitch = (long)(2 * (size_t)h->pad_bytes + ((dev_row + 15) & ~(size_t)15));
+    // a multiple of 128: the tensor maps of the staged kernel see a row as pitch/128 segments of 128 bytes
+    h->pitch = (long)((2 * (size_t)h->pad_bytes + dev_row + 127) & ~(size_t)127);
     cudaStream_t st = (cudaStream_t)stream;
     g_alloc_stream = st;
     h->last_stream = st;
@@ -634,6 +675,17 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
     CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
     CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));   // the padding must read as zero
+    {
+        // tensor maps of the staged kernel (SumParams::tmaps); without the driver entry point the kernel
+        // falls back to one 1-D bulk copy per row
+        std::vector<CUtensorMap> maps;
+        if (encode_box_maps(h->d_spec, h->pitch, n_sft, maps)) {
+            CREATE_TRY(dev_alloc((void **)&h->d_tmaps, maps.size() * sizeof(CUtensorMap), st));
+            CREATE_TRY(cudaMemcpyAsync(h->d_tmaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, st));
+            CREATE_TRY(cudaStreamSynchronize(st));     // `maps` is pageable host memory
+            h->max_seg = (int)maps.size() - 1;
+        }
+    }
     if (format == TCW_BIT_COUNT) {
         // bit-packed input: stage the words on the device, then expand to one byte per bin
         const size_t wrow = row_bytes(format, n_bins);
@@ -778,6 +830,7 @@ int tcw_destroy(tcw_handle *h)
     g_alloc_stream = h->last_stream;
     dev_free(h->up_staging, h->last_stream);
     dev_free(h->d_spec, h->last_stream);
+    dev_free(h->d_tmaps, h->last_stream);
     dev_free(h->d_ts, h->last_stream);
     dev_free(h->d_vel, h->last_stream);
     dev_free(h->d_status, h->last_stream);
@@ -935,9 +988,14 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
             long w_bins = max_window_bins(grid, 32 * all[c], p.dmaxT);
             // equally spaced f0: the lanes past the end of a ragged last tile still form addresses (their sums
             // are discarded), so every slot holds the window of a whole tile
-            if (p.d32 != 0.0) w_bins = std::max(w_bins, (long)std::floor((32 * all[c] - 1) * (p.d32 / 32.0) * p.dmaxT) + 3);
+            if (p.d32 != 0.0)
+                w_bins = std::max(w_bins, (long)std::floor((32 * all[c] - 1) * (p.d32 / 32.0) * p.dmaxT * (1.0 + 1e-9) + 1e-6) + 2);
             if (w_bins > tcw::PAD_BINS) continue;
-            const int sb = slot_bytes_for(h->fmt_dev, w_bins);
+            // one tensor-map copy per slot where the rows allow it (not for the weighted search: its wider row
+            // metadata leaves no shared memory for 128-byte granular rows at three CTAs per SM)
+            const bool box = !wgt && h->d_tmaps != nullptr;
+            if (!box) { p.tmaps = nullptr; p.max_seg = 0; }
+            const int sb = slot_bytes_for(h->fmt_dev, w_bins, box);
             // rings holding at least six rows per warp (a slot is RB rows) hide the L2 latency; TCW_MINB CTAs of four warps per SM
             const int per_sm = TCW_MINB;
             for (int s = h->opt_stages ? std::min(h->opt_stages, 8) : (tcw::RB >= 4 ? 2 : 6 / tcw::RB); s >= 2; --s) {

@@ -70,6 +70,11 @@ struct SumParams {
     void *cpart;                // chunked: float32 / int32 [n_chunks][n_groups][n_f0] partial sums
     unsigned char *clive;       // chunked: [n_chunks][n_groups][n_tiles] 1 where the CTA wrote its partial sums
     int *status;                // device status word
+    // staged kernel, one tensor-map copy per ring slot: tmaps + 128*n is the CUtensorMap whose box is
+    // {128 bytes, n segments, RB rows} over the library's copy seen as [n_sft][pitch/128][128 bytes]
+    // (n = 1 .. max_seg); NULL = every row travels by its own 1-D bulk copy
+    const unsigned char *tmaps;
+    int max_seg;
     // staged kernel, fast bin index (one fused multiply-add per lookup, see RowMeta below)
     double fix_add;             // 0.5 + thr, thr = thr2 / 2^33 bins
     double d32;                 // equally spaced f0 axis: 32 * spacing (Hz), else 0
@@ -247,6 +252,13 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// TMA tiled copy of a {128 bytes, n segments, RB rows} box of the spectrogram (tensor map `map`, coordinates
+// {0, segment, row}) into shared memory, completion counted in bytes on an mbarrier.  dst is 128-byte aligned.
+__device__ __forceinline__ void tensor3_g2s(uint32_t dst, const void *map, int seg, int row, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(map), "r"(0), "r"(seg), "r"(row), "r"(bar) : "memory");
 }
 __device__ __forceinline__ float lds_f32(uint32_t a)
 {
@@ -449,16 +461,18 @@ sum_staged_kernel(const SumParams p)
         if constexpr (!UNI) df[r] = __dsub_rn(p.f0[min(i0 + r * 32 + lane, i_last)], f_first);
         if (WGT) w1p[r] = w2p[r] = 0.0f;
     }
-    const int jw = j0 + warp;
-    const int n_rows = jw < j1 ? (j1 - jw + NW - 1) / NW : 0;
+    // warp w owns the ring slots w, w + NW, w + 2*NW, ... of the chunk; a slot is RB CONSECUTIVE SFT rows, so that one
+    // tensor-map copy can fetch it.  Row n of the warp (n = RB*slot + q) is SFT row_of(n); rows at or past j1 do not exist.
+    const int jw = j0 + RB * warp;
+    auto row_of = [&](int n) { return jw + (NW * RB) * (n / RB) + (n % RB); };
 
     // Row metadata is computed 32 rows at a time, one row per lane (rows 32*m + lane of this warp),
     // and written to the warp's metadata ring; (g, D) of the next batch are loaded ahead of use.
     double gn = 0, dn = 1;
     float wn = 1.0f;
-    if (lane < n_rows) {
-        gn = __ldg(g + jw + NW * lane); dn = __ldg(d + jw + NW * lane);
-        if (WGT && wr) wn = __ldg(wr + jw + NW * lane);
+    if (row_of(lane) < j1) {
+        gn = __ldg(g + row_of(lane)); dn = __ldg(d + row_of(lane));
+        if (WGT && wr) wn = __ldg(wr + row_of(lane));
     }
 
     int m_pos = lane;                            // (32*m + lane) mod MR: the row's place in the metadata ring
@@ -466,6 +480,7 @@ sum_staged_kernel(const SumParams p)
     const int slot_step = (32 / RB) % D;
     auto compute_batch = [&](int m) {
         const int n = 32 * m + lane;
+        const int jn = row_of(n);
         const double gj = gn, dj = dn;
         const double Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
         Meta mt;
@@ -475,42 +490,82 @@ sum_staged_kernel(const SumParams p)
         mt.by16 = -1;
         mt.src_lo = mt.src_hi = 0;
         if constexpr (WGT) { mt.w = wn; mt.full = 0; mt.ktest = 0; mt.pad = 0; }
-        if (n + 32 < n_rows) {
-            gn = __ldg(g + jw + NW * (n + 32)); dn = __ldg(d + jw + NW * (n + 32));
-            if (WGT && wr) wn = __ldg(wr + jw + NW * (n + 32));
+        if (jn + 32 * NW < j1) {          // row_of(n + 32) = jn + 32*NW
+            gn = __ldg(g + jn + 32 * NW); dn = __ldg(d + jn + 32 * NW);
+            if (WGT && wr) wn = __ldg(wr + jn + 32 * NW);
         }
         // once the highest template of the tile is below the band for the largest possible Doppler
         // factor, no later SFT can contribute
-        if (n < n_rows && !(f_last * gj * p.dmaxT < below)) {
-            const int lo_f = bin_lo<TPOW2>(f_first, gj, Dp, p.T);
-            const int kf = lo_f - p.k_min;
-            const int kl = bin_lo<TPOW2>(f_last, gj, Dp, p.T) - p.k_min;
+        int kf = 0, kl = -1, lo_f = 0;
+        bool bad = false;                                   // the row's own 1-D window breaks the host's bound
+        if (jn < j1 && !(f_last * gj * p.dmaxT < below)) {
+            lo_f = bin_lo<TPOW2>(f_first, gj, Dp, p.T);
+            kf = lo_f - p.k_min;
+            kl = bin_lo<TPOW2>(f_last, gj, Dp, p.T) - p.k_min;
             mt.by16 = 0;
             if (kl >= 0 && kf < p.n_bins) {
                 const int a_byte = (BPB * kf) & ~15;                 // rounds towards -inf: may reach into the left padding
                 const int e_byte = (BPB * (kl + 1) + 15) & ~15;
-                if (e_byte - a_byte > p.slot_limit || kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
+                if (kf < -PAD_BINS || kl >= p.n_bins + PAD_BINS) {
                     atomicOr(p.status, 1);  // host-side window bound violated: the search reports TCW_EINTERNAL
                 } else {
-                    const long src = (long)(jw + NW * n) * p.pitch + p.pad_bytes + a_byte;
-                    mt.src_lo = (uint32_t)src;
-                    mt.src_hi = (uint32_t)(src >> 32);
+                    bad = e_byte - a_byte > p.slot_limit;
                     mt.by16 = e_byte - a_byte;
-                    const uint32_t S = slots_s + (uint32_t)m_slot * slot_stride + (uint32_t)(lane % RB) * (uint32_t)p.slot_bytes;
-                    // byte address of band-relative bin b: S + BPB*b - a_byte (S and a_byte are multiples of 16), so the
-                    // tile's first bin kf sits at element W = (S - a_byte)/BPB + kf of shared memory (W < 2^16)
-                    const int W = (((int)S - a_byte) >> SH) + kf;     // exact: (S - a_byte) is a multiple of 16, kf - a_byte/BPB >= 0
-                    mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add + (double)W), TCW_FIX_BASE);
-                    if constexpr (WGT) {
-                        mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
-                        mt.ktest = (uint32_t)(kf - W) - FIX_HC;
-                    }
                 }
+            }
+        }
+        // A slot whose RB rows are all live and whose windows fit one {128 B x nseg x RB} box travels by ONE
+        // tensor-map copy (the rows of a slot are consecutive in memory and the track drifts slowly); otherwise
+        // (band edges, gaps in the data, the steep start of a fast spin-down) every row gets its own 1-D copy.
+        bool use2d = false;
+        int seg0 = 0, nseg = 0;
+        if (p.tmaps) {
+            int kfm = mt.by16 > 0 ? kf : INT32_MAX, klm = mt.by16 > 0 ? kl : INT32_MIN;
+            bool all = mt.by16 > 0;
+#pragma unroll
+            for (int o = 1; o < RB; o <<= 1) {
+                kfm = min(kfm, __shfl_xor_sync(0xffffffffu, kfm, o));
+                klm = max(klm, __shfl_xor_sync(0xffffffffu, klm, o));
+                all = __shfl_xor_sync(0xffffffffu, (int)all, o) && all;
+            }
+            if (all) {
+                seg0 = ((int)p.pad_bytes + BPB * kfm) >> 7;
+                nseg = (((int)p.pad_bytes + BPB * (klm + 1) + 127) >> 7) - seg0;
+                use2d = nseg <= p.max_seg && nseg * 128 <= p.slot_limit;
+            }
+        }
+        if (mt.by16 > 0 && bad && !use2d) {
+            atomicOr(p.status, 1);
+            mt.by16 = 0;
+        }
+        if (mt.by16 > 0) {
+            const int a_byte = use2d ? 128 * seg0 - (int)p.pad_bytes : (BPB * kf) & ~15;   // first staged byte, relative to bin 0
+            const uint32_t row_stride = use2d ? (uint32_t)(128 * nseg) : (uint32_t)p.slot_bytes;
+            const long src = (long)jn * p.pitch + p.pad_bytes + a_byte;
+            mt.src_lo = (uint32_t)src;
+            mt.src_hi = (uint32_t)(src >> 32);
+            const uint32_t S = slots_s + (uint32_t)m_slot * slot_stride + (uint32_t)(lane % RB) * row_stride;
+            // byte address of band-relative bin b: S + BPB*b - a_byte (both multiples of BPB), so the tile's
+            // first bin kf sits at element W = (S - a_byte)/BPB + kf of shared memory (W < 2^16)
+            const int W = (((int)S - a_byte) >> SH) + kf;
+            mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add + (double)W), TCW_FIX_BASE);
+            if constexpr (WGT) {
+                mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
+                mt.ktest = (uint32_t)(kf - W) - FIX_HC;
             }
         }
         // the first row of every ring slot carries the slot's summary for the consumer
         const unsigned live = __ballot_sync(0xffffffffu, mt.by16 > 0);
         mt.flags = ((live >> (lane & ~(RB - 1))) & ((1u << RB) - 1u)) | (mt.by16 < 0 ? 256u : 0u);
+        if (use2d) {
+            // the slot's first row carries the box: bytes the copy delivers, first segment, first SFT row
+            mt.flags |= 512u | ((uint32_t)nseg << 16);
+            if (lane % RB == 0) {
+                mt.by16 = 128 * nseg * RB;
+                mt.src_lo = (uint32_t)seg0;
+                mt.src_hi = (uint32_t)jn;
+            }
+        }
         meta[m_pos] = mt;
         m_pos += 32;
         if (m_pos >= MR) m_pos -= MR;
@@ -528,14 +583,27 @@ sum_staged_kernel(const SumParams p)
         if (elect_one()) {
             uint32_t u[RB], lo[RB], hi[RB];
             int by[RB], tot = 0;
-#pragma unroll
-            for (int q = 0; q < RB; ++q) {
+            {
                 uint32_t b;
-                lds_v4(meta_i + (uint32_t)(q * MB) + 16u, u[q], b, lo[q], hi[q]);
-                by[q] = (int)b;
-                tot += max(by[q], 0);
+                lds_v4(meta_i + 16u, u[0], b, lo[0], hi[0]);
+                by[0] = (int)b;
             }
-            if (tot > 0) {
+            if (u[0] & 512u) {
+                mbar_arrive_expect_tx(bar_i, (uint32_t)by[0]);
+                tensor3_g2s(slot_i, p.tmaps + ((u[0] >> 16) << 7), (int)lo[0], (int)hi[0], bar_i);
+                tot = -1;
+            } else {
+                tot = max(by[0], 0);
+#pragma unroll
+                for (int q = 1; q < RB; ++q) {
+                    uint32_t b;
+                    lds_v4(meta_i + (uint32_t)(q * MB) + 16u, u[q], b, lo[q], hi[q]);
+                    by[q] = (int)b;
+                    tot += max(by[q], 0);
+                }
+            }
+            if (tot < 0) {
+            } else if (tot > 0) {
                 mbar_arrive_expect_tx(bar_i, (uint32_t)tot);
 #pragma unroll
                 for (int q = 0; q < RB; ++q)
@@ -593,13 +661,17 @@ sum_staged_kernel(const SumParams p)
     };
     // the same indices by the defining chain (bin_lo): taken where a lookup of this lane lies within thr of a
     // rounding boundary, or always when the fast index is switched off.  S = shared address of the row's slot.
-    auto exact_row = [&](int n, uint32_t S, uint32_t (&hi)[R]) {
-        const int j = jw + NW * n;
+    auto exact_row = [&](int n, uint32_t mc, uint32_t sc_, uint32_t (&hi)[R]) {
+        const int j = row_of(n);
         const double gj = __ldg(g + j), dj = __ldg(d + j);
         const double Dp = TPOW2 ? __dmul_rn(dj, p.T) : dj;
         const int lo_f = bin_lo<TPOW2>(f_first, gj, Dp, p.T);
         const int kf = lo_f - p.k_min;
-        const int a_byte = (BPB * kf) & ~15;
+        // where the row was staged: mc = metadata of the slot's first row, sc_ = the slot's first byte
+        const uint32_t fl = lds_u32(mc + 16u);
+        const bool box = (fl & 512u) != 0;
+        const int a_byte = box ? 128 * (int)lds_u32(mc + 24u) - (int)p.pad_bytes : (BPB * kf) & ~15;
+        const uint32_t S = sc_ + (uint32_t)(n % RB) * (box ? ((fl >> 16) << 7) : (uint32_t)p.slot_bytes);
         const uint32_t base = FIX_HC + (uint32_t)((((int)S - a_byte) >> SH) + kf) - (uint32_t)lo_f;
 #pragma unroll
         for (int r = 0; r < R; ++r)
@@ -650,8 +722,9 @@ sum_staged_kernel(const SumParams p)
     int sc = 0, nc = 0;   // slot of the ring and slot count of the consumer
     for (;;) {
         stage_next();     // refills the slot consumed in the previous iteration
-        const uint32_t flags = lds_u32(meta_c + 16u);     // bit q: row q of the slot is staged; bit 8: no further rows
-        if (flags & 256u) break;
+        const uint32_t flags_w = lds_u32(meta_c + 16u);   // bit q: row q of the slot is staged; bit 8: no further rows;
+        if (flags_w & 256u) break;                        // bit 9 and bits 16-23: one box copy of that many segments
+        const uint32_t flags = flags_w & 255u;
         if (flags) {
             mbar_wait(bar_c, ph);
             if (PAIR && flags == (1u << RB) - 1u) {
@@ -671,8 +744,8 @@ sum_staged_kernel(const SumParams p)
                     if constexpr (WGT || !UNI) {
                         if (min(mn0, mn1) <= p.thr2) {
                             uint32_t ex0[R], ex1[R];
-                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex0);
-                            exact_row(RB * nc + q + 1, slot_c + (uint32_t)((q + 1) * p.slot_bytes), ex1);
+                            exact_row(RB * nc + q, meta_c, slot_c, ex0);
+                            exact_row(RB * nc + q + 1, meta_c, slot_c, ex1);
                             add_row(mq0, ex0);
                             add_row(mq1, ex1);
                         } else {
@@ -704,8 +777,8 @@ sum_staged_kernel(const SumParams p)
                         }
                         if (min(mn0, mn1) <= p.thr2) {
                             uint32_t ex0[R], ex1[R];
-                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex0);
-                            exact_row(RB * nc + q + 1, slot_c + (uint32_t)((q + 1) * p.slot_bytes), ex1);
+                            exact_row(RB * nc + q, meta_c, slot_c, ex0);
+                            exact_row(RB * nc + q + 1, meta_c, slot_c, ex1);
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
                                 const uint32_t a0 = addr0 + (ex0[r] << SH), a1 = addr0 + (ex1[r] << SH);
@@ -730,7 +803,7 @@ sum_staged_kernel(const SumParams p)
                         uint32_t hi[R];
                         if (fast_row(mq, hi) <= p.thr2) {
                             uint32_t ex[R];
-                            exact_row(RB * nc + q, slot_c + (uint32_t)(q * p.slot_bytes), ex);
+                            exact_row(RB * nc + q, meta_c, slot_c, ex);
                             add_row(mq, ex);
                         } else {
                             add_row(mq, hi);
