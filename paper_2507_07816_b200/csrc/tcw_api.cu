@@ -1500,7 +1500,12 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
     if (smem > SMEM_MAX) return fail(TCW_EUNSUPPORTED, "band too wide for one CTA's shared memory (%zu bytes)", smem);
 
     cudaStream_t st = (cudaStream_t)stream;
+    // Transforms run in batches whose samples (64 MB) stay in L2 between the window kernel and cuFFT; their spectra
+    // are kept for a SUPER-batch of up to 2 GiB (16 384 eight-second SFTs at 4096 Hz) and normalised by ONE launch:
+    // a batch of 512 SFTs is only 128 CTAs (fewer than the 148 SMs, eight warps each), and a kernel whose threads
+    // each walk a long dependent loop needs the whole machine full of warps.
     const int batch = (int)std::min<long>(n_seg, std::max<long>(1, (64L << 20) / ((long)N * 4)));
+    const long super = std::min<long>(n_seg, std::max<long>(batch, ((2L << 30) / ((long)n_half * 8)) / batch * batch));
     float *d_x = nullptr, *d_win = nullptr;
     float2 *d_spec = nullptr;
     cufftHandle plan = 0;
@@ -1519,7 +1524,7 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         }                                                                                           \
     } while (0)
     PREP_TRY(dev_alloc((void **)&d_x, (size_t)batch * N * sizeof(float), st));
-    PREP_TRY(dev_alloc((void **)&d_spec, (size_t)batch * n_half * sizeof(float2), st));
+    PREP_TRY(dev_alloc((void **)&d_spec, (size_t)(super + batch) * n_half * sizeof(float2), st));   // + batch: cuFFT always writes whole batches
     PREP_TRY(dev_alloc((void **)&d_win, (size_t)N * sizeof(float), st));
     tcw::prep_window_table_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, d_win);
     PREP_TRY(cudaGetLastError());
@@ -1543,21 +1548,24 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         if (cufftSetStream(plan, st) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftSetStream failed"); goto done; }
     }
     PREP_TRY(cudaFuncSetAttribute(tcw::prep_normalise_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    for (long j0 = 0; j0 < n_seg; j0 += batch) {
-        const int nb = (int)std::min<long>(batch, n_seg - j0);
-        if (nb < batch)   // zero the tail of the batch buffer: cuFFT always transforms `batch` segments
-            PREP_TRY(cudaMemsetAsync(d_x + (size_t)nb * N, 0, (size_t)(batch - nb) * N * sizeof(float), st));
-        if (!on_device)
-            PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyHostToDevice, st));
-        {
-            const float *src = on_device ? strain + j0 * N : d_x;
-            if ((N & 3) == 0 && ((uintptr_t)src & 15) == 0)
-                tcw::prep_window4_kernel<<<dim3((unsigned)((N / 4 + 255) / 256), (unsigned)std::min(nb, 64)), 256, 0, st>>>(src, d_win, nb, N, d_x);
-            else
-                tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(src, d_win, nb, N, d_x);
+    for (long s0 = 0; s0 < n_seg; s0 += super) {
+        const long ns = std::min<long>(super, n_seg - s0);
+        for (long j0 = s0; j0 < s0 + ns; j0 += batch) {
+            const int nb = (int)std::min<long>(batch, s0 + ns - j0);
+            if (nb < batch)   // zero the tail of the batch buffer: cuFFT always transforms `batch` segments
+                PREP_TRY(cudaMemsetAsync(d_x + (size_t)nb * N, 0, (size_t)(batch - nb) * N * sizeof(float), st));
+            if (!on_device)
+                PREP_TRY(cudaMemcpyAsync(d_x, strain + j0 * N, (size_t)nb * N * sizeof(float), cudaMemcpyHostToDevice, st));
+            {
+                const float *src = on_device ? strain + j0 * N : d_x;
+                if ((N & 3) == 0 && ((uintptr_t)src & 15) == 0)
+                    tcw::prep_window4_kernel<<<dim3((unsigned)((N / 4 + 255) / 256), (unsigned)std::min(nb, 64)), 256, 0, st>>>(src, d_win, nb, N, d_x);
+                else
+                    tcw::prep_window_kernel<<<148 * 8, 256, 0, st>>>(src, d_win, nb, N, d_x);
+            }
+            PREP_TRY(cudaGetLastError());
+            if (cufftExecR2C(plan, d_x, (cufftComplex *)(d_spec + (size_t)(j0 - s0) * n_half)) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftExecR2C failed"); goto done; }
         }
-        PREP_TRY(cudaGetLastError());
-        if (cufftExecR2C(plan, d_x, (cufftComplex *)d_spec) != CUFFT_SUCCESS) { rc = fail(TCW_ECUDA, "cufftExecR2C failed"); goto done; }
         tcw::PrepParams p;
         p.spec = d_spec;
         p.n_half = n_half;
@@ -1566,9 +1574,9 @@ int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int f
         p.h = h;
         p.threshold = (float)prep->threshold;
         p.out_format = format;
-        p.out = (unsigned char *)out_spectrogram + j0 * out_pitch_bytes;
+        p.out = (unsigned char *)out_spectrogram + s0 * out_pitch_bytes;
         p.out_pitch = out_pitch_bytes;
-        tcw::prep_normalise_kernel<<<(nb + spc - 1) / spc, tcw::PREP_THREADS, smem, st>>>(p, nb, spc);
+        tcw::prep_normalise_kernel<<<(unsigned)((ns + spc - 1) / spc), tcw::PREP_THREADS, smem, st>>>(p, (int)ns, spc);
         PREP_TRY(cudaGetLastError());
     }
     PREP_TRY(cudaStreamSynchronize(st));

@@ -121,21 +121,48 @@ prep_normalise_kernel(const PrepParams p, int n_batch, int spc)
             for (int q = 0; q < W; ++q) c += Pu[k0 + q] < cand;
             if (c <= h) key = cand;
         }
-        // the re-count works on the float bits: per window element two compares and four predicated integer instructions
+        // Slides.  With L = #(x < mu) and LE = #(x <= mu) over the slid window, the new median is the largest element
+        // below mu if L > h, the smallest above it if LE <= h, else mu.  Every slide scans the window once, branch-free
+        // and identical in every lane, for three things: pred - mu (the unsigned maximum of x - mu is attained by the
+        // largest x < mu, whose difference wraps to the top of the range), succ - mu - 1 (the unsigned minimum of
+        // x - mu - 1: elements <= mu wrap to the top), and ONE of the two counts, C = #(x < mu + s), from the sign of
+        // x - mu - s (keys are float bits of non-negative numbers, below 2^31).  The other count K is carried: it moves
+        // by (entering element) - (leaving element), and when the median moves it is known exactly -- moving down to
+        // pred gives LE(pred) = L, so K := L and the scans count L (s = 0); moving up to succ gives L(succ) = LE, so
+        // K := LE and the scans count LE (s = 1).
         unsigned int mu = key;
+        unsigned int sflag = 0u;
+        int K = 0;
+        for (int q = 0; q < W; ++q) K += Pu[k0 + q] <= mu;          // LE of the first window
         for (int k = k0; k < k1; ++k) {
             if (k > k0) {
-                int c_less = 0, c_gt = 0;
-                unsigned int pred = 0u, succ = 0xffffffffu;
                 const unsigned int *wq = Pu + k;
+                const unsigned int x_out = wq[-1], x_in = wq[W - 1];
+                const unsigned int mk = mu + 1u - sflag;            // K = #(x < mk)
+                K += (int)(x_in < mk) - (int)(x_out < mk);
+                const unsigned int nmu = 0u - mu, nmu1 = nmu - 1u, nms = nmu - sflag;
+                unsigned int maxd0 = 0u, maxd1 = 0u, mine0 = 0xffffffffu, mine1 = 0xffffffffu;
+                unsigned int c0 = 0u, c1 = 0u;
 #pragma unroll 4
-                for (int q = 0; q < W; ++q) {
-                    const unsigned int x = wq[q];
-                    if (x < mu) { ++c_less; pred = max(pred, x); }
-                    if (x > mu) { ++c_gt; succ = min(succ, x); }
+                for (int q = 0; q + 1 < W; q += 2) {
+                    const unsigned int x0 = wq[q], x1 = wq[q + 1];
+                    maxd0 = max(maxd0, x0 + nmu);
+                    maxd1 = max(maxd1, x1 + nmu);
+                    mine0 = min(mine0, x0 + nmu1);
+                    mine1 = min(mine1, x1 + nmu1);
+                    c0 += (x0 + nms) >> 31;
+                    c1 += (x1 + nms) >> 31;
                 }
-                if (c_less > h) mu = pred;
-                else if (W - c_gt <= h) mu = succ;
+                {
+                    const unsigned int x0 = wq[W - 1];              // W is odd
+                    maxd0 = max(maxd0, x0 + nmu);
+                    mine0 = min(mine0, x0 + nmu1);
+                    c0 += (x0 + nms) >> 31;
+                }
+                const int C = (int)(c0 + c1);
+                const int L = sflag ? K : C, LE = sflag ? C : K;
+                if (L > h) { mu += max(maxd0, maxd1); K = L; sflag = 0u; }
+                else if (LE <= h) { mu += 1u + min(mine0, mine1); K = LE; sflag = 1u; }
             }
             const float m = __uint_as_float(mu);
             const float rho = P[k + h] * 0.69314718055994531f / m;
