@@ -1414,21 +1414,24 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
         int nb;
         sel_grid(n, &seg, &nb);
         const int vec = ((uintptr_t)values & 15) == 0;
-        const size_t zbytes = (size_t)nb * 2048 * 4 + 2 * (size_t)tcw::SEL_MAX_BLOCKS * 4 + (size_t)tcw::SEL_MAX_CAND * 12 + 64;
+        const size_t n_rows = (size_t)((n + tcw::SEL_ROW - 1) / tcw::SEL_ROW);
+        const size_t zbytes = (size_t)nb * 2048 * 4 + 2 * (size_t)tcw::SEL_MAX_BLOCKS * 4 + (size_t)tcw::SEL_MAX_CAND * 12 + 64 + n_rows * 2;
         if ((rc = h->d_selzoom.reserve(zbytes)) != TCW_OK) return rc;
         long long *z_idx = (long long *)h->d_selzoom.p;
         unsigned int *z_bits = (unsigned int *)(z_idx + tcw::SEL_MAX_CAND);
         unsigned int *z_off = z_bits + tcw::SEL_MAX_CAND;
         unsigned int *z_cnt = z_off + tcw::SEL_MAX_BLOCKS;
         unsigned int *z_hist = z_cnt + tcw::SEL_MAX_BLOCKS;
-        tcw::sel_sample_kernel<<<1, 1024, 0, st>>>(v, n, dtype, sc.state);
-        if (dtype) tcw::sel_zoom_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist);
-        else tcw::sel_zoom_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist);
+        unsigned short *z_rows = (unsigned short *)(z_hist + (size_t)nb * 2048);      // largest zoom bin of every row of 128 values
+        CUDA_TRY(cudaMemsetAsync(z_rows, 0, n_rows * 2, st));
+        tcw::sel_sample_kernel<<<1, 1024, 0, st>>>(v, n, dtype, (unsigned int)K, sc.state);
+        if (dtype) tcw::sel_zoom_hist_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist, z_rows);
+        else tcw::sel_zoom_hist_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, sc.hist, z_hist, z_rows);
         tcw::sel_zoom_pick_kernel<<<1, 256, 0, st>>>(sc.hist, sc.state, (unsigned int)K, dtype);
         tcw::sel_zoom_count_kernel<<<(nb + 7) / 8, 256, 0, st>>>(z_hist, nb, sc.state, z_cnt);
         tcw::sel_zoom_scan_kernel<<<1, 256, 0, st>>>(z_cnt, nb, z_off);
-        if (dtype) tcw::sel_zoom_compact_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_bits, z_idx);
-        else tcw::sel_zoom_compact_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_bits, z_idx);
+        if (dtype) tcw::sel_zoom_compact_kernel<1><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_rows, z_bits, z_idx);
+        else tcw::sel_zoom_compact_kernel<0><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, vec, sc.state, z_off, z_rows, z_bits, z_idx);
         run_select(z_bits, tcw::SEL_MAX_CAND, 2, z_idx);
         run_select(v, n, 1, nullptr);
     } else {
@@ -1459,11 +1462,15 @@ int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, doubl
     sel_grid(n, &seg, &nb);
     const unsigned int *v = (const unsigned int *)values;
     const int vec = ((uintptr_t)values & 15) == 0;
-    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, threshold, sc.blk_gt, sc.blk_eq);
+    // the count pass leaves, per row of 128 values, how many are selected (n/128 bytes); the scatter pass opens only those rows
+    const size_t n_rows = (size_t)((n + tcw::SEL_ROW - 1) / tcw::SEL_ROW);
+    if ((rc = h->d_selzoom.reserve(n_rows)) != TCW_OK) return rc;
+    unsigned char *row_cnt = (unsigned char *)h->d_selzoom.p;
+    CUDA_TRY(cudaMemsetAsync(row_cnt, 0, n_rows, st));
+    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, threshold, sc.blk_gt, sc.blk_eq, 0, row_cnt);
     tcw::sel_scan_kernel<<<1, 256, 0, st>>>(sc.blk_gt, sc.blk_eq, nb, sc.off_gt, sc.off_eq, sc.state);
     if (capacity > 0)
-        tcw::sel_scatter_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, sc.state, threshold, sc.blk_gt,
-                                                                       sc.blk_eq, sc.off_gt, sc.off_eq, capacity, nullptr, out_idx);
+        tcw::sel_scatter_rows_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, threshold, row_cnt, sc.off_gt, capacity, out_idx);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(out_count, &sc.state->count, sizeof(long long), cudaMemcpyDeviceToDevice, st));
     h->last_stream = st;

@@ -38,20 +38,25 @@ struct SelState {
     unsigned int k_eff;         // min(K, number of selectable values)
     unsigned int n_greater;     // keys strictly above the K-th largest (after the last pass)
     unsigned long long count;   // threshold selection: number of values above the threshold
-    // two-read route: monotone bin map  bin(key) = 0 if key >> z_top < z_prefix, 2047 if >, else
-    // clamp(((key >> z_shift) & 2047), 0, 2047); z_bin = the bin of the K-th largest key; n_cand = keys
-    // in bins >= z_bin; cand_ok = 1 when they fit the candidate buffer
-    unsigned int z_shift, z_top, z_prefix, z_bin, n_cand, cand_ok;
+    // two-read route: monotone bin map  bin(key) = 0 if key < z_lo, else min(((key - z_lo) >> z_shift) + 1, 2047);
+    // z_bin = the bin of the K-th largest key; n_cand = keys in bins >= z_bin; cand_ok = 1 when they fit the
+    // candidate buffer
+    unsigned int z_shift, z_lo, z_bin, n_cand, cand_ok;
     unsigned int z_val_lo;      // raw value (float bits / int) of the lowest key in a bin >= 1: smaller values skip the key arithmetic
     unsigned int z_val_bin;     // raw value of the lowest key in a bin >= z_bin: only values at or above it can be candidates
 };
 
 // the monotone bin of a key under the zoom window (non-decreasing in key)
-__device__ __forceinline__ unsigned int sel_zoom_bin(unsigned int key, unsigned int z_shift, unsigned int z_top, unsigned int z_prefix)
+__device__ __forceinline__ unsigned int sel_zoom_bin(unsigned int key, unsigned int z_shift, unsigned int z_lo)
 {
-    const unsigned int hi = z_top >= 32u ? 0u : key >> z_top;
-    if (hi != z_prefix) return hi < z_prefix ? 0u : 2047u;
-    return (key >> z_shift) & 2047u;
+    if (key < z_lo) return 0u;
+    return min(((key - z_lo) >> z_shift) + 1u, 2047u);
+}
+// the lowest key of bin d >= 1 (saturating)
+__device__ __forceinline__ unsigned int sel_zoom_bin_lo(unsigned int d, unsigned int z_shift, unsigned int z_lo)
+{
+    const unsigned long long k = (unsigned long long)z_lo + ((unsigned long long)(d - 1u) << z_shift);
+    return k > 0xffffffffull ? 0xffffffffu : (unsigned int)k;
 }
 
 // order-preserving key of a float32 (NaN -> 0 = "not selectable"), or of an int32
@@ -105,6 +110,7 @@ __device__ __forceinline__ SelSeg sel_segment(long n, long seg)
 // four consecutive elements tile + 4t .. tile + 4t + 3 (one 16-byte load when the array is 16-byte
 // aligned; segments start on multiples of 1024 elements).  nv = how many of the four are in range.
 constexpr int SEL_TILE = 4 * SEL_THREADS;
+constexpr int SEL_ROW = 128;      // a row: the 128 consecutive values one warp fetches with one 16-byte load per lane
 __device__ __forceinline__ void sel_load4(const unsigned int *__restrict__ vals, long i, long end, bool vec,
                                           unsigned int (&b)[4], int &nv)
 {
@@ -234,11 +240,13 @@ sel_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ state, u
 __device__ __forceinline__ unsigned int sel_block_scan(unsigned int cnt, unsigned int *warp_tot, unsigned int &total);
 
 // ---- two-read route -------------------------------------------------------------------------
-// One CTA: SEL_SAMPLE keys at a fixed stride, sorted descending; the zoom window is placed on the highest
-// bit in which the sample's largest key and its 16th largest differ (a window of 11 bits from there down),
-// so that the bins resolve the upper tail.  Any window gives exact results; this one gives few candidates.
+// One CTA: SEL_SAMPLE keys at a fixed stride, sorted descending.  The zoom window starts at the sample's r-th
+// largest key, r as small as still leaves an expected 8 K values above it (2 <= r <= 16): everything below is
+// settled by one compare in pass A, and the fewer values reach the window the fewer warps leave that fast path.
+// The bins are 1/128 of the spread between the sample's largest and 16th largest key wide, so that 2047 of them
+// resolve the tail far above the sample's maximum.  Any window gives exact results; this one gives few candidates.
 __global__ void __launch_bounds__(1024)
-sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, SelState *__restrict__ state)
+sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, unsigned int K, SelState *__restrict__ state)
 {
     __shared__ unsigned int key[SEL_SAMPLE];
     const long stride = n / SEL_SAMPLE > 0 ? n / SEL_SAMPLE : 1;
@@ -258,14 +266,14 @@ sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, Sel
             __syncthreads();
         }
     if (threadIdx.x == 0) {
-        const unsigned int diff = key[0] ^ key[15];
-        const int top_bit = diff ? 31 - __clz(diff) : 10;            // highest differing bit
-        const int shift = top_bit >= 10 ? top_bit - 10 : 0;
+        const unsigned int spread = key[0] - key[15];
+        const int bits = spread ? 32 - __clz(spread) : 0;
+        const int shift = bits > 7 ? bits - 7 : 0;                   // spread >> shift < 128
+        long r = ((long)8 * K * SEL_SAMPLE + n - 1) / n;
+        r = r < 2 ? 2 : (r > 16 ? 16 : r);
         state->z_shift = (unsigned int)shift;
-        state->z_top = (unsigned int)(shift + 11);
-        state->z_prefix = shift + 11 >= 32 ? 0u : key[0] >> (shift + 11);
-        const unsigned int base = shift + 11 >= 32 ? 0u : (key[0] >> (shift + 11)) << (shift + 11);
-        state->z_val_lo = sel_unkey(base | (1u << shift), is_int);
+        state->z_lo = key[r - 1];
+        state->z_val_lo = sel_unkey(key[r - 1], is_int);
         state->z_val_bin = state->z_val_lo;
         state->z_bin = 0;
         state->n_cand = 0;
@@ -281,12 +289,13 @@ sel_sample_kernel(const unsigned int *__restrict__ vals, long n, int is_int, Sel
 template <int IS_INT>
 __global__ void __launch_bounds__(SEL_THREADS)
 sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, int vec,
-                     const SelState *__restrict__ state, unsigned int *__restrict__ hist, unsigned int *__restrict__ blk_hist)
+                     const SelState *__restrict__ state, unsigned int *__restrict__ hist, unsigned int *__restrict__ blk_hist,
+                     unsigned short *__restrict__ row_max)
 {
     __shared__ unsigned int h[2048];
     for (int t = threadIdx.x; t < 2048; t += SEL_THREADS) h[t] = 0;
     __syncthreads();
-    const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, vlo = state->z_val_lo;
+    const unsigned int zs = state->z_shift, zl = state->z_lo, vlo = state->z_val_lo;
     const SelSeg sg = sel_segment(n, seg);
     unsigned int below = 0;
     for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
@@ -307,13 +316,27 @@ sel_zoom_hist_kernel(const unsigned int *__restrict__ vals, long n, long seg, in
             below += (inr && lt) ? 1u : 0u;
             rest |= (inr && !lt) ? (1u << c) : 0u;
         }
+        unsigned int m0 = 0, m1 = 0;                            // largest zoom bin among this thread's values of either tile
         if (rest) {
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
                 if ((rest >> c & 1u) && sel_valid(b[c], IS_INT)) {
-                    const unsigned int d = sel_zoom_bin(sel_key(b[c], IS_INT), zs, zt, zp);
+                    const unsigned int d = sel_zoom_bin(sel_key(b[c], IS_INT), zs, zl);
                     if (d) atomicAdd(&h[d], 1u); else ++below;
+                    if (c < 4) m0 = max(m0, d); else m1 = max(m1, d);
                 }
+            }
+        }
+        // the largest bin of each ROW (the 128 consecutive values one warp loads): pass B opens only the rows that can
+        // hold a candidate, a few thousand of three million, instead of reading the array again
+        // (row_max is zeroed by the host; only warps that met the window write)
+        if (__any_sync(0xffffffffu, rest != 0u)) {
+            m0 = __reduce_max_sync(0xffffffffu, m0);
+            m1 = __reduce_max_sync(0xffffffffu, m1);
+            if ((threadIdx.x & 31) == 0) {
+                const long r0 = (t0 >> 7) + (threadIdx.x >> 5), r1 = r0 + SEL_TILE / SEL_ROW;
+                if (m0) row_max[r0] = (unsigned short)m0;
+                if (m1) row_max[r1] = (unsigned short)m1;
             }
         }
     }
@@ -357,9 +380,7 @@ sel_zoom_pick_kernel(unsigned int *__restrict__ hist, SelState *__restrict__ sta
         state->z_bin = (unsigned int)d;
         {
             // the lowest key of bin d (d >= 1) as a raw value: pass B tests values against it before any key arithmetic
-            const unsigned int zt = state->z_top, zs = state->z_shift;
-            const unsigned int base = zt >= 32u ? 0u : state->z_prefix << zt;
-            state->z_val_bin = sel_unkey(base | ((unsigned int)(d > 0 ? d : 1) << zs), is_int);
+            state->z_val_bin = sel_unkey(sel_zoom_bin_lo((unsigned int)(d > 0 ? d : 1), state->z_shift, state->z_lo), is_int);
         }
         state->n_cand = n_cand > 0xffffffffull ? 0xffffffffu : (unsigned int)n_cand;
         state->cand_ok = (k > 0 && n_cand <= (unsigned long long)SEL_MAX_CAND) ? 1u : 0u;
@@ -402,55 +423,92 @@ sel_zoom_scan_kernel(const unsigned int *__restrict__ blk_cnt, int n_blocks, uns
     }
 }
 
-// Pass B: the keys in bins >= z_bin with their indices, in index order, into the candidate buffer.
-// One compare per value rules out everything below the lowest value of that bin; a tile pair without a
-// possible candidate costs two vector loads and one barrier.
+// Rows: a row is SEL_ROW = 128 consecutive values, what one warp fetches with one 16-byte load per lane.  The
+// streaming passes leave one small summary per row (largest zoom bin, or number of selected values); the passes
+// below read only the summaries and open the few rows that matter.  Warp w of a CTA owns a contiguous run of
+// the CTA's rows, lanes scan 32 summaries at a time, and an open row is loaded by the whole warp: lane order,
+// then the four values of a lane, is index order.
+//   open(r)  -> the row may hold a wanted value     take(bits) -> the value is wanted
+//   WRITE = false: returns the number of wanted values in the warp's rows (warp-uniform);
+//   WRITE = true:  emit(rank, bits, index) for each of them, ranks ascending from `pos`.
+template <bool WRITE, class Open, class Take, class Emit>
+__device__ __forceinline__ unsigned int sel_walk_rows(const unsigned int *__restrict__ vals, long end, bool vec, long w0, long w1,
+                                                      Open open, Take take, unsigned long long pos, Emit emit)
+{
+    const unsigned int lane = threadIdx.x & 31, lt = (1u << lane) - 1u;
+    unsigned int total = 0;
+    for (long rb = w0; rb < w1; rb += 32) {
+        const long r = rb + lane;
+        unsigned int m = __ballot_sync(0xffffffffu, r < w1 && open(r));
+        while (m) {
+            const long row = rb + (__ffs(m) - 1);
+            m &= m - 1;
+            const long i = row * SEL_ROW + 4 * lane;
+            unsigned int b[4];
+            int nv;
+            sel_load4(vals, i, end, vec, b, nv);
+            unsigned int c = 0, t[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { t[q] = (q < nv && take(b[q])) ? 1u : 0u; c += t[q]; }
+            if (!WRITE) {
+                total += __reduce_add_sync(0xffffffffu, c);
+            } else {
+                // exclusive prefix of c over the lanes: four ballots of the per-value flags, counted below the lane
+                unsigned int before = 0, all = 0;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const unsigned int bm = __ballot_sync(0xffffffffu, t[q] != 0u);
+                    before += __popc(bm & lt);
+                    all += __popc(bm);
+                }
+                unsigned long long at = pos + before;
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (t[q]) { emit(at, b[q], i + q); ++at; }
+                pos += all;
+                total += all;
+            }
+        }
+    }
+    return total;
+}
+// the contiguous run of rows warp `warp` of this CTA owns
+__device__ __forceinline__ void sel_warp_rows(const SelSeg &sg, long &w0, long &w1)
+{
+    const long r_begin = sg.begin / SEL_ROW, r_end = (sg.end + SEL_ROW - 1) / SEL_ROW;
+    const long rpw = (r_end - r_begin + SEL_THREADS / 32 - 1) / (SEL_THREADS / 32);
+    w0 = min(r_begin + rpw * (threadIdx.x >> 5), r_end);
+    w1 = min(w0 + rpw, r_end);
+}
+
+// Pass B: the keys in bins >= z_bin with their indices, in index order, into the candidate buffer.  It does not
+// read the array again: pass A left the largest bin of every row, and only rows whose maximum reaches z_bin are
+// opened (counted first, then written behind the per-CTA offsets from the stored histograms).
 template <int IS_INT>
 __global__ void __launch_bounds__(SEL_THREADS)
 sel_zoom_compact_kernel(const unsigned int *__restrict__ vals, long n, long seg, int vec,
                         const SelState *__restrict__ state, const unsigned int *__restrict__ blk_off,
+                        const unsigned short *__restrict__ row_max,
                         unsigned int *__restrict__ cand_bits, long long *__restrict__ cand_idx)
 {
     __shared__ unsigned int wt[SEL_THREADS / 32];
     if (!state->cand_ok) return;
-    const unsigned int zs = state->z_shift, zt = state->z_top, zp = state->z_prefix, d0 = state->z_bin, vbin = state->z_val_bin;
-    unsigned int base = blk_off[blockIdx.x];
+    const unsigned int zs = state->z_shift, zl = state->z_lo, d0 = state->z_bin, vbin = state->z_val_bin;
     const SelSeg sg = sel_segment(n, seg);
-    for (long t0 = sg.begin; t0 < sg.end; t0 += 2 * SEL_TILE) {
-        unsigned int b[8];
-        int nv[2];
-        {
-            unsigned int b0[4], b1[4];
-            sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, nv[0]);
-            sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, nv[1]);
-#pragma unroll
-            for (int c = 0; c < 4; ++c) { b[c] = b0[c]; b[4 + c] = b1[c]; }
-        }
-        unsigned int maybe = 0;
-#pragma unroll
-        for (int c = 0; c < 8; ++c)
-            maybe |= ((c & 3) < nv[c >> 2] && (d0 == 0u || !sel_raw_below(b[c], vbin, IS_INT))) ? (1u << c) : 0u;
-        if (!__syncthreads_or((int)maybe)) continue;
-        // some thread of the CTA may hold a candidate: exact test, then the two tiles in index order
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {
-            bool take[4];
-            unsigned int cnt = 0;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int c = 4 * half + q;
-                take[q] = (maybe >> c & 1u) && sel_valid(b[c], IS_INT) && sel_zoom_bin(sel_key(b[c], IS_INT), zs, zt, zp) >= d0;
-                cnt += take[q];
-            }
-            unsigned int tot;
-            unsigned int r = sel_block_scan(cnt, wt, tot);
-            const long i = t0 + (long)half * SEL_TILE + 4 * threadIdx.x;
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if (take[q]) { cand_bits[base + r] = b[4 * half + q]; cand_idx[base + r] = i + q; ++r; }
-            base += tot;
-        }
-    }
+    long w0, w1;
+    sel_warp_rows(sg, w0, w1);
+    auto open = [&](long r) { return (unsigned int)row_max[r] >= d0; };
+    auto take = [&](unsigned int bits) {
+        return (d0 == 0u || !sel_raw_below(bits, vbin, IS_INT)) && sel_valid(bits, IS_INT) &&
+               sel_zoom_bin(sel_key(bits, IS_INT), zs, zl) >= d0;
+    };
+    auto emit = [&](unsigned long long at, unsigned int bits, long i) { cand_bits[at] = bits; cand_idx[at] = i; };
+    const unsigned int cnt = sel_walk_rows<false>(vals, sg.end, vec != 0, w0, w1, open, take, 0ull, emit);
+    if ((threadIdx.x & 31) == 0) wt[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    unsigned long long pos = blk_off[blockIdx.x];
+    for (unsigned int w = 0; w < (threadIdx.x >> 5); ++w) pos += wt[w];
+    if (cnt) sel_walk_rows<true>(vals, sg.end, vec != 0, w0, w1, open, take, pos, emit);
 }
 
 // ---- ordered compaction -------------------------------------------------------------------
@@ -477,7 +535,8 @@ template <bool THR>
 __global__ void __launch_bounds__(SEL_THREADS)
 sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec,
                  const SelState *__restrict__ state, double thr,
-                 unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq, int gate = 0)
+                 unsigned int *__restrict__ blk_gt, unsigned int *__restrict__ blk_eq, int gate = 0,
+                 unsigned char *__restrict__ row_cnt = nullptr)
 {
     __shared__ unsigned int s_gt, s_eq;
     if (!THR && !sel_gate(state, gate, n)) return;
@@ -491,12 +550,29 @@ sel_count_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is
         int n0, n1;
         sel_load4(vals, t0 + 4 * threadIdx.x, sg.end, vec != 0, b0, n0);
         sel_load4(vals, t0 + SEL_TILE + 4 * threadIdx.x, sg.end, vec != 0, b1, n1);
+        unsigned int g0 = 0, g1 = 0;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const int c0 = c < n0 ? sel_class<THR>(b0[c], is_int, kth, thr) : 0;
             const int c1 = c < n1 ? sel_class<THR>(b1[c], is_int, kth, thr) : 0;
-            gt += (c0 == 2) + (c1 == 2);
+            g0 += c0 == 2;
+            g1 += c1 == 2;
             eq += (c0 == 1) + (c1 == 1);
+        }
+        gt += g0 + g1;
+        if (THR && row_cnt) {
+            // how many values of each ROW (128 consecutive values, one warp's load) are selected: the scatter pass
+            // then opens only the rows that hold one instead of reading the array again
+            // (row_cnt is zeroed by the host; only warps that hold a selected value write)
+            if (__any_sync(0xffffffffu, (g0 | g1) != 0u)) {
+                g0 = __reduce_add_sync(0xffffffffu, g0);
+                g1 = __reduce_add_sync(0xffffffffu, g1);
+                if ((threadIdx.x & 31) == 0) {
+                    const long r0 = (t0 >> 7) + (threadIdx.x >> 5), r1 = r0 + SEL_TILE / SEL_ROW;
+                    if (g0) row_cnt[r0] = (unsigned char)g0;
+                    if (g1) row_cnt[r1] = (unsigned char)g1;
+                }
+            }
         }
     }
     for (int o = 16; o; o >>= 1) {
@@ -622,6 +698,32 @@ sel_scatter_kernel(const unsigned int *__restrict__ vals, long n, long seg, int 
         base_gt += tot2;
         base_eq += tot1;
     }
+}
+
+// Threshold selection, second pass: out_idx[rank] = i for the values above the threshold, ascending i, up to
+// `capacity`.  Reads the per-row counts of the count pass (n/128 bytes) and opens only the rows that hold a selected
+// value (sel_walk_rows).
+__global__ void __launch_bounds__(SEL_THREADS)
+sel_scatter_rows_kernel(const unsigned int *__restrict__ vals, long n, long seg, int is_int, int vec, double thr,
+                        const unsigned char *__restrict__ row_cnt, const unsigned long long *__restrict__ off_gt,
+                        long capacity, long long *__restrict__ out_idx)
+{
+    __shared__ unsigned int wt[SEL_THREADS / 32];
+    const SelSeg sg = sel_segment(n, seg);
+    long w0, w1;
+    sel_warp_rows(sg, w0, w1);
+    unsigned int cnt = 0;
+    for (long r = w0 + (threadIdx.x & 31); r < w1; r += 32) cnt += row_cnt[r];
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if ((threadIdx.x & 31) == 0) wt[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    unsigned long long pos = off_gt[blockIdx.x];
+    for (unsigned int w = 0; w < (threadIdx.x >> 5); ++w) pos += wt[w];
+    if (cnt == 0) return;
+    auto open = [&](long r) { return row_cnt[r] != 0; };
+    auto take = [&](unsigned int bits) { return sel_class<true>(bits, is_int, 0u, thr) == 2; };
+    auto emit = [&](unsigned long long at, unsigned int, long i) { if ((long)at < capacity) out_idx[at] = i; };
+    sel_walk_rows<true>(vals, sg.end, vec != 0, w0, w1, open, take, pos, emit);
 }
 
 // one CTA: bitonic sort of the k_eff candidates by (key descending, index ascending)
