@@ -384,6 +384,9 @@ enum {
     TCW_OPT_GENERAL_F0 = 7, /* staged kernel: 1 = treat the f0 axis as arbitrary even when it is equally spaced (the
                                equally spaced instantiation derives the templates of a lane from one product
                                and a stride; same bins either way); 0 default                              */
+    TCW_OPT_ROW_COPIES = 8, /* staged kernel: 1 = stage every SFT row by its own 1-D bulk copy; 0 default: a ring slot (four
+                               consecutive SFT rows) travels by ONE tensor-map copy wherever its rows' windows fit one
+                               box (same bins, same sums bit for bit; the tests compare the two)            */
     TCW_OPT_DEBUG_SHRINK_SLOT = 100 /* test hook: the kernels check their staged windows against the planned
                                bound minus this many bytes, which forces the device status word and
                                hence TCW_EINTERNAL; 0 default.  Not for production use.               */
@@ -406,7 +409,8 @@ int tcw_get_timing(tcw_handle *h, float ms[4], int *n_searches);
  * info[5] kernels launched by the call, info[6] ring depth per warp (slots of four SFT rows in the staged kernel), info[7] sky points per
  * block (sky-block kernel, else 0), info[8] SFT chunks of the staged kernel (1 = not chunked),
  * info[9] SFT rows per chunk, info[10] tau ranges of the progressive read-back of the last search (tcw_search_host
- * with a large out_stat; 0 = none), info[11] reserved (0).
+ * with a large out_stat; 0 = none), info[11] 1 when the staged kernel staged ring slots by tensor-map copies
+ * (0: one 1-D bulk copy per row, see TCW_OPT_ROW_COPIES).
  * Synchronises the search's stream. */
 int tcw_get_info(tcw_handle *h, long info[12]);
 

@@ -26,6 +26,7 @@ TCW_OPT_KERNEL, TCW_OPT_TIMING, TCW_OPT_F0_PER_LANE, TCW_OPT_STAGES, TCW_OPT_SKY
 TCW_OPT_CHUNK_ROWS = 5
 TCW_OPT_EXACT_INDEX = 6
 TCW_OPT_GENERAL_F0 = 7
+TCW_OPT_ROW_COPIES = 8
 TCW_OPT_DEBUG_SHRINK_SLOT = 100
 KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
@@ -438,7 +439,8 @@ class Handle:
             _check(rc)
         return dict(kernel={1: "gather", 2: "staged", 3: "skyblock", 4: "bank"}.get(v[0], "?"), tile=int(v[1]), ctas=int(v[2]),
                     smem_bytes=int(v[3]), status=int(v[4]), launches=int(v[5]), stages=int(v[6]),
-                    sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]), readback_parts=int(v[10]))
+                    sky_block=int(v[7]), chunks=int(v[8]), chunk_rows=int(v[9]), readback_parts=int(v[10]),
+                    box_copies=int(v[11]))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

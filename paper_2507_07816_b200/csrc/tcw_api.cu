@@ -275,6 +275,7 @@ struct tcw_handle {
     unsigned int progress_target[16] = {0};  // CTAs per part
     int progress_a0[17] = {0};               // tau index where each part starts
     int opt_nonuniform = 0;   // 1: never take the equally-spaced-f0 instantiation of the staged kernel
+    int opt_row_copies = 0;   // 1: never stage a ring slot by one tensor-map copy
     bool keep_status = false; // a multi-part search (tcw_search_groups, tcw_search_host) clears the status word once
     int dbg_slot_shrink = 0;  // test hook: bytes taken off the kernels' own window bound
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
@@ -896,6 +897,10 @@ int tcw_set_option(tcw_handle *h, int key, long value)
         if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_GENERAL_F0 must be 0 or 1");
         h->opt_nonuniform = (int)value;
         return TCW_OK;
+    case TCW_OPT_ROW_COPIES:
+        if (value != 0 && value != 1) return fail(TCW_EINVAL, "TCW_OPT_ROW_COPIES must be 0 or 1");
+        h->opt_row_copies = (int)value;
+        return TCW_OK;
     case TCW_OPT_DEBUG_SHRINK_SLOT:
         if (value < 0 || value > (1 << 20)) return fail(TCW_EINVAL, "TCW_OPT_DEBUG_SHRINK_SLOT must be 0..2^20");
         h->dbg_slot_shrink = (int)value;
@@ -993,7 +998,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
             if (w_bins > tcw::PAD_BINS) continue;
             // one tensor-map copy per slot where the rows allow it (not for the weighted search: its wider row
             // metadata leaves no shared memory for 128-byte granular rows at three CTAs per SM)
-            const bool box = !wgt && h->d_tmaps != nullptr;
+            const bool box = !wgt && h->d_tmaps != nullptr && !h->opt_row_copies;
             if (!box) { p.tmaps = nullptr; p.max_seg = 0; }
             const int sb = slot_bytes_for(h->fmt_dev, w_bins, box);
             // rings holding at least six rows per warp (a slot is RB rows) hide the L2 latency; TCW_MINB CTAs of four warps per SM
@@ -1199,6 +1204,7 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
     h->info[8] = p.n_chunks;
     h->info[9] = p.chunk_rows;
     h->info[10] = h->progress_active ? h->progress_np : 0;
+    h->info[11] = kernel == 2 && p.tmaps ? 1 : 0;     // the staged kernel may stage slots by tensor-map copies
     return TCW_OK;
 }
 

@@ -302,3 +302,41 @@ def test_cfg3_full_size_sampled_groups(tcw, fmt):
         first = (st == bmax.values[:, None]).int().argmax(dim=1)
         assert torch.equal(first, idx)
         assert (stat >= 0).all().item() and (stat <= w.n_sft).all().item()
+
+
+@pytest.mark.parametrize("fmt", ["f32", "u8"])
+def test_box_copies_are_bit_identical_to_row_copies(tcw, fmt):
+    """The staged kernel fetches a ring slot (four consecutive SFT rows) with ONE tensor-map copy where the rows'
+    windows fit one box, and with one 1-D bulk copy per row otherwise (band edges, gaps in the data, the steep
+    start of a fast spin-down).  Both stagings feed the same arithmetic in the same order, so whole searches must
+    agree bit for bit with TCW_OPT_ROW_COPIES, and with the oracle: on cfg1, on random shapes with holes (rows of
+    one slot far apart in time), on a steep track (3000 Hz, tau = 3500 s, n = 3: 27 bins per SFT at the start) and
+    on an SFT-chunked search."""
+    rng = np.random.default_rng(20251105)
+    base = tcw_inputs.make_workload("cfg1")
+    cases = [(base if fmt == "f32" else base.with_format("u8"), {})]
+    for trial in range(6):
+        w = _random_workload(rng, fmt, int(rng.integers(70, 400)), int(rng.integers(600, 5000)),
+                             int(rng.integers(40, 1500)), float(rng.choice([0.5, 1.0, 2.0])),
+                             T=float(rng.choice([8.0, 10.0])), uniform=bool(trial % 2))
+        cases.append((w, {tcw.TCW_OPT_CHUNK_ROWS: 64} if trial % 3 == 0 else {}))
+    # steep: a band of 2600 bins below 3000 Hz, 600 templates, short tau, low braking index, and a gap of two hours
+    T, n_bins, f_min = 8.0, 2600, 2700.0
+    ts = np.concatenate([T * np.arange(300) + T / 2, 7200.0 + T * np.arange(300, 520) + T / 2])
+    rho = rng.standard_exponential((len(ts), n_bins), dtype=np.float32)
+    spec = rho if fmt == "f32" else (rho > 1.6).astype(np.uint8)
+    steep = Workload("steep", fmt, spec, len(ts), n_bins, f_min, T, ts, detector_velocity(ts), 0.0,
+                     f_min + 150.0 + 0.125 * np.arange(600), np.array([3500.0, 5000.0]), np.array([3.0, 5.0]),
+                     sky_vector(1.0, 0.3)[None])
+    cases.append((steep, {}))
+    n_box = 0
+    for w, opts in cases:
+        ref = oracle.evaluate(w)
+        s_box, b_box, i_box = _search_with(tcw, w, {tcw.TCW_OPT_KERNEL: 2, **opts})
+        s_row, b_row, i_row = _search_with(tcw, w, {tcw.TCW_OPT_KERNEL: 2, tcw.TCW_OPT_ROW_COPIES: 1, **opts})
+        assert i_row["box_copies"] == 0 and i_box["status"] == 0 and i_row["status"] == 0
+        n_box += i_box["box_copies"]
+        assert np.array_equal(s_box.view(np.uint32), s_row.view(np.uint32)), w.name
+        assert np.array_equal(b_box.view(np.uint8), b_row.view(np.uint8)), w.name
+        assert_stat_parity(w, s_box.reshape(-1), ref.stat)
+    assert n_box > 0, "no case exercised the tensor-map copies"
