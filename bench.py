@@ -439,7 +439,7 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
             block["roofline_binding"]["lookup_chain"] = {
                 "achieved_inband_lookups_per_s": inband / (sum_ms * 1e-3), "peak_lookups_per_s": pk["chain_lookups_per_s"],
                 "frac": inband / (sum_ms * 1e-3) / pk["chain_lookups_per_s"],
-                "note": "the bare lookup chain of the staged kernel (DFMA, address, LDS.32, FADD, half a VIMNMX3 per lookup) "
+                "note": "the bare lookup chain of the staged kernel as it ships (two rows per block: DFMA, address, LDS.32, half a FADD2, half a VIMNMX3 per lookup) "
                         "measured alone by tcw_measure_peaks: staging, row metadata and band edges are what separates the two"}
     if world == 1 and cpu_seconds > 0:
         cb = time_oracle(w, cpu_seconds)

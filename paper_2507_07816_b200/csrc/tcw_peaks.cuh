@@ -8,14 +8,16 @@
 //   * independent FP32 FFMA                            -- the schedulers' warp-instruction issue rate,
 //   * independent LDS.32 gathers of the access pattern the staged kernel has (lanes on consecutive
 //     templates read words at a stride below one) -- the shared-memory gather rate,
-//   * the bare lookup chain of the staged kernel (one DFMA, one address LEA, one LDS.32, one FADD,
-//     half a VIMNMX3 per lookup, 16 lookups per straight-line block) -- the speed of light of the
+//   * the bare lookup chain of the staged kernel as it ships (one DFMA, one address LEA, one LDS.32, half a FADD2,
+//     half a VIMNMX3 per lookup, two rows of 16 lookups per straight-line block) -- the speed of light of the
 //     design's instruction mix, in lookups per second.
 // Rates are whole-GPU, per second.  The numbers are only as good as the clocks of the moment; bench.py
 // measures them in the same process as the timed search and prints the SM clock beside them.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include "tcw_sum.cuh"   // fadd2
 
 namespace tcw {
 
@@ -110,8 +112,9 @@ peak_lds_kernel(int iters, float *out)
     if (s == 12345.678f) out[0] = s;
 }
 
-// The bare lookup chain of sum_staged_kernel: per row 16 x { DFMA, address, LDS.32, FADD } plus the
-// minimum of the fraction words; nothing else (no staging, no metadata, no band edges).
+// The bare lookup chain of sum_staged_kernel as it ships: two rows per straight-line block, per row 16 x { DFMA,
+// address, LDS.32 } plus the minimum of the fraction words, the two rows' elements added pairwise and accumulated
+// with packed float32 adds (FADD2); nothing else (no staging, no metadata, no band edges).
 __global__ void __launch_bounds__(128, 3)
 peak_chain_kernel(int rows, double c0, double q0, float *out)
 {
@@ -126,30 +129,37 @@ peak_chain_kernel(int rows, double c0, double q0, float *out)
     for (int r = 0; r < 16; ++r) acc[r] = 0.0f;
     uint32_t mn_all = 0xffffffffu;
     double c = c0, q = q0;
-    for (int j = 0; j < rows; ++j) {
-        // c drifts a little from row to row like g*D does; q keeps y in [2^20 + 2^19, +600)
-        c = __dadd_rn(c, -1e-9);
-        const double y0 = __fma_rn(dlane, c, q);
-        const double step = __dmul_rn(4.0, c);
-        uint32_t hi[16], lo[16];
-        hi[0] = (uint32_t)__double2hiint(y0);
-        lo[0] = (uint32_t)__double2loint(y0);
+    for (int j = 0; j < rows; j += 2) {
+        uint32_t hi[2][16], lo[2][16];
 #pragma unroll
-        for (int r = 1; r < 16; ++r) {
-            const double y = __fma_rn(step, (double)r, y0);
-            hi[r] = (uint32_t)__double2hiint(y);
-            lo[r] = (uint32_t)__double2loint(y);
+        for (int z = 0; z < 2; ++z) {
+            // c drifts a little from row to row like g*D does; q keeps y in [2^20 + 2^19, +600)
+            c = __dadd_rn(c, -1e-9);
+            const double y0 = __fma_rn(dlane, c, q);
+            const double step = __dmul_rn(4.0, c);
+            hi[z][0] = (uint32_t)__double2hiint(y0);
+            lo[z][0] = (uint32_t)__double2loint(y0);
+#pragma unroll
+            for (int r = 1; r < 16; ++r) {
+                const double y = __fma_rn(step, (double)r, y0);
+                hi[z][r] = (uint32_t)__double2hiint(y);
+                lo[z][r] = (uint32_t)__double2loint(y);
+            }
+            uint32_t m = min(lo[z][0], min(lo[z][1], lo[z][2]));
+#pragma unroll
+            for (int r = 3; r + 1 < 16; r += 2) m = min(m, min(lo[z][r], lo[z][r + 1]));
+            mn_all = min(mn_all, min(m, lo[z][15]));
         }
-        uint32_t m = min(lo[0], min(lo[1], lo[2]));
-#pragma unroll
-        for (int r = 3; r + 1 < 16; r += 2) m = min(m, min(lo[r], lo[r + 1]));
-        mn_all = min(mn_all, min(m, lo[15]));
+        float v0[16], v1[16], t[16];
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
-            float v;
-            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + (hi[r] << 2)));
-            acc[r] += v;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v0[r]) : "r"(base + (hi[0][r] << 2)));
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v1[r]) : "r"(base + (hi[1][r] << 2)));
         }
+#pragma unroll
+        for (int r = 0; r < 16; r += 2) fadd2(t[r], t[r + 1], v0[r], v0[r + 1], v1[r], v1[r + 1]);
+#pragma unroll
+        for (int r = 0; r < 16; r += 2) fadd2(acc[r], acc[r + 1], acc[r], acc[r + 1], t[r], t[r + 1]);
     }
     float s = 0;
 #pragma unroll

@@ -519,7 +519,7 @@ sum_staged_kernel(const SumParams p)
         // (band edges, gaps in the data, the steep start of a fast spin-down) every row gets its own 1-D copy.
         bool use2d = false;
         int seg0 = 0, nseg = 0;
-        if (p.tmaps) {
+        if (!WGT && p.tmaps) {     // (the weighted instantiation always stages row by row: keep the box code out of it)
             int kfm = mt.by16 > 0 ? kf : INT32_MAX, klm = mt.by16 > 0 ? kl : INT32_MIN;
             bool all = mt.by16 > 0;
 #pragma unroll
@@ -588,7 +588,7 @@ sum_staged_kernel(const SumParams p)
                 lds_v4(meta_i + 16u, u[0], b, lo[0], hi[0]);
                 by[0] = (int)b;
             }
-            if (u[0] & 512u) {
+            if (!WGT && (u[0] & 512u)) {
                 mbar_arrive_expect_tx(bar_i, (uint32_t)by[0]);
                 tensor3_g2s(slot_i, p.tmaps + ((u[0] >> 16) << 7), (int)lo[0], (int)hi[0], bar_i);
                 tot = -1;
@@ -669,7 +669,7 @@ sum_staged_kernel(const SumParams p)
         const int kf = lo_f - p.k_min;
         // where the row was staged: mc = metadata of the slot's first row, sc_ = the slot's first byte
         const uint32_t fl = lds_u32(mc + 16u);
-        const bool box = (fl & 512u) != 0;
+        const bool box = !WGT && (fl & 512u) != 0;
         const int a_byte = box ? 128 * (int)lds_u32(mc + 24u) - (int)p.pad_bytes : (BPB * kf) & ~15;
         const uint32_t S = sc_ + (uint32_t)(n % RB) * (box ? ((fl >> 16) << 7) : (uint32_t)p.slot_bytes);
         const uint32_t base = FIX_HC + (uint32_t)((((int)S - a_byte) >> SH) + kf) - (uint32_t)lo_f;
