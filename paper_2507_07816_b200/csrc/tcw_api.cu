@@ -996,9 +996,8 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
             if (p.d32 != 0.0)
                 w_bins = std::max(w_bins, (long)std::floor((32 * all[c] - 1) * (p.d32 / 32.0) * p.dmaxT * (1.0 + 1e-9) + 1e-6) + 2);
             if (w_bins > tcw::PAD_BINS) continue;
-            // one tensor-map copy per slot where the rows allow it (not for the weighted search: its wider row
-            // metadata leaves no shared memory for 128-byte granular rows at three CTAs per SM)
-            const bool box = !wgt && h->d_tmaps != nullptr && !h->opt_row_copies;
+            // one tensor-map copy per slot where the rows allow it
+            const bool box = h->d_tmaps != nullptr && !h->opt_row_copies;
             if (!box) { p.tmaps = nullptr; p.max_seg = 0; }
             const int sb = slot_bytes_for(h->fmt_dev, w_bins, box);
             // rings holding at least six rows per warp (a slot is RB rows) hide the L2 latency; TCW_MINB CTAs of four warps per SM

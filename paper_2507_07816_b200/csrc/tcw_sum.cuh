@@ -318,34 +318,28 @@ struct __align__(16) RowMeta {
     int by16;         // bytes staged (> 0, a multiple of 16), 0 row with no in-band bin, -1 no further rows
     uint32_t src_lo, src_hi;   // first staged byte of the row's window, relative to SumParams::spec_pad
 };
-// weighted search: the row's weight, whether every template of the tile is in band in this row
-// (then the weight sums W1, W2 advance by the same amount for the whole tile: one warp-uniform
-// add), and the constant that turns the fast index into a band-relative bin for the edge rows
-struct __align__(16) RowMetaW {
-    double c, Q;
-    uint32_t flags;
-    int by16;
-    uint32_t src_lo, src_hi;
+// weighted search: per row also the row's weight and the constant that turns the fast index into a band-relative
+// bin for the edge rows, in a second ring of 8-byte entries (the 32-byte RowMeta ring keeps its pitch, so that the
+// weighted instantiation still fits 128-byte granular slot rows at three CTAs per SM); RowMeta::flags bit 10 of
+// the row says that every template of the tile is in band in this row (then the weight sums W1, W2 advance by
+// the same amount for the whole tile: one warp-uniform add)
+struct __align__(8) RowWgt {
     float w;
-    int full;
     uint32_t ktest;   // bin - k_min = HI + ktest
-    int pad;
 };
-template <bool WGT> struct MetaT { typedef RowMeta type; };
-template <> struct MetaT<true> { typedef RowMetaW type; };
-static_assert(sizeof(RowMeta) == 32 && sizeof(RowMetaW) == 48, "RowMeta layout");
+static_assert(sizeof(RowMeta) == 32 && sizeof(RowWgt) == 8, "RowMeta layout");
 
 // rows of the per-warp metadata ring: one batch of 32 rows plus the rows still in flight
 __host__ __device__ inline int staged_meta_rows(int stages) { return 32 + RB * stages; }
 
-// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*meta_rows] [slot NW*D*RB*slot_bytes].  The slot
+// dynamic shared memory: [mbarrier NW*D] [RowMeta NW*meta_rows] [weighted: RowWgt NW*meta_rows] [slot NW*D*RB*slot_bytes].  The slot
 // region is reused for the cross-warp reduction (NW * 32*R accumulators) once every copy has
 // completed; the mbarrier words are never reused as data (they are updated through the async proxy,
 // and a generic store to the same bytes is not ordered against that without a proxy fence).
 __host__ __device__ inline size_t staged_bar_bytes(int stages) { return ((size_t)NW * stages * 8 + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t staged_header_bytes(int stages, bool wgt)
 {
-    return (staged_bar_bytes(stages) + (size_t)NW * staged_meta_rows(stages) * (wgt ? sizeof(RowMetaW) : sizeof(RowMeta)) + 127) & ~(size_t)127;
+    return (staged_bar_bytes(stages) + (size_t)NW * staged_meta_rows(stages) * (sizeof(RowMeta) + (wgt ? sizeof(RowWgt) : 0)) + 127) & ~(size_t)127;
 }
 __host__ __device__ inline size_t staged_smem_bytes(int stages, int slot_bytes, int tile, bool wgt)
 {
@@ -395,7 +389,7 @@ sum_staged_kernel(const SumParams p)
     constexpr bool PAIR = TCW_PAIR && RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
                                                    // per-lane weight sums leave no registers for that)
     typedef typename AccW<FMT, WGT>::type V;
-    typedef typename MetaT<WGT>::type Meta;
+    typedef RowMeta Meta;
     constexpr int MB = (int)sizeof(Meta);
     constexpr int F = 32 * R;                      // templates per tile
     constexpr int BPB = FMT == FMT_F32 ? 4 : 1;    // bytes per bin
@@ -414,6 +408,9 @@ sum_staged_kernel(const SumParams p)
     const uint32_t slots_e = slots_s + (uint32_t)D * slot_stride;
     const uint32_t bars_s = smem_u32(bars);
     const uint32_t meta_s = smem_u32(meta), meta_e = meta_s + (uint32_t)(MR * MB);
+    // weighted: the warp's ring of RowWgt entries, row for row beside its RowMeta ring
+    RowWgt *wmeta = (RowWgt *)(smem + staged_bar_bytes(D) + (size_t)NW * MR * MB) + warp * MR;
+    const uint32_t wmeta_s = smem_u32(wmeta);
 
     // block -> (SFT chunk, group, f0 tile).  Chunks are the slowest index: the CTAs in flight work
     // on the same few hundred SFT rows, which therefore stay in L2 while every group reads them.
@@ -489,7 +486,8 @@ sum_staged_kernel(const SumParams p)
         mt.flags = 0;
         mt.by16 = -1;
         mt.src_lo = mt.src_hi = 0;
-        if constexpr (WGT) { mt.w = wn; mt.full = 0; mt.ktest = 0; mt.pad = 0; }
+        RowWgt mw = {wn, 0u};
+        bool full = false;
         if (jn + 32 * NW < j1) {          // row_of(n + 32) = jn + 32*NW
             gn = __ldg(g + jn + 32 * NW); dn = __ldg(d + jn + 32 * NW);
             if (WGT && wr) wn = __ldg(wr + jn + 32 * NW);
@@ -519,7 +517,7 @@ sum_staged_kernel(const SumParams p)
         // (band edges, gaps in the data, the steep start of a fast spin-down) every row gets its own 1-D copy.
         bool use2d = false;
         int seg0 = 0, nseg = 0;
-        if (!WGT && p.tmaps) {     // (the weighted instantiation always stages row by row: keep the box code out of it)
+        if (p.tmaps) {
             int kfm = mt.by16 > 0 ? kf : INT32_MAX, klm = mt.by16 > 0 ? kl : INT32_MIN;
             bool all = mt.by16 > 0;
 #pragma unroll
@@ -550,8 +548,8 @@ sum_staged_kernel(const SumParams p)
             const int W = (((int)S - a_byte) >> SH) + kf;
             mt.Q = __dadd_rn(__dadd_rn(__dsub_rn(__dmul_rn(f_first, mt.c), (double)lo_f), p.fix_add + (double)W), TCW_FIX_BASE);
             if constexpr (WGT) {
-                mt.full = (kf >= 0 && kl < p.n_bins) ? 1 : 0;
-                mt.ktest = (uint32_t)(kf - W) - FIX_HC;
+                full = kf >= 0 && kl < p.n_bins;
+                mw.ktest = (uint32_t)(kf - W) - FIX_HC;
             }
         }
         // the first row of every ring slot carries the slot's summary for the consumer
@@ -565,6 +563,10 @@ sum_staged_kernel(const SumParams p)
                 mt.src_lo = (uint32_t)seg0;
                 mt.src_hi = (uint32_t)jn;
             }
+        }
+        if constexpr (WGT) {
+            if (full) mt.flags |= 1024u;
+            wmeta[m_pos] = mw;
         }
         meta[m_pos] = mt;
         m_pos += 32;
@@ -588,7 +590,7 @@ sum_staged_kernel(const SumParams p)
                 lds_v4(meta_i + 16u, u[0], b, lo[0], hi[0]);
                 by[0] = (int)b;
             }
-            if (!WGT && (u[0] & 512u)) {
+            if (u[0] & 512u) {
                 mbar_arrive_expect_tx(bar_i, (uint32_t)by[0]);
                 tensor3_g2s(slot_i, p.tmaps + ((u[0] >> 16) << 7), (int)lo[0], (int)hi[0], bar_i);
                 tot = -1;
@@ -669,7 +671,7 @@ sum_staged_kernel(const SumParams p)
         const int kf = lo_f - p.k_min;
         // where the row was staged: mc = metadata of the slot's first row, sc_ = the slot's first byte
         const uint32_t fl = lds_u32(mc + 16u);
-        const bool box = !WGT && (fl & 512u) != 0;
+        const bool box = (fl & 512u) != 0;
         const int a_byte = box ? 128 * (int)lds_u32(mc + 24u) - (int)p.pad_bytes : (BPB * kf) & ~15;
         const uint32_t S = sc_ + (uint32_t)(n % RB) * (box ? ((fl >> 16) << 7) : (uint32_t)p.slot_bytes);
         const uint32_t base = FIX_HC + (uint32_t)((((int)S - a_byte) >> SH) + kf) - (uint32_t)lo_f;
@@ -682,8 +684,9 @@ sum_staged_kernel(const SumParams p)
     const uint32_t addr0 = 0u - ((uint32_t)BPB * FIX_HC);
     auto add_row = [&](uint32_t mq, const uint32_t (&hi)[R]) {
         if constexpr (WGT) {
-            const float wj = lds_f32(mq + 32u);
-            if (lds_u32(mq + 36u)) {          // warp-uniform: the whole tile is in band
+            const uint32_t wq = wmeta_s + ((mq - meta_s) >> 2);     // the row's RowWgt entry (8 bytes per 32 of RowMeta)
+            const float wj = lds_f32(wq);
+            if (lds_u32(mq + 16u) & 1024u) {  // warp-uniform: the whole tile is in band
                 const double wd = (double)wj;
                 W1u = __dadd_rn(W1u, wd);
                 W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
@@ -695,7 +698,7 @@ sum_staged_kernel(const SumParams p)
                 }
             } else {
                 const float wj2 = __fmul_rn(wj, wj);
-                const uint32_t ktest = lds_u32(mq + 40u);
+                const uint32_t ktest = lds_u32(wq + 4u);
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const uint32_t a = addr0 + (hi[r] << SH);

@@ -213,3 +213,31 @@ def test_multi_sky_count_weighted_uses_staged_kernel(tcw):
     ref = oracle.evaluate_weighted(w, wt, mean1, var1, sel=oracle.group_templates(w, groups))
     sel = (groups[:, None] * n_f0 + np.arange(n_f0)[None, :]).reshape(-1)
     assert_weighted_parity(w, ref, mean1, var1, psi[sel], stat[sel], bs[groups], bi[groups])
+
+
+@pytest.mark.parametrize("fmt", ["f32", "u8"])
+def test_weighted_box_copies_are_bit_identical_to_row_copies(tcw, fmt):
+    """The weighted instantiation stages ring slots by one tensor-map copy like the unweighted one (its weights and
+    band-edge constants live in a second metadata ring); with TCW_OPT_ROW_COPIES it stages row by row.  Same
+    arithmetic in the same order: Psi, s and the best templates must agree bit for bit (cfg1 with and without SFT
+    chunks, which exercises whole-tile rows, band-edge rows and rows past the band)."""
+    import torch
+    w = tcw_inputs.make_workload("cfg1")
+    if fmt != "f32":
+        w = w.with_format(fmt)
+    wts = tcw_inputs.synthetic_weights(w.sky, w.timestamps, 5)
+    mean1, var1 = MOMENTS[fmt]
+    for chunk in (0, 64):
+        out = []
+        for row_copies in (0, 1):
+            with tcw.Handle.from_workload(w) as h:
+                h.set_option(tcw.TCW_OPT_KERNEL, KERNELS["staged"])
+                h.set_option(tcw.TCW_OPT_CHUNK_ROWS, chunk)
+                h.set_option(tcw.TCW_OPT_ROW_COPIES, row_copies)
+                psi, stat, best = h.search_weighted(tcw.Grid.of(w), wts, mean1, var1)
+                torch.cuda.synchronize()
+                info = h.info()
+                assert info["status"] == 0 and info["box_copies"] == 1 - row_copies, info
+                out.append((psi.cpu().numpy().view(np.uint32), stat.cpu().numpy().view(np.uint32), best.cpu().numpy().view(np.uint8)))
+        for a, b in zip(out[0], out[1]):
+            assert np.array_equal(a, b)
