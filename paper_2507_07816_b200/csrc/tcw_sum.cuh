@@ -7,11 +7,12 @@
 // Two kernels compute it:
 //   * sum_staged_kernel -- the product path.  One CTA owns (group, tile of 32*R consecutive f0).
 //     Consecutive f0 of one group select a narrow contiguous bin window per SFT (g <= 1).  Every
-//     warp owns the SFT rows j = j_begin + warp + NW*n and runs its own software pipeline: it
-//     computes the window [k(f_first, j), k(f_last, j)] of a row a few rows ahead, one lane
-//     issues ONE TMA bulk copy (cp.async.bulk, mbarrier complete_tx) of exactly that window
-//     into the warp's private shared-memory ring, and all lanes gather row n from shared memory,
-//     each lane carrying R templates in registers.  The library's spectrogram copy carries
+//     warp owns ring slots of RB consecutive SFT rows (slots warp, warp + NW, ...) and runs its own
+//     software pipeline: it computes the windows [k(f_first, j), k(f_last, j)] of the rows a few slots
+//     ahead, one lane issues ONE TMA copy per slot -- a tensor-map box of {128 B, n segments, RB rows}
+//     (cp.async.bulk.tensor.3d, mbarrier complete_tx) where the rows' windows fit one box, else one 1-D
+//     bulk copy per row -- into the warp's private shared-memory ring, and all lanes gather the rows from
+//     shared memory, each lane carrying R templates in registers.  The library's spectrogram copy carries
 //     PAD_BINS zero bins on both sides of every row, so a window that is partly out of band is
 //     still copied whole and no per-lookup bounds test is needed (out-of-band bins add 0).
 //   * sum_gather_kernel -- one thread per template gathering from global memory.  It serves f0
@@ -578,8 +579,8 @@ sum_staged_kernel(const SumParams p)
 
     int ni = 0;                                  // next slot (RB rows) to stage
     uint32_t bar_i = bars_s, slot_i = slots_s, meta_i = meta_s;
-    // Stage the rows RB*ni .. RB*ni + RB-1: one elected lane reads the rows' copy descriptors and
-    // issues one TMA bulk copy per staged row, all counted on the slot's mbarrier.
+    // Stage the rows RB*ni .. RB*ni + RB-1: one elected lane reads the slot's descriptor and issues one
+    // tensor-map copy for the slot, or one TMA bulk copy per staged row, counted on the slot's mbarrier.
     auto stage_next = [&]() {
         if ((ni & (32 / RB - 1)) == 0) compute_batch(ni / (32 / RB));
         if (elect_one()) {
