@@ -75,11 +75,11 @@ def test_library_is_sm100a_and_has_tma_bulk_copies():
         assert "DMUL" in sass and "DADD" in sass
         # ring slots of four SFT rows travel by one tensor-map TMA copy (cp.async.bulk.tensor.3d)
         assert "UTMALDG.3D" in sass
+        assert ("FFMA" in sass) == (wgt == "1")   # only the weighted sum fuses weight * element + acc
     # the headline instantiation (float32, 16 templates per lane, equally spaced f0) adds row pairs with packed
     # float32 adds
     head = _sass_of("_ZN3tcw17sum_staged_kernelILi0ELi16ELb1ELb0ELb1EEEvNS_9SumParamsE")
     assert "UTMALDG.3D" in head and "UBLKCP" in head and head.count("FADD2") >= 32
-        assert ("FFMA" in sass) == (wgt == "1")   # only the weighted sum fuses weight * element + acc
 
 
 def test_defining_chain_is_never_contracted():
