@@ -435,6 +435,15 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
             "peak_source": "tcw_measure_peaks in this process: independent FFMA streams, one warp instruction per scheduler per cycle",
             "note": "warp instructions of one launch (ncu capture of the shipped build) over the live CUDA-event time of the "
                     "kernel, against the measured issue rate; the instruction count per lookup is what a faster kernel lowers"}
+        if info.get("kernel") == "staged" and ncu.get("l2_sectors") and pk.get("stage_box_copies_bytes_per_s"):
+            # the other co-limit of the staged kernel: bytes its TMA copies draw from L2 (32-byte sectors of the ncu
+            # capture) over the live kernel time, against what the same ring draws when it stages alone
+            l2b = 32.0 * float(ncu["l2_sectors"])
+            block["roofline_binding"]["staging"] = {
+                "achieved_l2_bytes_per_s": l2b / (sum_ms * 1e-3), "peak_bytes_per_s": pk["stage_box_copies_bytes_per_s"],
+                "frac": l2b / (sum_ms * 1e-3) / pk["stage_box_copies_bytes_per_s"], "l2_bytes_per_launch": l2b,
+                "note": "L2 -> shared-memory traffic of the launch (lts__t_sectors of the ncu capture x 32 B) over the live kernel "
+                        "time, against the rate the per-warp rings reach with tensor-map copies and no consumer (tcw_measure_peaks)"}
         if info.get("kernel") == "staged" and inband:
             block["roofline_binding"]["lookup_chain"] = {
                 "achieved_inband_lookups_per_s": inband / (sum_ms * 1e-3), "peak_lookups_per_s": pk["chain_lookups_per_s"],

@@ -349,13 +349,17 @@ int tcw_tables(tcw_handle *h, double *out_g, double *out_d, void *stream);
  *  out[0] FP64 DFMA warp instructions/s   out[1] FP64 DMUL   out[2] FP64 DADD
  *  out[3] FP32 FFMA warp instructions/s (= the schedulers' issue limit, one per scheduler per cycle)
  *  out[4] LDS.32 warp instructions/s for the staged kernel's gather pattern (conflict-free, stride < 1 word)
- *  out[5] lookups/s of the bare lookup chain of sum_staged_kernel (DFMA, address, LDS.32, FADD, half a
- *         VIMNMX3 per lookup; no staging, metadata or band edges): the speed of light of the instruction mix
+ *  out[5] lookups/s of the bare lookup chain of sum_staged_kernel as it ships (two rows per block: DFMA, address,
+ *         LDS.32, half a FADD2, half a VIMNMX3 per lookup; no staging, metadata or band edges): the speed of light
+ *         of the instruction mix
  *  out[6] number of SMs   out[7] nominal maximum SM clock in Hz
  *  out[8] lookups/s of the count formats' chain with one byte per bin (the device layout: LDS.U8 + IADD)
  *  out[9] the same chain gathering from bit-packed windows (LDS.U8 of byte k >> 3, shift by k & 7, mask):
  *         the measurement behind keeping one byte per bin on the device
- * n_out must be >= 10.  Synchronous; takes about 0.15 s. */
+ *  out[10] bytes/s the staged kernel's per-warp ring draws from L2 into shared memory when it stages alone (no
+ *          consumer) with four 1-D bulk copies per slot, out[11] the same with one tensor-map copy per slot
+ *          (both only when n_out >= 12; 0 if the tensor maps cannot be encoded)
+ * n_out must be >= 10.  Synchronous; takes about 0.2 s. */
 int tcw_measure_peaks(double *out, int n_out, void *stream);
 
 /* Options.  tcw_set_option returns TCW_EINVAL for an unknown key or value. */

@@ -492,11 +492,12 @@ def prepare(strain, fs: float, T_sft: float, f_min: float, n_bins: int, median_b
 
 def measure_peaks(stream=None) -> dict:
     """tcw_measure_peaks: measured whole-GPU rates of the limits that bind the kernels (per second)."""
-    out = (ctypes.c_double * 10)()
-    _check(load_library().tcw_measure_peaks(out, 10, _stream_ptr(stream)))
+    out = (ctypes.c_double * 12)()
+    _check(load_library().tcw_measure_peaks(out, 12, _stream_ptr(stream)))
     keys = ("fp64_dfma_winst_per_s", "fp64_dmul_winst_per_s", "fp64_dadd_winst_per_s", "issue_winst_per_s",
             "lds32_winst_per_s", "chain_lookups_per_s", "n_sm", "sm_clock_max_hz",
-            "count_chain_u8_lookups_per_s", "count_chain_bitpacked_lookups_per_s")
+            "count_chain_u8_lookups_per_s", "count_chain_bitpacked_lookups_per_s",
+            "stage_row_copies_bytes_per_s", "stage_box_copies_bytes_per_s")
     return dict(zip(keys, (float(x) for x in out)))
 
 

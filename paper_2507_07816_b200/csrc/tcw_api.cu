@@ -1817,6 +1817,32 @@ int tcw_measure_peaks(double *out, int n_out, void *stream)
         timed([&] { tcw::peak_count_chain_kernel<false><<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, (int *)d_out); }, work, &out[8]);
         timed([&] { tcw::peak_count_chain_kernel<true><<<c_ctas, 128, 0, st>>>(rows, 0.93, 1572864.0 + 8.5, (int *)d_out); }, work, &out[9]);
     }
+    if (n_out >= 12) {
+        // staging alone (peak_stage_kernel): 2048 rows of a 20 000-bin float32 band, 2080-byte windows
+        out[10] = out[11] = 0.0;
+        const long pitch = 81920 + 8448;
+        const int n_rows = 2048, slots = 128, c_ctas = n_sm * 3 * 8;
+        unsigned char *d_arr = nullptr, *d_maps = nullptr;
+        const size_t smem = 128 + (size_t)4 * 2 * tcw::RB * tcw::PEAK_STAGE_ROW;
+        if (cudaMalloc((void **)&d_arr, (size_t)pitch * n_rows) == cudaSuccess) {
+            cudaMemsetAsync(d_arr, 1, (size_t)pitch * n_rows, st);
+            cudaFuncSetAttribute(tcw::peak_stage_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(tcw::peak_stage_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            const double n_slots = (double)c_ctas * 4 * slots;
+            timed([&] { tcw::peak_stage_kernel<false><<<c_ctas, 128, smem, st>>>(d_arr, pitch, n_rows, slots, 2080, nullptr, 0, (unsigned *)d_out); },
+                  n_slots * tcw::RB * 2080.0, &out[10]);
+            std::vector<CUtensorMap> maps;
+            if (encode_box_maps(d_arr, pitch, n_rows, maps) && cudaMalloc((void **)&d_maps, maps.size() * sizeof(CUtensorMap)) == cudaSuccess) {
+                cudaMemcpy(d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice);
+                timed([&] { tcw::peak_stage_kernel<true><<<c_ctas, 128, smem, st>>>(d_arr, pitch, n_rows, slots, 0, d_maps, 17, (unsigned *)d_out); },
+                      n_slots * tcw::RB * 17.0 * 128.0, &out[11]);
+            }
+            cudaStreamSynchronize(st);
+            cudaFree(d_maps);
+            cudaFree(d_arr);
+        }
+        cudaGetLastError();
+    }
     out[6] = (double)n_sm;
     int khz = 0;
     cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);

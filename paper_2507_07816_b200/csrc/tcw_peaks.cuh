@@ -11,6 +11,8 @@
 //   * the bare lookup chain of the staged kernel as it ships (one DFMA, one address LEA, one LDS.32, half a FADD2,
 //     half a VIMNMX3 per lookup, two rows of 16 lookups per straight-line block) -- the speed of light of the
 //     design's instruction mix, in lookups per second.
+//   * the staged kernel's ring alone (no consumer): four 1-D bulk copies per slot against one tensor-map copy per
+//     slot -- the L2 -> shared-memory staging rate, in bytes per second.
 // Rates are whole-GPU, per second.  The numbers are only as good as the clocks of the moment; bench.py
 // measures them in the same process as the timed search and prints the SM clock beside them.
 #pragma once
@@ -220,6 +222,58 @@ peak_count_chain_kernel(int rows, double c0, double q0, int *out)
 #pragma unroll
     for (int r = 0; r < 16; ++r) s += acc[r];
     if (s == 123456789 || mn_all == 1u) out[0] = s;
+}
+
+// Staging alone: every warp runs the staged kernel's two-slot ring over a spectrogram-like array (rows of a 20 000-bin
+// float32 band, windows drifting like a track) and consumes nothing.  BOX = false: four 1-D bulk copies of `bytes`
+// per slot (round 1's staging); BOX = true: one tensor-map copy of {128 B, nseg, RB rows} per slot.  The rate is the
+// L2 -> shared-memory throughput the ring can draw with twelve warps per SM.
+constexpr int PEAK_STAGE_ROW = 2304;     // shared-memory bytes per staged row
+template <bool BOX>
+__global__ void __launch_bounds__(128, 3)
+peak_stage_kernel(const unsigned char *spec, long pitch, int n_rows, int slots, int bytes, const unsigned char *tmaps, int nseg, unsigned *out)
+{
+    extern __shared__ __align__(128) unsigned char peak_smem[];
+    const int warp = (int)__reduce_or_sync(0xffffffffu, threadIdx.x >> 5), lane = threadIdx.x & 31;
+    const uint32_t bar0 = smem_u32(peak_smem) + 16u * warp;
+    unsigned char *ring = peak_smem + 128 + (size_t)warp * 2 * RB * PEAK_STAGE_ROW;
+    const uint32_t ring0 = smem_u32(ring);
+    if (lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8u, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    const long gw = (long)blockIdx.x * 4 + warp;
+    const int row = (int)((gw * 37) % (n_rows - RB * slots - 8));
+    const int col = 4096 + (int)((gw * 53) % 4096) * 16;      // byte offset in the row, 16-byte aligned
+    unsigned acc = 0;
+    uint32_t ph = 0;
+    auto issue = [&](int s, int n) {
+        if (elect_one()) {
+            const int r0 = row + RB * n, c0 = col - 48 * n;
+            const uint32_t bar = bar0 + 8u * s, dst = ring0 + (uint32_t)(s * RB * PEAK_STAGE_ROW);
+            if (!BOX) {
+                mbar_arrive_expect_tx(bar, (uint32_t)(RB * bytes));
+#pragma unroll
+                for (int q = 0; q < RB; ++q)
+                    bulk_g2s(dst + q * PEAK_STAGE_ROW, spec + (long)(r0 + q) * pitch + c0 - 16 * q, (uint32_t)bytes, bar);
+            } else {
+                mbar_arrive_expect_tx(bar, (uint32_t)(RB * 128 * nseg));
+                tensor3_g2s(dst, tmaps + 128 * nseg, c0 >> 7, r0, bar);
+            }
+        }
+    };
+    issue(0, 0);
+    for (int n = 0; n < slots; ++n) {
+        const int s = n & 1;
+        if (n + 1 < slots) issue(s ^ 1, n + 1);
+        mbar_wait(bar0 + 8u * s, ph);
+        acc += *(volatile unsigned *)(ring + (size_t)s * RB * PEAK_STAGE_ROW + 4 * lane);
+        __syncwarp();
+        if (s == 1) ph ^= 1u;
+    }
+    if (acc == 0x12345678u) out[0] = acc;
 }
 
 }  // namespace tcw

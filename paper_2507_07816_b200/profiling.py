@@ -148,6 +148,7 @@ def summary(argv):
             "fp64_pipe_pct": get("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_elapsed", False),
             "lds_wavefronts": get("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", False),
             "l2_hit_pct": get("lts__t_sector_hit_rate.pct", False),
+            "l2_sectors": get("lts__t_sectors.sum", False),
             "registers_per_thread": get("launch__registers_per_thread", False),
             "grid_size": get("launch__grid_size", False),
         }
