@@ -277,6 +277,17 @@ __device__ __forceinline__ void fadd2(float &o0, float &o1, float a0, float a1, 
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     asm("mov.b64 {%0, %1}, %2;" : "=f"(o0), "=f"(o1) : "l"(r));
 }
+// two float32 fused multiply-adds in one instruction (fma.rn.f32x2, SASS FFMA2): each half rounds exactly like a
+// scalar __fmaf_rn
+__device__ __forceinline__ void ffma2(float &o0, float &o1, float w, float b0, float b1, float c0, float c1)
+{
+    unsigned long long a, b, c, r;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(a) : "f"(w));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(b0), "f"(b1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c) : "f"(c0), "f"(c1));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(o0), "=f"(o1) : "l"(r));
+}
 __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 {
     uint32_t v;
@@ -691,26 +702,36 @@ sum_staged_kernel(const SumParams p)
                 const double wd = (double)wj;
                 W1u = __dadd_rn(W1u, wd);
                 W2u = __dadd_rn(W2u, __dmul_rn(wd, wd));
+                float v[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const uint32_t a = addr0 + (hi[r] << SH);
-                    const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
-                    acc[r] = __fmaf_rn(wj, v, acc[r]);
+                    v[r] = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
                 }
+#pragma unroll
+                for (int r = 0; r < R; r += 2) ffma2(acc[r], acc[r + 1], wj, v[r], v[r + 1], acc[r], acc[r + 1]);
             } else {
                 const float wj2 = __fmul_rn(wj, wj);
                 const uint32_t ktest = lds_u32(wq + 4u);
+                float v[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     const uint32_t a = addr0 + (hi[r] << SH);
-                    const float v = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
-                    acc[r] = __fmaf_rn(wj, v, acc[r]);
+                    v[r] = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
                     if (hi[r] + ktest < (uint32_t)p.n_bins) {
                         w1p[r] = __fadd_rn(w1p[r], wj);
                         w2p[r] = __fadd_rn(w2p[r], wj2);
                     }
                 }
+#pragma unroll
+                for (int r = 0; r < R; r += 2) ffma2(acc[r], acc[r + 1], wj, v[r], v[r + 1], acc[r], acc[r + 1]);
             }
+        } else if constexpr (FMT == FMT_F32 && TCW_FADD2) {
+            float v[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[r] = lds_f32(addr0 + (hi[r] << SH));
+#pragma unroll
+            for (int r = 0; r < R; r += 2) fadd2(acc[r], acc[r + 1], acc[r], acc[r + 1], v[r], v[r + 1]);
         } else {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
