@@ -398,8 +398,10 @@ sum_staged_kernel(const SumParams p)
 #ifndef TCW_FADD2
 #define TCW_FADD2 1
 #endif
-    constexpr bool PAIR = TCW_PAIR && RB % 2 == 0 && !WGT;     // live slots are consumed two rows at a time (the weighted kernel's
-                                                   // per-lane weight sums leave no registers for that)
+#ifndef TCW_WGT_PAIR
+#define TCW_WGT_PAIR 1
+#endif
+    constexpr bool PAIR = TCW_PAIR && RB % 2 == 0 && (!WGT || TCW_WGT_PAIR);     // live slots are consumed two rows at a time
     typedef typename AccW<FMT, WGT>::type V;
     typedef RowMeta Meta;
     constexpr int MB = (int)sizeof(Meta);
@@ -767,7 +769,44 @@ sum_staged_kernel(const SumParams p)
                     const uint32_t mn0 = fast_row(mq0, hi0);
                     const uint32_t mn1 = fast_row(mq1, hi1);
                     if constexpr (WGT || !UNI) {
-                        if (min(mn0, mn1) <= p.thr2) {
+                        bool done = false;
+                        if constexpr (WGT && FMT == FMT_F32) {
+                            if (lds_u32(mq0 + 16u) & lds_u32(mq1 + 16u) & 1024u) {
+                                // weighted, the whole tile in band in both rows (warp-uniform): both rows' elements are
+                                // gathered with the fast indices before the guard band is consulted, then accumulated
+                                // in the order of the one-row path (row q, then row q + 1: bit-identical to it), so the
+                                // gathers of one row overlap the arithmetic of the other
+                                const uint32_t wq0 = wmeta_s + ((mq0 - meta_s) >> 2);
+                                const float wa = lds_f32(wq0), wb = lds_f32(wq0 + (uint32_t)sizeof(RowWgt));
+                                float v0[R], v1[R];
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    v0[r] = lds_f32(addr0 + (hi0[r] << SH));
+                                    v1[r] = lds_f32(addr0 + (hi1[r] << SH));
+                                }
+                                if (min(mn0, mn1) <= p.thr2) {
+                                    uint32_t ex0[R], ex1[R];
+                                    exact_row(RB * nc + q, meta_c, slot_c, ex0);
+                                    exact_row(RB * nc + q + 1, meta_c, slot_c, ex1);
+#pragma unroll
+                                    for (int r = 0; r < R; ++r) {
+                                        v0[r] = lds_f32(addr0 + (ex0[r] << SH));
+                                        v1[r] = lds_f32(addr0 + (ex1[r] << SH));
+                                    }
+                                }
+                                const double wda = (double)wa, wdb = (double)wb;
+                                W1u = __dadd_rn(__dadd_rn(W1u, wda), wdb);
+                                W2u = __dadd_rn(__dadd_rn(W2u, __dmul_rn(wda, wda)), __dmul_rn(wdb, wdb));
+#pragma unroll
+                                for (int r = 0; r < R; r += 2) {
+                                    ffma2(acc[r], acc[r + 1], wa, v0[r], v0[r + 1], acc[r], acc[r + 1]);
+                                    ffma2(acc[r], acc[r + 1], wb, v1[r], v1[r + 1], acc[r], acc[r + 1]);
+                                }
+                                done = true;
+                            }
+                        }
+                        if (done) {
+                        } else if (min(mn0, mn1) <= p.thr2) {
                             uint32_t ex0[R], ex1[R];
                             exact_row(RB * nc + q, meta_c, slot_c, ex0);
                             exact_row(RB * nc + q + 1, meta_c, slot_c, ex1);
