@@ -284,7 +284,7 @@ struct tcw_handle {
     // asynchronous upload (tcw_create_async): pieces of rows copied on up_stream, one event per piece
     cudaStream_t up_stream = nullptr;
     std::vector<cudaEvent_t> up_ev;
-    long up_rows = 0;            // rows per piece
+    std::vector<long> up_end;    // one past the last row of each piece
     bool up_pending = false;     // the first search still has to wait for the pieces
     void *up_staging = nullptr;  // tightly packed device copy the pieces land in before the re-lay
     long info[12] = {0, 0, 0, 0, 0, 0, 0, 0, 1, 0, 0, 0};
@@ -675,7 +675,10 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
     CREATE_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned long long), st));
     CREATE_TRY(cudaEventCreateWithFlags(&h->ev_stage, cudaEventDisableTiming));
     CREATE_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
-    CREATE_TRY(cudaMemsetAsync(h->d_spec, 0, (size_t)h->pitch * n_sft, st));   // the padding must read as zero
+    // the padding on either side of every row must read as zero (the payload is overwritten by the copies below)
+    CREATE_TRY(cudaMemset2DAsync(h->d_spec, (size_t)h->pitch, 0, (size_t)h->pad_bytes, (size_t)n_sft, st));
+    CREATE_TRY(cudaMemset2DAsync(h->d_spec + h->pad_bytes + dev_row, (size_t)h->pitch, 0,
+                                 (size_t)h->pitch - (size_t)h->pad_bytes - dev_row, (size_t)n_sft, st));
     {
         // tensor maps of the staged kernel (SumParams::tmaps); without the driver entry point the kernel
         // falls back to one 1-D bulk copy per row
@@ -726,9 +729,12 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
             cudaEventRecord(ready, st);                       // allocations and the zero fill precede the pieces
             cudaStreamWaitEvent(h->up_stream, ready, 0);
             cudaEventDestroy(ready);
-            h->up_rows = std::max<long>(64, (long)((16 << 20) / dev_row));
-            for (long j0 = 0; j0 < n_sft; j0 += h->up_rows) {
-                const size_t nr = (size_t)std::min<long>(h->up_rows, n_sft - j0);
+            // pieces of 16 MB while the first search is waiting to start, 64 MB afterwards (fewer calls and events)
+            const long rows16 = std::max<long>(64, (long)((16 << 20) / dev_row));
+            long up_rows = rows16;
+            for (long j0 = 0; j0 < n_sft; j0 += up_rows) {
+                up_rows = h->up_end.size() < 8 ? rows16 : 4 * rows16;
+                const size_t nr = (size_t)std::min<long>(up_rows, n_sft - j0);
                 unsigned char *stg = (unsigned char *)h->up_staging + (size_t)j0 * dev_row;
                 CREATE_TRY(cudaMemcpyAsync(stg, (const unsigned char *)spectrogram + (size_t)j0 * dev_row, nr * dev_row,
                                            cudaMemcpyHostToDevice, h->up_stream));
@@ -737,6 +743,7 @@ static int create_impl(tcw_handle **out, const void *spectrogram, int format, lo
                 cudaEvent_t e;
                 CREATE_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
                 h->up_ev.push_back(e);
+                h->up_end.push_back(j0 + (long)nr);
                 CREATE_TRY(cudaEventRecord(e, h->up_stream));
             }
             h->up_pending = true;
@@ -791,7 +798,7 @@ int tcw_create_async(tcw_handle **out, const void *spectrogram, int format, long
 static void upload_wait_rows(tcw_handle *h, long j_end, cudaStream_t st)
 {
     if (!h->up_pending || h->up_ev.empty()) return;
-    long k = (std::max<long>(j_end, 1) - 1) / h->up_rows;
+    long k = (long)(std::lower_bound(h->up_end.begin(), h->up_end.end(), std::max<long>(j_end, 1)) - h->up_end.begin());
     k = std::min<long>(k, (long)h->up_ev.size() - 1);
     cudaStreamWaitEvent(st, h->up_ev[(size_t)k], 0);
 }
