@@ -720,10 +720,7 @@ sum_staged_kernel(const SumParams p)
                 for (int r = 0; r < R; ++r) {
                     const uint32_t a = addr0 + (hi[r] << SH);
                     v[r] = FMT == FMT_F32 ? lds_f32(a) : (float)lds_u8(a);
-                    if (hi[r] + ktest < (uint32_t)p.n_bins) {
-                        w1p[r] = __fadd_rn(w1p[r], wj);
-                        w2p[r] = __fadd_rn(w2p[r], wj2);
-                    }
+                    if (hi[r] + ktest < (uint32_t)p.n_bins) fadd2(w1p[r], w2p[r], w1p[r], w2p[r], wj, wj2);   // both counters in one add
                 }
 #pragma unroll
                 for (int r = 0; r < R; r += 2) ffma2(acc[r], acc[r + 1], wj, v[r], v[r + 1], acc[r], acc[r + 1]);
