@@ -340,3 +340,17 @@ def test_box_copies_are_bit_identical_to_row_copies(tcw, fmt):
         assert np.array_equal(b_box.view(np.uint8), b_row.view(np.uint8)), w.name
         assert_stat_parity(w, s_box.reshape(-1), ref.stat)
     assert n_box > 0, "no case exercised the tensor-map copies"
+
+
+def test_measured_peaks_are_sane(tcw):
+    """tcw_measure_peaks: every rate is positive and in the order the hardware imposes -- FP64 at about half the
+    issue rate, the shipped lookup chain below 32 lookups per issued instruction, a tensor-map copy per slot staging
+    at least as fast as four bulk copies per slot (within noise), bit-packed gathers slower than byte gathers."""
+    import torch
+    torch.cuda.set_device(0)
+    p = tcw.measure_peaks()
+    assert all(v > 0 for v in p.values()), p
+    assert 0.35 < p["fp64_dfma_winst_per_s"] / p["issue_winst_per_s"] < 0.6
+    assert p["chain_lookups_per_s"] < 32 * p["issue_winst_per_s"] / 3.5
+    assert p["stage_box_copies_bytes_per_s"] > 0.9 * p["stage_row_copies_bytes_per_s"] > 5e12
+    assert p["count_chain_bitpacked_lookups_per_s"] < p["count_chain_u8_lookups_per_s"]
