@@ -289,6 +289,37 @@ int tcw_topk(tcw_handle *h, const void *values, int dtype, long n, int K, void *
 int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, double threshold,
                      long capacity, long long *out_idx, long long *out_count, void *stream);
 
+/* tcw_select_above_static -- tcw_select_above for callers that must not allocate device memory.
+ *
+ * Who that is: a search job that sized its spectrograms and result arrays to fill the GPU and has
+ * nothing left for a library to take; a host program whose own caching allocator owns the device
+ * memory, so that a cudaMalloc from inside a library can fail even though "free" memory exists; and a
+ * follow-up loop that runs beside searches on other streams, where cudaMalloc / cudaFree would
+ * synchronise the whole device and stall them.  The other selection calls take their scratch from
+ * the handle's grow-only pool block, and making a handle allocates; this call needs no handle.
+ *
+ * Same selection, same kernels, same results as tcw_select_above (the templates with
+ * Psi > Psi_noise max): the indices i with values[i] > threshold, ascending; NaN never selected.
+ * The scratch (per-CTA counts and offsets, one byte per row of 128 values) lives in ONE array that
+ * is part of the library image: about 2.1 MB on every GPU that loads libtcw.so, held until the
+ * process exits.  The call makes no cudaMalloc, cudaFree, pool or library allocation; the caller
+ * supplies inputs and outputs.
+ *  values     DEVICE [n], dtype 0: float32, 1: int32;  1 <= n <= TCW_SELECT_STATIC_MAX_N.
+ *             A larger n returns TCW_EUNSUPPORTED and touches nothing (use tcw_select_above).
+ *  out_idx    DEVICE [capacity] int64 (may be NULL when capacity == 0): the first `capacity` hits;
+ *  out_count  DEVICE int64: the total number of hits (may exceed capacity).
+ * Works on the CURRENT device (cudaSetDevice before calling); asynchronous on `stream`.
+ * First call on each device: looks up the device address of the array (cudaGetSymbolAddress) and
+ * keeps it.  Make that first call during set-up, before any stream capture is begun.
+ * Sharing: every call on a device uses the same array, and the array keeps what the previous call
+ * left in it.  The call itself clears the part that must start at zero (the per-row counts of the
+ * rows it covers), so back-to-back calls on one stream are independent.  Two calls that may run
+ * at the same time on one GPU (different streams, or different threads) RACE on the array and give
+ * wrong results: order them on one stream or with events. */
+#define TCW_SELECT_STATIC_MAX_N (1L << 28)
+int tcw_select_above_static(const void *values, int dtype, long n, double threshold, long capacity,
+                            long long *out_idx, long long *out_count, void *stream);
+
 /* ---- data preparation ----------------------------------------
  *
  * "The data used in this study are 8-second Han-windowed Short Fourier Transforms (SFTs), which

@@ -32,7 +32,7 @@ KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
 EXPORTS = (
-    "tcw_create", "tcw_create_async", "tcw_upload_wait", "tcw_search", "tcw_search_groups", "tcw_split_groups", "tcw_check", "tcw_measure_peaks", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_prepare", "tcw_destroy", "tcw_last_error",
+    "tcw_create", "tcw_create_async", "tcw_upload_wait", "tcw_search", "tcw_search_groups", "tcw_split_groups", "tcw_check", "tcw_measure_peaks", "tcw_search_host", "tcw_search_weighted", "tcw_search_bank", "tcw_get_counter", "tcw_topk", "tcw_select_above", "tcw_select_above_static", "tcw_prepare", "tcw_destroy", "tcw_last_error",
     "tcw_track_indices", "tcw_tables", "tcw_set_option", "tcw_get_timing", "tcw_get_info",
 )
 
@@ -112,6 +112,8 @@ def load_library(rebuild: bool = False) -> ctypes.CDLL:
     L.tcw_topk.argtypes = [vp, vp, ci, cl, ci, vp, vp, vp, vp]
     L.tcw_select_above.restype = ci
     L.tcw_select_above.argtypes = [vp, vp, ci, cl, ctypes.c_double, cl, vp, vp, vp]
+    L.tcw_select_above_static.restype = ci
+    L.tcw_select_above_static.argtypes = [vp, ci, cl, ctypes.c_double, cl, vp, vp, vp]
     L.tcw_prepare.restype = ci
     L.tcw_prepare.argtypes = [vp, cl, ctypes.POINTER(_CPrep), ci, vp, cl, ctypes.POINTER(ci), vp]
     L.tcw_destroy.restype = ci
@@ -488,6 +490,30 @@ def prepare(strain, fs: float, T_sft: float, f_min: float, n_bins: int, median_b
     _check(L.tcw_prepare(ptr, n, ctypes.byref(cp), FORMATS[fmt], out.data_ptr(), out.stride(0) * out.element_size(),
                          ctypes.byref(got), _stream_ptr(stream)))
     return out[: got.value]
+
+
+SELECT_STATIC_MAX_N = 1 << 28   # TCW_SELECT_STATIC_MAX_N of include/tcw.h
+
+
+def select_above_static(values, threshold: float, out_idx, out_count, stream=None) -> None:
+    """tcw_select_above_static: Handle.select_above for callers that may not allocate on the GPU
+    (the job already filled the device with its own arrays, the host program's allocator owns the
+    memory, or a cudaMalloc would stall searches running on other streams).  No handle, and nothing
+    is allocated here either: the caller passes the outputs, `out_idx` an int64 CUDA tensor whose
+    length is the capacity (may be empty) and `out_count` an int64 CUDA tensor with one element.
+    The scratch is a fixed array inside libtcw.so, so `values` holds at most SELECT_STATIC_MAX_N
+    entries (TcwError beyond that) and calls that overlap on one GPU race; on one stream they are
+    safe back to back.  Runs on the current device; make the first call before any stream capture.
+    Asynchronous."""
+    import torch
+    if not values.is_contiguous():
+        raise ValueError("values must be contiguous (this call makes no copy)")
+    if out_idx.dtype != torch.int64 or out_count.dtype != torch.int64 or out_count.numel() < 1 or not out_idx.is_contiguous():
+        raise ValueError("out_idx and out_count must be contiguous int64 CUDA tensors, out_count with one element")
+    cap = out_idx.numel()
+    _check(load_library().tcw_select_above_static(values.data_ptr(), Handle._sel_dtype(values), values.numel(), float(threshold),
+                                                  cap, out_idx.data_ptr() if cap > 0 else None, out_count.data_ptr(),
+                                                  _stream_ptr(stream)))
 
 
 def measure_peaks(stream=None) -> dict:

@@ -1489,6 +1489,93 @@ int tcw_select_above(tcw_handle *h, const void *values, int dtype, long n, doubl
     return TCW_OK;
 }
 
+// ---- tcw_select_above_static: the threshold selection with its scratch inside the library image ---------
+// For callers that cannot let a library allocate (a job that filled the GPU with its own arrays, a host
+// program whose allocator owns the device memory, a loop that must not take the device-wide synchronisation of
+// cudaMalloc / cudaFree while searches run on other streams): include/tcw.h has the contract.  The scratch that
+// tcw_select_above takes from the handle is here one file-scope device array, laid out as
+//   [SSEL_OFF_GT]  off_gt   SEL_MAX_BLOCKS x u64    exclusive scan of the per-CTA hit counts
+//   [SSEL_OFF_EQ]  off_eq   SEL_MAX_BLOCKS x u64    (written by the shared scan kernel, unused by this selection)
+//   [SSEL_STATE]   SelState 256 bytes               .count = total hits
+//   [SSEL_BLK_GT]  blk_gt   SEL_MAX_BLOCKS x u32    hits per CTA, every launched CTA writes its entry
+//   [SSEL_BLK_EQ]  blk_eq   SEL_MAX_BLOCKS x u32
+//   [SSEL_ROWS]    row_cnt  one byte per row of SEL_ROW values: must be ZERO where no value is selected, and
+//                           the count kernel writes only rows that hold a hit -> cleared on every call
+// Every GPU that loads the library carries the array (SSEL_BYTES, about 2.1 MB) until the process exits.
+namespace {
+constexpr size_t SSEL_OFF_GT = 0;
+constexpr size_t SSEL_OFF_EQ = SSEL_OFF_GT + (size_t)tcw::SEL_MAX_BLOCKS * 8;
+constexpr size_t SSEL_STATE = SSEL_OFF_EQ + (size_t)tcw::SEL_MAX_BLOCKS * 8;
+constexpr size_t SSEL_BLK_GT = SSEL_STATE + 256;
+constexpr size_t SSEL_BLK_EQ = SSEL_BLK_GT + (size_t)tcw::SEL_MAX_BLOCKS * 4;
+constexpr size_t SSEL_ROWS = SSEL_BLK_EQ + (size_t)tcw::SEL_MAX_BLOCKS * 4;
+constexpr size_t SSEL_MAX_ROWS = (size_t)(TCW_SELECT_STATIC_MAX_N / tcw::SEL_ROW);
+constexpr size_t SSEL_BYTES = SSEL_ROWS + SSEL_MAX_ROWS;
+static_assert(sizeof(tcw::SelState) <= 256 && SSEL_ROWS % 256 == 0 && TCW_SELECT_STATIC_MAX_N % tcw::SEL_ROW == 0,
+              "static selection scratch layout");
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_static_select_scratch[SSEL_BYTES];
+
+namespace {
+// In host code `g_static_select_scratch` is only the host-side handle of the symbol, not an address a kernel can
+// use: the device address differs per GPU and comes from cudaGetSymbolAddress with that GPU current.  Looked up
+// once per device and kept (the lookup allocates nothing; it may load the module, hence "before stream capture").
+int static_select_scratch(unsigned char **out)
+{
+    static std::mutex mu;
+    static unsigned char *ptr[64];
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(TCW_EUNSUPPORTED, "device ordinal %d is outside 0..63", dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void *p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_static_select_scratch));
+        if (!p) return fail(TCW_ECUDA, "cudaGetSymbolAddress gave a NULL address for the static selection scratch");
+        ptr[dev] = (unsigned char *)p;
+    }
+    *out = ptr[dev];
+    return TCW_OK;
+}
+}  // namespace
+
+int tcw_select_above_static(const void *values, int dtype, long n, double threshold, long capacity, long long *out_idx,
+                            long long *out_count, void *stream)
+{
+    if (!values || !out_count || (capacity > 0 && !out_idx)) return fail(TCW_EINVAL, "NULL array pointer");
+    if (dtype != 0 && dtype != 1) return fail(TCW_EINVAL, "dtype must be 0 (float32) or 1 (int32)");
+    if (n <= 0 || capacity < 0) return fail(TCW_EINVAL, "n must be positive and capacity >= 0");
+    if (std::isnan(threshold)) return fail(TCW_EINVAL, "threshold is NaN");
+    if (n > TCW_SELECT_STATIC_MAX_N)
+        return fail(TCW_EUNSUPPORTED, "n = %ld exceeds TCW_SELECT_STATIC_MAX_N = %ld, the size the library's built-in scratch "
+                    "covers; use tcw_select_above (scratch from a handle) for larger arrays", n, (long)TCW_SELECT_STATIC_MAX_N);
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *base = nullptr;
+    int rc = static_select_scratch(&base);
+    if (rc != TCW_OK) return rc;
+    unsigned long long *off_gt = (unsigned long long *)(base + SSEL_OFF_GT), *off_eq = (unsigned long long *)(base + SSEL_OFF_EQ);
+    tcw::SelState *state = (tcw::SelState *)(base + SSEL_STATE);
+    unsigned int *blk_gt = (unsigned int *)(base + SSEL_BLK_GT), *blk_eq = (unsigned int *)(base + SSEL_BLK_EQ);
+    unsigned char *row_cnt = base + SSEL_ROWS;
+    long seg;
+    int nb;
+    sel_grid(n, &seg, &nb);
+    const unsigned int *v = (const unsigned int *)values;
+    const int vec = ((uintptr_t)values & 15) == 0;
+    const size_t n_rows = (size_t)((n + tcw::SEL_ROW - 1) / tcw::SEL_ROW);
+    // the previous call's row counts are still there: clear the rows this call covers (everything else in the
+    // array is written before it is read: blk_* by every CTA of the count pass, off_* and state->count by the scan)
+    CUDA_TRY(cudaMemsetAsync(row_cnt, 0, n_rows, st));
+    tcw::sel_count_kernel<true><<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, state, threshold, blk_gt, blk_eq, 0, row_cnt);
+    tcw::sel_scan_kernel<<<1, 256, 0, st>>>(blk_gt, blk_eq, nb, off_gt, off_eq, state);
+    if (capacity > 0)
+        tcw::sel_scatter_rows_kernel<<<nb, tcw::SEL_THREADS, 0, st>>>(v, n, seg, dtype, vec, threshold, row_cnt, off_gt, capacity, out_idx);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(out_count, &state->count, sizeof(long long), cudaMemcpyDeviceToDevice, st));
+    return TCW_OK;
+}
+
 int tcw_prepare(const float *strain, long n_samples, const tcw_prep *prep, int format, void *out_spectrogram,
                 long out_pitch_bytes, int *n_sft, void *stream)
 {
