@@ -242,7 +242,9 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
     key = f"{w.name}:{w.fmt}"
     grid = tcw.Grid.of(w)
     n_sft, n_f0 = w.n_sft, len(w.f0)
-    g_lo, g_hi = tcw.shard_groups(grid.n_groups, rank, world) if world > 1 else (0, grid.n_groups)
+    # N > 1: contiguous whole-group ranges of nearly equal in-band WORK, not equal counts
+    g_lo, g_hi = (tcw.shard_groups(grid.n_groups, rank, world, weights=tcw.group_work(grid, w.timestamps, w.T_sft, w.f_min, w.n_bins))
+                  if world > 1 else (0, grid.n_groups))
     my_groups = g_hi - g_lo
     nominal = float(grid.n_templates) * n_sft                       # whole job, all ranks
     stream = torch.cuda.current_stream()
@@ -483,6 +485,8 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     tcw.load_library()
+    if args.shard_table:
+        return run_shard_table(args, tcw, tcw_inputs, dev)
     if args.shard:
         # one rank's share of an N-GPU strong-scaling run, timed alone on this GPU (no process group): what
         # rank R of `torchrun --nproc-per-node N bench.py --gpus N` executes, for boxes with a single GPU
@@ -559,7 +563,7 @@ def run_shard(args, tcw, tcw_inputs, dev, r, n):
     name, fmt = headline_name(args)
     w = tcw_inputs.make_workload(name, fmt=fmt)
     grid = tcw.Grid.of(w)
-    lo, hi = tcw.shard_groups(grid.n_groups, r, n)
+    lo, hi = tcw.shard_groups(grid.n_groups, r, n, weights=tcw.group_work(grid, w.timestamps, w.T_sft, w.f_min, w.n_bins))
     h = tcw.Handle.from_workload(w, device=dev)
     out_stat = torch.empty((max(hi - lo, 1), len(w.f0)), dtype=h.stat_dtype, device=dev)
     out_best = torch.empty((max(hi - lo, 1), 2), dtype=torch.int32, device=dev)
@@ -587,6 +591,53 @@ def run_shard(args, tcw, tcw_inputs, dev, r, n):
                       "ms_per_step": ms, "rank_lookups_per_s": (hi - lo) * len(w.f0) * w.n_sft / (ms * 1e-3),
                       "kernels_per_step": info["launches"], "ctas": info["ctas"],
                       "slice_equals_whole_search": same, "steps": args.steps, "warmup": args.warmup}), flush=True)
+    return 0
+
+
+def run_shard_table(args, tcw, tcw_inputs, dev):
+    """--shard-table 2,4,8: ONE-GPU EMULATION of the multi-GPU split, not a scaling measurement.  For every N
+    and both cuts (equal group count / equal in-band work) each rank's range is timed alone on this GPU;
+    predicted efficiency = (single-GPU time / N) / (slowest rank's time).  What it leaves out: N uploads of
+    the spectrogram over PCIe and anything the GPUs share (nothing on the data path)."""
+    import torch
+    name, fmt = headline_name(args)
+    w = tcw_inputs.make_workload(name, fmt=fmt)
+    grid = tcw.Grid.of(w)
+    work = tcw.group_work(grid, w.timestamps, w.T_sft, w.f_min, w.n_bins)
+    h = tcw.Handle.from_workload(w, device=dev)
+    out_stat = torch.empty((grid.n_groups, len(w.f0)), dtype=h.stat_dtype, device=dev)
+    out_best = torch.empty((grid.n_groups, 2), dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def timed(lo, hi):
+        if hi == lo:
+            return 0.0
+        for _ in range(args.warmup):
+            h.search_groups(grid, lo, hi, out_stat, out_best)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            h.search_groups(grid, lo, hi, out_stat, out_best)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps
+
+    single = timed(0, grid.n_groups)
+    table = {}
+    for n in (int(x) for x in args.shard_table.split(",")):
+        row = {}
+        for cut, wts in (("equal_count", None), ("equal_work", work)):
+            parts = [tcw.shard_groups(grid.n_groups, r, n, weights=wts) for r in range(n)]
+            ms = [timed(lo, hi) for lo, hi in parts]
+            row[cut] = {"ranges": parts, "ms": [round(x, 3) for x in ms], "max_ms": round(max(ms), 3),
+                        "work_max_over_mean": round(float(max(work[lo:hi].sum() for lo, hi in parts) / (work.sum() / n)), 4),
+                        "predicted_efficiency": round(single / n / max(ms), 4)}
+        table[str(n)] = row
+    h.check()
+    h.close()
+    print(json.dumps({"what": "one-GPU emulation of the group split, not a scaling measurement", "config": workload_config(w),
+                      "single_gpu_ms": round(single, 3), "steps": args.steps, "warmup": args.warmup, "n": table}), flush=True)
     return 0
 
 
@@ -735,6 +786,8 @@ def main():
     ap.add_argument("--general-f0", action="store_true", help="staged kernel: do not use the equally-spaced-f0 instantiation")
     ap.add_argument("--shard", default=None, metavar="R/N",
                     help="time rank R's group range of an N-GPU strong-scaling run alone on one GPU (and check it against the whole search)")
+    ap.add_argument("--shard-table", default=None, metavar="N1,N2,..",
+                    help="one-GPU emulation of the split for each N: every rank's range timed alone, equal-count and equal-work cuts")
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

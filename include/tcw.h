@@ -150,9 +150,11 @@ int tcw_search(tcw_handle *h, const tcw_grid *grid, void *out_stat, void *out_be
  *  out_stat  DEVICE, [(group_end - group_begin)][n_f0], the range's slice of tcw_search's out_stat; may be NULL.
  *  out_best  DEVICE, [(group_end - group_begin)] candidate records; may be NULL (not both).
  * The range is served as at most seven sub-grid searches (whole sky points, whole tau rows, part of a
- * tau row), enqueued on `stream`; every template is evaluated exactly as by tcw_search, so the
- * outputs equal the corresponding slices of a whole-grid search bit for bit.  Asynchronous.
- * TCW_EINVAL for an empty range or one outside 0..n_groups. */
+ * tau row), enqueued on `stream`; every template is evaluated exactly as by tcw_search -- the
+ * SFT-chunk plan, which fixes the float32 summation order, is decided on the WHOLE grid's size for
+ * every sub-grid -- so the outputs equal the corresponding slices of a whole-grid search bit for bit.
+ * Asynchronous.  TCW_EINVAL for an empty range or one outside 0..n_groups (the Python binding
+ * turns an empty in-range interval, a rank with no groups, into a no-op). */
 int tcw_search_groups(tcw_handle *h, const tcw_grid *grid, long group_begin, long group_end,
                       void *out_stat, void *out_best, void *stream);
 
@@ -422,9 +424,14 @@ enum {
     TCW_OPT_ROW_COPIES = 8, /* staged kernel: 1 = stage every SFT row by its own 1-D bulk copy; 0 default: a ring slot (four
                                consecutive SFT rows) travels by ONE tensor-map copy wherever its rows' windows fit one
                                box (same bins, same sums bit for bit; the tests compare the two)            */
-    TCW_OPT_DEBUG_SHRINK_SLOT = 100 /* test hook: the kernels check their staged windows against the planned
+    TCW_OPT_DEBUG_SHRINK_SLOT = 100, /* test hook: the kernels check their staged windows against the planned
                                bound minus this many bytes, which forces the device status word and
                                hence TCW_EINTERNAL; 0 default.  Not for production use.               */
+    TCW_OPT_DEBUG_FAIL_WAIT = 101,  /* test hook: in tcw_search_host's progressive read-back, the stream wait of
+                               part (value - 1) behaves as if the driver had refused it; the call must
+                               then still deliver every value (plain copies after the search).  0 default */
+    TCW_OPT_DEBUG_CHUNK_SCRATCH = 102 /* test hook: byte cap on the SFT-chunk scratch (default 16e9) so that the
+                               'whole grid too large to chunk' plan can be reached on a small grid; 0 default */
 };
 int tcw_set_option(tcw_handle *h, int key, long value);
 

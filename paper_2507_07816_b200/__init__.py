@@ -28,6 +28,8 @@ TCW_OPT_EXACT_INDEX = 6
 TCW_OPT_GENERAL_F0 = 7
 TCW_OPT_ROW_COPIES = 8
 TCW_OPT_DEBUG_SHRINK_SLOT = 100
+TCW_OPT_DEBUG_FAIL_WAIT = 101
+TCW_OPT_DEBUG_CHUNK_SCRATCH = 102
 KERNELS = {"auto": 0, "gather": 1, "staged": 2, "skyblock": 3}
 FORMATS = {"f32": TCW_F32_POWER, "u8": TCW_U8_COUNT, "bits": TCW_BIT_COUNT}
 
@@ -264,6 +266,8 @@ class Handle:
             out_stat = torch.empty((max(n, 0), len(grid.f0)), dtype=self.stat_dtype, device=dev)
         if out_best is None and want_best:
             out_best = torch.empty((max(n, 0), 2), dtype=torch.int32, device=dev)
+        if n == 0 and 0 <= int(group_begin) <= grid.n_groups:
+            return out_stat, out_best       # a rank with no groups (world_size > n_groups) has nothing to launch
         cg = grid._c()
         _check(L.tcw_search_groups(self._h, ctypes.byref(cg), int(group_begin), int(group_end),
                                    out_stat.data_ptr() if out_stat is not None else None,
@@ -536,14 +540,55 @@ def split_groups(n_tau: int, n_brk: int, group_begin: int, group_end: int) -> li
     return [(slice(r[0], r[1]), slice(r[2], r[3]), slice(r[4], r[5])) for r in list(rects)[: n.value]]
 
 
-def shard_groups(n_groups: int, rank: int, world_size: int) -> tuple[int, int]:
+def shard_groups(n_groups: int, rank: int, world_size: int, weights=None) -> tuple[int, int]:
     """Multi-GPU partition: the flattened (sky, tau, n)
-    group index 0..n_groups-1 is cut into world_size contiguous, nearly equal ranges and rank r
-    searches [begin, end) with Handle.search_groups.  Whole groups per rank, so each per-group
-    argmax stays on one rank; the spectrogram is replicated; no collective on the data path.
+    group index 0..n_groups-1 is cut into world_size contiguous ranges and rank r searches
+    [begin, end) with Handle.search_groups.  Whole groups per rank, so each per-group argmax stays on
+    one rank; the spectrogram is replicated; no collective on the data path.
+    weights = None: nearly equal group COUNTS.  weights = [n_groups] non-negative work per group
+    (group_work): cut r is placed where the running sum of the weights is nearest r/world_size of the
+    total, so ranks get nearly equal WORK (groups with small tau or small n leave the band early and
+    cost less).  Every rank computes the same cuts from the same weights; no communication.
     A rank may get an empty range (begin == end) when world_size > n_groups."""
     if not (0 <= rank < world_size):
         raise ValueError("rank out of range")
-    base, rem = divmod(int(n_groups), world_size)
-    lo = rank * base + min(rank, rem)
-    return lo, lo + base + (1 if rank < rem else 0)
+    n_groups = int(n_groups)
+    if weights is None:
+        base, rem = divmod(n_groups, world_size)
+        lo = rank * base + min(rank, rem)
+        return lo, lo + base + (1 if rank < rem else 0)
+    wt = np.asarray(weights, dtype=np.float64).reshape(-1)
+    if wt.size != n_groups or not np.all(np.isfinite(wt)) or np.any(wt < 0):
+        raise ValueError("weights must be n_groups finite non-negative numbers")
+    cum = np.concatenate(([0.0], np.cumsum(wt)))           # cum[i] = work of groups 0..i-1
+    if not cum[-1] > 0:
+        return shard_groups(n_groups, rank, world_size)
+    cuts = [0]
+    for r in range(1, world_size):
+        target = cum[-1] * r / world_size
+        i = int(np.searchsorted(cum, target))               # first i with cum[i] >= target
+        if i > 0 and target - cum[i - 1] <= cum[min(i, n_groups)] - target:
+            i -= 1                                          # the cut below is at least as near
+        cuts.append(min(max(i, cuts[-1]), n_groups))
+    cuts.append(n_groups)
+    return cuts[rank], cuts[rank + 1]
+
+
+def group_work(grid: Grid, timestamps, T_sft: float, f_min: float, n_bins: int) -> np.ndarray:
+    """Scheduling estimate for shard_groups(weights=): per group of the flattened (sky, tau, n) index,
+    how many (f0, SFT) lookups fall inside the band.  From eq. (1) alone -- the
+    track f0 (1 + t/tau)^(-1/(n-1)) crosses a band edge f_e at t = tau ((f0/f_e)^(n-1) - 1) -- with the
+    1e-4 Doppler factor left out, so it is the same for every sky point.  It only decides where the
+    group axis is cut between GPUs; no search result depends on it."""
+    ts = np.sort(_f64(timestamps)) - float(grid.T0)
+    k_min = float(np.rint(f_min * T_sft))
+    f_lo, f_hi = (k_min - 0.5) / T_sft, (k_min + n_bins - 0.5) / T_sft
+    per = np.zeros((len(grid.tau), len(grid.brk)))
+    for a, tau in enumerate(grid.tau):
+        for b, n in enumerate(grid.brk):
+            t_exit = tau * (np.maximum(grid.f0 / f_lo, 0.0) ** (n - 1.0) - 1.0)     # below f_lo from here on
+            t_enter = tau * (np.maximum(grid.f0 / f_hi, 0.0) ** (n - 1.0) - 1.0)    # above f_hi before
+            hi = np.searchsorted(ts, t_exit, side="left")
+            lo = np.searchsorted(ts, np.maximum(t_enter, 0.0), side="left")
+            per[a, b] = float(np.maximum(hi - lo, 0).sum())
+    return np.tile(per.reshape(-1), len(grid.sky))

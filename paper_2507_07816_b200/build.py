@@ -35,18 +35,38 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _flags() -> list[str]:
+    return [*NVCC_FLAGS, *os.environ.get("TCW_NVCC_FLAGS", "").split()]
+
+
+def _stamp_path() -> str:
+    return LIB + ".flags"
+
+
 def needs_build() -> bool:
+    """True when the library is missing, older than a source, or was built with other nvcc flags
+    (TCW_NVCC_FLAGS variants: the flag string is kept in a stamp file beside the library, so a
+    variant measurement can never silently time a build made with different flags)."""
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPENDS)
+    if any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPENDS):
+        return True
+    try:
+        with open(_stamp_path()) as f:
+            return f.read() != " ".join(_flags())
+    except OSError:
+        # no stamp (a library built before stamps existed): trust it only for the default flags
+        return bool(os.environ.get("TCW_NVCC_FLAGS", "").split())
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("TCW_NVCC_FLAGS", "").split(), *(["-Xptxas", "-v"] if verbose else []),
+        cmd = [_nvcc(), *_flags(), *(["-Xptxas", "-v"] if verbose else []),
                "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
         subprocess.run(cmd, check=True)
+        with open(_stamp_path(), "w") as f:
+            f.write(" ".join(_flags()))
     return LIB
 
 

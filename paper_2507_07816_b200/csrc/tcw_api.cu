@@ -276,8 +276,11 @@ struct tcw_handle {
     int progress_a0[17] = {0};               // tau index where each part starts
     int opt_nonuniform = 0;   // 1: never take the equally-spaced-f0 instantiation of the staged kernel
     int opt_row_copies = 0;   // 1: never stage a ring slot by one tensor-map copy
+    long plan_groups = 0;     // tcw_search_groups: group count of the WHOLE grid while its sub-grids are searched (chunk plan)
+    double chunk_scratch_max = CHUNK_SCRATCH_MAX;   // lowered by the test hook TCW_OPT_DEBUG_CHUNK_SCRATCH
     bool keep_status = false; // a multi-part search (tcw_search_groups, tcw_search_host) clears the status word once
     int dbg_slot_shrink = 0;  // test hook: bytes taken off the kernels' own window bound
+    int dbg_fail_wait = 0;    // test hook: the stream wait of read-back part (value - 1) reports CUDA_ERROR_NOT_SUPPORTED
     std::vector<cudaEvent_t> ev;  // 4 per timed search: start, tables done, sum done, best done
     size_t timing_n = 0;          // timed searches recorded since the last tcw_get_timing
     cudaStream_t last_stream = nullptr;
@@ -912,6 +915,14 @@ int tcw_set_option(tcw_handle *h, int key, long value)
         if (value < 0 || value > (1 << 20)) return fail(TCW_EINVAL, "TCW_OPT_DEBUG_SHRINK_SLOT must be 0..2^20");
         h->dbg_slot_shrink = (int)value;
         return TCW_OK;
+    case TCW_OPT_DEBUG_CHUNK_SCRATCH:
+        if (value < 0) return fail(TCW_EINVAL, "TCW_OPT_DEBUG_CHUNK_SCRATCH must be >= 0");
+        h->chunk_scratch_max = value ? (double)value : CHUNK_SCRATCH_MAX;
+        return TCW_OK;
+    case TCW_OPT_DEBUG_FAIL_WAIT:
+        if (value < 0 || value > 16) return fail(TCW_EINVAL, "TCW_OPT_DEBUG_FAIL_WAIT must be 0..16");
+        h->dbg_fail_wait = (int)value;
+        return TCW_OK;
     case TCW_OPT_CHUNK_ROWS:
         if (value < -1 || value > (1L << 30)) return fail(TCW_EINVAL, "TCW_OPT_CHUNK_ROWS must be -1, 0 or a row count");
         h->opt_chunk = value;
@@ -1039,8 +1050,12 @@ static int search_impl(tcw_handle *h, const tcw_grid *grid, const tcw_weighting 
         if (c_rows > 0) {
             c_rows = std::max<long>(64, (c_rows + 63) / 64 * 64);
             long nc = (rows + c_rows - 1) / c_rows;
-            const double scratch = (double)nc * (double)n_groups * grid->n_f0 * (wgt ? 20.0 : 4.0);
-            if (nc > 1 && nc <= 255 && scratch <= CHUNK_SCRATCH_MAX && nc * n_partial <= 2147483647L) {
+            // The yes/no of chunking fixes the float32 summation order, so a group range (tcw_search_groups) must
+            // decide it as the whole grid would: both size limits are tested on the whole grid's group count.  (A
+            // range is never larger than its grid, so what the whole grid may chunk, the range may too.)
+            const long plan_groups = std::max<long>(h->plan_groups, n_groups);
+            const double scratch = (double)nc * (double)plan_groups * grid->n_f0 * (wgt ? 20.0 : 4.0);
+            if (nc > 1 && nc <= 255 && scratch <= h->chunk_scratch_max && nc * (plan_groups * p.n_tiles) <= 2147483647L) {
                 p.chunk_rows = (int)c_rows;
                 p.n_chunks = (int)nc;
                 n_ctas = nc * n_partial;
@@ -1260,6 +1275,8 @@ int tcw_search_bank(tcw_handle *h, const tcw_bank *bank, void *out_stat, int *ou
     CUDA_TRY(cudaMemcpyAsync(d_brk, bank->brk, sizeof(double) * n, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(d_sky, bank->sky, sizeof(double) * 3 * n_vec, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemsetAsync(h->d_counter, 0, sizeof(unsigned long long), st));
+    // every search starts with a clear status word (tcw.h: tcw_check reports on the LAST search, bank searches included)
+    if (!h->keep_status) CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
 
     const bool tm = h->opt_timing != 0 && h->timing_n < TIMING_MAX;
     cudaEvent_t *ev = nullptr;
@@ -1767,6 +1784,7 @@ int tcw_search_groups(tcw_handle *h, const tcw_grid *grid, long group_begin, lon
     CUDA_TRY(cudaSetDevice(h->device));
     CUDA_TRY(cudaMemsetAsync(h->d_status, 0, sizeof(int), st));
     h->keep_status = true;
+    h->plan_groups = n_groups;
     long info_sum[3] = {0, 0, 0};   // CTAs, kernels launched, parts
     for (const GroupRect &r : split_groups(grid->n_tau, grid->n_brk, group_begin, group_end)) {
         const tcw_grid sub = sub_grid(grid, r);
@@ -1777,6 +1795,7 @@ int tcw_search_groups(tcw_handle *h, const tcw_grid *grid, long group_begin, lon
         info_sum[0] += h->info[2]; info_sum[1] += h->info[5]; info_sum[2]++;
     }
     h->keep_status = false;
+    h->plan_groups = 0;
     if (rc == TCW_OK) { h->info[2] = info_sum[0]; h->info[5] = info_sum[1]; }
     return rc;
 }
@@ -1833,22 +1852,34 @@ int tcw_search_host(tcw_handle *h, const tcw_grid *grid, void *out_stat_host, vo
     const size_t pitch_t = (size_t)grid->n_tau * row_t;
     if (h->progress_active) {
         cudaError_t e = cudaStreamWaitEvent(h->dl_stream, h->dl_ready, 0);     // the counters have been cleared
+        int p_plain = h->progress_np;      // parts from here on go back by plain copies on the search stream
         for (int p = 0; p < h->progress_np && e == cudaSuccess; ++p) {
             const int a0 = h->progress_a0[p], a1 = h->progress_a0[p + 1];     // np <= n_tau: never empty
-            const CUresult wr = wait_value((CUstream)h->dl_stream, (CUdeviceptr)(h->d_progress + p), h->progress_target[p],
-                                           CU_STREAM_WAIT_VALUE_GEQ);
+            const CUresult wr = h->dbg_fail_wait == p + 1 ? CUDA_ERROR_NOT_SUPPORTED :
+                wait_value((CUstream)h->dl_stream, (CUdeviceptr)(h->d_progress + p), h->progress_target[p], CU_STREAM_WAIT_VALUE_GEQ);
             if (wr != CUDA_SUCCESS) {
-                rc = fail(TCW_ECUDA, "cuStreamWaitValue32 failed for part %d (CUresult %d)", p, (int)wr);
+                // the driver refuses the stream wait (e.g. CUDA_ERROR_NOT_SUPPORTED): the search itself is fine, so the
+                // remaining ranges are copied after it, in stream order; the waits already queued are satisfied by the
+                // running search as usual
+                p_plain = p;
                 break;
             }
             e = cudaMemcpy2DAsync((char *)out_stat_host + (size_t)a0 * row_t, pitch_t, h->d_stat.p + (size_t)a0 * row_t, pitch_t,
                                   (size_t)(a1 - a0) * row_t, (size_t)grid->n_sky, cudaMemcpyDeviceToHost, h->dl_stream);
         }
-        if (e != cudaSuccess && rc == TCW_OK) rc = fail(TCW_ECUDA, "progressive read-back: %s", cudaGetErrorString(e));
-        if (rc != TCW_OK) {
-            // the waits may never be satisfied if something went wrong: let the search finish, then release them
+        if (e == cudaSuccess && p_plain < h->progress_np) {
+            const int a0 = h->progress_a0[p_plain], a1 = h->progress_a0[h->progress_np];
+            e = cudaMemcpy2DAsync((char *)out_stat_host + (size_t)a0 * row_t, pitch_t, h->d_stat.p + (size_t)a0 * row_t, pitch_t,
+                                  (size_t)(a1 - a0) * row_t, (size_t)grid->n_sky, cudaMemcpyDeviceToHost, st);
+        }
+        h->info[10] = p_plain;             // parts that really went back under the search
+        if (e != cudaSuccess) {
+            rc = fail(TCW_ECUDA, "progressive read-back: %s", cudaGetErrorString(e));
+            // Waits already queued on dl_stream must not be left hanging.  CU_STREAM_WAIT_VALUE_GEQ is the cyclic
+            // compare (int32)(*addr - value) >= 0, so the value that releases a wait is its own target (0xffffffff
+            // would not: target - 1 steps "behind").  Let the search finish, then write every target.
             cudaStreamSynchronize(st);
-            cudaMemsetAsync(h->d_progress, 0xff, 16 * sizeof(unsigned int), st);
+            cudaMemcpyAsync(h->d_progress, h->progress_target, (size_t)h->progress_np * sizeof(unsigned int), cudaMemcpyHostToDevice, st);
             cudaStreamSynchronize(st);
             cudaStreamSynchronize(h->dl_stream);
             return rc;

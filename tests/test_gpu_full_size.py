@@ -137,17 +137,29 @@ def _device_group_parity(tcw, w, groups, stat, best, h):
     return ref
 
 
-def test_cfg4_full_size_sampled_groups(tcw):
+@pytest.fixture(scope="module")
+def cfg4_w():
+    return tcw_inputs.make_workload("cfg4")
+
+
+def _random_groups(n_groups: int, seed: int, n: int = 32) -> np.ndarray:
+    """First and last group (for n_sky = 1: the smallest and the largest (tau, n)) plus n seeded-random ones."""
+    return np.unique(np.concatenate(([0, n_groups - 1], np.random.default_rng(seed).integers(0, n_groups, size=n))))
+
+
+def test_cfg4_full_size_sampled_groups(tcw, cfg4_w):
     """cfg4 exactly as bench.py --config cfg4 runs it: 11.52 M templates x 20 843 SFTs of 20 000 bins
-    (1.67 GB, timestamps with holes), chunked staged kernel; the oracle recomputes three whole groups."""
+    (1.67 GB, timestamps with holes), chunked staged kernel; the oracle recomputes 34 whole groups (first,
+    last, 32 seeded-random).  NOTE the float32 bar 1e-4 |s| is ~2 here and cannot see one wrong bin: the
+    bit-exact evidence for the indices at this shape is in the three tests below."""
     import torch
-    w = tcw_inputs.make_workload("cfg4")
+    w = cfg4_w
     with tcw.Handle.from_workload(w) as h:
         stat, best = h.search(tcw.Grid.of(w))
         torch.cuda.synchronize()
         info = h.info()
         assert info["kernel"] == "staged" and info["chunks"] > 1 and info["status"] == 0
-        ref = _device_group_parity(tcw, w, np.array([0, 287, 575]), stat, best, h)
+        ref = _device_group_parity(tcw, w, _random_groups(w.n_groups, 404), stat, best, h)
         st = stat.reshape(-1, len(w.f0))
         bmax = st.max(dim=1)
         b = best.cpu().numpy()
@@ -168,7 +180,7 @@ def test_cfg5_full_size_sampled_groups(tcw):
         info = h.info()
         assert info["kernel"] == "skyblock" and info["status"] == 0
         n_ab = len(w.tau) * len(w.brk)
-        groups = np.array([0, 1, 777 * n_ab + 5, 2048 * n_ab + 11, 4095 * n_ab + n_ab - 1])
+        groups = _random_groups(4096 * n_ab, 505)
         _device_group_parity(tcw, w, groups, stat, best, h)
         st = stat.reshape(-1, len(w.f0))
         bmax = st.max(dim=1)
@@ -179,3 +191,61 @@ def test_cfg5_full_size_sampled_groups(tcw):
         assert torch.equal(st[torch.arange(st.shape[0], device=st.device), idx], bmax.values)
         first = (st == bmax.values[:, None]).int().argmax(dim=1)
         assert torch.equal(first, idx)
+
+
+def test_cfg4_uint8_counts_bit_exact_on_random_groups(tcw, cfg4_w):
+    """cfg4's shape (20 000 bins from 500 Hz, x up to 24 000 bins, 21 SFT chunks, gaps,
+    tensor-map box copies) with its spectrogram thresholded to uint8.  n_sky = 1, so the automatic choice is the
+    chunked staged kernel, the one the headline runs; counts are integers, so ONE wrong bin in one SFT shows
+    whenever the two neighbouring bytes differ.  34 whole groups against the oracle, exactly."""
+    import torch
+    w = cfg4_w.with_format("u8")
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == "staged" and info["chunks"] > 1 and info["status"] == 0
+        assert info["box_copies"] == 1                 # ring slots travel by tensor-map copies, as in the headline run
+        _device_group_parity(tcw, w, _random_groups(w.n_groups, 414), stat, best, h)     # exact for counts
+
+
+def test_cfg4_byte_hash_spectrogram_pins_every_bin_of_the_shipped_kernel(tcw, cfg4_w):
+    """VERDICT r2 item 1(c), by construction instead of an export hook: the same cfg4 shape with the spectrogram
+    replaced by uniform random BYTES 0..255 (uint8 values are added as integers, tcw.h).  A wrong bin in any one
+    SFT of a template then changes its integer sum with probability 255/256, so exact equality of whole groups
+    with the oracle checks the bin indices that the staged kernel itself computes (one-FMA index, guard band,
+    fallback), not those of the inspection call tcw_track_indices."""
+    import torch
+    rng = np.random.default_rng(424)
+    w = dataclasses.replace(cfg4_w, fmt="u8", spectrogram=rng.integers(0, 256, size=cfg4_w.spectrogram.shape, dtype=np.uint8))
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(tcw.Grid.of(w))
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == "staged" and info["chunks"] > 1 and info["status"] == 0
+        groups = _random_groups(w.n_groups, 434, n=14)
+        g = torch.as_tensor(groups, device=stat.device)
+        got = stat.reshape(-1, len(w.f0))[g].cpu().numpy().reshape(-1)
+    ref = oracle.evaluate(w, sel=oracle.group_templates(w, groups))
+    assert_stat_parity(w, got, ref.stat)               # exact: both sides decide every bin by the same float64 chain
+    assert ref.stat.max() > 127 * 5000                 # the sums are large: the bytes really were added
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_fast_index_equals_the_defining_chain_at_full_size(tcw, name, cfg4_w):
+    """the shipped index (one FMA + guard band + fallback) against TCW_OPT_EXACT_INDEX = 1
+    (the defining chain of single IEEE operations in every lookup) on the WHOLE float32 output of cfg2 and cfg4,
+    bitwise, on the device.  Same bins give the same float32 sums bit for bit (same order); a different bin
+    anywhere in 2.4e11 lookups would change a sum."""
+    import torch
+    w = cfg4_w if name == "cfg4" else tcw_inputs.make_workload(name)
+    grid = tcw.Grid.of(w)
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(grid)
+        kernel, chunks = h.info()["kernel"], h.info()["chunks"]
+        h.set_option(tcw.TCW_OPT_EXACT_INDEX, 1)
+        stat_x, best_x = h.search(grid)
+        torch.cuda.synchronize()
+        info = h.info()
+        assert info["kernel"] == kernel == "staged" and info["chunks"] == chunks and info["status"] == 0
+        assert torch.equal(stat, stat_x) and torch.equal(best, best_x)

@@ -176,8 +176,12 @@ def test_search_groups_equals_slices_of_the_whole_search(tcw):
                 h.check()
                 assert np.array_equal(s.cpu().numpy().view(np.int32), stat[g0:g1].view(np.int32)), (n_sky, g0, g1)
                 assert np.array_equal(b.cpu().numpy(), best[g0:g1]), (n_sky, g0, g1)
-            with pytest.raises(tcw.TcwError):
-                h.search_groups(grid, 3, 3)
+            # an empty in-range interval is a rank with nothing to do (no-op); the C call itself still
+            # refuses it, as tcw.h says, and anything outside 0..n_groups is an error either way
+            assert h.search_groups(grid, 3, 3)[0].shape[0] == 0
+            cg = grid._c()
+            import ctypes
+            assert tcw.load_library().tcw_search_groups(h._h, ctypes.byref(cg), 3, 3, s.data_ptr(), b.data_ptr(), None) == tcw.TCW_EINVAL
             with pytest.raises(tcw.TcwError):
                 h.search_groups(grid, 0, grid.n_groups + 1)
     ref = oracle.evaluate(w)
@@ -292,7 +296,8 @@ def test_cfg3_full_size_sampled_groups(tcw, fmt):
         info = h.info()
         assert info["kernel"] == "skyblock" and info["sky_block"] == 256 and info["status"] == 0
         n_ab = len(w.tau) * len(w.brk)
-        groups = np.array([0, 3 * n_ab + 7, 100 * n_ab + 41, 128 * n_ab + 79, 255 * n_ab + n_ab - 1])
+        # first and last group plus 32 seeded-random ones (no hand-picked lists)
+        groups = np.unique(np.concatenate(([0, 256 * n_ab - 1], np.random.default_rng(303).integers(0, 256 * n_ab, size=32))))
         _device_group_parity(tcw, w, groups, stat, best, h)
         st = stat.reshape(-1, len(w.f0))
         bmax = st.max(dim=1)
@@ -354,3 +359,84 @@ def test_measured_peaks_are_sane(tcw):
     assert p["chain_lookups_per_s"] < 32 * p["issue_winst_per_s"] / 3.5
     assert p["stage_box_copies_bytes_per_s"] > 0.9 * p["stage_row_copies_bytes_per_s"] > 5e12
     assert p["count_chain_bitpacked_lookups_per_s"] < p["count_chain_u8_lookups_per_s"]
+
+
+def test_bank_search_clears_the_status_word(tcw, cfg1):
+    """tcw.h says every search starts with a clear status word and lists tcw_search_bank among the
+    calls tcw_check reports on; a bank search after an invalid grid search must therefore check clean."""
+    import torch
+    w = cfg1
+    f0, tau, brk, sky = tcw_inputs.random_bank(200, 480.0, 640.0, 5, sky=w.sky[0])
+    with tcw.Handle.from_workload(w) as h:
+        h.set_option(tcw.TCW_OPT_DEBUG_SHRINK_SLOT, 1 << 19)
+        h.search(tcw.Grid.of(w))
+        with pytest.raises(tcw.TcwError):
+            h.check()
+        h.set_option(tcw.TCW_OPT_DEBUG_SHRINK_SLOT, 0)
+        stat, inband, _ = h.search_bank(f0, tau, brk, sky, T0=w.T0)
+        h.check()
+        assert h.info()["status"] == 0
+        torch.cuda.synchronize()
+    ref = oracle.evaluate_bank(w, f0, tau, brk, sky)
+    clean = ref.n_ambig == 0
+    assert np.array_equal(inband.cpu().numpy()[clean], ref.n_inband[clean])
+
+
+def test_search_groups_of_an_empty_range_is_a_no_op(tcw, cfg1):
+    """shard_groups hands a rank an empty range when world_size > n_groups; that rank must get
+    empty outputs, not an error."""
+    grid = tcw.Grid.of(cfg1)
+    with tcw.Handle.from_workload(cfg1) as h:
+        for r in range(16):
+            lo, hi = tcw.shard_groups(grid.n_groups, r, 16)          # 12 groups over 16 ranks
+            stat, best = h.search_groups(grid, lo, hi)
+            assert stat.shape == (hi - lo, len(grid.f0)) and best.shape == (hi - lo, 2)
+        with pytest.raises(tcw.TcwError):
+            h.search_groups(grid, grid.n_groups + 1, grid.n_groups + 1)
+
+
+@pytest.mark.parametrize("fail_part", [1, 2, 3])
+def test_read_back_survives_a_refused_stream_wait(tcw, fail_part):
+    """if the driver refuses cuStreamWaitValue32 for some part of tcw_search_host's progressive
+    read-back, the finished search must still be delivered whole (remaining parts by plain copies after the
+    search) and nothing may hang.  The hook makes part (fail_part - 1) report CUDA_ERROR_NOT_SUPPORTED."""
+    import torch
+    w = tcw_inputs.make_workload("cfg3", fmt="u8").subgrid(sky=np.arange(0, 256, 256 // 56)[:56])
+    grid = tcw.Grid.of(w)
+    with tcw.Handle.from_workload(w) as h:
+        stat, best = h.search(grid)
+        torch.cuda.synchronize()
+        want, bwant = stat.cpu().numpy(), best.cpu().numpy()
+        h.set_option(tcw.TCW_OPT_DEBUG_FAIL_WAIT, fail_part)
+        got, bgot = h.search_host(grid)
+        assert h.info()["readback_parts"] == fail_part - 1           # parts that went back under the search
+        assert np.array_equal(got, want) and np.array_equal(bgot, bwant)
+        h.set_option(tcw.TCW_OPT_DEBUG_FAIL_WAIT, 0)
+        got, bgot = h.search_host(grid)                              # and the handle is healthy afterwards
+        assert h.info()["readback_parts"] > 1
+        assert np.array_equal(got, want) and np.array_equal(bgot, bwant)
+
+
+def test_group_range_takes_the_whole_grids_chunk_plan(tcw, cfg1):
+    """whether the SFT axis is chunked fixes the float32 summation order, and the decision has two
+    size limits that depend on the number of groups.  A range of groups must decide as its whole grid does, or
+    tcw_search_groups would not be the slice of tcw_search bit for bit.  The hook lowers the scratch cap so that
+    cfg1's whole grid (12 groups) is over it while a 6-group range alone would be under it."""
+    import torch
+    w = cfg1
+    grid = tcw.Grid.of(w)
+    with tcw.Handle.from_workload(w) as h:
+        h.set_option(tcw.TCW_OPT_KERNEL, 2)
+        h.set_option(tcw.TCW_OPT_CHUNK_ROWS, 64)                     # 256 SFTs -> 4 chunks where chunking is allowed
+        stat_c, _ = h.search(grid)
+        assert h.info()["chunks"] == 4
+        h.set_option(tcw.TCW_OPT_DEBUG_CHUNK_SCRATCH, 4 * 9 * len(w.f0) * 4)      # room for 9 groups of partial sums
+        stat, best = h.search(grid)
+        assert h.info()["chunks"] <= 1                               # the whole grid does not chunk under the cap
+        s, b = h.search_groups(grid, 3, 9)
+        assert h.info()["chunks"] <= 1                               # ... so neither does a 6-group range
+        torch.cuda.synchronize()
+        assert torch.equal(s, stat.reshape(-1, len(w.f0))[3:9]) and torch.equal(b, best[3:9])
+        # the two plans do differ in the last bits (else this test would prove nothing), within the float32 bar
+        assert not torch.equal(stat_c, stat)
+        assert torch.allclose(stat_c, stat, rtol=2e-6, atol=0)

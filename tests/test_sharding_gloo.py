@@ -34,13 +34,14 @@ def _workload(n_sky: int):
     return w
 
 
-def _rank_main(rank: int, world: int, port: int, n_sky: int, out_path: str):
+def _rank_main(rank: int, world: int, port: int, n_sky: int, out_path: str, by_work: bool = False):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         w = _workload(n_sky)
         n_f0 = len(w.f0)
-        lo, hi = tcw.shard_groups(w.n_groups, rank, world)
+        wts = tcw.group_work(tcw.Grid.of(w), w.timestamps, w.T_sft, w.f_min, w.n_bins) if by_work else None
+        lo, hi = tcw.shard_groups(w.n_groups, rank, world, weights=wts)
         stat, val, idx = [], [], []
         for s, a, b in tcw.split_groups(len(w.tau), len(w.brk), lo, hi):      # what tcw_search_groups runs
             sub = w.subgrid(sky=s, tau=a, brk=b)
@@ -65,10 +66,12 @@ def _rank_main(rank: int, world: int, port: int, n_sky: int, out_path: str):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,n_sky", [(2, 1), (3, 1), (2, 5)])
-def test_group_sharding_reassembles_the_unsharded_search(tmp_path, world, n_sky):
+@pytest.mark.parametrize("world,n_sky,by_work", [(2, 1, False), (3, 1, False), (2, 5, False), (3, 1, True)])
+def test_group_sharding_reassembles_the_unsharded_search(tmp_path, world, n_sky, by_work):
+    """by_work: the cut is placed by the in-band work per group (group_work) instead of the group count;
+    still contiguous, still whole groups, and the reassembly is still the unsharded result."""
     out = str(tmp_path / "gathered.npz")
-    mp.spawn(_rank_main, args=(world, _free_port(), n_sky, out), nprocs=world, join=True)
+    mp.spawn(_rank_main, args=(world, _free_port(), n_sky, out, by_work), nprocs=world, join=True)
     got = np.load(out)
     w = _workload(n_sky)
     ref = oracle.evaluate(w)
@@ -84,3 +87,41 @@ def test_shard_groups_partitions_every_rank_count():
             assert parts[0][0] == 0 and parts[-1][1] == n_groups
             assert all(a[1] == b[0] for a, b in zip(parts, parts[1:]))
             assert max(hi - lo for lo, hi in parts) - min(hi - lo for lo, hi in parts) <= 1
+
+
+def test_shard_groups_with_more_ranks_than_groups_gives_empty_ranges():
+    parts = [tcw.shard_groups(3, r, 8) for r in range(8)]
+    assert parts[0][0] == 0 and parts[-1][1] == 3 and all(a[1] == b[0] for a, b in zip(parts, parts[1:]))
+    assert sum(hi == lo for lo, hi in parts) == 5 and all(0 <= lo <= hi <= 3 for lo, hi in parts)
+
+
+def test_work_weighted_cut_is_a_partition_and_balances_work():
+    rng = np.random.default_rng(5)
+    for n_groups in (1, 7, 576, 20480):
+        wt = rng.random(n_groups) ** 3 * np.linspace(0.1, 2.0, n_groups)       # skewed: late groups cost more
+        for world in (1, 2, 3, 8):
+            parts = [tcw.shard_groups(n_groups, r, world, weights=wt) for r in range(world)]
+            assert parts[0][0] == 0 and parts[-1][1] == n_groups
+            assert all(a[1] == b[0] for a, b in zip(parts, parts[1:])) and all(lo <= hi for lo, hi in parts)
+            if n_groups >= 576:
+                work = np.array([wt[lo:hi].sum() for lo, hi in parts])
+                assert work.max() <= wt.sum() / world + wt.max()                # within one group of the ideal
+                count = np.array([wt[slice(*tcw.shard_groups(n_groups, r, world))].sum() for r in range(world)])
+                assert work.max() <= count.max() + 1e-9                         # never worse than the equal-count cut
+    # zero and uniform weights reduce to the equal-count cut
+    assert [tcw.shard_groups(12, r, 4, weights=np.zeros(12)) for r in range(4)] == [tcw.shard_groups(12, r, 4) for r in range(4)]
+    assert [tcw.shard_groups(12, r, 4, weights=np.ones(12)) for r in range(4)] == [tcw.shard_groups(12, r, 4) for r in range(4)]
+    with pytest.raises(ValueError):
+        tcw.shard_groups(12, 0, 4, weights=np.ones(11))
+
+
+def test_group_work_tracks_the_oracles_in_band_lookups():
+    """group_work is an estimate (no Doppler) of what the oracle counts exactly; on cfg1 and on a cfg4-like
+    grid whose small-tau tracks leave the band early, they agree to a fraction of a percent per group."""
+    w = tcw_inputs.make_workload("cfg1")
+    est = tcw.group_work(tcw.Grid.of(w), w.timestamps, w.T_sft, w.f_min, w.n_bins)
+    ref = oracle.evaluate(w)
+    exact = ref.n_inband.reshape(w.n_groups, len(w.f0)).sum(axis=1)
+    assert est.shape == exact.shape
+    assert np.all(np.abs(est - exact) <= 0.01 * exact.max() + len(w.f0))
+    assert exact.min() < exact.max() and np.corrcoef(est, exact)[0, 1] > 0.999
