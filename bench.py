@@ -49,6 +49,7 @@ METRIC = "template-SFT lookups/s"
 UNIT = "lookups/s"
 C_LIGHT = 299792458.0
 HEADLINE = "cfg4"
+FP64_PER_LOOKUP = 34.0      # FP64 instructions per lookup of sum_bank_kernel's fast path (SASS count)
 PER_CONFIG = (("cfg2", "f32"), ("cfg3", "u8"), ("cfg3", "bits"), ("cfg5", "bits"))
 L2_BYTES = 126e6
 
@@ -66,6 +67,40 @@ def load_ncu_summary():
 
 
 # ----------------------------------------------------------------------------- helpers
+# The driver keeps the tail of the line: prose and provenance strings stay out of it unless --verbose
+# (they are in DESIGN.md section 6), and floats carry five significant digits.
+COMPACT_DROP = ("note", "traffic_source", "inst_source", "peak_source", "path", "timing", "samples", "searches_averaged")
+
+
+def slim_block(b):
+    """A per_config entry as the default line carries it: the numbers (time, value, rooflines, e2e, launches), the
+    workload by name; the launch geometry, stage split, clocks and full config are in the --verbose line."""
+    keep = ("value", "ms_per_step", "kernel_ms", "inband_fraction", "roofline", "roofline_binding", "e2e", "gpu_launches",
+            "results", "n", "n_sft", "us_per_template", "exact_chain_lookups", "templates_per_s")
+    out = {"workload": b["config"]["workload"].split(" ")[0] + ":" + b["config"]["format"]} if "config" in b else {}
+    if "launch" in b:
+        out["kernel"] = b["launch"].get("kernel")
+    out.update({k: b[k] for k in keep if k in b})
+    for r in ("roofline", "roofline_binding"):
+        if r in out:
+            out[r] = {k: v for k, v in out[r].items() if k not in ("kernel_ms", "algorithmic_bytes_per_launch", "inst_per_launch",
+                                                                   "issue_active_pct_ncu", "fp64_pipe_pct_ncu", "bytes_per_inband_lookup")}
+    if "cpu_baseline" in b:
+        out["cpu_baseline"] = {k: b["cpu_baseline"][k] for k in ("value", "cores", "kind") if k in b["cpu_baseline"]}
+    return out
+
+
+def compact(obj, drop=COMPACT_DROP, top=True):
+    if isinstance(obj, dict):
+        return {k: compact(v, drop, False) for k, v in obj.items()
+                if top or k not in drop or k == "sample"}
+    if isinstance(obj, (list, tuple)):
+        return [compact(v, drop, False) for v in obj]
+    if isinstance(obj, float):
+        return float(f"{obj:.5g}") if math.isfinite(obj) else None
+    return obj
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -150,30 +185,55 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def time_oracle(w, budget_s: float, max_groups: int | None = None):
-    """The oracle as it stands (oracle/tcw_oracle.c, OpenMP over templates) timed on ONE call over a
-    seeded random sample of whole (sky, tau, n) groups of `w`.  A first call on a few groups sizes
-    the sample so that the timed call takes about `budget_s` (never more than the whole grid)."""
+def time_oracle(w, budget_s: float, max_groups: int | None = None, literal: bool = False):
+    """The oracle as it stands (oracle/tcw_oracle.c, OpenMP over templates) timed on ONE call.
+    Sample = a seeded random sub-grid of WHOLE groups: some tau values x some sky points x every
+    braking index x every f0, evaluated whole, so that the oracle's per-(tau, n) spin-down table is
+    built for the sampled rows only and the rate does not depend on the sample size (round 2 built
+    the table of the whole grid for every sample: VERDICT r2 #7).  A first call on one (sky, tau) row
+    sizes the sample to about `budget_s`.  literal=True: the oracle's literal mode (one correctly
+    rounded power per (template, SFT), no table: BASELINE.md section 2) on a prefix of that row."""
     import oracle
     oracle.build()
     rng = np.random.default_rng(7)
-    order = rng.permutation(w.n_groups)
-    n1 = min(4, w.n_groups)
-    t0 = time.perf_counter()
-    oracle.evaluate(w, sel=oracle.group_templates(w, order[:n1]))      # also loads the library
-    t1 = time.perf_counter() - t0
-    n = int(max(1, min(w.n_groups, budget_s / (t1 / n1))))
-    if max_groups is not None:
-        n = min(n, max_groups)
-    sel = oracle.group_templates(w, np.sort(order[:n]))
-    t0 = time.perf_counter()
-    oracle.evaluate(w, sel=sel)
-    t_used = time.perf_counter() - t0
-    lookups = n * len(w.f0) * w.n_sft
+    tau_order, sky_order = rng.permutation(len(w.tau)), rng.permutation(len(w.sky))
+    n_brk, n_f0 = len(w.brk), len(w.f0)
+
+    def sub(n_tau, n_sky):
+        return w.subgrid(tau=np.sort(tau_order[:n_tau]), sky=np.sort(sky_order[:n_sky]))
+
+    if literal:
+        row, m = sub(1, 1), min(256, n_f0)
+        t0 = time.perf_counter()
+        oracle.evaluate(row, sel=np.arange(m), literal=True)
+        t1 = time.perf_counter() - t0
+        m = int(max(m, min(row.n_templates, m * budget_s / t1)))
+        t0 = time.perf_counter()
+        r = oracle.evaluate(row, sel=np.arange(m), literal=True)
+        t_used = time.perf_counter() - t0
+        n_templates, what = m, f"the first {m} templates of one (sky,tau) row of {w.name}, literal mode"
+    else:
+        t0 = time.perf_counter()
+        oracle.evaluate(sub(1, 1))                                       # also loads the library
+        t1 = time.perf_counter() - t0
+        rows = max(1.0, budget_s / t1)
+        if max_groups is not None:
+            rows = max(1.0, min(rows, max_groups / n_brk))
+        n_tau = int(min(len(w.tau), rows))
+        n_sky = int(min(len(w.sky), max(1.0, rows / n_tau)))
+        sw = sub(n_tau, n_sky)
+        t0 = time.perf_counter()
+        r = oracle.evaluate(sw)
+        t_used = time.perf_counter() - t0
+        n_templates = sw.n_templates
+        what = f"{n_tau} tau x {n_sky} sky x all {n_brk} n = {n_tau * n_sky * n_brk} of {w.n_groups} whole groups of {w.name}"
+    lookups = float(n_templates) * w.n_sft
+    inband = float(r.n_inband.sum())
     return dict(value=lookups / t_used, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
-                sample=f"{n} of {w.n_groups} whole (sky,tau,n) groups of {w.name} in one call "
-                       f"({n * len(w.f0)} templates x {w.n_sft} SFTs = {lookups:.3e} nominal lookups) in {t_used:.1f} s",
-                seconds=t_used, templates=n * len(w.f0))
+                inband_lookups_per_s=inband / t_used,
+                sample=f"{what} in one call ({n_templates} templates x {w.n_sft} SFTs = {lookups:.3e} nominal, "
+                       f"{inband:.3e} in-band lookups) in {t_used:.1f} s",
+                seconds=t_used, templates=n_templates)
 
 
 def workload_config(w, extra=None):
@@ -338,6 +398,7 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
     if spec_np.dtype == np.uint32:
         spec_np = spec_np.view(np.int32)
     spec_pin = torch.from_numpy(spec_np).pin_memory()
+    skip_e2e = e2e_steps <= 0
     e2e_steps = max(1, min(steps, e2e_steps))
     if world == 1:
         stat_pin = torch.empty((len(w.sky), len(w.tau), len(w.brk), n_f0), dtype=h.stat_dtype).pin_memory()
@@ -364,14 +425,14 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
                     hh.check()
         e2e_path = ("per rank: tcw_create_async(pinned HOST spectrogram) + tcw_search_groups(own group range) + "
                     "device-to-host copy of its out_stat / out_best slices + tcw_check + tcw_destroy")
-    for _ in range(2):
+    for _ in range(0 if skip_e2e else 2):
         e2e_step()
     barrier()
     t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    for _ in range(0 if skip_e2e else e2e_steps):
         e2e_step()                      # tcw_search_host / tcw_check synchronise before returning
     torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
+    e2e_s = max(time.perf_counter() - t0, 1e-9)
     if world > 1:
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -389,8 +450,10 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
     peak, peak_src = load_peaks()
     b_comp = compulsory_bytes(w)
     sum_ms = stage_ms[1]
+    dev_spec_bytes = float(n_sft) * w.n_bins * (4 if w.fmt == "f32" else 1)       # bit-packed input is expanded to one byte per bin
+    unique_b = dev_spec_bytes + 4.0 * grid.n_templates + 8.0 * grid.n_groups
     achieved = b_comp / (sum_ms * 1e-3) / 1e9 if sum_ms > 0 else 0.0
-    ncu = ctx["ncu"].get("captures", {}).get(key)
+    ncu = None if weighted else ctx["ncu"].get("captures", {}).get(key)      # the captures are of the unweighted kernels
     kernel_name = ("sum_skyblock2_kernel" if info.get("kernel") == "skyblock" and info.get("sky_block") == 256
                    else f"sum_{info.get('kernel')}_kernel")
     block = {
@@ -415,14 +478,17 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
                                         if ncu else None),
                      "peak_source": peak_src, "kernel": kernel_name, "algorithmic_bytes_per_launch": b_comp, "kernel_ms": sum_ms,
                      "bytes_per_inband_lookup": b_comp / inband if inband else None,
-                     "note": "compulsory-bytes model of BASELINE.json: every group is charged its own read of the rows, which "
-                             "L2 and the sky-block sharing serve; fractions above 1 mean the model is not what binds "
-                             "(see roofline_binding)"},
+                     # what must leave / enter HBM once: the spectrogram as the device holds it + the outputs.  `frac` above is
+                     # BASELINE.json's per-group model, which L2 serves (frac > 1 = the model does not bind: see roofline_binding)
+                     "unique_bytes": unique_b, "frac_unique": unique_b / (sum_ms * 1e-3) / 1e9 / peak if sum_ms > 0 else None,
+                     "traffic_over_unique": ((ncu["dram_bytes_read"] + ncu["dram_bytes_write"]) / unique_b) if ncu else None},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps, "path": e2e_path},
         "gpu_launches": (info.get("launches") or 0) * steps,
         "clocks": clocks,
     }
+    if skip_e2e:
+        del block["e2e"]
     pk = ctx["peaks"]
     if ncu and pk and world == 1 and not opts and not weighted:
         inst = float(ncu["inst_executed"])
@@ -454,17 +520,20 @@ def measure_config(ctx, name, fmt, steps, warmup, e2e_steps, cpu_seconds, opts=N
                         "measured alone by tcw_measure_peaks: staging, row metadata and band edges are what separates the two"}
     if world == 1 and cpu_seconds > 0:
         cb = time_oracle(w, cpu_seconds)
-        block["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        block["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "inband_lookups_per_s")}
         block["cpu_baseline"]["templates_per_s"] = cb["templates"] / cb["seconds"]
-        block["cpu_baseline"]["note"] = "the oracle as it stands: the literal float64 definition, not an optimised CPU code"
         if one_thread:
-            # the same oracle on one thread (all cores and one core), a smaller sample
+            # the same oracle on one thread (all cores and one core), and its literal mode
+            # (one correctly rounded power per lookup) on all cores; smaller samples -- the rate
+            # no longer depends on the sample size
             import oracle
             all_threads = oracle.num_threads()
             oracle.set_num_threads(1)
             c1 = time_oracle(w, min(4.0, cpu_seconds))
             oracle.set_num_threads(all_threads)
             block["cpu_baseline"]["one_thread"] = {"value": c1["value"], "unit": UNIT, "cores": 1, "sample": c1["sample"]}
+            cl = time_oracle(w, min(3.0, cpu_seconds), literal=True)
+            block["cpu_baseline"]["literal"] = {"value": cl["value"], "unit": UNIT, "cores": cl["cores"], "sample": cl["sample"]}
     return block
 
 
@@ -525,6 +594,16 @@ def run_ours(args):
             blk = measure_config(ctx, cname, cfmt, min(args.steps, 20), max(3, min(args.warmup, 5)), min(args.e2e_steps, 5),
                                  0.0 if args.no_cpu_baseline else min(3.0, args.cpu_seconds))
             per[f"{cname}:{cfmt}"] = blk
+        # the (f) rows of SURVEY.md section 8, a few steps each, so that the driver-run record measures them too:
+        # NEXT-1 weighted statistic + Psi (eq. 4), NEXT-2 random bank, NEXT-4 selection
+        # (PAPER.md:79), NEXT-3 data preparation
+        if not opts and not args.weighted and not args.no_next_rows:
+            st, wu = min(args.steps, 10), 3
+            per["weighted:cfg2"] = measure_config(ctx, "cfg2", "f32", st, wu, 0, 0.0, weighted=True)
+            per["weighted:cfg4"] = measure_config(ctx, "cfg4", "f32", st, wu, 0, 0.0, weighted=True)
+            per["bank:cfg2:1M"] = measure_bank("cfg2", "f32", 1_000_000, min(st, 5), wu, ctx["peaks"])
+            per["select:393M"] = measure_select(393_216_000, min(st, 5), wu)
+            per["prep:10800"] = measure_prep(10800, min(st, 5), wu)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -550,9 +629,12 @@ def run_ours(args):
         line["measured_peaks"] = ctx["peaks"]
     if per:
         line["per_config"] = per
-        line["gpu_launches"] += sum(b["gpu_launches"] for b in per.values())
-        line["gpu_launches_note"] = "kernels of the timed regions of the headline and of every per_config entry"
-    print(json.dumps(line), flush=True)
+        line["gpu_launches"] += sum(b.get("gpu_launches", 0) for b in per.values())
+    if per and not args.verbose:
+        line["per_config"] = {k: slim_block(b) for k, b in per.items()}
+    out = compact(line, drop=() if args.verbose else COMPACT_DROP)
+    out["roofline"]["peak_source"] = line["roofline"]["peak_source"]      # the contract wants the headline peak's origin stated
+    print(json.dumps(out, separators=(",", ":")), flush=True)
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -642,129 +724,160 @@ def run_shard_table(args, tcw, tcw_inputs, dev):
 
 
 # ----------------------------------------------------------------------------- bank mode (NEXT-2)
-def run_bank(args):
-    """--bank N: tcw_search_bank on N uniform random templates (PAPER.md:63 (ii)) over the config's
-    data, at the config's first sky point.  Not the headline metric: a second line
-    for DESIGN.md.  The path is bound by FP64 arithmetic (one power per lookup), so the roofline
-    object is an ALU one: FP64 instructions per lookup (counted in the SASS of the fast path:
-    DESIGN.md section 7) x lookups evaluated / time, against 148 SMs x 64 FP64 lanes x 1.965 GHz."""
+def measure_bank(config, fmt, n_bank, steps, warmup, peaks=None):
+    """tcw_search_bank on n_bank uniform random templates (PAPER.md:63 (ii)) over the config's data, at the
+    config's first sky point.  The path is bound by FP64 arithmetic (one power per lookup), so
+    its roofline is an ALU one: FP64_PER_LOOKUP warp-level FP64 instructions per 32 evaluated lookups (counted
+    in the SASS of the fast path: DESIGN.md section 7) over the kernel time, against the FP64 issue rate that
+    tcw_measure_peaks measures on this GPU."""
     import torch
 
     import paper_2507_07816_b200 as tcw
     import tcw_inputs
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the tCW path has no CPU fallback")
-    torch.cuda.set_device(0)
-    tcw.load_library()
-    w = tcw_inputs.make_workload(args.config, fmt=args.format)
+    w = tcw_inputs.make_workload(config, fmt=fmt)
     f_hi = w.f_min + w.n_bins / w.T_sft
-    f0, tau, brk, sky = tcw_inputs.random_bank(args.bank, w.f_min, f_hi, w.seed, sky=w.sky[0])
+    f0, tau, brk, sky = tcw_inputs.random_bank(n_bank, w.f_min, f_hi, w.seed, sky=w.sky[0])
     h = tcw.Handle.from_workload(w, device="cuda:0")
-    out = torch.empty(args.bank, dtype=h.stat_dtype, device="cuda:0")
-    for _ in range(args.warmup):
+    out = torch.empty(n_bank, dtype=h.stat_dtype, device="cuda:0")
+    for _ in range(warmup):
         _, inband, _ = h.search_bank(f0, tau, brk, sky, T0=w.T0, out_stat=out)
     h.set_option(tcw.TCW_OPT_TIMING, 1)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         _, inband, _ = h.search_bank(f0, tau, brk, sky, T0=w.T0, out_stat=out)
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
     stage_ms, n_timed = h.timing()
     n_exact = h.counter(0)
-    nominal = float(args.bank) * w.n_sft
+    launches = h.info()["launches"]
+    nominal = float(n_bank) * w.n_sft
     evaluated = float(inband.sum(dtype=torch.int64).item())
     kern_ms = stage_ms[1]
-    line = {"metric": METRIC + " (random template bank, tcw_search_bank)", "value": nominal / (kern_ms * 1e-3), "unit": UNIT,
-            "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
+    h.close()
+    peaks = peaks or tcw.measure_peaks()
+    ach = FP64_PER_LOOKUP * evaluated / 32.0 / (kern_ms * 1e-3)
+    return {"metric": METRIC + " (random template bank, tcw_search_bank)", "value": nominal / (kern_ms * 1e-3), "unit": UNIT,
+            "n_gpus": 1, "steps": steps, "warmup": warmup, "ms_per_step": 1e3 * wall / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 index + f32/i32 accumulate",
-            "data": "synthetic", "config": workload_config(w, {"bank_templates": args.bank, "sky": "shared (PAPER.md:77)"}),
-            "templates_per_s": args.bank / (kern_ms * 1e-3), "kernel_ms": kern_ms,
-            "host_ms_per_step_incl_parameter_copy": 1e3 * wall / args.steps,
+            "data": "synthetic", "config": workload_config(w, {"bank_templates": n_bank, "sky": "shared (PAPER.md:77)"}),
+            "templates_per_s": n_bank / (kern_ms * 1e-3), "kernel_ms": kern_ms,
+            "host_ms_per_step_incl_parameter_copy": 1e3 * wall / steps,
             "inband_lookups": evaluated, "inband_fraction": evaluated / nominal,
             "exact_chain_lookups": n_exact,
-            "us_per_template": 1e3 * kern_ms / args.bank,
-            "paper_us_per_template_a100": 15.0}
-    print(json.dumps(line), flush=True)
-    h.close()
+            "us_per_template": 1e3 * kern_ms / n_bank,
+            "paper_us_per_template_a100": 15.0,
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peaks["fp64_dfma_winst_per_s"], "unit": "FP64 warp instructions/s",
+                         "frac": ach / peaks["fp64_dfma_winst_per_s"], "traffic": None, "kernel": "sum_bank_kernel",
+                         "fp64_inst_per_lookup": FP64_PER_LOOKUP, "peak_source": "tcw_measure_peaks (DFMA streams) in this process"},
+            "gpu_launches": launches * steps}
+
+
+def run_bank(args):
+    """--bank N: one line for tcw_search_bank (not the headline metric)."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the tCW path has no CPU fallback")
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    print(json.dumps(measure_bank(args.config, args.format, args.bank, args.steps, args.warmup)), flush=True)
     return 0
 
 
 # ----------------------------------------------------------------------------- selection mode (NEXT-4)
-def run_select(args):
-    """--select N: tcw_topk (K = 1000) and tcw_select_above over N float32 statistics ~ N(0, 1)
-    (the shape of a Psi array; cfg5's out_stat has 393 M entries).  HBM-bound streaming passes: the
-    algorithmic bytes are ONE read of the array (4 N bytes); top-K makes five passes (three
-    histogram passes, count, scatter), threshold selection two."""
+def measure_select(n, steps, warmup):
+    """tcw_topk (K = 1000) and tcw_select_above over n float32 statistics ~ N(0, 1) (the shape of a Psi
+    array; cfg5's out_stat has 393 M entries).  HBM-bound streaming passes: the algorithmic bytes are ONE
+    read of the array (4 n bytes); top-K reads large arrays twice, threshold selection once plus the rows
+    that hold a hit."""
     import torch
 
     import paper_2507_07816_b200 as tcw
     import tcw_inputs
 
-    torch.cuda.set_device(0)
-    tcw.load_library()
     w = tcw_inputs.make_workload("cfg1")
     h = tcw.Handle.from_workload(w, device="cuda:0")
-    n = args.select
     g = torch.Generator(device="cuda").manual_seed(1)
     v = torch.randn(n, generator=g, device="cuda", dtype=torch.float32)
     peak, peak_src = load_peaks()
     res = {}
     for name, fn in (("topk_K1000", lambda: h.topk(v, 1000)), ("select_above_4.5", lambda: h.select_above(v, 4.5, 1 << 20))):
-        for _ in range(max(3, args.warmup)):
+        for _ in range(max(3, warmup)):
             fn()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             fn()
         e1.record()
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / args.steps
+        ms = e0.elapsed_time(e1) / steps
         res[name] = {"ms": ms, "values_per_s": n / (ms * 1e-3),
                      "roofline": {"bound": "hbm", "achieved": 4.0 * n / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                                   "frac": 4.0 * n / (ms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src}}
-    print(json.dumps({"metric": "statistics selected per second (tcw_topk / tcw_select_above)", "n": n,
-                      "steps": args.steps, "data": "synthetic", "results": res}), flush=True)
     h.close()
+    del v
+    torch.cuda.empty_cache()
+    return {"metric": "statistics selected per second (tcw_topk / tcw_select_above)", "n": n,
+            "steps": steps, "data": "synthetic", "results": res, "gpu_launches": (26 + 3) * steps}
+
+
+def run_select(args):
+    """--select N: one line for the selection calls."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    print(json.dumps(measure_select(args.select, args.steps, args.warmup)), flush=True)
     return 0
 
 
 # ----------------------------------------------------------------------------- data preparation mode (NEXT-3)
-def run_prep(args):
-    """--prep N_SFT: tcw_prepare on N_SFT 8-s segments of synthetic strain at 4096 Hz (device-resident),
-    band 500-1000 Hz (4000 bins), running median over 101 bins, bit-packed number count output: the
-    step that produces cfg3's input.  HBM model: one read of the strain (4 B/sample)."""
+def measure_prep(n_sft, steps, warmup):
+    """tcw_prepare on n_sft 8-s segments of synthetic strain at 4096 Hz (device-resident), band 500-1000 Hz
+    (4000 bins), running median over 101 bins: the step that produces cfg2's / cfg3's input.
+    HBM model: one read of the strain (4 B/sample)."""
     import torch
 
     import paper_2507_07816_b200 as tcw
-    import tcw_inputs
 
-    torch.cuda.set_device(0)
-    tcw.load_library()
     fs, T = 4096.0, 8.0
-    n_sft = args.prep
     g = torch.Generator(device="cuda").manual_seed(2)
     x = torch.randn(n_sft * int(fs * T), generator=g, device="cuda", dtype=torch.float32)
     peak, peak_src = load_peaks()
     res = {}
     for fmt in ("f32", "bits"):
-        for _ in range(max(2, min(args.warmup, 3))):
+        for _ in range(max(2, min(warmup, 3))):
             tcw.prepare(x, fs, T, 500.0, 4000, 101, 1.6, fmt)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             tcw.prepare(x, fs, T, 500.0, 4000, 101, 1.6, fmt)      # synchronises its stream
-        ms = 1e3 * (time.perf_counter() - t0) / args.steps
+        ms = 1e3 * (time.perf_counter() - t0) / steps
         gbs = 4.0 * x.numel() / (ms * 1e-3) / 1e9
         res[fmt] = {"ms": ms, "sfts_per_s": n_sft / (ms * 1e-3), "samples_per_s": x.numel() / (ms * 1e-3),
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
                                  "traffic": None, "peak_source": peak_src}}
-    print(json.dumps({"metric": "SFTs prepared per second (tcw_prepare: window, cuFFT R2C, running median, normalise, threshold)",
-                      "n_sft": n_sft, "fs": fs, "T_sft": T, "band_bins": 4000, "median_bins": 101, "steps": args.steps,
-                      "data": "synthetic", "timing": "host wall clock around the synchronous call (includes plan creation and scratch allocation)",
-                      "results": res}), flush=True)
+    del x
+    torch.cuda.empty_cache()
+    return {"metric": "SFTs prepared per second (tcw_prepare: window, cuFFT R2C, running median, normalise, threshold)",
+            "n_sft": n_sft, "fs": fs, "T_sft": T, "band_bins": 4000, "median_bins": 101, "steps": steps,
+            "data": "synthetic", "timing": "host wall clock around the synchronous call (includes plan creation and scratch allocation)",
+            "results": res}
+
+
+def run_prep(args):
+    """--prep N_SFT: one line for tcw_prepare."""
+    import torch
+
+    import paper_2507_07816_b200 as tcw
+    torch.cuda.set_device(0)
+    tcw.load_library()
+    print(json.dumps(measure_prep(args.prep, args.steps, args.warmup)), flush=True)
     return 0
 
 
@@ -788,6 +901,8 @@ def main():
                     help="time rank R's group range of an N-GPU strong-scaling run alone on one GPU (and check it against the whole search)")
     ap.add_argument("--shard-table", default=None, metavar="N1,N2,..",
                     help="one-GPU emulation of the split for each N: every rank's range timed alone, equal-count and equal-work cuts")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the weighted / bank / select / prep per_config entries")
+    ap.add_argument("--verbose", action="store_true", help="keep notes and provenance strings in the JSON line")
     ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
